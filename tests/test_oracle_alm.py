@@ -1,0 +1,163 @@
+"""Pins for oracle Part 2 (oracle/alm.py): exact line search against a brute-force scan, Lanczos
+against a dense eigen-solver, and the full ALORA loop against closed-form optima (MaxCut K_n and
+odd cycles, Lovasz theta) and the paper's Prop. 6 instance (the pass/fail test for rank
+adaptation: without the growth step ALM never leaves the spurious point).  CPU only."""
+import json
+import os
+
+import numpy as np
+import pytest
+
+from paper_2505_15775_b200 import inputs
+from tests.test_oracle_pins import _graph_maxcut, prop6_instance
+
+GOLD = json.load(open(os.path.join(os.path.dirname(__file__), "golden", "paper_examples.json")))
+
+
+@pytest.fixture(scope="module")
+def Oracle(oracle_mod):
+    return oracle_mod.Oracle
+
+
+@pytest.fixture(scope="module")
+def alm():
+    from oracle import alm
+    return alm
+
+
+def test_counter_uniform(alm):
+    v = alm.counter_uniform(7, 100000)
+    assert np.all(np.abs(v) < 1) and abs(v.mean()) < 0.01 and abs(v.var() - 1 / 3) < 0.01
+    np.testing.assert_array_equal(v, inputs.counter_uniform(7, 100000))
+    assert not np.array_equal(v[:100], alm.counter_uniform(8, 100))
+
+
+def test_quartic_argmin_bruteforce(alm):
+    rng = np.random.default_rng(3)
+    for _ in range(200):
+        p = rng.standard_normal(5)
+        p[4] = abs(p[4]) + 1e-3
+        p[1] = -abs(p[1])
+        a, flag = alm.quartic_argmin(p)
+        assert flag == 0 and a > 0
+        grid = np.linspace(0, 2 * a + 5, 200001)[1:]
+        phi = np.polyval(p[::-1], grid)
+        assert np.polyval(p[::-1], a) <= phi.min() + 1e-9 * (1 + abs(phi.min()))
+        assert abs(p[1] + a * (2 * p[2] + a * (3 * p[3] + 4 * p[4] * a))) < 1e-8 * (1 + np.abs(p).sum() * max(1, a) ** 3)
+    assert alm.quartic_argmin([0, -2.0, 4.0, 0, 0]) == (0.25, 0)
+    assert alm.quartic_argmin([0, -2.0, -1.0, 0, 0])[1] == 1
+
+
+def test_lanczos_dense(alm, Oracle):
+    w = inputs.small(0)
+    o = Oracle(w.problem)
+    lam, _ = o.lam(np.random.default_rng(1).standard_normal(w.problem.m), 1.0, w.R)
+    S = o.smatvec(lam, np.eye(w.problem.n))
+    ev, Q = np.linalg.eigh(S)
+    theta, v, k, resid = alm.lanczos(lambda x: o.smatvec(lam, x), w.problem.n, 42, 300, 1e-8)
+    assert abs(theta - ev[0]) < 1e-8 and k < 300
+    assert np.linalg.norm(S @ v - theta * v) < 1e-6
+    # breakdown: Prop. 6 operator has two distinct eigenvalues -> exact after 2 steps
+    P, y, F, rho, eps, a = prop6_instance()
+    o6 = Oracle(P)
+    theta, v, k, resid = alm.lanczos(lambda x: o6.smatvec(y, x), P.n, 1, 50, 1e-12)
+    assert k == 2 and abs(theta + eps) < 1e-14 and abs(abs(v[-1]) - 1) < 1e-12
+
+
+@pytest.mark.parametrize("n", [9, 20])
+def test_solve_Kn(alm, Oracle, n):
+    P = _graph_maxcut(n, [(i, j) for i in range(n) for j in range(i + 1, n)])
+    o = Oracle(P)
+    R0 = inputs._unit_rows(np.random.default_rng(n), n, 4)
+    res = alm.solve(o, R0, np.zeros(n), 1.0, alm.Params(eps=1e-7))
+    assert res.converged
+    assert abs(o.inner_C(res.R, res.R) + n * n / 4) < 1e-4
+    assert np.abs(res.y + n / 4).max() < 1e-4
+
+
+@pytest.mark.parametrize("n", [7, 51])
+def test_solve_odd_cycle(alm, Oracle, n):
+    P = _graph_maxcut(n, [(i, (i + 1) % n) for i in range(n)])
+    o = Oracle(P)
+    R0 = inputs._unit_rows(np.random.default_rng(n), n, 3)
+    res = alm.solve(o, R0, np.zeros(n), 1.0, alm.Params(eps=1e-7))
+    opt = -(n / 2) * (1 + np.cos(np.pi / n))
+    assert res.converged and abs(o.inner_C(res.R, res.R) - opt) < 1e-5 * abs(opt)
+    assert np.abs(res.y + 0.5 * (1 + np.cos(np.pi / n))).max() < 1e-4
+
+
+def test_solve_from_rank_one_grows(alm, Oracle):
+    """MaxCut on G(60,150) started from r0 = 1 must grow and reach the optimum found from r0 = 12."""
+    rng = inputs._rng(77)
+    lo, hi = inputs.gnm_edges(rng, 60, 150)
+    P = inputs.maxcut_problem(60, lo, hi, np.ones(150))
+    o = Oracle(P)
+    a = alm.solve(o, inputs._unit_rows(rng, 60, 12), np.zeros(60), 1.0, alm.Params(eps=1e-7))
+    b = alm.solve(o, inputs._unit_rows(rng, 60, 1), np.zeros(60), 1.0, alm.Params(eps=1e-7))
+    assert a.converged and b.converged and any(r.grew for r in b.log)
+    assert abs(o.inner_C(a.R, a.R) - o.inner_C(b.R, b.R)) < 1e-4
+
+
+@pytest.mark.parametrize("name,n,edges,theta", [
+    ("C5", 5, [(i, (i + 1) % 5) for i in range(5)], GOLD["theta"]["C5"]),
+    ("C7", 7, [(i, (i + 1) % 7) for i in range(7)], 7 * np.cos(np.pi / 7) / (1 + np.cos(np.pi / 7))),
+    ("K6", 6, [(i, j) for i in range(6) for j in range(i + 1, 6)], 1.0),
+    ("empty6", 6, [], 6.0)])
+def test_solve_theta(alm, Oracle, name, n, edges, theta):
+    lo = np.array([e[0] for e in edges], np.int64); hi = np.array([e[1] for e in edges], np.int64)
+    P = inputs.theta_problem(n, lo, hi)
+    o = Oracle(P)
+    R0 = np.random.default_rng(5).standard_normal((n, 3)) / np.sqrt(3 * n)
+    res = alm.solve(o, R0, np.zeros(P.m), 1.0, alm.Params(eps=1e-7))
+    assert res.converged, res.kkt
+    assert abs(o.inner_C(res.R, res.R) + theta) < 2e-5 * theta
+
+
+def test_prop6_escape(alm, Oracle):
+    """Started at the spurious local minimiser F-hat with y = [0,..,0,2]: with the
+    growth step ALORA reaches X* = a e_d e_d^T (objective eps*a, y* = [0,..,0,1]); with growth
+    disabled it halts at F-hat forever (zero inner iterations, dual infeasible)."""
+    P, y, F, rho, eps, a = prop6_instance()
+    o = Oracle(P)
+    fixed = dict(gamma=1.0, eps=1e-8)
+    res = alm.solve(o, F, y, rho, alm.Params(**fixed))
+    assert res.converged and res.log[0].grew == 1 and res.log[0].inner_iters == 0
+    X = res.R @ res.R.T
+    Xs = np.zeros((P.n, P.n)); Xs[-1, -1] = a
+    assert np.abs(X - Xs).max() < 1e-5 and abs(o.inner_C(res.R, res.R) - eps * a) < 1e-6
+    assert np.abs(res.y - np.r_[np.zeros(P.n - 1), 1.0]).max() < 1e-5
+    stuck = alm.solve(o, F, y, rho, alm.Params(tau_neg=1e30, T_max=40, **fixed))
+    assert not stuck.converged and all(r.inner_iters == 0 for r in stuck.log)
+    assert abs(o.inner_C(stuck.R, stuck.R) - 2 * eps * a) < 1e-12 and stuck.kkt[1] > 1e-3
+
+
+def test_config0_full_solve(alm, Oracle):
+    """BASELINE.json config 0 to KKT <= 1e-6; first-order condition (5a) holds at
+    the end: A(X) - b = (y_prev - y)/sigma by construction, and ||AX - b|| decreases overall."""
+    w = inputs.full(0)
+    o = Oracle(w.problem)
+    res = alm.solve(o, w.R, w.y, w.sigma, alm.Params(eps=1e-6))
+    assert res.converged and max(res.kkt) <= 1e-6
+    assert res.log[-1].qnorm < 1e-3 * res.log[0].qnorm
+    assert res.log[-1].r < 40 and any(r.shrank for r in res.log)
+    # Barvinok-Pataki: final rank r(r+1)/2 <= m
+    r = res.R.shape[1]
+    assert r * (r + 1) // 2 <= w.problem.m
+
+
+def test_thm1_bound_7b(alm, Oracle):
+    """(7b) PAPER.md:250: ||A X_{y,rho} - b|| <= ||y - y*||/rho for an exact subproblem solution;
+    K_9 with y* = -(9/4) 1, one outer iteration with a tight inner tolerance."""
+    n = 9
+    P = _graph_maxcut(n, [(i, j) for i in range(n) for j in range(i + 1, n)])
+    o = Oracle(P)
+    rng = np.random.default_rng(2)
+    ystar = np.full(n, -n / 4)
+    for rho in [0.5, 3.0]:
+        y = ystar + 0.3 * rng.standard_normal(n)
+        res = alm.solve(o, inputs._unit_rows(rng, n, n), y, rho,
+                        alm.Params(T_max=1, tol0=1e-10, tol_min=1e-12, it_max=5000, tau_neg=1e30, gamma=1.0))
+        q = o.A_op(res.R) - P.b
+        assert np.linalg.norm(q) <= np.linalg.norm(y - ystar) / rho * (1 + 1e-6)
+        # (8a) dual non-expansiveness: z = y - rho q is the updated dual
+        assert np.linalg.norm(res.y - ystar) <= np.linalg.norm(y - ystar) * (1 + 1e-6)
