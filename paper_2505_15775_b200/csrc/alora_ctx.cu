@@ -1,0 +1,411 @@
+// alora_ctx.cu -- context creation (validation, re-layout of the sparse data, upload) and the
+// small non-templated kernels (ordered final reductions, long-constraint finish, low-rank term).
+#include <algorithm>
+#include <cmath>
+#include <cstring>
+#include <numeric>
+
+#include "alora_internal.h"
+
+namespace alora {
+
+alora_status fail(alora_ctx* c, alora_status s, const std::string& msg) {
+  if (c) c->err = msg;
+  return s;
+}
+
+// ---------------------------------------------------------------------------------------------
+// small kernels
+// ---------------------------------------------------------------------------------------------
+// out[s] = sum over the partial rows of up to three regions, fixed order (one block, 8 warps)
+__global__ void k_finalize(const double* p0, int n0, const double* p1, int n1, const double* p2, int n2,
+                           double* out) {
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  for (int s = warp; s < kNStat; s += kBlock / 32) {
+    double v = 0.0;
+    for (int i = lane; i < n0; i += 32) v += p0[(int64_t)i * kNStat + s];
+    for (int i = lane; i < n1; i += 32) v += p1[(int64_t)i * kNStat + s];
+    for (int i = lane; i < n2; i += 32) v += p2[(int64_t)i * kNStat + s];
+    v = warp_sum(v);
+    if (lane == 0) out[s] = v;
+  }
+}
+
+// one block per long slot: ordered sum of its chunk partials, then the per-constraint finish.
+// slot cons id == m denotes C's sym-upper list (line search only): its sums are <C,RR^T>,
+// <C,RD^T>+<C,DR^T> (=2<C,RD^T>, halved here) and <C,DD^T>.
+__global__ void k_long_finish(int mode, int64_t m, const int* long_cons, const int64_t* long_chptr,
+                              const double* ch_out, const double* y, const double* b, double sigma,
+                              double* z, double* lam, double* partials) {
+  __shared__ double sm[3][kBlock / 32];
+  const int slot = blockIdx.x, lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int64_t c0 = long_chptr[slot], c1 = long_chptr[slot + 1];
+  double v[3] = {0.0, 0.0, 0.0};
+  for (int64_t c = c0 + threadIdx.x; c < c1; c += kBlock) {
+    v[0] += ch_out[3 * c]; v[1] += ch_out[3 * c + 1]; v[2] += ch_out[3 * c + 2];
+  }
+  for (int k = 0; k < 3; ++k) { double t = warp_sum(v[k]); if (lane == 0) sm[k][warp] = t; }
+  __syncthreads();
+  if (threadIdx.x < kNStat) partials[(int64_t)slot * kNStat + threadIdx.x] = 0.0;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    double t[3] = {0.0, 0.0, 0.0};
+    for (int k = 0; k < 3; ++k) for (int wv = 0; wv < kBlock / 32; ++wv) t[k] += sm[k][wv];
+    double st[kNStat];
+    for (int s = 0; s < kNStat; ++s) st[s] = 0.0;
+    const int64_t i = long_cons[slot];
+    if (i == m) {
+      st[LS_CRR] = t[0]; st[LS_CRD] = 0.5 * t[1]; st[LS_CDD] = t[2];
+    } else if (mode == CONS_EVAL) {
+      cons_finish<CONS_EVAL>(st, i, t[0], t[1], t[2], y, b, sigma, z, lam);
+    } else {
+      cons_finish<CONS_LS>(st, i, t[0], t[1], t[2], y, b, sigma, z, lam);
+    }
+    for (int s = 0; s < kNStat; ++s) partials[(int64_t)slot * kNStat + s] = st[s];
+  }
+}
+
+// Low-rank cost term, stage 1: per-block partials of T = U^T X (pC x r).  blockDim.x = r * rpb.
+template <typename T>
+__global__ void k_lowrank(const T* X, int64_t n, int r, int64_t ld, const T* U, int pC, double* part) {
+  extern __shared__ double lsm[];  // [pC][blockDim.x]
+  const int c = threadIdx.x % r, slot = threadIdx.x / r, rpb = blockDim.x / r;
+  double acc[8];
+  for (int p = 0; p < 8; ++p) acc[p] = 0.0;
+  for (int64_t row = (int64_t)blockIdx.x * rpb + slot; row < n; row += (int64_t)gridDim.x * rpb) {
+    const double xv = (double)X[row * ld + c];
+    for (int p = 0; p < pC; ++p) acc[p] += (double)U[row * pC + p] * xv;
+  }
+  for (int p = 0; p < pC; ++p) lsm[p * blockDim.x + threadIdx.x] = acc[p];
+  __syncthreads();
+  if (slot == 0) {
+    for (int p = 0; p < pC; ++p) {
+      double v = 0.0;
+      for (int s2 = 0; s2 < rpb; ++s2) v += lsm[p * blockDim.x + s2 * r + c];
+      part[((int64_t)blockIdx.x * pC + p) * r + c] = v;
+    }
+  }
+}
+// stage 2: Tm[p][c] = sum over blocks; Ts = s_p * Tm (optional)
+__global__ void k_lowrank_reduce(const double* part, int nblk, int pC, int r, const double* s, double* Tm,
+                                 double* Ts) {
+  for (int idx = threadIdx.x; idx < pC * r; idx += blockDim.x) {
+    double v = 0.0;
+    for (int bk = 0; bk < nblk; ++bk) v += part[(int64_t)bk * pC * r + idx];
+    Tm[idx] = v;
+    if (Ts) Ts[idx] = s[idx / r] * v;
+  }
+}
+
+// lambda = y - sigma (z - b)
+__global__ void k_lambda(int64_t m, const double* y, const double* z, const double* b, double sigma, double* lam) {
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < m; i += (int64_t)gridDim.x * blockDim.x)
+    lam[i] = y[i] - sigma * (z[i] - b[i]);
+}
+
+int pick_vec(const alora_ctx* c, int64_t ld, const void* p0, const void* p1, const void* p2) {
+  const int maxv = (int)(16 / c->esz);
+  for (int v = maxv; v > 1; v /= 2) {
+    const size_t al = (size_t)v * c->esz;
+    if (ld % v) continue;
+    if (((uintptr_t)p0 % al) || ((uintptr_t)p1 % al) || ((uintptr_t)p2 % al)) continue;
+    return v;
+  }
+  return 1;
+}
+
+}  // namespace alora
+
+// ---------------------------------------------------------------------------------------------
+// hot-path calls: alora_eval / alora_linesearch / alora_smatvec
+// ---------------------------------------------------------------------------------------------
+namespace alora {
+namespace {
+
+int vec_slot(int vec) { return vec == 1 ? 0 : vec == 2 ? 1 : 2; }
+
+template <typename T> int grid_rows(alora_ctx* c, int vec, int shape, int mode, int64_t items) {
+  int& occ = c->occ_cache[vec_slot(vec)][shape][mode];
+  if (!occ) occ = std::max(1, occ_rows(T(), vec, shape, mode));
+  const int gpb = kBlock / kShapes[shape].gs;
+  const int64_t need = (items + gpb - 1) / gpb;
+  return (int)std::max<int64_t>(1, std::min<int64_t>(need, std::min<int64_t>((int64_t)c->num_sms * occ, c->part_cap)));
+}
+template <typename T> int grid_cons(alora_ctx* c, int vec, int shape, int mode, int chunked, int64_t items) {
+  int& occ = c->occ_cache[vec_slot(vec)][shape][3 + mode * 2 + chunked];
+  if (!occ) occ = std::max(1, occ_cons(T(), vec, shape, mode, chunked));
+  const int gpb = kBlock / kShapes[shape].gs;
+  const int64_t need = (items + gpb - 1) / gpb;
+  return (int)std::max<int64_t>(1, std::min<int64_t>(need, std::min<int64_t>((int64_t)c->num_sms * occ, c->part_cap)));
+}
+
+struct Geo { int vec, nvec, shape, exact; };
+alora_status geometry(alora_ctx* c, int32_t r, int64_t ld, const void* p0, const void* p1, const void* p2, Geo& g) {
+  if (r < 1 || ld < r) return fail(c, ALORA_EINVAL, "need 1 <= r <= ld");
+  if (((uintptr_t)p0 % c->esz) || ((uintptr_t)p1 % c->esz) || ((uintptr_t)p2 % c->esz)) return fail(c, ALORA_EINVAL, "misaligned pointer");
+  g.vec = pick_vec(c, ld, p0, p1, p2);
+  g.nvec = (r + g.vec - 1) / g.vec;
+  g.shape = shape_index(g.nvec);
+  g.exact = (g.nvec * g.vec == r);
+  if (g.shape < 0) return fail(c, ALORA_EINVAL, "r too large for this alignment (<= 64 packs per row)");
+  return ALORA_OK;
+}
+
+template <typename T> void fill_rows(alora_ctx* c, RowArgs<T>& a, const Geo& g, const T* X, int r, int64_t ld) {
+  a.n = c->n; a.r = r; a.ld = ld; a.nvec = g.nvec; a.exact = g.exact; a.X = X; a.X2 = nullptr; a.Out = nullptr;
+  a.c_rowptr = c->c_rowptr; a.c_col = c->c_col; a.c_val = (const T*)c->c_val; a.dC = (const T*)c->dC;
+  a.dcons = c->dcons; a.da = (const T*)c->da;
+  a.a_rowptr = c->a_rowptr; a.a_col = c->a_col; a.a_val = (const T*)c->a_val; a.a_cons = c->a_cons;
+  a.y = c->y; a.b = c->b; a.sigma = c->sigma; a.w = nullptr; a.z = nullptr;
+  a.pC = 0; a.U = (const T*)c->U; a.Ts = c->Ts; a.scale = 1.0; a.diag_class = (c->cls == 0);
+  a.partials = c->part_rows;
+}
+template <typename T> void fill_cons(alora_ctx* c, ConsArgs<T>& a, const Geo& g, const T* X, const T* X2, int r, int64_t ld) {
+  a.n = c->n; a.r = r; a.ld = ld; a.nvec = g.nvec; a.exact = g.exact; a.X = X; a.X2 = X2; a.m = c->m;
+  a.ptr = c->f_ptr; a.e_row = c->f_row; a.e_col = c->f_col; a.e_val = (const T*)c->f_val;
+  a.y = c->y; a.b = c->b; a.sigma = c->sigma; a.z = nullptr; a.lam = c->lam;
+  a.nchunk = 0; a.ch_beg = c->ch_beg; a.ch_end = c->ch_end; a.ch_out = c->ch_out; a.partials = c->part_cons;
+}
+
+// T = U^T X (pC x r) into Tm, optionally Ts = s * Tm
+template <typename T> alora_status lowrank(alora_ctx* c, const T* X, int r, int64_t ld, double* Tm, bool want_Ts) {
+  if (r > c->lr_rmax) return fail(c, ALORA_EINVAL, "low-rank cost term supports r <= 256");
+  const int rpb = std::max(1, kBlock / r), threads = r * rpb;
+  k_lowrank<T><<<c->lr_grid, threads, sizeof(double) * c->pC * threads, c->stream>>>(X, c->n, r, ld, (const T*)c->U, c->pC, c->lr_part);
+  k_lowrank_reduce<<<1, kBlock, 0, c->stream>>>(c->lr_part, c->lr_grid, c->pC, r, c->s_dev, Tm, want_Ts ? c->Ts : nullptr);
+  c->launches += 2;
+  ALORA_CUDA(c, cudaGetLastError());
+  return ALORA_OK;
+}
+
+template <typename T> alora_status eval_impl(alora_ctx* c, const T* R, int32_t r, int64_t ld, T* G, double* z_dev) {
+  Geo g;
+  alora_status s = geometry(c, r, ld, R, G, nullptr, g);
+  if (s != ALORA_OK) return s;
+  if (G && (const void*)G == (const void*)R) return fail(c, ALORA_EINVAL, "G must not alias R");
+  double* zout = z_dev ? z_dev : c->z_int;
+  RowArgs<T> a;
+  fill_rows(c, a, g, R, r, ld);
+  a.Out = G; a.scale = 2.0;
+  if (c->cls == 0) {
+    a.z = zout;
+    const int grid = grid_rows<T>(c, g.vec, g.shape, ROWS_FUSED_EVAL, c->n);
+    ALORA_CUDA(c, launch_rows(g.vec, g.shape, ROWS_FUSED_EVAL, a, grid, c->stream));
+    k_finalize<<<1, kBlock, 0, c->stream>>>(c->part_rows, grid, nullptr, 0, nullptr, 0, c->stats_dev);
+    c->launches += 2;
+  } else {
+    if (c->pC) { s = lowrank<T>(c, R, r, ld, c->TmR, true); if (s != ALORA_OK) return s; a.pC = c->pC; }
+    ConsArgs<T> ca;
+    fill_cons(c, ca, g, R, (const T*)nullptr, r, ld);
+    ca.z = zout;
+    int gc = 0;
+    if (c->m > 0) {
+      gc = grid_cons<T>(c, g.vec, g.shape, CONS_EVAL, 0, c->m);
+      ALORA_CUDA(c, launch_cons(g.vec, g.shape, CONS_EVAL, 0, ca, gc, c->stream));
+      c->launches++;
+    }
+    if (c->nchunk_A > 0) {
+      ca.nchunk = c->nchunk_A;
+      const int gk = grid_cons<T>(c, g.vec, g.shape, CONS_EVAL, 1, c->nchunk_A);
+      ALORA_CUDA(c, launch_cons(g.vec, g.shape, CONS_EVAL, 1, ca, gk, c->stream));
+      k_long_finish<<<c->nlong_A, kBlock, 0, c->stream>>>(CONS_EVAL, c->m, c->long_cons, c->long_chptr, c->ch_out, c->y,
+                                                         c->b, c->sigma, zout, c->lam, c->part_long);
+      c->launches += 2;
+    }
+    a.w = c->lam; a.diag_class = 0;
+    const int grid = grid_rows<T>(c, g.vec, g.shape, ROWS_ADJ, c->n);
+    ALORA_CUDA(c, launch_rows(g.vec, g.shape, ROWS_ADJ, a, grid, c->stream));
+    k_finalize<<<1, kBlock, 0, c->stream>>>(c->part_rows, grid, c->part_cons, gc, c->part_long, c->nlong_A, c->stats_dev);
+    c->launches += 2;
+  }
+  ALORA_CUDA(c, cudaGetLastError());
+  c->z_last = zout; c->have_eval = true;
+  return ALORA_OK;
+}
+
+alora_status fetch_stats(alora_ctx* c, int r_lowrank, double stats[8]) {
+  ALORA_CUDA(c, cudaMemcpyAsync(c->pinned, c->stats_dev, sizeof(double) * kNStat, cudaMemcpyDeviceToHost, c->stream));
+  if (c->pC && c->cls == 1)
+    ALORA_CUDA(c, cudaMemcpyAsync(c->pinned + 64, c->TmR, sizeof(double) * c->pC * r_lowrank, cudaMemcpyDeviceToHost, c->stream));
+  ALORA_CUDA(c, cudaStreamSynchronize(c->stream));
+  const double* p = c->pinned;
+  double cx = p[ES_CX];
+  if (c->pC && c->cls == 1)
+    for (int q = 0; q < c->pC; ++q) {
+      double t = 0.0;
+      for (int k = 0; k < r_lowrank; ++k) t += p[64 + q * r_lowrank + k] * p[64 + q * r_lowrank + k];
+      cx += c->s_host[q] * t;
+    }
+  stats[1] = cx; stats[2] = p[ES_YQ]; stats[3] = p[ES_QQ]; stats[4] = p[ES_GG]; stats[5] = p[ES_GR]; stats[6] = p[ES_LZ]; stats[7] = 0.0;
+  stats[0] = cx - p[ES_YQ] + 0.5 * c->sigma * p[ES_QQ];
+  return ALORA_OK;
+}
+
+template <typename T> alora_status ls_impl(alora_ctx* c, const T* R, const T* D, int32_t r, int64_t ld) {
+  Geo g;
+  alora_status s = geometry(c, r, ld, R, D, nullptr, g);
+  if (s != ALORA_OK) return s;
+  if (c->cls == 0) {
+    RowArgs<T> a;
+    fill_rows(c, a, g, R, r, ld);
+    a.X2 = D;
+    const int grid = grid_rows<T>(c, g.vec, g.shape, ROWS_LS_FUSED, c->n);
+    ALORA_CUDA(c, launch_rows(g.vec, g.shape, ROWS_LS_FUSED, a, grid, c->stream));
+    k_finalize<<<1, kBlock, 0, c->stream>>>(c->part_rows, grid, nullptr, 0, nullptr, 0, c->ls_dev);
+    c->launches += 2;
+  } else {
+    if (c->pC) {
+      s = lowrank<T>(c, R, r, ld, c->TmR, false); if (s != ALORA_OK) return s;
+      s = lowrank<T>(c, D, r, ld, c->TmD, false); if (s != ALORA_OK) return s;
+    }
+    ConsArgs<T> ca;
+    fill_cons(c, ca, g, R, D, r, ld);
+    int gc = 0;
+    if (c->m > 0) {
+      gc = grid_cons<T>(c, g.vec, g.shape, CONS_LS, 0, c->m);
+      ALORA_CUDA(c, launch_cons(g.vec, g.shape, CONS_LS, 0, ca, gc, c->stream));
+      c->launches++;
+    }
+    if (c->nchunk_all > 0) {
+      ca.nchunk = c->nchunk_all;
+      const int gk = grid_cons<T>(c, g.vec, g.shape, CONS_LS, 1, c->nchunk_all);
+      ALORA_CUDA(c, launch_cons(g.vec, g.shape, CONS_LS, 1, ca, gk, c->stream));
+      k_long_finish<<<c->nlong_all, kBlock, 0, c->stream>>>(CONS_LS, c->m, c->long_cons, c->long_chptr, c->ch_out, c->y,
+                                                           c->b, c->sigma, nullptr, nullptr, c->part_long);
+      c->launches += 2;
+    }
+    k_finalize<<<1, kBlock, 0, c->stream>>>(c->part_cons, gc, c->part_long, c->nlong_all, nullptr, 0, c->ls_dev);
+    c->launches++;
+  }
+  ALORA_CUDA(c, cudaGetLastError());
+  c->have_ls = true;
+  return ALORA_OK;
+}
+
+
+alora_status fetch_ls(alora_ctx* c, int r, double p[5]) {
+  ALORA_CUDA(c, cudaMemcpyAsync(c->pinned, c->ls_dev, sizeof(double) * kNStat, cudaMemcpyDeviceToHost, c->stream));
+  const bool lr = c->pC && c->cls == 1;
+  if (lr) {
+    ALORA_CUDA(c, cudaMemcpyAsync(c->pinned + 64, c->TmR, sizeof(double) * c->pC * r, cudaMemcpyDeviceToHost, c->stream));
+    ALORA_CUDA(c, cudaMemcpyAsync(c->pinned + 64 + 8 * 256, c->TmD, sizeof(double) * c->pC * r, cudaMemcpyDeviceToHost, c->stream));
+  }
+  ALORA_CUDA(c, cudaStreamSynchronize(c->stream));
+  const double* s = c->pinned;
+  double cRR = s[LS_CRR], cRD = s[LS_CRD], cDD = s[LS_CDD];
+  if (lr)
+    for (int q = 0; q < c->pC; ++q) {
+      const double* tr = s + 64 + q * r; const double* td = s + 64 + 8 * 256 + q * r;
+      double rr = 0, rd = 0, dd = 0;
+      for (int k = 0; k < r; ++k) { rr += tr[k] * tr[k]; rd += tr[k] * td[k]; dd += td[k] * td[k]; }
+      cRR += c->s_host[q] * rr; cRD += c->s_host[q] * rd; cDD += c->s_host[q] * dd;
+    }
+  const double sg = c->sigma;
+  p[0] = cRR - s[LS_YQ] + 0.5 * sg * s[LS_QQ];
+  p[1] = 2.0 * cRD - s[LS_YQ1] + sg * s[LS_QQ1];
+  p[2] = cDD - s[LS_YQ2] + 0.5 * sg * s[LS_Q11] + sg * s[LS_QQ2];
+  p[3] = sg * s[LS_Q12];
+  p[4] = 0.5 * sg * s[LS_Q22];
+  return ALORA_OK;
+}
+
+template <typename T> alora_status matvec_impl(alora_ctx* c, const double* mu, const T* V, int32_t p, T* W) {
+  Geo g;
+  alora_status s = geometry(c, p, p, V, W, nullptr, g);
+  if (s != ALORA_OK) return s;
+  RowArgs<T> a;
+  fill_rows(c, a, g, V, p, p);
+  a.Out = W; a.scale = 1.0; a.w = mu; a.diag_class = (c->cls == 0);
+  if (c->pC) { s = lowrank<T>(c, V, p, p, c->TmD, true); if (s != ALORA_OK) return s; a.pC = c->pC; }
+  const int grid = grid_rows<T>(c, g.vec, g.shape, ROWS_ADJ, c->n);
+  ALORA_CUDA(c, launch_rows(g.vec, g.shape, ROWS_ADJ, a, grid, c->stream));
+  k_finalize<<<1, kBlock, 0, c->stream>>>(c->part_rows, grid, nullptr, 0, nullptr, 0, c->mv_dev);
+  c->launches += 2;
+  ALORA_CUDA(c, cudaGetLastError());
+  return ALORA_OK;
+}
+
+
+}  // namespace
+}  // namespace alora
+
+using namespace alora;
+
+extern "C" alora_status alora_eval(alora_ctx* c, const void* R, int32_t r, int64_t ld, void* G, double* z_dev, double stats[8]) {
+  if (!c || !R) return c ? fail(c, ALORA_EINVAL, "alora_eval: NULL argument") : ALORA_EINVAL;
+  if (!c->have_dual) return fail(c, ALORA_ESTATE, "alora_eval before alora_set_dual");
+  ALORA_CUDA(c, cudaSetDevice(c->device));
+  alora_status s = c->dtype == ALORA_F32 ? eval_impl<float>(c, (const float*)R, r, ld, (float*)G, z_dev)
+                                         : eval_impl<double>(c, (const double*)R, r, ld, (double*)G, z_dev);
+  if (s != ALORA_OK) return s;
+  c->last_eval_r = r;
+  return stats ? fetch_stats(c, r, stats) : ALORA_OK;
+}
+
+extern "C" alora_status alora_get_stats(alora_ctx* c, double stats[8]) {
+  if (!c || !stats) return ALORA_EINVAL;
+  if (!c->have_eval) return fail(c, ALORA_ESTATE, "alora_get_stats before alora_eval");
+  return fetch_stats(c, c->last_eval_r, stats);
+}
+
+extern "C" alora_status alora_get_lambda(alora_ctx* c, double* lam_dev) {
+  if (!c || !lam_dev) return ALORA_EINVAL;
+  if (!c->have_eval) return fail(c, ALORA_ESTATE, "alora_get_lambda before alora_eval");
+  const int grid = (int)std::max<int64_t>(1, std::min<int64_t>((c->m + 255) / 256, (int64_t)c->num_sms * 8));
+  k_lambda<<<grid, 256, 0, c->stream>>>(c->m, c->y, c->z_last, c->b, c->sigma, lam_dev);
+  c->launches++;
+  ALORA_CUDA(c, cudaGetLastError());
+  return ALORA_OK;
+}
+
+extern "C" alora_status alora_eval_host(alora_ctx* c, const void* R_host, int32_t r, int64_t ld, void* G_host, double* z_host,
+                                        double stats[8]) {
+  if (!c || !R_host || !stats) return c ? fail(c, ALORA_EINVAL, "alora_eval_host: NULL argument") : ALORA_EINVAL;
+  if (r < 1 || ld < r) return fail(c, ALORA_EINVAL, "need 1 <= r <= ld");
+  ALORA_CUDA(c, cudaSetDevice(c->device));
+  const size_t nb = (size_t)c->n * (size_t)ld * c->esz;
+  if (nb > c->stage_bytes) {
+    if (c->stageR) { c->pool.release(c->stageR); c->pool.release(c->stageG); }
+    ALORA_CUDA(c, c->pool.alloc(&c->stageR, nb));
+    ALORA_CUDA(c, c->pool.alloc(&c->stageG, nb));
+    c->stage_bytes = nb;
+  }
+  ALORA_CUDA(c, cudaMemcpyAsync(c->stageR, R_host, nb, cudaMemcpyHostToDevice, c->stream));
+  alora_status s = alora_eval(c, c->stageR, r, ld, G_host ? c->stageG : nullptr, nullptr, nullptr);
+  if (s != ALORA_OK) return s;
+  if (G_host) ALORA_CUDA(c, cudaMemcpyAsync(G_host, c->stageG, nb, cudaMemcpyDeviceToHost, c->stream));
+  if (z_host) ALORA_CUDA(c, cudaMemcpyAsync(z_host, c->z_int, sizeof(double) * c->m, cudaMemcpyDeviceToHost, c->stream));
+  return fetch_stats(c, r, stats);
+}
+
+extern "C" alora_status alora_linesearch(alora_ctx* c, const void* R, const void* D, int32_t r, int64_t ld, double p[5]) {
+  if (!c || !R || !D) return c ? fail(c, ALORA_EINVAL, "alora_linesearch: NULL argument") : ALORA_EINVAL;
+  if (!c->have_dual) return fail(c, ALORA_ESTATE, "alora_linesearch before alora_set_dual");
+  ALORA_CUDA(c, cudaSetDevice(c->device));
+  alora_status s = c->dtype == ALORA_F32 ? ls_impl<float>(c, (const float*)R, (const float*)D, r, ld)
+                                         : ls_impl<double>(c, (const double*)R, (const double*)D, r, ld);
+  if (s != ALORA_OK) return s;
+  c->last_ls_r = r;
+  return p ? fetch_ls(c, r, p) : ALORA_OK;
+}
+
+extern "C" alora_status alora_get_linesearch(alora_ctx* c, double p[5]) {
+  if (!c || !p) return ALORA_EINVAL;
+  if (!c->have_ls) return fail(c, ALORA_ESTATE, "alora_get_linesearch before alora_linesearch");
+  return fetch_ls(c, c->last_ls_r, p);
+}
+
+extern "C" alora_status alora_smatvec(alora_ctx* c, const double* mu_dev, const void* V, int32_t p, void* W, double* vw) {
+  if (!c || !V || !W || (!mu_dev && c->m > 0)) return c ? fail(c, ALORA_EINVAL, "alora_smatvec: NULL argument") : ALORA_EINVAL;
+  if (V == W) return fail(c, ALORA_EINVAL, "W must not alias V");
+  ALORA_CUDA(c, cudaSetDevice(c->device));
+  alora_status s = c->dtype == ALORA_F32 ? matvec_impl<float>(c, mu_dev, (const float*)V, p, (float*)W)
+                                         : matvec_impl<double>(c, mu_dev, (const double*)V, p, (double*)W);
+  if (s != ALORA_OK) return s;
+  if (vw) {
+    ALORA_CUDA(c, cudaMemcpyAsync(c->pinned + 32, c->mv_dev, sizeof(double) * kNStat, cudaMemcpyDeviceToHost, c->stream));
+    ALORA_CUDA(c, cudaStreamSynchronize(c->stream));
+    *vw = c->pinned[32 + ES_GR];
+  }
+  return ALORA_OK;
+}

@@ -1,0 +1,103 @@
+// alora_internal.h -- the context behind include/alora.h (host side).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <string>
+#include <vector>
+
+#include "../../include/alora.h"
+#include "dispatch.h"
+
+namespace alora {
+
+// device array with byte accounting
+struct DevPool {
+  std::vector<void*> ptrs;
+  size_t bytes = 0;
+  cudaError_t alloc(void** p, size_t nbytes) {
+    *p = nullptr;
+    if (nbytes == 0) nbytes = 16;
+    cudaError_t e = cudaMalloc(p, nbytes);
+    if (e == cudaSuccess) { ptrs.push_back(*p); bytes += nbytes; }
+    return e;
+  }
+  void release(void* p) {
+    for (auto& q : ptrs) if (q == p) { cudaFree(q); q = nullptr; }
+  }
+  void free_all() {
+    for (void* p : ptrs) if (p) cudaFree(p);
+    ptrs.clear();
+  }
+};
+
+struct SolveWorkspace;  // alora_solve.cu
+
+}  // namespace alora
+
+struct alora_ctx {
+  int device = 0;
+  cudaStream_t stream = nullptr;
+  alora_dtype dtype = ALORA_F32;
+  size_t esz = 4;
+  int64_t n = 0, m = 0;
+  int cls = 0;  // 0: diagonal class (one fused pass), 1: general (forward + adjoint)
+  int num_sms = 148;
+  std::string err;
+  alora::DevPool pool;
+
+  // C: diagonal + off-diagonal full-pattern CSR (columns ascending within a row)
+  int* c_rowptr = nullptr; int* c_col = nullptr; void* c_val = nullptr; void* dC = nullptr;
+  int64_t c_nnz = 0;
+  // diagonal class: constraint of row j (-1: none) and its coefficient; null = identity / ones
+  int* dcons = nullptr; void* da = nullptr;
+  // general class: row-oriented full pattern of the constraints
+  int* a_rowptr = nullptr; int* a_col = nullptr; void* a_val = nullptr; int* a_cons = nullptr;
+  int64_t a_nnz = 0;
+  // forward list: coalesced constraint entries [0, nf_A), then C's sym-upper entries [nf_A, nf_A+nf_C)
+  int64_t* f_ptr = nullptr; int* f_row = nullptr; int* f_col = nullptr; void* f_val = nullptr;
+  int64_t nf_A = 0, nf_C = 0;
+  // chunks of long constraints (first nchunk_A) and of C (the rest); slots: long constraints, then C
+  int64_t* ch_beg = nullptr; int64_t* ch_end = nullptr; int64_t nchunk_A = 0, nchunk_all = 0;
+  int* long_cons = nullptr; int64_t* long_chptr = nullptr; int nlong_A = 0, nlong_all = 0;
+  double* ch_out = nullptr;
+  // vectors
+  double* b = nullptr; const double* y = nullptr; double sigma = 0.0; bool have_dual = false;
+  double* z_int = nullptr; double* lam = nullptr; const double* z_last = nullptr;
+  double normb = 0.0, normC = 0.0;
+  // low-rank cost
+  int pC = 0; void* U = nullptr; double* s_dev = nullptr; std::vector<double> s_host;
+  double* lr_part = nullptr; double* TmR = nullptr; double* TmD = nullptr; double* Ts = nullptr; double* lr_scal = nullptr;
+  int lr_grid = 0; int lr_rmax = 256;
+  // partial sums / results
+  int part_cap = 0;
+  double* part_rows = nullptr; double* part_cons = nullptr; double* part_long = nullptr;
+  double* stats_dev = nullptr; double* ls_dev = nullptr; double* mv_dev = nullptr;
+  double* pinned = nullptr;  // 64 doubles
+  bool have_eval = false, have_ls = false;
+  int last_eval_r = 0, last_ls_r = 0;
+  int64_t launches = 0;
+  // staging for alora_eval_host
+  void* stageR = nullptr; void* stageG = nullptr; size_t stage_bytes = 0;
+  void* pinR = nullptr; size_t pin_bytes = 0;
+  // occupancy cache [vec idx][shape][kind]
+  int occ_cache[3][7][8];
+  alora::SolveWorkspace* ws = nullptr;
+};
+
+namespace alora {
+
+alora_status fail(alora_ctx* c, alora_status s, const std::string& msg);
+#define ALORA_CUDA(c, expr)                                                                        \
+  do {                                                                                             \
+    cudaError_t e__ = (expr);                                                                      \
+    if (e__ != cudaSuccess)                                                                        \
+      return alora::fail((c), e__ == cudaErrorMemoryAllocation ? ALORA_ENOMEM : ALORA_ECUDA,      \
+                         std::string(#expr) + ": " + cudaGetErrorString(e__));                     \
+  } while (0)
+
+// alora_ctx.cu
+int pick_vec(const alora_ctx* c, int64_t ld, const void* p0, const void* p1, const void* p2);
+void free_solve_workspace(alora_ctx* c);
+
+}  // namespace alora

@@ -1,0 +1,50 @@
+// dispatch.h -- host-side launchers for the templated kernels, one translation unit per
+// (element type, vector width) so the instantiations compile in parallel.
+#pragma once
+#include "kernels.cuh"
+
+namespace alora {
+
+#define ALORA_DECL_INST(T, SUF)                                                                       \
+  cudaError_t launch_rows_##SUF(int shape, int mode, const RowArgs<T>& a, int grid, cudaStream_t s);  \
+  cudaError_t launch_cons_##SUF(int shape, int mode, int chunked, const ConsArgs<T>& a, int grid,     \
+                                cudaStream_t s);                                                      \
+  int occ_rows_##SUF(int shape, int mode);                                                            \
+  int occ_cons_##SUF(int shape, int mode, int chunked);
+
+ALORA_DECL_INST(float, f32v4)
+ALORA_DECL_INST(float, f32v2)
+ALORA_DECL_INST(float, f32v1)
+ALORA_DECL_INST(double, f64v2)
+ALORA_DECL_INST(double, f64v1)
+#undef ALORA_DECL_INST
+
+// generic front-ends: vec = elements per vector load
+inline cudaError_t launch_rows(int vec, int shape, int mode, const RowArgs<float>& a, int grid, cudaStream_t s) {
+  return vec == 4 ? launch_rows_f32v4(shape, mode, a, grid, s)
+       : vec == 2 ? launch_rows_f32v2(shape, mode, a, grid, s) : launch_rows_f32v1(shape, mode, a, grid, s);
+}
+inline cudaError_t launch_rows(int vec, int shape, int mode, const RowArgs<double>& a, int grid, cudaStream_t s) {
+  return vec == 2 ? launch_rows_f64v2(shape, mode, a, grid, s) : launch_rows_f64v1(shape, mode, a, grid, s);
+}
+inline cudaError_t launch_cons(int vec, int shape, int mode, int chunked, const ConsArgs<float>& a, int grid, cudaStream_t s) {
+  return vec == 4 ? launch_cons_f32v4(shape, mode, chunked, a, grid, s)
+       : vec == 2 ? launch_cons_f32v2(shape, mode, chunked, a, grid, s) : launch_cons_f32v1(shape, mode, chunked, a, grid, s);
+}
+inline cudaError_t launch_cons(int vec, int shape, int mode, int chunked, const ConsArgs<double>& a, int grid, cudaStream_t s) {
+  return vec == 2 ? launch_cons_f64v2(shape, mode, chunked, a, grid, s) : launch_cons_f64v1(shape, mode, chunked, a, grid, s);
+}
+inline int occ_rows(float, int vec, int shape, int mode) {
+  return vec == 4 ? occ_rows_f32v4(shape, mode) : vec == 2 ? occ_rows_f32v2(shape, mode) : occ_rows_f32v1(shape, mode);
+}
+inline int occ_rows(double, int vec, int shape, int mode) {
+  return vec == 2 ? occ_rows_f64v2(shape, mode) : occ_rows_f64v1(shape, mode);
+}
+inline int occ_cons(float, int vec, int shape, int mode, int ch) {
+  return vec == 4 ? occ_cons_f32v4(shape, mode, ch) : vec == 2 ? occ_cons_f32v2(shape, mode, ch) : occ_cons_f32v1(shape, mode, ch);
+}
+inline int occ_cons(double, int vec, int shape, int mode, int ch) {
+  return vec == 2 ? occ_cons_f64v2(shape, mode, ch) : occ_cons_f64v1(shape, mode, ch);
+}
+
+}  // namespace alora

@@ -1,0 +1,408 @@
+// kernels.cuh -- templated sm_100a kernels of the ALM-BM hot path.
+//
+// Two kernel families, both HBM-bound gather/stream kernels (no dense contraction => no tensor cores):
+//   k_rows : one sub-warp group of GS lanes per row j of R (thin row, r = 10..40 elements, held in
+//            registers as NIT vectors of VEC elements per lane).  Streams the row-oriented CSR,
+//            gathers neighbour rows with vector loads, writes the output row, and accumulates every
+//            scalar of the evaluation lane-locally in fp64 (one block reduction at the very end).
+//              ROWS_FUSED_EVAL : "diagonal" class (MaxCut): z_j = a_j |R_j|^2 is row-local, so
+//                                z, q, lambda, G = 2 S(lambda) R, <C,RR^T>, y.q, |q|^2, |G|^2, <G,R>
+//                                come out of ONE pass                       (a1-a4 fused)
+//              ROWS_ADJ        : weighted-adjoint SpMM  Out = scale * (C - sum_i w_i A_i) X with the
+//                                weights w gathered by constraint id        (a3; a6 with scale = 1)
+//              ROWS_LS_FUSED   : line-search sums for the diagonal class    (a5)
+//   k_cons : SDDMM-style forward evaluator, one group per constraint (or per chunk of a long
+//            constraint): sum_e w_e a_e <R_j,R_k>  and the bilinear forms with D   (a1, a2, a5)
+// Sums across rows / constraints are fp64 and two-stage (per-block partials, then one ordered
+// reduction), so results do not depend on block scheduling.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace alora {
+
+constexpr int kBlock = 256;
+constexpr int kLongThreshold = 128;  // constraints with more stored entries are split into chunks
+constexpr int kChunk = 64;           // entries per chunk of a long constraint
+
+enum RowsMode { ROWS_FUSED_EVAL = 0, ROWS_ADJ = 1, ROWS_LS_FUSED = 2 };
+enum ConsMode { CONS_EVAL = 0, CONS_LS = 1 };
+
+// stat slots written by the kernels (per-block partial rows have this many doubles)
+constexpr int kNStat = 16;
+enum EvalStat { ES_CX = 0, ES_YQ = 1, ES_QQ = 2, ES_GG = 3, ES_GR = 4, ES_LZ = 5 };
+enum LsStat { LS_CRR = 0, LS_CRD = 1, LS_CDD = 2, LS_YQ = 3, LS_YQ1 = 4, LS_YQ2 = 5, LS_QQ = 6,
+              LS_QQ1 = 7, LS_QQ2 = 8, LS_Q11 = 9, LS_Q12 = 10, LS_Q22 = 11 };
+
+template <typename T> struct RowArgs {
+  int64_t n; int r; int64_t ld; int nvec; int exact;  // exact: r == nvec*VEC (no tail masking)
+  const T* X;    // R (or V)
+  const T* X2;   // D (ROWS_LS_FUSED)
+  T* Out;        // G / W, may be null
+  const int* c_rowptr; const int* c_col; const T* c_val; const T* dC;  // off-diagonal C (full pattern) + diag
+  const int* dcons; const T* da;       // diagonal class: constraint on row j and its coefficient (null: j / 1)
+  const int* a_rowptr; const int* a_col; const T* a_val; const int* a_cons;  // general class, full pattern
+  const double* y; const double* b; double sigma;
+  const double* w;   // ROWS_ADJ weights (lambda or mu), fp64[m]
+  double* z;         // ROWS_FUSED_EVAL: z out (fp64[m]) or null
+  int pC; const T* U; const double* Ts;  // low-rank cost: U n x pC row-major, Ts[p][r] = s_p (U^T X)_p
+  double scale;
+  int diag_class;    // ROWS_ADJ: 1 = constraints are the per-row diagonal ones, 0 = use a_* CSR
+  double* partials;  // [gridDim.x][kNStat]
+};
+
+template <typename T> struct ConsArgs {
+  int64_t n; int r; int64_t ld; int nvec; int exact;
+  const T* X; const T* X2;
+  int64_t m;                      // number of real constraints
+  const int64_t* ptr;             // m+1 (short kernel)
+  const int* e_row; const int* e_col; const T* e_val;  // forward entries (constraints, then C)
+  const double* y; const double* b; double sigma;
+  double* z; double* lam;         // CONS_EVAL outputs
+  // chunk kernel
+  int64_t nchunk; const int64_t* ch_beg; const int64_t* ch_end;
+  double* ch_out;                 // [nchunk][3]
+  double* partials;
+};
+
+// ---------------------------------------------------------------------------------------------
+template <typename T, int VEC> struct alignas(sizeof(T) * VEC) Pack { T v[VEC]; };
+
+template <typename T, int VEC> __device__ __forceinline__ Pack<T, VEC> ldg_pack(const T* p);
+template <> __device__ __forceinline__ Pack<float, 4> ldg_pack<float, 4>(const float* p) {
+  float4 t = __ldg(reinterpret_cast<const float4*>(p)); Pack<float, 4> o; o.v[0] = t.x; o.v[1] = t.y; o.v[2] = t.z; o.v[3] = t.w; return o; }
+template <> __device__ __forceinline__ Pack<float, 2> ldg_pack<float, 2>(const float* p) {
+  float2 t = __ldg(reinterpret_cast<const float2*>(p)); Pack<float, 2> o; o.v[0] = t.x; o.v[1] = t.y; return o; }
+template <> __device__ __forceinline__ Pack<float, 1> ldg_pack<float, 1>(const float* p) {
+  Pack<float, 1> o; o.v[0] = __ldg(p); return o; }
+template <> __device__ __forceinline__ Pack<double, 2> ldg_pack<double, 2>(const double* p) {
+  double2 t = __ldg(reinterpret_cast<const double2*>(p)); Pack<double, 2> o; o.v[0] = t.x; o.v[1] = t.y; return o; }
+template <> __device__ __forceinline__ Pack<double, 1> ldg_pack<double, 1>(const double* p) {
+  Pack<double, 1> o; o.v[0] = __ldg(p); return o; }
+
+template <typename T, int VEC> __device__ __forceinline__ void st_pack(T* p, const Pack<T, VEC>& x) {
+  *reinterpret_cast<Pack<T, VEC>*>(p) = x;
+}
+
+template <int GS> __device__ __forceinline__ unsigned group_mask() {
+  if (GS >= 32) return 0xffffffffu;
+  return ((1u << GS) - 1u) << (((threadIdx.x & 31) / GS) * GS);
+}
+template <int GS> __device__ __forceinline__ double group_sum(double v, unsigned mask) {
+#pragma unroll
+  for (int o = GS / 2; o > 0; o >>= 1) v += __shfl_xor_sync(mask, v, o);
+  return v;
+}
+__device__ __forceinline__ double warp_sum(double v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+
+// Ordered block reduction of NST per-thread fp64 partials -> out[0..NST)
+template <int NST> __device__ __forceinline__ void block_reduce_store(double (&st)[NST], double* out) {
+  __shared__ double sm[NST][kBlock / 32];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+#pragma unroll
+  for (int s = 0; s < NST; ++s) {
+    double v = warp_sum(st[s]);
+    if (lane == 0) sm[s][warp] = v;
+  }
+  __syncthreads();
+  if (threadIdx.x < kNStat) {  // unused slots of the partial row are written as zero
+    double v = 0.0;
+    if (threadIdx.x < NST) {
+#pragma unroll
+      for (int wv = 0; wv < kBlock / 32; ++wv) v += sm[threadIdx.x][wv];
+    }
+    out[threadIdx.x] = v;
+  }
+}
+
+// Row vector held by one lane: NIT packs of VEC elements, pack index vi = lane + it*GS.
+template <typename T, int VEC, int GS, int NIT> struct RowReg {
+  Pack<T, VEC> p[NIT];
+  __device__ __forceinline__ void zero() {
+#pragma unroll
+    for (int it = 0; it < NIT; ++it)
+#pragma unroll
+      for (int i = 0; i < VEC; ++i) p[it].v[i] = T(0);
+  }
+  // load row `base` (pointer to the first element of the row); masks the tail beyond r
+  __device__ __forceinline__ void load(const T* base, int lane, int nvec, int r, int exact) {
+#pragma unroll
+    for (int it = 0; it < NIT; ++it) {
+      const int vi = lane + it * GS;
+      if (vi < nvec) {
+        p[it] = ldg_pack<T, VEC>(base + vi * VEC);
+        if (VEC > 1 && !exact && vi == nvec - 1) {
+#pragma unroll
+          for (int i = 0; i < VEC; ++i) if (vi * VEC + i >= r) p[it].v[i] = T(0);
+        }
+      } else {
+#pragma unroll
+        for (int i = 0; i < VEC; ++i) p[it].v[i] = T(0);
+      }
+    }
+  }
+  __device__ __forceinline__ void store(T* base, int lane, int nvec, int r, int exact) const {
+#pragma unroll
+    for (int it = 0; it < NIT; ++it) {
+      const int vi = lane + it * GS;
+      if (vi < nvec) {
+        if (VEC > 1 && !exact && vi == nvec - 1) {
+#pragma unroll
+          for (int i = 0; i < VEC; ++i) if (vi * VEC + i < r) base[vi * VEC + i] = p[it].v[i];
+        } else {
+          st_pack<T, VEC>(base + vi * VEC, p[it]);
+        }
+      }
+    }
+  }
+  __device__ __forceinline__ void axpy(T a, const RowReg& x) {
+#pragma unroll
+    for (int it = 0; it < NIT; ++it)
+#pragma unroll
+      for (int i = 0; i < VEC; ++i) p[it].v[i] = fma(a, x.p[it].v[i], p[it].v[i]);
+  }
+  __device__ __forceinline__ T dot(const RowReg& x) const {  // lane-local part of the dot product
+    T s = T(0);
+#pragma unroll
+    for (int it = 0; it < NIT; ++it)
+#pragma unroll
+      for (int i = 0; i < VEC; ++i) s = fma(p[it].v[i], x.p[it].v[i], s);
+    return s;
+  }
+};
+
+// acc += sum_e val[e] * X[col[e], :]   (unrolled so several gathers are in flight per group)
+template <typename T, int VEC, int GS, int NIT>
+__device__ __forceinline__ void gather_axpy(RowReg<T, VEC, GS, NIT>& acc, const T* __restrict__ X, int64_t ld,
+                                            const int* __restrict__ col, const T* __restrict__ val, int beg, int end,
+                                            int lane, int nvec, int r, int exact) {
+  using Row = RowReg<T, VEC, GS, NIT>;
+  constexpr int UN = (NIT == 1) ? 4 : 2;
+  int e = beg;
+  for (; e + UN <= end; e += UN) {
+    int cj[UN]; T vj[UN]; Row xn[UN];
+#pragma unroll
+    for (int u = 0; u < UN; ++u) { cj[u] = __ldg(col + e + u); vj[u] = __ldg(val + e + u); }
+#pragma unroll
+    for (int u = 0; u < UN; ++u) xn[u].load(X + (int64_t)cj[u] * ld, lane, nvec, r, exact);
+#pragma unroll
+    for (int u = 0; u < UN; ++u) acc.axpy(vj[u], xn[u]);
+  }
+  for (; e < end; ++e) {
+    Row xn; xn.load(X + (int64_t)__ldg(col + e) * ld, lane, nvec, r, exact);
+    acc.axpy(__ldg(val + e), xn);
+  }
+}
+
+template <typename T, int VEC, int GS, int NIT, int MODE>
+__global__ void __launch_bounds__(kBlock) k_rows(const RowArgs<T> a) {
+  using Row = RowReg<T, VEC, GS, NIT>;
+  constexpr int GPB = kBlock / GS;
+  constexpr int NST = (MODE == ROWS_LS_FUSED) ? 12 : 6;
+  const int lane = threadIdx.x % GS, grp = threadIdx.x / GS;
+  const unsigned gmask = group_mask<GS>();
+  const int nvec = a.nvec, r = a.r, exact = a.exact;
+  double st[NST];
+#pragma unroll
+  for (int s = 0; s < NST; ++s) st[s] = 0.0;
+
+  for (int64_t row = (int64_t)blockIdx.x * GPB + grp; row < a.n; row += (int64_t)gridDim.x * GPB) {
+    Row x; x.load(a.X + row * a.ld, lane, nvec, r, exact);
+    const int cb = __ldg(a.c_rowptr + row), ce = __ldg(a.c_rowptr + row + 1);
+    const T dc = __ldg(a.dC + row);
+
+    if (MODE == ROWS_LS_FUSED) {
+      Row d; d.load(a.X2 + row * a.ld, lane, nvec, r, exact);
+      const T rr_l = x.dot(x), rd_l = x.dot(d), dd_l = d.dot(d);
+      const double rr = group_sum<GS>((double)rr_l, gmask), rd = group_sum<GS>((double)rd_l, gmask),
+                   dd = group_sum<GS>((double)dd_l, gmask);
+      const int c = a.dcons ? __ldg(a.dcons + row) : (int)row;
+      if (c >= 0 && lane == 0) {
+        const double av = a.da ? (double)__ldg(a.da + row) : 1.0;
+        const double q = av * rr - __ldg(a.b + c), q1 = 2.0 * av * rd, q2 = av * dd, yv = __ldg(a.y + c);
+        st[LS_YQ] += yv * q; st[LS_YQ1] += yv * q1; st[LS_YQ2] += yv * q2;
+        st[LS_QQ] += q * q; st[LS_QQ1] += q * q1; st[LS_QQ2] += q * q2;
+        st[LS_Q11] += q1 * q1; st[LS_Q12] += q1 * q2; st[LS_Q22] += q2 * q2;
+      }
+      // <C, .> bilinear forms over the upper triangle (col > row), each off-diagonal pair once
+      T sRR = T(0), sRD = T(0), sDD = T(0);
+      for (int e = cb; e < ce; ++e) {
+        const int k = __ldg(a.c_col + e);
+        if (k > row) {
+          const T cv = __ldg(a.c_val + e);
+          Row xn, dn;
+          xn.load(a.X + (int64_t)k * a.ld, lane, nvec, r, exact);
+          dn.load(a.X2 + (int64_t)k * a.ld, lane, nvec, r, exact);
+          sRR = fma(cv, x.dot(xn), sRR);
+          sRD = fma(cv, x.dot(dn) + d.dot(xn), sRD);
+          sDD = fma(cv, d.dot(dn), sDD);
+        }
+      }
+      st[LS_CRR] += (double)dc * (double)rr_l + 2.0 * (double)sRR;
+      st[LS_CRD] += (double)dc * (double)rd_l + (double)sRD;
+      st[LS_CDD] += (double)dc * (double)dd_l + 2.0 * (double)sDD;
+    } else {
+      double coef = 0.0;  // weight of the row's own diagonal constraint times its coefficient
+      if (MODE == ROWS_FUSED_EVAL) {
+        const double nrm = group_sum<GS>((double)x.dot(x), gmask);
+        const int c = a.dcons ? __ldg(a.dcons + row) : (int)row;
+        if (c >= 0) {
+          const double av = a.da ? (double)__ldg(a.da + row) : 1.0;
+          const double z = av * nrm, q = z - __ldg(a.b + c), yv = __ldg(a.y + c), lam = yv - a.sigma * q;
+          coef = lam * av;
+          if (lane == 0) {
+            if (a.z) a.z[c] = z;
+            st[ES_YQ] += yv * q; st[ES_QQ] += q * q; st[ES_LZ] += lam * z;
+          }
+        }
+      }
+      // (C X)_row : diagonal + off-diagonal gathers
+      Row acc; acc.zero(); acc.axpy(dc, x);
+      gather_axpy<T, VEC, GS, NIT>(acc, a.X, a.ld, a.c_col, a.c_val, cb, ce, lane, nvec, r, exact);
+      st[ES_CX] += (double)acc.dot(x);
+      if (MODE == ROWS_ADJ) {
+        if (a.diag_class) {
+          const int c = a.dcons ? __ldg(a.dcons + row) : (int)row;
+          if (c >= 0) coef = __ldg(a.w + c) * (a.da ? (double)__ldg(a.da + row) : 1.0);
+        } else {
+          const int ab = __ldg(a.a_rowptr + row), ae = __ldg(a.a_rowptr + row + 1);
+          constexpr int UN = (NIT == 1) ? 4 : 2;
+          int e = ab;
+          for (; e + UN <= ae; e += UN) {
+            int cj[UN]; T wj[UN]; Row xn[UN];
+#pragma unroll
+            for (int u = 0; u < UN; ++u) {
+              cj[u] = __ldg(a.a_col + e + u);
+              wj[u] = (T)(-__ldg(a.w + __ldg(a.a_cons + e + u)) * (double)__ldg(a.a_val + e + u));
+            }
+#pragma unroll
+            for (int u = 0; u < UN; ++u) xn[u].load(a.X + (int64_t)cj[u] * a.ld, lane, nvec, r, exact);
+#pragma unroll
+            for (int u = 0; u < UN; ++u) acc.axpy(wj[u], xn[u]);
+          }
+          for (; e < ae; ++e) {
+            Row xn; xn.load(a.X + (int64_t)__ldg(a.a_col + e) * a.ld, lane, nvec, r, exact);
+            acc.axpy((T)(-__ldg(a.w + __ldg(a.a_cons + e)) * (double)__ldg(a.a_val + e)), xn);
+          }
+        }
+        for (int p = 0; p < a.pC; ++p) {  // low-rank cost term: + U[row,p] * s_p (U^T X)_p
+          const T up = __ldg(a.U + row * a.pC + p);
+#pragma unroll
+          for (int it = 0; it < NIT; ++it) {
+            const int vi = lane + it * GS;
+            if (vi < nvec) {
+#pragma unroll
+              for (int i = 0; i < VEC; ++i) {
+                const int cidx = vi * VEC + i;
+                if (cidx < r) acc.p[it].v[i] = fma(up, (T)__ldg(a.Ts + p * r + cidx), acc.p[it].v[i]);
+              }
+            }
+          }
+        }
+      }
+      acc.axpy((T)(-coef), x);
+      const T sc = (T)a.scale;
+#pragma unroll
+      for (int it = 0; it < NIT; ++it)
+#pragma unroll
+        for (int i = 0; i < VEC; ++i) acc.p[it].v[i] *= sc;
+      st[ES_GG] += (double)acc.dot(acc);
+      st[ES_GR] += (double)acc.dot(x);
+      if (a.Out) acc.store(a.Out + row * a.ld, lane, nvec, r, exact);
+    }
+  }
+  block_reduce_store<NST>(st, a.partials + (int64_t)blockIdx.x * kNStat);
+}
+
+// ---------------------------------------------------------------------------------------------
+// Forward (SDDMM-style) evaluator.  One entry e = (j, k, a), j <= k, contributes
+//   w a <X_j, X_k>                 with w = 1 (j == k) or 2 (j < k)            -> z
+//   w a (<X_j,D_k> + <D_j,X_k>)    (= <A, XD^T + DX^T> restricted to the entry)  -> q1
+//   w a <D_j, D_k>                                                               -> q2
+template <typename T, int VEC, int GS, int NIT, int MODE>
+__device__ __forceinline__ void cons_entry(const ConsArgs<T>& a, int64_t e, int lane, T& s0, T& s1, T& s2) {
+  using Row = RowReg<T, VEC, GS, NIT>;
+  const int j = __ldg(a.e_row + e), k = __ldg(a.e_col + e);
+  T av = __ldg(a.e_val + e);
+  Row xj, xk;
+  xj.load(a.X + (int64_t)j * a.ld, lane, a.nvec, a.r, a.exact);
+  if (j != k) { av += av; xk.load(a.X + (int64_t)k * a.ld, lane, a.nvec, a.r, a.exact); } else { xk = xj; }
+  s0 = fma(av, xj.dot(xk), s0);
+  if (MODE == CONS_LS) {
+    Row dj, dk;
+    dj.load(a.X2 + (int64_t)j * a.ld, lane, a.nvec, a.r, a.exact);
+    if (j != k) dk.load(a.X2 + (int64_t)k * a.ld, lane, a.nvec, a.r, a.exact); else dk = dj;
+    s1 = fma(av, xj.dot(dk) + dj.dot(xk), s1);
+    s2 = fma(av, dj.dot(dk), s2);
+  }
+}
+
+// per-constraint finalisation (a2): q = z - b, lambda = y - sigma q, scalar sums
+template <int MODE>
+__device__ __forceinline__ void cons_finish(double* st, int64_t i, double z, double q1, double q2,
+                                            const double* y, const double* b, double sigma, double* zout,
+                                            double* lam) {
+  const double q = z - __ldg(b + i), yv = __ldg(y + i);
+  if (MODE == CONS_EVAL) {
+    const double l = yv - sigma * q;
+    zout[i] = z; lam[i] = l;
+    st[ES_YQ] += yv * q; st[ES_QQ] += q * q; st[ES_LZ] += l * z;
+  } else {
+    st[LS_YQ] += yv * q; st[LS_YQ1] += yv * q1; st[LS_YQ2] += yv * q2;
+    st[LS_QQ] += q * q; st[LS_QQ1] += q * q1; st[LS_QQ2] += q * q2;
+    st[LS_Q11] += q1 * q1; st[LS_Q12] += q1 * q2; st[LS_Q22] += q2 * q2;
+  }
+}
+
+template <typename T, int VEC, int GS, int NIT, int MODE>
+__global__ void __launch_bounds__(kBlock) k_cons(const ConsArgs<T> a) {
+  constexpr int GPB = kBlock / GS;
+  constexpr int NST = (MODE == CONS_LS) ? 12 : 6;
+  const int lane = threadIdx.x % GS, grp = threadIdx.x / GS;
+  const unsigned gmask = group_mask<GS>();
+  double st[NST];
+#pragma unroll
+  for (int s = 0; s < NST; ++s) st[s] = 0.0;
+  for (int64_t i = (int64_t)blockIdx.x * GPB + grp; i < a.m; i += (int64_t)gridDim.x * GPB) {
+    const int64_t e0 = __ldg(a.ptr + i), e1 = __ldg(a.ptr + i + 1);
+    if (e1 - e0 > kLongThreshold) continue;  // long constraints: k_cons_chunk + k_long_finish
+    T s0 = T(0), s1 = T(0), s2 = T(0);
+    for (int64_t e = e0; e < e1; ++e) cons_entry<T, VEC, GS, NIT, MODE>(a, e, lane, s0, s1, s2);
+    const double z = group_sum<GS>((double)s0, gmask);
+    double q1 = 0.0, q2 = 0.0;
+    if (MODE == CONS_LS) { q1 = group_sum<GS>((double)s1, gmask); q2 = group_sum<GS>((double)s2, gmask); }
+    if (lane == 0) cons_finish<MODE>(st, i, z, q1, q2, a.y, a.b, a.sigma, a.z, a.lam);
+  }
+  block_reduce_store<NST>(st, a.partials + (int64_t)blockIdx.x * kNStat);
+}
+
+// one group per chunk of <= kChunk entries of a long constraint (or of C's sym-upper list)
+template <typename T, int VEC, int GS, int NIT, int MODE>
+__global__ void __launch_bounds__(kBlock) k_cons_chunk(const ConsArgs<T> a) {
+  constexpr int GPB = kBlock / GS;
+  const int lane = threadIdx.x % GS, grp = threadIdx.x / GS;
+  const unsigned gmask = group_mask<GS>();
+  for (int64_t c = (int64_t)blockIdx.x * GPB + grp; c < a.nchunk; c += (int64_t)gridDim.x * GPB) {
+    const int64_t e0 = __ldg(a.ch_beg + c), e1 = __ldg(a.ch_end + c);
+    T s0 = T(0), s1 = T(0), s2 = T(0);
+    for (int64_t e = e0; e < e1; ++e) cons_entry<T, VEC, GS, NIT, MODE>(a, e, lane, s0, s1, s2);
+    const double z = group_sum<GS>((double)s0, gmask);
+    double q1 = 0.0, q2 = 0.0;
+    if (MODE == CONS_LS) { q1 = group_sum<GS>((double)s1, gmask); q2 = group_sum<GS>((double)s2, gmask); }
+    if (lane == 0) { a.ch_out[3 * c] = z; a.ch_out[3 * c + 1] = q1; a.ch_out[3 * c + 2] = q2; }
+  }
+}
+
+// shapes (GS, NIT) by number of VEC-packs per row
+struct Shape { int gs, nit; };
+__host__ inline int shape_index(int nvec) {
+  if (nvec <= 1) return 0; if (nvec <= 2) return 1; if (nvec <= 4) return 2; if (nvec <= 8) return 3;
+  if (nvec <= 16) return 4; if (nvec <= 32) return 5; if (nvec <= 64) return 6; return -1;
+}
+constexpr Shape kShapes[7] = {{1, 1}, {2, 1}, {4, 1}, {8, 1}, {8, 2}, {16, 2}, {16, 4}};
+
+}  // namespace alora

@@ -1,0 +1,121 @@
+"""GPU parity: the CUDA path (through the C ABI) against the oracle, element by element, on the
+same seeded inputs.  Tolerances (BASELINE.json north_star; definitions in DESIGN.md reading 22):
+rel <= 1e-10 in fp64 and <= 2e-5 in fp32 on f, ||G||_F and z = A(RR^T); additionally on G itself,
+on p0..p4 (relative to sum |p_k|) and on S(mu)v."""
+import numpy as np
+import pytest
+
+from paper_2505_15775_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+
+TOL = {inputs.F64: 1e-10, inputs.F32: 2e-5}
+
+
+@pytest.fixture(scope="module")
+def torch():
+    import torch
+    assert torch.cuda.is_available(), "these tests need a CUDA device"
+    return torch
+
+
+@pytest.fixture(scope="module")
+def binding():
+    from paper_2505_15775_b200 import binding
+    return binding
+
+
+def tdtype(torch, w):
+    return torch.float32 if w.dtype == inputs.F32 else torch.float64
+
+
+def dev(torch, a, dt):
+    return torch.as_tensor(np.ascontiguousarray(a), dtype=dt).cuda()
+
+
+def rel(a, b):
+    return float(np.linalg.norm(np.asarray(a, float) - np.asarray(b, float)) / max(1e-300, np.linalg.norm(np.asarray(b, float))))
+
+
+def check_workload(torch, binding, oracle_mod, w, ld=None, label=""):
+    P, tol = w.problem, TOL[w.dtype]
+    o = oracle_mod.Oracle(P)
+    dt = tdtype(torch, w)
+    r = w.r
+    ld = ld or r
+    ctx = binding.Context(P, w.dtype)
+    Rh = np.zeros((P.n, ld)); Rh[:, :r] = w.R
+    Dh = np.zeros((P.n, ld)); Dh[:, :r] = w.D
+    if ld > r:  # pads hold garbage the kernels must ignore
+        Rh[:, r:] = 7.0; Dh[:, r:] = -3.0
+    R, D = dev(torch, Rh, dt), dev(torch, Dh, dt)
+    G = torch.full_like(R, 5.0)
+    y = dev(torch, w.y, torch.float64)
+    z = torch.zeros(P.m, dtype=torch.float64, device="cuda")
+    ctx.set_dual(y, w.sigma)
+    st = ctx.eval(R, r, ld, G, z)
+    torch.cuda.synchronize()
+    # oracle on the same (fp32-rounded) inputs, all arithmetic in double
+    parts = o.f(w.y, w.sigma, w.R, parts=True)
+    Go = o.grad(w.y, w.sigma, w.R)
+    zo = o.A_op(w.R)
+    fden = abs(parts["cx"]) + abs(parts["yq"]) + 0.5 * w.sigma * parts["qq"]
+    assert abs(st[0] - parts["f"]) <= tol * fden, (label, st[0], parts["f"])
+    assert abs(st[1] - parts["cx"]) <= tol * fden
+    assert rel(z.cpu().numpy(), zo) <= tol, label
+    Gg = G.cpu().numpy().astype(float)
+    assert rel(Gg[:, :r], Go) <= tol, label
+    assert abs(np.sqrt(st[4]) - np.linalg.norm(Go)) <= tol * np.linalg.norm(Go)
+    assert abs(st[5] - np.vdot(Go, w.R)) <= tol * (np.linalg.norm(Go) * np.linalg.norm(w.R))
+    if ld > r:
+        assert np.all(Gg[:, r:] == 5.0), "pad columns of G must not be touched"
+    # value-only call gives the same scalars
+    st2 = ctx.eval(R, r, ld, None, None)
+    assert st2[0] == st[0] and st2[3] == st[3]
+    # lambda
+    lam = torch.zeros(P.m, dtype=torch.float64, device="cuda")
+    ctx.eval(R, r, ld, G, z)
+    ctx.get_lambda(lam)
+    lamo, _ = o.lam(w.y, w.sigma, w.R)
+    torch.cuda.synchronize()
+    assert np.linalg.norm(lam.cpu().numpy() - lamo) <= tol * (np.linalg.norm(w.y) + w.sigma * np.linalg.norm(zo)), label
+    # line search
+    p = ctx.linesearch(R, D, r, ld)
+    po = o.linesearch(w.y, w.sigma, w.R, w.D)
+    assert np.abs(p - po).max() <= tol * np.abs(po).sum(), (label, p, po)
+    # matvec
+    mu = dev(torch, lamo, torch.float64)
+    V = dev(torch, w.V, dt)
+    W = torch.zeros_like(V)
+    vw = ctx.smatvec(mu, V, 1, W)
+    Wo = o.smatvec(lamo, w.V)
+    assert rel(W.cpu().numpy(), Wo) <= tol, label
+    assert abs(vw - w.V @ Wo) <= tol * np.linalg.norm(w.V) * np.linalg.norm(Wo)
+    # block matvec with p = 3 columns
+    V3h = np.stack([w.V, np.roll(w.V, 1), w.V ** 2], axis=1)
+    if w.dtype == inputs.F32:
+        V3h = V3h.astype(np.float32).astype(float)
+    V3 = dev(torch, V3h, dt); W3 = torch.zeros_like(V3)
+    ctx.smatvec(mu, V3, 3, W3, fetch=False)
+    torch.cuda.synchronize()
+    assert rel(W3.cpu().numpy(), o.smatvec(lamo, V3h)) <= tol, label
+    ctx.close()
+
+
+@pytest.mark.parametrize("idx", [0, 1, 2, 3, 4])
+def test_small_configs(torch, binding, oracle_mod, idx):
+    check_workload(torch, binding, oracle_mod, inputs.small(idx), label=f"small{idx}")
+
+
+@pytest.mark.parametrize("idx,ld", [(1, 20), (3, 12), (4, 11), (0, 41), (2, 26)])
+def test_padded_leading_dimension(torch, binding, oracle_mod, idx, ld):
+    """ld > r, including odd ld (element-wise path) and ld that allows wider vectors than r."""
+    check_workload(torch, binding, oracle_mod, inputs.small(idx), ld=ld, label=f"small{idx}/ld{ld}")
+
+
+@pytest.mark.parametrize("r", [1, 2, 3, 5, 7, 13, 33, 64])
+def test_ranks(torch, binding, oracle_mod, r):
+    """every (GS, NIT) shape and ragged tails, both classes and dtypes."""
+    for maker in (lambda: inputs.config1(side=23, r=r), lambda: inputs.config3(n=700, m=900, nnzC=2000, r=r),
+                  lambda: inputs.config2(n=300, M=900, r=r), lambda: inputs.config0(n=300, M=700, r=r)):
+        check_workload(torch, binding, oracle_mod, maker(), label=f"r{r}")
