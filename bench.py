@@ -1,0 +1,305 @@
+"""bench.py -- throughput of the ALM-BM hot path (BASELINE.json metric) on synthetic inputs.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 1]
+    python -m torch.distributed.run --nnodes=1 --nproc-per-node N --master-addr 127.0.0.1 \
+        --master-port P bench.py --gpus N --steps K --warmup W
+
+One "step" = one pass of the whole hot path at one point R:
+alora_eval (f + grad), alora_linesearch (quartic coefficients along D) and one alora_smatvec
+(Lanczos matvec S(lambda)v).  `value` = steps/s, i.e. f+grad evaluations/s with each evaluation
+accompanied by its line-search and matvec work, inputs resident in HBM.  Extra keys give the
+eval-only rate, the dominant kernel's roofline, the end-to-end rate through host buffers and the
+oracle timed on the host cores.  N > 1 runs N independent replicas (DESIGN.md "Multi-GPU":
+replicas only), one process per GPU, value = total steps of all ranks / max-over-ranks time.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from paper_2505_15775_b200 import inputs  # noqa: E402
+
+METRIC = "ALM-BM f+grad evals/sec (each step = f+grad, line-search coefficients, S(lambda)v matvec)"
+UNIT = "evals/s"
+
+
+def workload(idx: int):
+    return inputs.full(idx)
+
+
+def algorithmic_bytes(w, info) -> int:
+    """Minimum bytes of one f+grad evaluation, SURVEY.md 8(d) / DESIGN.md "Algorithmic bytes":
+    every array once (nonzeros + indices + R read + G write + y, b read + z write)."""
+    P = w.problem
+    s = 4 if w.dtype == inputs.F32 else 8
+    v = s
+    n, m, r = P.n, P.m, w.r
+    if info["cls"] == 0:
+        full = info["c_nnz"]  # 2|E|
+        return 4 * (n + 1) + (full + n) * (4 + v) + 2 * n * r * s + 24 * n
+    e_up, e_full, c_full = info["nf_A"], info["a_nnz"], info["c_nnz"]
+    fwd = e_up * (8 + v) + 8 * (m + 1) + n * r * s + 8 * m
+    wts = 24 * m
+    adj = e_full * (8 + v) + 4 * (n + 1) + (c_full + n) * (4 + v) + 4 * (n + 1) + 8 * m + 2 * n * r * s
+    return fwd + wts + adj
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled during the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu: int):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(gpu), f"--query-gpu={self.Q}",
+                                       "--format=csv,noheader,nounits", "-lms", "100"],
+                                      stdout=self.f, stderr=subprocess.DEVNULL)
+        except OSError:
+            self.p = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": []}
+        if self.p is None:
+            return out
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.p.kill()
+        self.f.flush(); self.f.seek(0)
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in self.f.read().splitlines():
+            parts = [x.strip() for x in line.split(",")]
+            if len(parts) < 6:
+                continue
+            try:
+                sm.append(float(parts[0])); mx.append(float(parts[1]))
+            except ValueError:
+                continue
+            for nm, val in zip(names, parts[2:6]):
+                if val.lower().startswith("active"):
+                    reasons.add(nm)
+        self.f.close()
+        os.unlink(self.f.name)
+        if sm:
+            out.update(sm_mhz=float(np.median(sm)), sm_max_mhz=float(max(mx)), reasons=sorted(reasons))
+        return out
+
+
+def oracle_step_seconds(w, reps_budget_s: float = 20.0):
+    """The oracle as it stands (single thread, fp64) on the same workload: one full step
+    (f, grad, line-search coefficients, one matvec).  Returns (seconds per step, steps timed)."""
+    from oracle.oracle import Oracle
+    o = Oracle(w.problem)
+    lam = None
+    t_all, k = 0.0, 0
+    while True:
+        t0 = time.perf_counter()
+        o.f(w.y, w.sigma, w.R)
+        o.grad(w.y, w.sigma, w.R)
+        o.linesearch(w.y, w.sigma, w.R, w.D)
+        if lam is None:
+            lam, _ = o.lam(w.y, w.sigma, w.R)
+        o.smatvec(lam, w.V)
+        t_all += time.perf_counter() - t0
+        k += 1
+        if t_all >= reps_budget_s or k >= 50:
+            break
+    return t_all / k, k
+
+
+def run_reference(args, w, rank, world):
+    """--impl reference: the oracle (kind: oracle, one host thread) timed on bounded work."""
+    if rank != 0:
+        return
+    from oracle.oracle import Oracle
+    o = Oracle(w.problem)
+    lam, _ = o.lam(w.y, w.sigma, w.R)
+
+    def step():
+        o.f(w.y, w.sigma, w.R); o.grad(w.y, w.sigma, w.R)
+        o.linesearch(w.y, w.sigma, w.R, w.D); o.smatvec(lam, w.V)
+
+    for _ in range(min(args.warmup, 1)):
+        step()
+    t0 = time.perf_counter()
+    k = 0
+    for _ in range(args.steps):
+        step(); k += 1
+        if time.perf_counter() - t0 > 150.0:   # keep the whole run within a few minutes
+            break
+    dt = time.perf_counter() - t0
+    val = k / dt
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": k,
+            "warmup": min(args.warmup, 1), "ms_per_step": 1e3 * dt / k, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": w.name, "n": w.problem.n, "m": w.problem.m, "r": w.r},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": 1, "kind": "oracle",
+                             "sample": f"{k} full steps (f, grad, line-search coefficients, matvec) of {w.name}"},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=1, help="BASELINE.json config index (default 1: torus MaxCut)")
+    ap.add_argument("--ld", type=int, default=0, help="leading dimension of R/G/D (default r)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    args = ap.parse_args()
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+
+    w = workload(args.config)
+    if args.impl == "reference":
+        run_reference(args, w, rank, world)
+        return
+
+    import torch
+    import torch.distributed as dist
+    from paper_2505_15775_b200 import binding
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (there is no CPU fallback)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    P = w.problem
+    r, ld = w.r, (args.ld or w.r)
+    tdt = torch.float32 if w.dtype == inputs.F32 else torch.float64
+    ndt = np.float32 if w.dtype == inputs.F32 else np.float64
+
+    def padded(a):
+        out = np.zeros((P.n, ld), ndt); out[:, :r] = a
+        return out
+
+    ctx = binding.Context(P, w.dtype, device=local)
+    info = ctx.info()
+    R, D = torch.from_numpy(padded(w.R)).cuda(), torch.from_numpy(padded(w.D)).cuda()
+    G = torch.empty_like(R)
+    y = torch.from_numpy(w.y).cuda()
+    z = torch.empty(P.m, dtype=torch.float64, device="cuda")
+    lam = torch.empty(P.m, dtype=torch.float64, device="cuda")
+    V = torch.from_numpy(w.V.astype(ndt)).cuda()
+    W = torch.empty_like(V)
+    ctx.set_dual(y, w.sigma)
+    ctx.eval(R, r, ld, G, z); ctx.get_lambda(lam)
+
+    def step():
+        ctx.eval(R, r, ld, G, z, stats=False)
+        ctx.linesearch(R, D, r, ld, fetch=False)
+        ctx.smatvec(lam, V, 1, W, fetch=False)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(3, args.warmup)):
+        step()
+    barrier()
+    sampler = ClockSampler(local) if rank == 0 else None
+    l0 = ctx.info()["launches"]
+    ctx.kernel_timing(True)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    e0.record()
+    for _ in range(args.steps):
+        step()
+    e1.record()
+    barrier()
+    ms = e0.elapsed_time(e1)
+    kern_ms, kern_n = ctx.kernel_timing_read()
+    ctx.kernel_timing(False)
+    launches = ctx.info()["launches"] - l0
+    clocks = sampler.stop() if sampler else None
+    t = torch.tensor([ms], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms = float(t.item())
+    value = world * args.steps / (ms * 1e-3)
+
+    # eval-only rate (the metric's bare "f+grad evals/s"), same hygiene
+    barrier(); e0.record()
+    for _ in range(args.steps):
+        ctx.eval(R, r, ld, G, z, stats=False)
+    e1.record(); barrier()
+    eval_only = args.steps / (e0.elapsed_time(e1) * 1e-3)
+    st = ctx.get_stats(); pls = ctx.get_linesearch()
+
+    # end to end through the C ABI with HOST buffers (pinned), copies inside the timed region
+    e2e = None
+    if not args.no_e2e:
+        Rh = torch.from_numpy(padded(w.R)).pin_memory()
+        Gh = torch.empty_like(Rh).pin_memory()
+        zh = torch.empty(P.m, dtype=torch.float64).pin_memory()
+        k2 = max(3, min(args.steps, 30))
+        for _ in range(3):
+            ctx.eval_host(Rh.numpy(), r, ld, Gh.numpy(), zh.numpy())
+        barrier(); e0.record()
+        for _ in range(k2):
+            ctx.eval_host(Rh.numpy(), r, ld, Gh.numpy(), zh.numpy())
+        e1.record(); barrier()
+        t2 = torch.tensor([e0.elapsed_time(e1)], dtype=torch.float64, device="cuda")
+        if world > 1:
+            dist.all_reduce(t2, op=dist.ReduceOp.MAX)
+        e2e = {"value": world * k2 / (float(t2.item()) * 1e-3), "unit": "evals/s (f+grad only, host R in, host G and z out)",
+               "h2d_bytes_per_step": int(Rh.numel() * Rh.element_size()),
+               "d2h_bytes_per_step": int(Gh.numel() * Gh.element_size() + zh.numel() * 8 + 64)}
+
+    if rank == 0:
+        peak, peak_src = peaks()
+        B = algorithmic_bytes(w, info)
+        kavg_ms = kern_ms / max(1, kern_n)
+        achieved = B / (kavg_ms * 1e-3) / 1e9 if kern_n else None
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                "warmup": max(3, args.warmup), "ms_per_step": ms / args.steps, "higher_is_better": True,
+                "scaling": "weak", "vs_baseline": None, "dtype": "f32" if w.dtype == inputs.F32 else "f64",
+                "data": "synthetic",
+                "config": {"workload": w.name, "n": P.n, "m": P.m, "edges": w.meta.get("edges"), "r": r, "ld": ld,
+                           "class": "diagonal (one fused pass)" if info["cls"] == 0 else "general (forward + adjoint)",
+                           "parallelism": f"replicas x{world}", "l2": "no flush: per-step working set > 126 MB L2"
+                           if B > 126e6 else "no flush: working set is L2-resident (latency-bound config)"},
+                "eval_only_per_s": eval_only,
+                "roofline": {"bound": "hbm", "kernel": "k_rows (fused f+grad pass)" if info["cls"] == 0 else "k_rows (adjoint pass)",
+                             "achieved": achieved, "peak": peak, "peak_source": peak_src, "unit": "GB/s",
+                             "frac": (achieved / peak) if achieved else None, "algorithmic_bytes": B,
+                             "kernel_ms": kavg_ms, "kernel_launches_timed": kern_n, "traffic": None},
+                "gpu_launches": int(launches), "clocks": clocks, "e2e": e2e,
+                "check": {"f": st[0], "gnorm": float(np.sqrt(st[4])), "p": [float(x) for x in pls]}}
+        if not args.no_cpu_baseline and world == 1:
+            sec, k = oracle_step_seconds(w)
+            line["cpu_baseline"] = {"value": 1.0 / sec, "unit": UNIT, "cores": 1, "kind": "oracle",
+                                    "sample": f"{k} full steps (f, grad, line-search coefficients, matvec) of {w.name}"}
+        print(json.dumps(line), flush=True)
+    ctx.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

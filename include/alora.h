@@ -122,6 +122,13 @@ alora_status alora_get_linesearch(alora_ctx *ctx, double p[5]);
 alora_status alora_smatvec(alora_ctx *ctx, const double *mu_dev, const void *V, int32_t p, void *W,
                            double *vw);
 
+/* Measurement hook (bench.py): when enabled, alora_eval brackets its dominant kernel (the fused
+ * row pass of the diagonal class, the adjoint pass of the general class) with CUDA events on the ctx
+ * stream; alora_kernel_timing_read synchronises, returns the summed kernel time and the number of
+ * launches timed since the last read (at most 8192 between reads), and resets. */
+alora_status alora_kernel_timing(alora_ctx *ctx, int enable);
+alora_status alora_kernel_timing_read(alora_ctx *ctx, double *total_ms, int64_t *count);
+
 /* Smallest Ritz pair of S(mu) by Lanczos with full re-orthogonalisation (reading 9):
  * start vector v0[i] = counter_uniform(seed, i), stops at step k when |beta_k s_k| <= tol_abs, on
  * breakdown, or at k = kmax (then returns ALORA_ENOTCONV with the best pair so far).

@@ -86,6 +86,8 @@ _lib.alora_eval_host.argtypes = [_vp, _vp, _i32, _i64, _vp, _vp, _vp]
 _lib.alora_linesearch.argtypes = [_vp, _vp, _vp, _i32, _i64, _vp]
 _lib.alora_get_linesearch.argtypes = [_vp, _vp]
 _lib.alora_smatvec.argtypes = [_vp, _vp, _vp, _i32, _vp, _vp]
+_lib.alora_kernel_timing.argtypes = [_vp, C.c_int]
+_lib.alora_kernel_timing_read.argtypes = [_vp, _vp, _vp]
 _lib.alora_lanczos.argtypes = [_vp, _vp, _i32, _dbl, C.c_uint64, _vp, _vp, _vp, _vp]
 _lib.alora_solve.argtypes = [_vp, C.POINTER(Params), _vp, _vp, _i32, _vp, _vp, _vp, _i32, _vp]
 
@@ -195,6 +197,14 @@ class Context:
         out = np.zeros(1) if fetch else None
         self._chk(_lib.alora_smatvec(self._h, _ptr(mu), _ptr(V), p, _ptr(W), _ptr(out)))
         return None if out is None else float(out[0])
+
+    def kernel_timing(self, enable: bool):
+        self._chk(_lib.alora_kernel_timing(self._h, int(enable)))
+
+    def kernel_timing_read(self):
+        ms, cnt = C.c_double(), C.c_int64()
+        self._chk(_lib.alora_kernel_timing_read(self._h, C.addressof(ms), C.addressof(cnt)))
+        return ms.value, cnt.value
 
     def lanczos(self, mu, kmax: int, tol_abs: float, seed: int, v=None):
         theta, resid, k = C.c_double(), C.c_double(), C.c_int32()

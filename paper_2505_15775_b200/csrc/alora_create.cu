@@ -281,6 +281,7 @@ extern "C" void alora_destroy(alora_ctx* c) {
   if (!c) return;
   cudaSetDevice(c->device);
   free_solve_workspace(c);
+  for (cudaEvent_t e : c->ev) cudaEventDestroy(e);
   c->pool.free_all();
   if (c->pinned) cudaFreeHost(c->pinned);
   if (c->pinR) cudaFreeHost(c->pinR);

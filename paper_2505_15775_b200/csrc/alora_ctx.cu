@@ -124,6 +124,18 @@ namespace {
 
 int vec_slot(int vec) { return vec == 1 ? 0 : vec == 2 ? 1 : 2; }
 
+// records an event on the ctx stream when kernel timing is on (pairs: before / after the dominant kernel)
+void time_mark(alora_ctx* c) {
+  if (!c->timing) return;
+  if (c->ev_used == c->ev.size()) {
+    if (c->ev.size() >= 16384) return;
+    cudaEvent_t e;
+    if (cudaEventCreate(&e) != cudaSuccess) return;
+    c->ev.push_back(e);
+  }
+  cudaEventRecord(c->ev[c->ev_used++], c->stream);
+}
+
 template <typename T> int grid_rows(alora_ctx* c, int vec, int shape, int mode, int64_t items) {
   int& occ = c->occ_cache[vec_slot(vec)][shape][mode];
   if (!occ) occ = std::max(1, occ_rows(T(), vec, shape, mode));
@@ -190,7 +202,9 @@ template <typename T> alora_status eval_impl(alora_ctx* c, const T* R, int32_t r
   if (c->cls == 0) {
     a.z = zout;
     const int grid = grid_rows<T>(c, g.vec, g.shape, ROWS_FUSED_EVAL, c->n);
+    time_mark(c);
     ALORA_CUDA(c, launch_rows(g.vec, g.shape, ROWS_FUSED_EVAL, a, grid, c->stream));
+    time_mark(c);
     k_finalize<<<1, kBlock, 0, c->stream>>>(c->part_rows, grid, nullptr, 0, nullptr, 0, c->stats_dev);
     c->launches += 2;
   } else {
@@ -214,7 +228,9 @@ template <typename T> alora_status eval_impl(alora_ctx* c, const T* R, int32_t r
     }
     a.w = c->lam; a.diag_class = 0;
     const int grid = grid_rows<T>(c, g.vec, g.shape, ROWS_ADJ, c->n);
+    time_mark(c);
     ALORA_CUDA(c, launch_rows(g.vec, g.shape, ROWS_ADJ, a, grid, c->stream));
+    time_mark(c);
     k_finalize<<<1, kBlock, 0, c->stream>>>(c->part_rows, grid, c->part_cons, gc, c->part_long, c->nlong_A, c->stats_dev);
     c->launches += 2;
   }
@@ -407,5 +423,23 @@ extern "C" alora_status alora_smatvec(alora_ctx* c, const double* mu_dev, const 
     ALORA_CUDA(c, cudaStreamSynchronize(c->stream));
     *vw = c->pinned[32 + ES_GR];
   }
+  return ALORA_OK;
+}
+
+extern "C" alora_status alora_kernel_timing(alora_ctx* c, int enable) {
+  if (!c) return ALORA_EINVAL;
+  c->timing = enable != 0; c->ev_used = 0;
+  return ALORA_OK;
+}
+
+extern "C" alora_status alora_kernel_timing_read(alora_ctx* c, double* total_ms, int64_t* count) {
+  if (!c || !total_ms || !count) return ALORA_EINVAL;
+  ALORA_CUDA(c, cudaStreamSynchronize(c->stream));
+  double tot = 0.0; int64_t k = 0;
+  for (size_t i = 0; i + 1 < c->ev_used; i += 2) {
+    float ms = 0.f;
+    if (cudaEventElapsedTime(&ms, c->ev[i], c->ev[i + 1]) == cudaSuccess) { tot += ms; ++k; }
+  }
+  *total_ms = tot; *count = k; c->ev_used = 0;
   return ALORA_OK;
 }

@@ -83,6 +83,8 @@ struct alora_ctx {
   // occupancy cache [vec idx][shape][kind]
   int occ_cache[3][7][8];
   alora::SolveWorkspace* ws = nullptr;
+  // optional CUDA-event timing of the dominant kernel of alora_eval (bench.py roofline)
+  bool timing = false; std::vector<cudaEvent_t> ev; size_t ev_used = 0;
 };
 
 namespace alora {
