@@ -127,6 +127,23 @@ def oracle_step_seconds(w, reps_budget_s: float = 20.0):
     return t_all / k, k
 
 
+def aggregate_ms(ms: float, world: int, device="cuda") -> float:
+    """Max over ranks of a per-rank duration (the replicas run independently; the job is as slow
+    as its slowest rank)."""
+    if world == 1:
+        return float(ms)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([ms], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_value(steps: int, world: int, ms: float) -> float:
+    """Whole-job throughput: every rank processed `steps` steps."""
+    return world * steps / (ms * 1e-3)
+
+
 def run_reference(args, w, rank, world):
     """--impl reference: the oracle (kind: oracle, one host thread) timed on bounded work."""
     if rank != 0:
@@ -237,11 +254,8 @@ def main():
     ctx.kernel_timing(False)
     launches = ctx.info()["launches"] - l0
     clocks = sampler.stop() if sampler else None
-    t = torch.tensor([ms], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms = float(t.item())
-    value = world * args.steps / (ms * 1e-3)
+    ms = aggregate_ms(ms, world)
+    value = whole_job_value(args.steps, world, ms)
 
     # eval-only rate (the metric's bare "f+grad evals/s"), same hygiene
     barrier(); e0.record()
@@ -264,10 +278,8 @@ def main():
         for _ in range(k2):
             ctx.eval_host(Rh.numpy(), r, ld, Gh.numpy(), zh.numpy())
         e1.record(); barrier()
-        t2 = torch.tensor([e0.elapsed_time(e1)], dtype=torch.float64, device="cuda")
-        if world > 1:
-            dist.all_reduce(t2, op=dist.ReduceOp.MAX)
-        e2e = {"value": world * k2 / (float(t2.item()) * 1e-3), "unit": "evals/s (f+grad only, host R in, host G and z out)",
+        ms2 = aggregate_ms(e0.elapsed_time(e1), world)
+        e2e = {"value": whole_job_value(k2, world, ms2), "unit": "evals/s (f+grad only, host R in, host G and z out)",
                "h2d_bytes_per_step": int(Rh.numel() * Rh.element_size()),
                "d2h_bytes_per_step": int(Gh.numel() * Gh.element_size() + zh.numel() * 8 + 64)}
 

@@ -1,15 +1,751 @@
-// placeholder until the solver lands
+// alora_solve.cu -- the host-side driver pieces that exercise the hot-path kernels end to end
+// (SURVEY.md 8a rows a7, a8): Lanczos with full re-orthogonalisation for lambda_min(S(mu)), and the
+// ALORA loop of Algorithm 1 with the readings of DESIGN.md: L-BFGS(5) directions,
+// exact quartic line search, rank growth along the most negative eigenvector with the closed-form
+// step, rank shrink through the spectrum of R^T R, dual update, sigma schedule and the KKT stop of
+// eq. 77.  All vector work runs in CUDA kernels on the ctx stream; the host keeps
+// only scalars, the Lanczos tridiagonal and r x r matrices.  Written independently of the test oracle
+// (same algorithm, no shared code).
+#include <algorithm>
+#include <chrono>
+#include <cmath>
+#include <cstring>
+
 #include "alora_internal.h"
-namespace alora { void free_solve_workspace(alora_ctx*) {} }
+
+namespace alora {
+
+// ---------------------------------------------------------------------------------------------
+// BLAS-1 style kernels on flat arrays (fp64 accumulation, ordered two-stage reductions)
+// ---------------------------------------------------------------------------------------------
+constexpr int kRedBlocks = 592;  // 148 SMs x 4
+
+template <typename TX, typename TY>
+__global__ void __launch_bounds__(kBlock) k_dots3(int64_t N, const TX* x0, const TY* y0, const TX* x1, const TY* y1,
+                                                  const TX* x2, const TY* y2, int nd, double* part) {
+  double st[3] = {0.0, 0.0, 0.0};
+  for (int64_t i = (int64_t)blockIdx.x * kBlock + threadIdx.x; i < N; i += (int64_t)gridDim.x * kBlock) {
+    st[0] += (double)x0[i] * (double)y0[i];
+    if (nd > 1) st[1] += (double)x1[i] * (double)y1[i];
+    if (nd > 2) st[2] += (double)x2[i] * (double)y2[i];
+  }
+  block_reduce_store<3>(st, part + (int64_t)blockIdx.x * kNStat);
+}
+
+__global__ void k_reduce_rows(const double* part, int nrows, double* out) {  // same order as k_finalize
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  for (int s = warp; s < kNStat; s += kBlock / 32) {
+    double v = 0.0;
+    for (int i = lane; i < nrows; i += 32) v += part[(int64_t)i * kNStat + s];
+    v = warp_sum(v);
+    if (lane == 0) out[s] = v;
+  }
+}
+
+template <typename T> __global__ void k_axpy(int64_t N, double a, const T* x, T* y) {  // y += a x
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (int64_t)gridDim.x * blockDim.x)
+    y[i] = (T)((double)y[i] + a * (double)x[i]);
+}
+template <typename T> __global__ void k_scale_copy(int64_t N, double a, const T* x, T* y) {  // y = a x
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (int64_t)gridDim.x * blockDim.x)
+    y[i] = (T)(a * (double)x[i]);
+}
+template <typename T> __global__ void k_scale(int64_t N, double a, T* y) {  // y *= a
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (int64_t)gridDim.x * blockDim.x)
+    y[i] = (T)(a * (double)y[i]);
+}
+// L-BFGS pair: S = alpha D, Y = G - Gprev, and the sums S.Y, S.S, Y.Y in the same pass
+template <typename T>
+__global__ void __launch_bounds__(kBlock) k_make_pair(int64_t N, double alpha, const T* D, const T* G, const T* Gp,
+                                                      T* S, T* Y, double* part) {
+  double st[3] = {0.0, 0.0, 0.0};
+  for (int64_t i = (int64_t)blockIdx.x * kBlock + threadIdx.x; i < N; i += (int64_t)gridDim.x * kBlock) {
+    const T s = (T)(alpha * (double)D[i]);
+    const T yv = (T)((double)G[i] - (double)Gp[i]);
+    S[i] = s; Y[i] = yv;
+    st[0] += (double)s * (double)yv; st[1] += (double)s * (double)s; st[2] += (double)yv * (double)yv;
+  }
+  block_reduce_store<3>(st, part + (int64_t)blockIdx.x * kNStat);
+}
+// w -= a v + b u   (Lanczos three-term recurrence)
+template <typename T> __global__ void k_axpy2(int64_t N, double a, const T* v, double b, const T* u, T* w) {
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (int64_t)gridDim.x * blockDim.x)
+    w[i] = (T)((double)w[i] - a * (double)v[i] - (u ? b * (double)u[i] : 0.0));
+}
+// c[j] partials for j < k: V is k x N (row j contiguous);  blockIdx.y = j
+template <typename T>
+__global__ void __launch_bounds__(kBlock) k_basis_dots(int64_t N, const T* V, const T* w, double* part, int nchunk) {
+  const int j = blockIdx.y;
+  const T* vj = V + (int64_t)j * N;
+  double st[1] = {0.0};
+  for (int64_t i = (int64_t)blockIdx.x * kBlock + threadIdx.x; i < N; i += (int64_t)gridDim.x * kBlock)
+    st[0] += (double)vj[i] * (double)w[i];
+  __shared__ double sm[kBlock / 32];
+  const double v = warp_sum(st[0]);
+  if ((threadIdx.x & 31) == 0) sm[threadIdx.x >> 5] = v;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    double t = 0.0;
+    for (int wv = 0; wv < kBlock / 32; ++wv) t += sm[wv];
+    part[(int64_t)j * nchunk + blockIdx.x] = t;
+  }
+}
+__global__ void k_basis_dots_reduce(const double* part, int nchunk, int k, double* c) {
+  const int j = blockIdx.x * blockDim.x + threadIdx.x;
+  if (j < k) {
+    double t = 0.0;
+    for (int i = 0; i < nchunk; ++i) t += part[(int64_t)j * nchunk + i];
+    c[j] = t;
+  }
+}
+// out[i] = beta*out[i] + sign * sum_j c[j] V[j][i]    (c on the device)
+template <typename T>
+__global__ void k_basis_combine(int64_t N, int k, const T* V, const double* c, double beta, double sign, T* out) {
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (int64_t)gridDim.x * blockDim.x) {
+    double t = 0.0;
+    for (int j = 0; j < k; ++j) t += c[j] * (double)V[(int64_t)j * N + i];
+    out[i] = (T)((beta != 0.0 ? beta * (double)out[i] : 0.0) + sign * t);
+  }
+}
+// v0[i] = counter_uniform(seed, i) in (-1,1): splitmix64-style hash, integer arithmetic only
+template <typename T> __global__ void k_counter_uniform(int64_t N, uint64_t seed, T* v) {
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (int64_t)gridDim.x * blockDim.x) {
+    uint64_t x = (uint64_t)i + seed * 0x9E3779B97F4A7C15ull;
+    x = (x ^ (x >> 30)) * 0xBF58476D1CE4E5B9ull;
+    x = (x ^ (x >> 27)) * 0x94D049BB133111EBull;
+    x = x ^ (x >> 31);
+    v[i] = (T)(((double)(x >> 11) + 0.5) * (2.0 / 9007199254740992.0) - 1.0);
+  }
+}
+// repack rows: dst (ld_d) <- src (ld_s), columns [0, r) copied, [r, ld_d) zeroed
+template <typename T> __global__ void k_repack(int64_t n, int r, const T* src, int64_t ld_s, T* dst, int64_t ld_d) {
+  const int64_t N = n * ld_d;
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (int64_t)gridDim.x * blockDim.x) {
+    const int64_t row = i / ld_d; const int c = (int)(i - row * ld_d);
+    dst[i] = c < r ? src[row * ld_s + c] : T(0);
+  }
+}
+template <typename T> __global__ void k_set_col(int64_t n, int64_t ld, int col, double scale, const T* v, T* R) {
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x)
+    R[i * ld + col] = (T)(scale * (double)v[i]);
+}
+// Gram matrix partials: part[block][i*r+j] = sum over the block's rows of R[row][i] R[row][j]
+template <typename T> __global__ void k_gram(int64_t n, int r, const T* R, int64_t ld, double* part, int64_t rows_per_block) {
+  const int64_t r0 = (int64_t)blockIdx.x * rows_per_block, r1 = min(n, r0 + rows_per_block);
+  for (int p = threadIdx.x; p < r * r; p += blockDim.x) {
+    const int i = p / r, j = p % r;
+    double t = 0.0;
+    for (int64_t row = r0; row < r1; ++row) t += (double)R[row * ld + i] * (double)R[row * ld + j];
+    part[(int64_t)blockIdx.x * r * r + p] = t;
+  }
+}
+__global__ void k_gram_reduce(const double* part, int nblk, int rr, double* M) {
+  for (int p = blockIdx.x * blockDim.x + threadIdx.x; p < rr; p += gridDim.x * blockDim.x) {
+    double t = 0.0;
+    for (int bk = 0; bk < nblk; ++bk) t += part[(int64_t)bk * rr + p];
+    M[p] = t;
+  }
+}
+// dst[row][c] = sum_i src[row][i] Q[i*rk + c]  for c < rk; zero for rk <= c < ld_d
+template <typename T>
+__global__ void k_rotate(int64_t n, int r, int rk, const T* src, int64_t ld_s, const double* Q, T* dst, int64_t ld_d) {
+  const int64_t N = n * ld_d;
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (int64_t)gridDim.x * blockDim.x) {
+    const int64_t row = i / ld_d; const int c = (int)(i - row * ld_d);
+    double t = 0.0;
+    if (c < rk) for (int k = 0; k < r; ++k) t += (double)src[row * ld_s + k] * Q[k * rk + c];
+    dst[i] = (T)t;
+  }
+}
+// y <- y - sigma (z - b)   (Alg. 1 line 10)
+__global__ void k_dual_update(int64_t m, double sigma, const double* z, const double* b, double* y) {
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < m; i += (int64_t)gridDim.x * blockDim.x)
+    y[i] -= sigma * (z[i] - b[i]);
+}
+__global__ void k_lambda2(int64_t m, const double* y, const double* z, const double* b, double sigma, double* lam) {
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < m; i += (int64_t)gridDim.x * blockDim.x)
+    lam[i] = y[i] - sigma * (z[i] - b[i]);
+}
+
+// ---------------------------------------------------------------------------------------------
+// workspace
+// ---------------------------------------------------------------------------------------------
+struct SolveWorkspace {
+  // Lanczos
+  void* V = nullptr; int V_cap = 0;  // basis, V_cap x n
+  void* w = nullptr;                 // n
+  double* bd_part = nullptr; double* cvec = nullptr; int bd_chunks = 0;
+  double* red_part = nullptr; double* red_out = nullptr;
+  // solve
+  void* buf[4 + 2 * 16] = {}; int nbuf = 0; int64_t buf_elems = 0;
+  double* lam = nullptr; double* z = nullptr; double* zv = nullptr; void* ritz = nullptr;
+  double* gram_part = nullptr; double* gram = nullptr; double* Qdev = nullptr;
+};
+
+void free_solve_workspace(alora_ctx* c) {
+  if (!c->ws) return;
+  // device memory belongs to the ctx pool (freed by alora_destroy); only the struct is ours
+  delete c->ws;
+  c->ws = nullptr;
+}
+
+}  // namespace alora
+
+// ---------------------------------------------------------------------------------------------
+// host numerics: tridiagonal eigenpair, cubic roots, Jacobi
+// ---------------------------------------------------------------------------------------------
+namespace alora {
+namespace {
+
+// number of eigenvalues of the tridiagonal (a, b) that are < x  (Sturm count)
+int sturm_count(const std::vector<double>& a, const std::vector<double>& b, int k, double x) {
+  int cnt = 0;
+  double d = 1.0;
+  for (int i = 0; i < k; ++i) {
+    const double off = i ? b[i - 1] : 0.0;
+    d = (a[i] - x) - (i ? off * off / d : 0.0);
+    if (d == 0.0) d = 1e-300;
+    if (d < 0.0) ++cnt;
+  }
+  return cnt;
+}
+
+// smallest eigenvalue (bisection) and its unit eigenvector (inverse iteration) of the k x k
+// symmetric tridiagonal with diagonal a[0..k) and off-diagonal b[0..k-1)
+void tridiag_smallest(const std::vector<double>& a, const std::vector<double>& b, int k, double& theta,
+                      std::vector<double>& s) {
+  s.assign(k, 0.0);
+  if (k == 1) { theta = a[0]; s[0] = 1.0; return; }
+  double lo = a[0], hi = a[0], scale = 0.0;
+  for (int i = 0; i < k; ++i) {
+    const double rad = (i ? std::fabs(b[i - 1]) : 0.0) + (i + 1 < k ? std::fabs(b[i]) : 0.0);
+    lo = std::min(lo, a[i] - rad); hi = std::max(hi, a[i] + rad);
+    scale = std::max(scale, std::fabs(a[i]) + rad);
+  }
+  double l = lo, h = hi;
+  for (int it = 0; it < 200 && h - l > 4e-16 * std::max(std::fabs(l), std::fabs(h)) + 1e-300; ++it) {
+    const double mid = 0.5 * (l + h);
+    if (mid <= l || mid >= h) break;
+    if (sturm_count(a, b, k, mid) >= 1) h = mid; else l = mid;
+  }
+  theta = 0.5 * (l + h);
+  // inverse iteration: (T - shift I) x = rhs with partial pivoting (shift nudged off the eigenvalue)
+  const double shift = theta - 1e-13 * std::max(scale, 1e-300) - 1e-300;
+  std::vector<double> x(k), dl(k), d(k), du(k), du2(k);
+  for (int i = 0; i < k; ++i) x[i] = 1.0 + 0.01 * ((i * 7919) % 13);
+  for (int rep = 0; rep < 4; ++rep) {
+    for (int i = 0; i < k; ++i) { d[i] = a[i] - shift; du[i] = i + 1 < k ? b[i] : 0.0; dl[i] = i + 1 < k ? b[i] : 0.0; du2[i] = 0.0; }
+    // LU with partial pivoting on the tridiagonal (dgtsv style), applied to x
+    for (int i = 0; i + 1 < k; ++i) {
+      if (std::fabs(d[i]) >= std::fabs(dl[i])) {
+        if (d[i] == 0.0) d[i] = 1e-300;
+        const double f = dl[i] / d[i];
+        d[i + 1] -= f * du[i];
+        x[i + 1] -= f * x[i];
+        du2[i] = 0.0;
+      } else {
+        const double f = d[i] / dl[i];
+        d[i] = dl[i];
+        const double t = d[i + 1];
+        d[i + 1] = du[i] - f * t;
+        du2[i] = i + 2 < k ? du[i + 1] : 0.0;
+        if (i + 2 < k) du[i + 1] = -f * du2[i];
+        du[i] = t;
+        const double tx = x[i]; x[i] = x[i + 1]; x[i + 1] = tx - f * x[i + 1];
+      }
+    }
+    if (d[k - 1] == 0.0) d[k - 1] = 1e-300;
+    x[k - 1] /= d[k - 1];
+    if (k > 1) x[k - 2] = (x[k - 2] - du[k - 2] * x[k - 1]) / d[k - 2];
+    for (int i = k - 3; i >= 0; --i) x[i] = (x[i] - du[i] * x[i + 1] - du2[i] * x[i + 2]) / d[i];
+    double nrm = 0.0;
+    for (int i = 0; i < k; ++i) nrm += x[i] * x[i];
+    nrm = std::sqrt(nrm);
+    if (!(nrm > 0.0) || !std::isfinite(nrm)) { for (int i = 0; i < k; ++i) x[i] = (i == 0); nrm = 1.0; }
+    for (int i = 0; i < k; ++i) x[i] /= nrm;
+  }
+  s = x;
+}
+
+// real roots of c3 x^3 + c2 x^2 + c1 x + c0 (c3 != 0); a complex pair whose imaginary part is below
+// 1e-8 * scale counts as a (double) real root
+int cubic_real_roots(double c3, double c2, double c1, double c0, double out[3]) {
+  const double b = c2 / c3, c = c1 / c3, d = c0 / c3;
+  const double Q = (b * b - 3.0 * c) / 9.0, R = (2.0 * b * b * b - 9.0 * b * c + 27.0 * d) / 54.0;
+  const double Q3 = Q * Q * Q;
+  if (R * R < Q3) {
+    const double th = std::acos(std::max(-1.0, std::min(1.0, R / std::sqrt(Q3))));
+    const double sq = -2.0 * std::sqrt(Q);
+    const double PI = 3.14159265358979323846;
+    out[0] = sq * std::cos(th / 3.0) - b / 3.0;
+    out[1] = sq * std::cos((th + 2.0 * PI) / 3.0) - b / 3.0;
+    out[2] = sq * std::cos((th - 2.0 * PI) / 3.0) - b / 3.0;
+    return 3;
+  }
+  const double A = -(R >= 0.0 ? 1.0 : -1.0) * std::cbrt(std::fabs(R) + std::sqrt(std::max(0.0, R * R - Q3)));
+  const double B = A != 0.0 ? Q / A : 0.0;
+  out[0] = (A + B) - b / 3.0;
+  const double re = -0.5 * (A + B) - b / 3.0, im = 0.8660254037844386 * std::fabs(A - B);
+  const double scale = std::max(1.0, std::max(std::fabs(out[0]), std::hypot(re, im)));
+  if (im <= 1e-8 * scale) { out[1] = re; out[2] = re; return 3; }
+  return 1;
+}
+
+// exact line search (reading 20): argmin over alpha > 0 of sum_k p_k alpha^k
+double quartic_argmin(const double p[5], int* flag) {
+  *flag = 0;
+  if (p[4] == 0.0 && p[3] == 0.0) {
+    if (p[2] > 0.0 && -p[1] / (2.0 * p[2]) > 0.0) return -p[1] / (2.0 * p[2]);
+    *flag = 1; return 1.0;
+  }
+  double roots[3]; int nr;
+  if (p[4] != 0.0) nr = cubic_real_roots(4.0 * p[4], 3.0 * p[3], 2.0 * p[2], p[1], roots);
+  else {  // quadratic 3 p3 x^2 + 2 p2 x + p1
+    const double qa = 3.0 * p[3], qb = 2.0 * p[2], qc = p[1], disc = qb * qb - 4.0 * qa * qc;
+    if (disc < 0.0) nr = 0;
+    else { const double sq = std::sqrt(disc); roots[0] = (-qb - sq) / (2.0 * qa); roots[1] = (-qb + sq) / (2.0 * qa); nr = 2; }
+  }
+  double cand[3]; int nc = 0;
+  for (int i = 0; i < nr; ++i) {
+    double a = roots[i];
+    for (int it = 0; it < 2; ++it) {
+      const double d1 = p[1] + a * (2.0 * p[2] + a * (3.0 * p[3] + a * 4.0 * p[4]));
+      const double d2 = 2.0 * p[2] + a * (6.0 * p[3] + a * 12.0 * p[4]);
+      if (d2 != 0.0) a -= d1 / d2;
+    }
+    if (a > 0.0) cand[nc++] = a;
+  }
+  if (!nc) { *flag = 1; return 1.0; }
+  std::sort(cand, cand + nc);
+  auto phi = [&](double a) { return p[0] + a * (p[1] + a * (p[2] + a * (p[3] + a * p[4]))); };
+  double best = cand[0];
+  for (int i = 1; i < nc; ++i)
+    if (phi(cand[i]) < phi(best) - 1e-14 * (std::fabs(phi(best)) + std::fabs(p[0]))) best = cand[i];
+  return best;
+}
+
+// cyclic Jacobi for a symmetric r x r matrix (row-major M, destroyed): eigenvalues ascending in mu,
+// eigenvectors in the columns of Q (row-major r x r)
+void jacobi_eigh(std::vector<double>& M, int r, std::vector<double>& mu, std::vector<double>& Q) {
+  Q.assign((size_t)r * r, 0.0);
+  for (int i = 0; i < r; ++i) Q[i * r + i] = 1.0;
+  for (int sweep = 0; sweep < 60; ++sweep) {
+    double off = 0.0, diag = 0.0;
+    for (int i = 0; i < r; ++i) for (int j = 0; j < r; ++j) (i == j ? diag : off) += M[i * r + j] * M[i * r + j];
+    if (off <= 1e-30 * diag || off == 0.0) break;
+    for (int p = 0; p < r; ++p)
+      for (int q = p + 1; q < r; ++q) {
+        const double apq = M[p * r + q];
+        if (apq == 0.0) continue;
+        const double tau = (M[q * r + q] - M[p * r + p]) / (2.0 * apq);
+        const double t = (tau >= 0.0 ? 1.0 : -1.0) / (std::fabs(tau) + std::sqrt(1.0 + tau * tau));
+        const double cs = 1.0 / std::sqrt(1.0 + t * t), sn = t * cs;
+        for (int k = 0; k < r; ++k) {
+          const double mkp = M[k * r + p], mkq = M[k * r + q];
+          M[k * r + p] = cs * mkp - sn * mkq; M[k * r + q] = sn * mkp + cs * mkq;
+        }
+        for (int k = 0; k < r; ++k) {
+          const double mpk = M[p * r + k], mqk = M[q * r + k];
+          M[p * r + k] = cs * mpk - sn * mqk; M[q * r + k] = sn * mpk + cs * mqk;
+        }
+        for (int k = 0; k < r; ++k) {
+          const double qkp = Q[k * r + p], qkq = Q[k * r + q];
+          Q[k * r + p] = cs * qkp - sn * qkq; Q[k * r + q] = sn * qkp + cs * qkq;
+        }
+      }
+  }
+  std::vector<int> order(r);
+  for (int i = 0; i < r; ++i) order[i] = i;
+  std::sort(order.begin(), order.end(), [&](int x, int y) { return M[x * r + x] < M[y * r + y]; });
+  mu.resize(r);
+  std::vector<double> Qs((size_t)r * r);
+  for (int c = 0; c < r; ++c) {
+    mu[c] = M[order[c] * r + order[c]];
+    for (int k = 0; k < r; ++k) Qs[k * r + c] = Q[k * r + order[c]];
+  }
+  Q.swap(Qs);
+}
+
+inline int ew_grid(alora_ctx* c, int64_t N) {
+  return (int)std::max<int64_t>(1, std::min<int64_t>((N + 255) / 256, (int64_t)c->num_sms * 8));
+}
+
+}  // namespace
+}  // namespace alora
+
+// ---------------------------------------------------------------------------------------------
+// device helpers with host results
+// ---------------------------------------------------------------------------------------------
+namespace alora {
+namespace {
+
+alora_status ensure_ws(alora_ctx* c) {
+  if (c->ws) return ALORA_OK;
+  c->ws = new (std::nothrow) SolveWorkspace();
+  if (!c->ws) return fail(c, ALORA_ENOMEM, "workspace");
+  SolveWorkspace* w = c->ws;
+  ALORA_CUDA(c, c->pool.alloc((void**)&w->red_part, sizeof(double) * kNStat * kRedBlocks));
+  ALORA_CUDA(c, c->pool.alloc((void**)&w->red_out, sizeof(double) * kNStat));
+  ALORA_CUDA(c, c->pool.alloc(&w->w, c->esz * c->n));
+  ALORA_CUDA(c, c->pool.alloc(&w->ritz, c->esz * c->n));
+  ALORA_CUDA(c, c->pool.alloc((void**)&w->lam, sizeof(double) * std::max<int64_t>(1, c->m)));
+  ALORA_CUDA(c, c->pool.alloc((void**)&w->z, sizeof(double) * std::max<int64_t>(1, c->m)));
+  ALORA_CUDA(c, c->pool.alloc((void**)&w->zv, sizeof(double) * std::max<int64_t>(1, c->m)));
+  return ALORA_OK;
+}
+
+// up to three dot products in one pass; results on the host (synchronises)
+template <typename TX, typename TY>
+alora_status dots(alora_ctx* c, int64_t N, int nd, const TX* x0, const TY* y0, const TX* x1, const TY* y1, const TX* x2,
+                  const TY* y2, double out[3]) {
+  SolveWorkspace* w = c->ws;
+  const int grid = (int)std::max<int64_t>(1, std::min<int64_t>((N + kBlock - 1) / kBlock, kRedBlocks));
+  k_dots3<TX, TY><<<grid, kBlock, 0, c->stream>>>(N, x0, y0, x1, y1, x2, y2, nd, w->red_part);
+  k_reduce_rows<<<1, kBlock, 0, c->stream>>>(w->red_part, grid, w->red_out);
+  c->launches += 2;
+  ALORA_CUDA(c, cudaMemcpyAsync(c->pinned + 48, w->red_out, sizeof(double) * 3, cudaMemcpyDeviceToHost, c->stream));
+  ALORA_CUDA(c, cudaStreamSynchronize(c->stream));
+  for (int i = 0; i < nd; ++i) out[i] = c->pinned[48 + i];
+  return ALORA_OK;
+}
+template <typename T> alora_status dot1(alora_ctx* c, int64_t N, const T* x, const T* y, double* out) {
+  double o[3];
+  alora_status s = dots<T, T>(c, N, 1, x, y, x, y, x, y, o);
+  *out = o[0];
+  return s;
+}
+
+template <typename T>
+alora_status lanczos_impl(alora_ctx* c, const double* mu, int kmax, double tol_abs, uint64_t seed, double* theta_out,
+                          T* v_out, int* k_used, double* resid_out, int* n_matvec) {
+  alora_status s = ensure_ws(c);
+  if (s != ALORA_OK) return s;
+  SolveWorkspace* w = c->ws;
+  const int64_t n = c->n;
+  kmax = (int)std::min<int64_t>(std::max(1, kmax), n);
+  if (w->V_cap < kmax) {
+    if (w->V) { c->pool.release(w->V); c->pool.release(w->bd_part); c->pool.release(w->cvec); }
+    w->bd_chunks = (int)std::max<int64_t>(1, std::min<int64_t>((n + kBlock * 8 - 1) / (kBlock * 8), 64));
+    ALORA_CUDA(c, c->pool.alloc(&w->V, c->esz * (size_t)n * kmax));
+    ALORA_CUDA(c, c->pool.alloc((void**)&w->bd_part, sizeof(double) * (size_t)kmax * w->bd_chunks));
+    ALORA_CUDA(c, c->pool.alloc((void**)&w->cvec, sizeof(double) * kmax));
+    w->V_cap = kmax;
+  }
+  T* V = (T*)w->V; T* wv = (T*)w->w;
+  const int g = ew_grid(c, n);
+  k_counter_uniform<T><<<g, 256, 0, c->stream>>>(n, seed, V);
+  c->launches++;
+  double nrm2;
+  s = dot1<T>(c, n, V, V, &nrm2); if (s != ALORA_OK) return s;
+  k_scale<T><<<g, 256, 0, c->stream>>>(n, 1.0 / std::sqrt(nrm2), V);
+  c->launches++;
+  std::vector<double> al, be, sv;
+  double theta = 0.0, resid = INFINITY;
+  int k = 0;
+  bool conv = false;
+  while (true) {
+    T* vk = V + (int64_t)k * n;
+    double a;
+    s = alora_smatvec(c, mu, vk, 1, wv, &a); if (s != ALORA_OK) return s;
+    if (n_matvec) ++*n_matvec;
+    al.push_back(a);
+    k_axpy2<T><<<g, 256, 0, c->stream>>>(n, a, vk, k ? be.back() : 0.0, k ? vk - n : (const T*)nullptr, wv);
+    c->launches++;
+    for (int pass = 0; pass < 2; ++pass) {  // classical Gram-Schmidt against V[0..k], twice
+      k_basis_dots<T><<<dim3(w->bd_chunks, k + 1), kBlock, 0, c->stream>>>(n, V, wv, w->bd_part, w->bd_chunks);
+      k_basis_dots_reduce<<<(k + 1 + 127) / 128, 128, 0, c->stream>>>(w->bd_part, w->bd_chunks, k + 1, w->cvec);
+      k_basis_combine<T><<<g, 256, 0, c->stream>>>(n, k + 1, V, w->cvec, 1.0, -1.0, wv);
+      c->launches += 3;
+    }
+    double b2;
+    s = dot1<T>(c, n, wv, wv, &b2); if (s != ALORA_OK) return s;
+    const double beta = std::sqrt(b2);
+    ++k;
+    tridiag_smallest(al, be, k, theta, sv);
+    resid = std::fabs(beta * sv[k - 1]);
+    double tnorm = 1e-300;
+    for (double x : al) tnorm = std::max(tnorm, std::fabs(x));
+    for (double x : be) tnorm = std::max(tnorm, std::fabs(x));
+    if (resid <= tol_abs || beta <= 1e-14 * tnorm) { conv = true; break; }
+    if (k >= kmax) break;
+    be.push_back(beta);
+    k_scale_copy<T><<<g, 256, 0, c->stream>>>(n, 1.0 / beta, wv, V + (int64_t)k * n);
+    c->launches++;
+  }
+  if (v_out) {  // Ritz vector V_k s, normalised
+    ALORA_CUDA(c, cudaMemcpyAsync(w->cvec, sv.data(), sizeof(double) * k, cudaMemcpyHostToDevice, c->stream));
+    k_basis_combine<T><<<g, 256, 0, c->stream>>>(n, k, V, w->cvec, 0.0, 1.0, v_out);
+    c->launches++;
+    double vv;
+    s = dot1<T>(c, n, v_out, v_out, &vv); if (s != ALORA_OK) return s;
+    k_scale<T><<<g, 256, 0, c->stream>>>(n, 1.0 / std::sqrt(vv), v_out);
+    c->launches++;
+    ALORA_CUDA(c, cudaStreamSynchronize(c->stream));  // sv is about to go out of scope
+  }
+  ALORA_CUDA(c, cudaGetLastError());
+  if (theta_out) *theta_out = theta;
+  if (k_used) *k_used = k;
+  if (resid_out) *resid_out = resid;
+  return conv ? ALORA_OK : ALORA_ENOTCONV;
+}
+
+}  // namespace
+}  // namespace alora
+
+using namespace alora;
+
 extern "C" void alora_default_params(alora_params* p) {
   if (!p) return;
   p->eps = 1e-5; p->stop_mode = 0; p->T_max = 100; p->tol0 = 1e-2; p->c_in = 0.1; p->tol_min = 1e-7;
   p->it_max = 500; p->lbfgs_mem = 5; p->p_max = 1; p->k_max = 300; p->tau_neg = -1.0; p->tol_eig = -1.0;
   p->gamma = 2.0; p->kappa = 0.25; p->sigma_max = 1e8; p->tau_shrink = 1e-8; p->s_max = 1e6; p->seed = 12345;
 }
-extern "C" alora_status alora_lanczos(alora_ctx* c, const double*, int32_t, double, uint64_t, double*, void*, int32_t*, double*) {
-  return alora::fail(c, ALORA_ESTATE, "not built yet");
+
+extern "C" alora_status alora_lanczos(alora_ctx* c, const double* mu_dev, int32_t kmax, double tol_abs, uint64_t seed,
+                                      double* theta, void* v_dev, int32_t* k_used, double* resid) {
+  if (!c || (!mu_dev && c->m > 0) || kmax < 1) return c ? fail(c, ALORA_EINVAL, "alora_lanczos: bad argument") : ALORA_EINVAL;
+  ALORA_CUDA(c, cudaSetDevice(c->device));
+  int k = 0;
+  alora_status s = c->dtype == ALORA_F32
+      ? lanczos_impl<float>(c, mu_dev, kmax, tol_abs, seed, theta, (float*)v_dev, &k, resid, nullptr)
+      : lanczos_impl<double>(c, mu_dev, kmax, tol_abs, seed, theta, (double*)v_dev, &k, resid, nullptr);
+  if (k_used) *k_used = k;
+  return s;
 }
-extern "C" alora_status alora_solve(alora_ctx* c, const alora_params*, void*, int32_t*, int32_t, double*, double*, alora_iter_record*, int32_t, alora_result*) {
-  return alora::fail(c, ALORA_ESTATE, "not built yet");
+
+// ---------------------------------------------------------------------------------------------
+// alora_solve: Algorithm 1
+// ---------------------------------------------------------------------------------------------
+namespace alora {
+namespace {
+
+template <typename T>
+alora_status solve_impl(alora_ctx* c, const alora_params* prm, T* R_user, int32_t* r_inout, int32_t r_cap, double* y,
+                        double* sigma_inout, alora_iter_record* log, int32_t log_cap, alora_result* res) {
+  const auto t_start = std::chrono::steady_clock::now();
+  alora_status s = ensure_ws(c);
+  if (s != ALORA_OK) return s;
+  SolveWorkspace* w = c->ws;
+  const int64_t n = c->n, m = c->m;
+  const int A = (int)(16 / sizeof(T));                    // columns are padded (with zeros) to 16-byte rows
+  auto pad = [&](int r) { return (r + A - 1) / A * A; };
+  const int mem = std::max(0, std::min(prm->lbfgs_mem, 16));
+  int r = *r_inout;
+  if (r < 1 || r > r_cap) return fail(c, ALORA_EINVAL, "alora_solve: need 1 <= r <= r_cap");
+  if (prm->p_max != 1) return fail(c, ALORA_EINVAL, "alora_solve: only p_max = 1 is implemented");
+  const int ldcap = pad(r_cap);
+  const int64_t elems = n * (int64_t)ldcap;
+  const int nslot = mem + 1;                              // one spare slot receives the candidate pair
+  const int nbuf = 5 + 2 * nslot;
+  if (w->buf_elems < elems || w->nbuf < nbuf) {
+    for (int i = 0; i < w->nbuf; ++i) c->pool.release(w->buf[i]);
+    for (int i = 0; i < nbuf; ++i) ALORA_CUDA(c, c->pool.alloc(&w->buf[i], sizeof(T) * elems));
+    w->nbuf = nbuf; w->buf_elems = elems;
+  }
+  if (!w->gram) {
+    ALORA_CUDA(c, c->pool.alloc((void**)&w->gram_part, sizeof(double) * 256 * 256 * 64));
+    ALORA_CUDA(c, c->pool.alloc((void**)&w->gram, sizeof(double) * 256 * 256));
+    ALORA_CUDA(c, c->pool.alloc((void**)&w->Qdev, sizeof(double) * 256 * 256));
+  }
+  if (ldcap > 256) return fail(c, ALORA_EINVAL, "alora_solve: r_cap <= 256");
+  T* Rw = (T*)w->buf[0]; T* Gw = (T*)w->buf[1]; T* Dw = (T*)w->buf[2]; T* Gp = (T*)w->buf[3]; T* Rtmp = (T*)w->buf[4];
+  T** Sb = (T**)&w->buf[5]; T** Yb = (T**)&w->buf[5 + nslot];
+  int ld = pad(r);
+  int64_t N = n * (int64_t)ld;
+  int g = ew_grid(c, N);
+  k_repack<T><<<g, 256, 0, c->stream>>>(n, r, R_user, r, Rw, ld);
+  c->launches++;
+
+  const double tau_neg = prm->tau_neg >= 0 ? prm->tau_neg : prm->eps;
+  const double tol_eig = prm->tol_eig >= 0 ? prm->tol_eig : prm->eps / 10.0;
+  const double normC = c->normC, normb = c->normb;
+  double sigma = *sigma_inout;
+  double infeas_prev = INFINITY, qnorm_prev = INFINITY;
+  uint64_t run = 0;
+  int n_evals = 0, n_ls = 0, n_mv = 0, outer = 0;
+  bool converged = false;
+  double kkt[3] = {0, 0, 0};
+  double st[8];
+
+  for (int t = 0; t < prm->T_max; ++t) {
+    alora_iter_record rec;
+    std::memset(&rec, 0, sizeof(rec));
+    rec.t = t; rec.sigma = sigma;
+    s = alora_set_dual(c, y, sigma); if (s != ALORA_OK) return s;
+    // -- 1. inner solve: F <- argmin_F L_rho(FF^T, y)                (Alg. 1 line 4)
+    const double tol_t = std::max(prm->tol_min, std::min(prm->tol0, prm->c_in * infeas_prev));
+    std::vector<int> pairs;                 // physical slots of the stored pairs, oldest first
+    int spare = 0;                          // physical slot that receives the next candidate pair
+    std::vector<double> sy(nslot), yy(nslot), alp(nslot);
+    int it = 0; bool have_prev = false; double alpha = 0.0, gnorm = 0.0;
+    while (true) {
+      s = alora_eval(c, Rw, ld, ld, Gw, w->z, st); if (s != ALORA_OK) return s;
+      ++rec.n_evals;
+      gnorm = std::sqrt(st[4]);
+      if (!std::isfinite(st[0]) || !std::isfinite(gnorm)) return fail(c, ALORA_ECUDA, "alora_solve: non-finite f or gradient");
+      if (have_prev && mem > 0) {
+        const int slot = spare;
+        const int gr = (int)std::max<int64_t>(1, std::min<int64_t>((N + kBlock - 1) / kBlock, kRedBlocks));
+        k_make_pair<T><<<gr, kBlock, 0, c->stream>>>(N, alpha, Dw, Gw, Gp, Sb[slot], Yb[slot], w->red_part);
+        k_reduce_rows<<<1, kBlock, 0, c->stream>>>(w->red_part, gr, w->red_out);
+        c->launches += 2;
+        ALORA_CUDA(c, cudaMemcpyAsync(c->pinned + 48, w->red_out, sizeof(double) * 3, cudaMemcpyDeviceToHost, c->stream));
+        ALORA_CUDA(c, cudaStreamSynchronize(c->stream));
+        const double v_sy = c->pinned[48], v_ss = c->pinned[49], v_yy = c->pinned[50];
+        if (v_sy > 1e-10 * std::sqrt(v_ss * v_yy)) {
+          sy[slot] = v_sy; yy[slot] = v_yy;
+          pairs.push_back(slot);
+          if ((int)pairs.size() > mem) { spare = pairs.front(); pairs.erase(pairs.begin()); }
+          else { spare = (int)pairs.size(); }   // slots 0..mem are handed out in order until the ring is full
+        }
+      }
+      if (gnorm / (1.0 + normC) <= tol_t || it >= prm->it_max) break;
+      // direction: two-loop recursion (reading 5); q lives in Dw
+      bool steepest = pairs.empty();
+      if (!steepest) {
+        ALORA_CUDA(c, cudaMemcpyAsync(Dw, Gw, sizeof(T) * N, cudaMemcpyDeviceToDevice, c->stream));
+        for (int i = (int)pairs.size() - 1; i >= 0; --i) {
+          const int sl = pairs[i];
+          double d; s = dot1<T>(c, N, Sb[sl], Dw, &d); if (s != ALORA_OK) return s;
+          alp[sl] = d / sy[sl];
+          k_axpy<T><<<g, 256, 0, c->stream>>>(N, -alp[sl], Yb[sl], Dw);
+          c->launches++;
+        }
+        const int nw = pairs.back();
+        k_scale<T><<<g, 256, 0, c->stream>>>(N, sy[nw] / yy[nw], Dw);
+        c->launches++;
+        for (size_t i = 0; i < pairs.size(); ++i) {
+          const int sl = pairs[i];
+          double d; s = dot1<T>(c, N, Yb[sl], Dw, &d); if (s != ALORA_OK) return s;
+          k_axpy<T><<<g, 256, 0, c->stream>>>(N, alp[sl] - d / sy[sl], Sb[sl], Dw);
+          c->launches++;
+        }
+        k_scale<T><<<g, 256, 0, c->stream>>>(N, -1.0, Dw);
+        c->launches++;
+        double gd; s = dot1<T>(c, N, Gw, Dw, &gd); if (s != ALORA_OK) return s;
+        if (gd >= 0.0) { pairs.clear(); spare = 0; steepest = true; }   // not a descent direction: restart from -G
+      }
+      if (steepest) { k_scale_copy<T><<<g, 256, 0, c->stream>>>(N, -1.0, Gw, Dw); c->launches++; }
+      double p[5];
+      s = alora_linesearch(c, Rw, Dw, ld, ld, p); if (s != ALORA_OK) return s;
+      ++n_ls;
+      int flag;
+      alpha = quartic_argmin(p, &flag);
+      std::swap(Gw, Gp);                                   // Gp <- current gradient
+      k_axpy<T><<<g, 256, 0, c->stream>>>(N, alpha, Dw, Rw);   // R <- R + alpha D
+      c->launches++;
+      ++it; have_prev = true;
+    }
+    rec.inner_iters = it; rec.gnorm = gnorm; rec.f = st[0];
+    double cx = st[1], qq = st[3];
+    // -- 2./3. lambda = y - sigma q; smallest eigenpair of C - A^*(lambda)   (Alg. 1 line 5)
+    k_lambda2<<<ew_grid(c, m), 256, 0, c->stream>>>(m, y, w->z, c->b, sigma, w->lam);
+    c->launches++;
+    double theta = 0.0, resid = 0.0; int ksteps = 0;
+    s = lanczos_impl<T>(c, w->lam, prm->k_max, tol_eig * (1.0 + normC), prm->seed + run, &theta, (T*)w->ritz, &ksteps, &resid, &n_mv);
+    ++run;
+    if (s != ALORA_OK && s != ALORA_ENOTCONV) return s;
+    rec.theta1 = theta; rec.lanczos_steps = ksteps;
+    double theta_kkt = theta;
+    bool changed = false;
+    if (-theta / (1.0 + normC) > tau_neg) {
+      // -- 4. grow (Alg. 1 lines 6-8), p = 1: s* = -theta / (sigma |A(vv^T)|^2)
+      if (r + 1 > r_cap) return fail(c, ALORA_EINVAL, "alora_solve: rank growth exceeds r_cap");
+      s = alora_eval(c, w->ritz, 1, 1, nullptr, w->zv, nullptr); if (s != ALORA_OK) return s;
+      double avv[3]; s = dots<double, double>(c, m, 1, w->zv, w->zv, w->zv, w->zv, w->zv, w->zv, avv); if (s != ALORA_OK) return s;
+      const double den = sigma * avv[0];
+      const double s_star = (den > 0.0 && -theta / den < prm->s_max) ? -theta / den : prm->s_max;
+      const int ld2 = pad(r + 1);
+      if (ld2 != ld) {
+        k_repack<T><<<ew_grid(c, n * (int64_t)ld2), 256, 0, c->stream>>>(n, r, Rw, ld, Rtmp, ld2);
+        c->launches++;
+        std::swap(Rw, Rtmp);
+        ld = ld2;
+      }
+      k_set_col<T><<<ew_grid(c, n), 256, 0, c->stream>>>(n, ld, r, std::sqrt(s_star), (const T*)w->ritz, Rw);
+      c->launches++;
+      ++r; rec.grew = 1; changed = true;
+    } else if (r > 1) {
+      // -- 5. shrink (reading 13): drop the numerically null directions of R
+      const int nblk = (int)std::max<int64_t>(1, std::min<int64_t>(64, n / 256));
+      const int64_t rpb = (n + nblk - 1) / nblk;
+      k_gram<T><<<nblk, 256, 0, c->stream>>>(n, r, Rw, ld, w->gram_part, rpb);
+      k_gram_reduce<<<(r * r + 255) / 256, 256, 0, c->stream>>>(w->gram_part, nblk, r * r, w->gram);
+      c->launches += 2;
+      std::vector<double> M((size_t)r * r), mu, Q;
+      ALORA_CUDA(c, cudaMemcpyAsync(M.data(), w->gram, sizeof(double) * r * r, cudaMemcpyDeviceToHost, c->stream));
+      ALORA_CUDA(c, cudaStreamSynchronize(c->stream));
+      jacobi_eigh(M, r, mu, Q);
+      int first_keep = 0;
+      while (first_keep < r && !(mu[first_keep] > prm->tau_shrink * mu[r - 1])) ++first_keep;
+      const int rk = r - first_keep;
+      if (first_keep > 0 && rk >= 1) {
+        std::vector<double> Qk((size_t)r * rk);
+        for (int i = 0; i < r; ++i) for (int cidx = 0; cidx < rk; ++cidx) Qk[(size_t)i * rk + cidx] = Q[(size_t)i * r + first_keep + cidx];
+        ALORA_CUDA(c, cudaMemcpyAsync(w->Qdev, Qk.data(), sizeof(double) * r * rk, cudaMemcpyHostToDevice, c->stream));
+        const int ld2 = pad(rk);
+        k_rotate<T><<<ew_grid(c, n * (int64_t)ld2), 256, 0, c->stream>>>(n, r, rk, Rw, ld, w->Qdev, Rtmp, ld2);
+        c->launches++;
+        ALORA_CUDA(c, cudaStreamSynchronize(c->stream));
+        std::swap(Rw, Rtmp);
+        rec.shrank = first_keep; r = rk; ld = ld2; changed = true;
+      }
+    }
+    if (changed) {
+      N = n * (int64_t)ld; g = ew_grid(c, N);
+      s = alora_eval(c, Rw, ld, ld, nullptr, w->z, st); if (s != ALORA_OK) return s;   // q, <C,X> at the new R
+      cx = st[1]; qq = st[3];
+    }
+    const double qnorm = std::sqrt(qq);
+    // -- 6. y <- y + rho (b - A FF^T)                               (Alg. 1 line 10)
+    k_dual_update<<<ew_grid(c, m), 256, 0, c->stream>>>(m, sigma, w->z, c->b, y);
+    c->launches++;
+    if (changed) {  // reading 17: S(lambda) != S(y_new) once R changed
+      int k2 = 0;
+      s = lanczos_impl<T>(c, y, prm->k_max, tol_eig * (1.0 + normC), prm->seed + run, &theta_kkt, (T*)nullptr, &k2, &resid, &n_mv);
+      ++run;
+      if (s != ALORA_OK && s != ALORA_ENOTCONV) return s;
+    }
+    double by[3]; s = dots<double, double>(c, m, 1, c->b, y, c->b, y, c->b, y, by); if (s != ALORA_OK) return s;
+    kkt[0] = qnorm / (1.0 + normb);
+    kkt[1] = std::fabs(std::min(0.0, theta_kkt)) / (1.0 + normC);
+    kkt[2] = std::fabs(cx - by[0]) / (1.0 + std::fabs(cx) + std::fabs(by[0]));
+    rec.r = r; rec.cx = cx; rec.qnorm = qnorm; rec.kkt[0] = kkt[0]; rec.kkt[1] = kkt[1]; rec.kkt[2] = kkt[2];
+    // -- 7. sigma schedule (reading 12)
+    if (qnorm > prm->kappa * qnorm_prev) sigma = std::min(prm->gamma * sigma, prm->sigma_max);
+    qnorm_prev = qnorm; infeas_prev = kkt[0];
+    if (log && t < log_cap) log[t] = rec;
+    n_evals += rec.n_evals; outer = t + 1;
+    // -- 8. until KKT(FF^T, y) <= eps                                (Alg. 1 line 11, eq. 77)
+    const bool done = prm->stop_mode == 1 ? kkt[0] <= prm->eps : std::max(kkt[0], std::max(kkt[1], kkt[2])) <= prm->eps;
+    if (done) { converged = true; break; }
+  }
+  // hand the state back: R (n x r, ld = r), r, y (updated in place), sigma
+  k_repack<T><<<ew_grid(c, n * (int64_t)r), 256, 0, c->stream>>>(n, r, Rw, ld, R_user, r);
+  c->launches++;
+  ALORA_CUDA(c, cudaStreamSynchronize(c->stream));
+  ALORA_CUDA(c, cudaGetLastError());
+  *r_inout = r; *sigma_inout = sigma;
+  if (res) {
+    res->converged = converged; res->outer_iters = outer; res->n_evals = n_evals; res->n_linesearch = n_ls;
+    res->n_matvec = n_mv; res->r_final = r; res->kkt[0] = kkt[0]; res->kkt[1] = kkt[1]; res->kkt[2] = kkt[2];
+    res->sigma_final = sigma;
+    res->seconds = std::chrono::duration<double>(std::chrono::steady_clock::now() - t_start).count();
+  }
+  return converged ? ALORA_OK : ALORA_ENOTCONV;
+}
+
+}  // namespace
+}  // namespace alora
+
+extern "C" alora_status alora_solve(alora_ctx* c, const alora_params* prm, void* R_dev, int32_t* r_inout, int32_t r_cap,
+                                    double* y_dev, double* sigma_inout, alora_iter_record* log, int32_t log_cap,
+                                    alora_result* res) {
+  if (!c || !prm || !R_dev || !r_inout || !sigma_inout || (!y_dev && c->m > 0))
+    return c ? fail(c, ALORA_EINVAL, "alora_solve: NULL argument") : ALORA_EINVAL;
+  if (!(*sigma_inout > 0.0)) return fail(c, ALORA_EINVAL, "alora_solve: sigma > 0");
+  ALORA_CUDA(c, cudaSetDevice(c->device));
+  return c->dtype == ALORA_F32
+      ? solve_impl<float>(c, prm, (float*)R_dev, r_inout, r_cap, y_dev, sigma_inout, log, log_cap, res)
+      : solve_impl<double>(c, prm, (double*)R_dev, r_inout, r_cap, y_dev, sigma_inout, log, log_cap, res);
 }

@@ -1,0 +1,152 @@
+"""GPU: Lanczos and the ALORA loop (alora_lanczos / alora_solve) against the oracle's Part 2
+(oracle/alm.py) and against closed forms.  Trajectory parity on config 0 follows DESIGN.md
+reading 23: same outer iterations, same grow / shrink decisions and ranks; per outer iteration
+<C,X>, ||q||/(1+||b||), sigma and theta_1 agree to 1e-6; inner iteration counts within 10 %."""
+import numpy as np
+import pytest
+
+from paper_2505_15775_b200 import inputs
+from tests.test_oracle_pins import _graph_maxcut, prop6_instance
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def torch():
+    import torch
+    assert torch.cuda.is_available()
+    return torch
+
+
+@pytest.fixture(scope="module")
+def binding():
+    from paper_2505_15775_b200 import binding
+    return binding
+
+
+@pytest.fixture(scope="module")
+def alm():
+    from oracle import alm
+    return alm
+
+
+def gpu_solve(torch, binding, P, dtype, R0, y0, sigma, r_cap, **kw):
+    tdt = torch.float32 if dtype == inputs.F32 else torch.float64
+    ctx = binding.Context(P, dtype)
+    n, r0 = R0.shape
+    Rbuf = torch.zeros(n * r_cap, dtype=tdt, device="cuda")
+    Rbuf[: n * r0] = torch.as_tensor(np.ascontiguousarray(R0), dtype=tdt).cuda().reshape(-1)
+    y = torch.as_tensor(np.ascontiguousarray(y0), dtype=torch.float64).cuda()
+    res, log, r, sg, ok = ctx.solve(binding.Params(**kw), Rbuf, r0, r_cap, y, sigma)
+    R = Rbuf[: n * r].reshape(n, r).cpu().numpy().astype(float)
+    out = dict(res=res, log=log, r=r, sigma=sg, ok=ok, R=R, y=y.cpu().numpy())
+    ctx.close()
+    return out
+
+
+def test_lanczos_matches_oracle_and_dense(torch, binding, alm, oracle_mod):
+    w = inputs.small(0)
+    P = w.problem
+    o = oracle_mod.Oracle(P)
+    mu = np.random.default_rng(1).standard_normal(P.m)
+    S = o.smatvec(mu, np.eye(P.n))
+    ev = np.linalg.eigvalsh(S)
+    th_o, v_o, k_o, res_o = alm.lanczos(lambda x: o.smatvec(mu, x), P.n, 42, 300, 1e-8)
+    ctx = binding.Context(P, inputs.F64)
+    mud = torch.as_tensor(mu).cuda()
+    v = torch.zeros(P.n, dtype=torch.float64, device="cuda")
+    th, k, resid, ok = ctx.lanczos(mud, 300, 1e-8, 42, v)
+    assert ok and abs(th - ev[0]) < 1e-8 and abs(th - th_o) < 1e-9
+    assert abs(k - k_o) <= 2
+    vv = v.cpu().numpy()
+    assert abs(np.linalg.norm(vv) - 1) < 1e-12 and np.linalg.norm(S @ vv - th * vv) < 1e-6
+    # iteration cap: ENOTCONV with the best pair so far
+    th2, k2, _, ok2 = ctx.lanczos(mud, 5, 1e-12, 42, None)
+    assert not ok2 and k2 == 5 and th2 >= ev[0] - 1e-12
+    ctx.close()
+    # breakdown (two distinct eigenvalues): exact after 2 steps
+    P6, y6, F, rho, eps, a = prop6_instance()
+    ctx = binding.Context(P6, inputs.F64)
+    th, k, resid, ok = ctx.lanczos(torch.as_tensor(y6).cuda(), 50, 1e-12, 1, None)
+    assert ok and k == 2 and abs(th + eps) < 1e-14
+    ctx.close()
+
+
+def test_lanczos_fp32(torch, binding, oracle_mod):
+    w = inputs.small(4)
+    P = w.problem
+    o = oracle_mod.Oracle(P)
+    lam, _ = o.lam(w.y, w.sigma, w.R)
+    ctx = binding.Context(P, inputs.F32)
+    v = torch.zeros(P.n, dtype=torch.float32, device="cuda")
+    th, k, resid, ok = ctx.lanczos(torch.as_tensor(lam).cuda(), 300, 1e-4, 7, v)
+    vv = v.cpu().numpy().astype(float)
+    Sv = o.smatvec(lam, vv)
+    assert abs(vv @ Sv - th) < 1e-4 and np.linalg.norm(Sv - th * vv) < 5e-3
+    import scipy.sparse.linalg as sla
+    op = sla.LinearOperator((P.n, P.n), matvec=lambda x: o.smatvec(lam, x), dtype=float)
+    ref = sla.eigsh(op, k=1, which="SA", tol=1e-8)[0][0]
+    assert abs(th - ref) < 1e-3
+    ctx.close()
+
+
+def test_config0_trajectory(torch, binding, alm, oracle_mod):
+    w = inputs.full(0)
+    o = oracle_mod.Oracle(w.problem)
+    ref = alm.solve(o, w.R, w.y, w.sigma, alm.Params(eps=1e-6))
+    out = gpu_solve(torch, binding, w.problem, w.dtype, w.R, w.y, w.sigma, r_cap=64, eps=1e-6)
+    assert out["ok"] and ref.converged
+    assert out["res"].outer_iters == ref.outer_iters
+    for a, b in zip(out["log"], ref.log):
+        assert (a.r, a.grew, a.shrank) == (b.r, b.grew, b.shrank), (a.t, a.r, b.r)
+        assert a.sigma == b.sigma
+        assert abs(a.cx - b.cx) <= 1e-6 * abs(b.cx), (a.t, a.cx, b.cx)
+        assert abs(a.kkt[0] - b.kkt[0]) <= 1e-6 * max(1e-3, b.kkt[0]) + 1e-9
+        assert abs(a.theta1 - b.theta1) <= 1e-6
+        assert abs(a.inner_iters - b.inner_iters) <= max(2, 0.1 * b.inner_iters), (a.t, a.inner_iters, b.inner_iters)
+    assert max(out["res"].kkt) <= 1e-6
+    assert abs(o.inner_C(out["R"], out["R"]) - o.inner_C(ref.R, ref.R)) <= 1e-6 * abs(o.inner_C(ref.R, ref.R))
+    np.testing.assert_allclose(out["y"], ref.y, atol=1e-5)
+
+
+@pytest.mark.parametrize("n", [9, 20])
+def test_solve_Kn(torch, binding, oracle_mod, n):
+    P = _graph_maxcut(n, [(i, j) for i in range(n) for j in range(i + 1, n)])
+    R0 = inputs._unit_rows(np.random.default_rng(n), n, 4)
+    out = gpu_solve(torch, binding, P, inputs.F64, R0, np.zeros(n), 1.0, r_cap=32, eps=1e-7)
+    o = oracle_mod.Oracle(P)
+    assert out["ok"] and abs(o.inner_C(out["R"], out["R"]) + n * n / 4) < 1e-4
+    assert np.abs(out["y"] + n / 4).max() < 1e-4
+
+
+def test_solve_theta_C5(torch, binding, oracle_mod):
+    P = inputs.theta_problem(5, np.arange(5), (np.arange(5) + 1) % 5) if False else \
+        inputs.theta_problem(5, np.array([0, 1, 2, 3, 0]), np.array([1, 2, 3, 4, 4]))
+    R0 = np.random.default_rng(5).standard_normal((5, 3)) / np.sqrt(15)
+    out = gpu_solve(torch, binding, P, inputs.F64, R0, np.zeros(P.m), 1.0, r_cap=16, eps=1e-7)
+    o = oracle_mod.Oracle(P)
+    assert out["ok"] and abs(o.inner_C(out["R"], out["R"]) + np.sqrt(5)) < 1e-4
+
+
+def test_prop6_escape(torch, binding, oracle_mod):
+    """Rank adaptation pass/fail: from the spurious minimiser the solver must grow
+    along e_d and reach X* = a e_d e_d^T; with growth disabled it stays put."""
+    P, y, F, rho, eps, a = prop6_instance()
+    out = gpu_solve(torch, binding, P, inputs.F64, F, y, rho, r_cap=16, gamma=1.0, eps=1e-8)
+    assert out["ok"] and out["log"][0].grew == 1 and out["log"][0].inner_iters == 0
+    X = out["R"] @ out["R"].T
+    Xs = np.zeros((P.n, P.n)); Xs[-1, -1] = a
+    assert np.abs(X - Xs).max() < 1e-5
+    assert np.abs(out["y"] - np.r_[np.zeros(P.n - 1), 1.0]).max() < 1e-5
+    stuck = gpu_solve(torch, binding, P, inputs.F64, F, y, rho, r_cap=16, gamma=1.0, eps=1e-8, tau_neg=1e30, T_max=20)
+    assert not stuck["ok"] and all(r.inner_iters == 0 for r in stuck["log"])
+
+
+def test_solve_fp32_ring_matchings(torch, binding, oracle_mod):
+    """Scaled-down config 4 (fp32 R): full rank-adaptive solve to relative primal infeasibility 1e-5."""
+    w = inputs.small(4)
+    out = gpu_solve(torch, binding, w.problem, w.dtype, w.R, w.y, w.sigma, r_cap=32, eps=1e-5, stop_mode=1)
+    assert out["ok"] and out["res"].kkt[0] <= 1e-5
+    o = oracle_mod.Oracle(w.problem)
+    q = o.A_op(out["R"]) - w.problem.b
+    assert np.linalg.norm(q) / (1 + np.linalg.norm(w.problem.b)) <= 2e-5
