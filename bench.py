@@ -176,6 +176,34 @@ def run_reference(args, w, rank, world):
     print(json.dumps(line), flush=True)
 
 
+def run_solve(args, w, local, torch, binding):
+    """ALM solve time (BASELINE.json metric, third part): alora_solve from a resident problem.
+    Config 0 stops at KKT <= 1e-6, config 4 at relative primal infeasibility <= 1e-5."""
+    P, r0 = w.problem, w.r
+    t0 = time.perf_counter()
+    ctx = binding.Context(P, w.dtype, device=local)
+    t_create = time.perf_counter() - t0
+    tdt = torch.float32 if w.dtype == inputs.F32 else torch.float64
+    r_cap = args.r_cap or (64 if P.n <= 100000 else r0 + 14)
+    Rbuf = torch.zeros(P.n * r_cap, dtype=tdt, device="cuda")
+    Rbuf[: P.n * r0] = torch.as_tensor(w.R, dtype=tdt).cuda().reshape(-1)
+    y = torch.as_tensor(w.y, dtype=torch.float64).cuda()
+    kw = dict(eps=1e-6, stop_mode=0) if P.n <= 1000 else dict(eps=1e-5, stop_mode=1)
+    l0 = ctx.info()["launches"]
+    torch.cuda.synchronize()
+    res, log, r, sg, ok = ctx.solve(binding.Params(**kw), Rbuf, r0, r_cap, y, w.sigma)
+    line = {"mode": "solve", "metric": "ALM solve time", "value": res.seconds, "unit": "s", "higher_is_better": False,
+            "config": {"workload": w.name, "n": P.n, "m": P.m, "r0": r0, "r_cap": r_cap, "stop": kw},
+            "converged": bool(ok), "outer_iters": res.outer_iters, "n_evals": res.n_evals,
+            "n_linesearch": res.n_linesearch, "n_matvec": res.n_matvec, "r_final": r, "sigma_final": sg,
+            "kkt": list(res.kkt), "create_seconds": t_create, "gpu_launches": ctx.info()["launches"] - l0,
+            "dtype": "f32" if w.dtype == inputs.F32 else "f64", "data": "synthetic",
+            "log": [dict(t=a.t, r=a.r, sigma=a.sigma, cx=a.cx, qnorm=a.qnorm, theta1=a.theta1, inner=a.inner_iters,
+                         lanczos=a.lanczos_steps, grew=a.grew, shrank=a.shrank, kkt=list(a.kkt)) for a in log]}
+    print(json.dumps(line), flush=True)
+    ctx.close()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -184,6 +212,9 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=1, help="BASELINE.json config index (default 1: torus MaxCut)")
     ap.add_argument("--ld", type=int, default=0, help="leading dimension of R/G/D (default r)")
+    ap.add_argument("--mode", default="path", choices=["path", "solve"],
+                    help="path: the hot-path step (default, the bench contract); solve: ALM solve time of the config")
+    ap.add_argument("--r-cap", type=int, default=0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
@@ -214,6 +245,9 @@ def main():
         out = np.zeros((P.n, ld), ndt); out[:, :r] = a
         return out
 
+    if args.mode == "solve":
+        run_solve(args, w, local, torch, binding)
+        return
     ctx = binding.Context(P, w.dtype, device=local)
     info = ctx.info()
     R, D = torch.from_numpy(padded(w.R)).cuda(), torch.from_numpy(padded(w.D)).cuda()

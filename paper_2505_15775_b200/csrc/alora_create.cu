@@ -17,10 +17,13 @@
 namespace alora {
 namespace {
 
+// every array gets 8 zeroed elements of slack: the bulk copies of rows_tiled.cuh read whole 16-byte
+// units and may run up to 3 elements past the logical end
 template <typename T> cudaError_t upload(alora_ctx* c, void** dst, const std::vector<T>& v) {
-  cudaError_t e = c->pool.alloc(dst, v.size() * sizeof(T));
+  cudaError_t e = c->pool.alloc(dst, (v.size() + 8) * sizeof(T));
   if (e != cudaSuccess) return e;
-  if (!v.empty()) e = cudaMemcpy(*dst, v.data(), v.size() * sizeof(T), cudaMemcpyHostToDevice);
+  e = cudaMemset(*dst, 0, (v.size() + 8) * sizeof(T));
+  if (e == cudaSuccess && !v.empty()) e = cudaMemcpy(*dst, v.data(), v.size() * sizeof(T), cudaMemcpyHostToDevice);
   return e;
 }
 
@@ -308,6 +311,7 @@ extern "C" alora_status alora_create(const alora_problem* P, alora_dtype dtype, 
   c->device = device; c->stream = (cudaStream_t)cuda_stream; c->dtype = dtype;
   c->esz = dtype == ALORA_F32 ? 4 : 8; c->n = P->n; c->m = P->m;
   std::memset(c->occ_cache, 0, sizeof(c->occ_cache));
+  std::memset(c->occ_ld, 0, sizeof(c->occ_ld));
   cudaDeviceProp prop;
   if (cudaGetDeviceProperties(&prop, device) == cudaSuccess) c->num_sms = prop.multiProcessorCount;
   alora_status s;

@@ -6,6 +6,7 @@
 #include <numeric>
 
 #include "alora_internal.h"
+#include "rows_tiled.cuh"
 
 namespace alora {
 
@@ -143,6 +144,49 @@ template <typename T> int grid_rows(alora_ctx* c, int vec, int shape, int mode, 
   const int64_t need = (items + gpb - 1) / gpb;
   return (int)std::max<int64_t>(1, std::min<int64_t>(need, std::min<int64_t>((int64_t)c->num_sms * occ, c->part_cap)));
 }
+// Row pass of the diagonal class: the tiled kernel on the full tiles plus k_rows on the ragged tail, or
+// k_rows alone when the tiled kernel's preconditions do not hold (non-identity diagonal constraints,
+// misaligned buffers, tile too large for shared memory).  *nparts = partial rows written.
+template <typename T>
+alora_status launch_diag_rows(alora_ctx* c, int vec, int nvec, int exact, int shape, int mode, RowArgs<T>& a,
+                              const void* dual, int* nparts) {
+  const int gs = kShapes[shape].gs, nit = kShapes[shape].nit, tr = tile_rows(gs);
+  const int full = (nvec == gs * nit) && exact;
+  const int64_t tiles = c->n / tr;
+  bool elig = !c->dcons && !c->da && tiles > 0 && !((uintptr_t)a.X % 16) && !((uintptr_t)a.X2 % 16) && !((uintptr_t)dual % 16);
+  int occ = 0;
+  if (elig) {
+    int& oc = c->occ_cache[vec_slot(vec)][shape][8 + mode];
+    int64_t& key = c->occ_ld[vec_slot(vec)][shape][mode];
+    const int64_t want = a.ld * 2 + full;
+    if (!oc || key != want) { oc = occ_tiled(T(), vec, shape, mode, full, a.ld); key = want; if (!oc) oc = -1; }
+    occ = oc;
+    elig = occ > 0;
+  }
+  if (!elig) {
+    const int grid = grid_rows<T>(c, vec, shape, mode, c->n);
+    a.row_begin = 0;
+    ALORA_CUDA(c, launch_rows(vec, shape, mode, a, grid, c->stream));
+    c->launches++;
+    *nparts = grid;
+    return ALORA_OK;
+  }
+  const int grid = (int)std::max<int64_t>(1, std::min<int64_t>(tiles, std::min<int64_t>((int64_t)c->num_sms * occ, c->part_cap / 2)));
+  a.tiles = tiles;
+  ALORA_CUDA(c, launch_tiled(vec, shape, mode, full, a, grid, c->stream));
+  c->launches++;
+  *nparts = grid;
+  if (tiles * tr < c->n) {
+    RowArgs<T> t = a;
+    t.row_begin = tiles * tr;
+    t.partials = a.partials + (int64_t)grid * kNStat;
+    const int gt = grid_rows<T>(c, vec, shape, mode, c->n - tiles * tr);
+    ALORA_CUDA(c, launch_rows(vec, shape, mode, t, gt, c->stream));
+    c->launches++;
+    *nparts = grid + gt;
+  }
+  return ALORA_OK;
+}
 template <typename T> int grid_cons(alora_ctx* c, int vec, int shape, int mode, int chunked, int64_t items) {
   int& occ = c->occ_cache[vec_slot(vec)][shape][3 + mode * 2 + chunked];
   if (!occ) occ = std::max(1, occ_cons(T(), vec, shape, mode, chunked));
@@ -170,7 +214,7 @@ template <typename T> void fill_rows(alora_ctx* c, RowArgs<T>& a, const Geo& g, 
   a.a_rowptr = c->a_rowptr; a.a_col = c->a_col; a.a_val = (const T*)c->a_val; a.a_cons = c->a_cons;
   a.y = c->y; a.b = c->b; a.sigma = c->sigma; a.w = nullptr; a.z = nullptr;
   a.pC = 0; a.U = (const T*)c->U; a.Ts = c->Ts; a.scale = 1.0; a.diag_class = (c->cls == 0);
-  a.partials = c->part_rows;
+  a.partials = c->part_rows; a.row_begin = 0; a.tiles = 0;
 }
 template <typename T> void fill_cons(alora_ctx* c, ConsArgs<T>& a, const Geo& g, const T* X, const T* X2, int r, int64_t ld) {
   a.n = c->n; a.r = r; a.ld = ld; a.nvec = g.nvec; a.exact = g.exact; a.X = X; a.X2 = X2; a.m = c->m;
@@ -201,12 +245,13 @@ template <typename T> alora_status eval_impl(alora_ctx* c, const T* R, int32_t r
   a.Out = G; a.scale = 2.0;
   if (c->cls == 0) {
     a.z = zout;
-    const int grid = grid_rows<T>(c, g.vec, g.shape, ROWS_FUSED_EVAL, c->n);
+    int nparts = 0;
     time_mark(c);
-    ALORA_CUDA(c, launch_rows(g.vec, g.shape, ROWS_FUSED_EVAL, a, grid, c->stream));
+    s = launch_diag_rows<T>(c, g.vec, g.nvec, g.exact, g.shape, ROWS_FUSED_EVAL, a, c->y, &nparts);
+    if (s != ALORA_OK) return s;
     time_mark(c);
-    k_finalize<<<1, kBlock, 0, c->stream>>>(c->part_rows, grid, nullptr, 0, nullptr, 0, c->stats_dev);
-    c->launches += 2;
+    k_finalize<<<1, kBlock, 0, c->stream>>>(c->part_rows, nparts, nullptr, 0, nullptr, 0, c->stats_dev);
+    c->launches++;
   } else {
     if (c->pC) { s = lowrank<T>(c, R, r, ld, c->TmR, true); if (s != ALORA_OK) return s; a.pC = c->pC; }
     ConsArgs<T> ca;
@@ -265,10 +310,11 @@ template <typename T> alora_status ls_impl(alora_ctx* c, const T* R, const T* D,
     RowArgs<T> a;
     fill_rows(c, a, g, R, r, ld);
     a.X2 = D;
-    const int grid = grid_rows<T>(c, g.vec, g.shape, ROWS_LS_FUSED, c->n);
-    ALORA_CUDA(c, launch_rows(g.vec, g.shape, ROWS_LS_FUSED, a, grid, c->stream));
-    k_finalize<<<1, kBlock, 0, c->stream>>>(c->part_rows, grid, nullptr, 0, nullptr, 0, c->ls_dev);
-    c->launches += 2;
+    int nparts = 0;
+    s = launch_diag_rows<T>(c, g.vec, g.nvec, g.exact, g.shape, ROWS_LS_FUSED, a, c->y, &nparts);
+    if (s != ALORA_OK) return s;
+    k_finalize<<<1, kBlock, 0, c->stream>>>(c->part_rows, nparts, nullptr, 0, nullptr, 0, c->ls_dev);
+    c->launches++;
   } else {
     if (c->pC) {
       s = lowrank<T>(c, R, r, ld, c->TmR, false); if (s != ALORA_OK) return s;
@@ -333,10 +379,17 @@ template <typename T> alora_status matvec_impl(alora_ctx* c, const double* mu, c
   fill_rows(c, a, g, V, p, p);
   a.Out = W; a.scale = 1.0; a.w = mu; a.diag_class = (c->cls == 0);
   if (c->pC) { s = lowrank<T>(c, V, p, p, c->TmD, true); if (s != ALORA_OK) return s; a.pC = c->pC; }
-  const int grid = grid_rows<T>(c, g.vec, g.shape, ROWS_ADJ, c->n);
-  ALORA_CUDA(c, launch_rows(g.vec, g.shape, ROWS_ADJ, a, grid, c->stream));
-  k_finalize<<<1, kBlock, 0, c->stream>>>(c->part_rows, grid, nullptr, 0, nullptr, 0, c->mv_dev);
-  c->launches += 2;
+  int nparts = 0;
+  if (c->cls == 0) {
+    s = launch_diag_rows<T>(c, g.vec, g.nvec, g.exact, g.shape, ROWS_ADJ, a, mu, &nparts);
+    if (s != ALORA_OK) return s;
+  } else {
+    nparts = grid_rows<T>(c, g.vec, g.shape, ROWS_ADJ, c->n);
+    ALORA_CUDA(c, launch_rows(g.vec, g.shape, ROWS_ADJ, a, nparts, c->stream));
+    c->launches++;
+  }
+  k_finalize<<<1, kBlock, 0, c->stream>>>(c->part_rows, nparts, nullptr, 0, nullptr, 0, c->mv_dev);
+  c->launches++;
   ALORA_CUDA(c, cudaGetLastError());
   return ALORA_OK;
 }

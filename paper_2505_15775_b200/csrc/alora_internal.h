@@ -81,7 +81,8 @@ struct alora_ctx {
   void* stageR = nullptr; void* stageG = nullptr; size_t stage_bytes = 0;
   void* pinR = nullptr; size_t pin_bytes = 0;
   // occupancy cache [vec idx][shape][kind]
-  int occ_cache[3][7][8];
+  int occ_cache[3][7][12];
+  int64_t occ_ld[3][7][4];   // ld for which the tiled-kernel occupancy was computed
   alora::SolveWorkspace* ws = nullptr;
   // optional CUDA-event timing of the dominant kernel of alora_eval (bench.py roofline)
   bool timing = false; std::vector<cudaEvent_t> ev; size_t ev_used = 0;

@@ -49,6 +49,8 @@ template <typename T> struct RowArgs {
   double scale;
   int diag_class;    // ROWS_ADJ: 1 = constraints are the per-row diagonal ones, 0 = use a_* CSR
   double* partials;  // [gridDim.x][kNStat]
+  int64_t row_begin; // k_rows: first row handled (rows [row_begin, n))
+  int64_t tiles;     // k_rows_tiled: number of full row tiles handled (rows [0, tiles * TR))
 };
 
 template <typename T> struct ConsArgs {
@@ -210,7 +212,7 @@ __global__ void __launch_bounds__(kBlock) k_rows(const RowArgs<T> a) {
 #pragma unroll
   for (int s = 0; s < NST; ++s) st[s] = 0.0;
 
-  for (int64_t row = (int64_t)blockIdx.x * GPB + grp; row < a.n; row += (int64_t)gridDim.x * GPB) {
+  for (int64_t row = a.row_begin + (int64_t)blockIdx.x * GPB + grp; row < a.n; row += (int64_t)gridDim.x * GPB) {
     Row x; x.load(a.X + row * a.ld, lane, nvec, r, exact);
     const int cb = __ldg(a.c_rowptr + row), ce = __ldg(a.c_rowptr + row + 1);
     const T dc = __ldg(a.dC + row);

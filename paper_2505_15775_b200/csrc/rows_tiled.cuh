@@ -1,0 +1,337 @@
+// rows_tiled.cuh -- the row kernel of the "diagonal" constraint class (MaxCut), B200 design.
+//
+// What the first design (k_rows) got wrong on B200 (profiles/r1a_*): per row it chains three
+// dependent global loads (rowptr -> col/val -> neighbour row) and keeps too few bytes in flight, so
+// the pass is latency bound at 0.34 of the HBM roofline while moving only the algorithmic bytes.
+//
+// Here every *streaming* input of a row tile -- the tile's rows of X (and D), its slices of dC, y, b
+// (or the weights w) and of the CSR (rowptr, col, val) -- is brought into shared memory by 1-D bulk
+// async copies (cp.async.bulk, SASS UBLKCP) issued by a dedicated producer warp into a ring of
+// kStages stages, completion signalled on mbarriers (full / empty), so tens of KB per block are in
+// flight to HBM independently of what the consumer warps are doing.  The 8 consumer warps read the
+// tile from shared memory, issue all neighbour-row gathers (the only dependent global access left;
+// they mostly hit L2) before the first FMA, write the output row with 16-byte stores and release the
+// stage per warp -- there is no block-wide barrier inside the tile loop.  Loop trip counts are
+// warp-uniform, so sub-warp reductions use full-mask shuffles.  Sums across rows are fp64, ordered,
+// two-stage as in kernels.cuh.
+#pragma once
+#include "kernels.cuh"
+
+namespace alora {
+
+constexpr int kStages = 4;            // tiles in flight per block
+constexpr int kUN = 4;                // neighbours gathered up front per row
+constexpr int kTiledThreads = kBlock + 32;   // 8 consumer warps + 1 producer warp
+
+__host__ __device__ constexpr int tile_rows(int gs) { return kBlock / gs; }   // one row per group per tile
+__host__ __device__ constexpr int tile_cap(int gs) {   // CSR entries staged per tile (denser tiles read global memory)
+  return tile_rows(gs) * 12 > 256 ? tile_rows(gs) * 12 : 256;
+}
+// per-stage shared memory: [X tile][D tile (line search)][dC][y|w][b][rowptr][col][val], 16-byte aligned pieces
+__host__ __device__ inline size_t tiled_stage_bytes(int gs, int esz, int64_t ld, int mode) {
+  const size_t tr = tile_rows(gs), cap = tile_cap(gs);
+  size_t b = tr * (size_t)ld * esz * (mode == ROWS_LS_FUSED ? 2 : 1);
+  b = (b + 15) & ~(size_t)15;
+  b += tr * esz;                 // dC
+  b = (b + 15) & ~(size_t)15;
+  b += tr * 8 * 2;               // y (or w), b
+  b += (tr + 4) * 4 + cap * 4 + cap * esz;
+  return (b + 15) & ~(size_t)15;
+}
+__host__ __device__ inline size_t tiled_smem_bytes(int gs, int esz, int64_t ld, int mode) {
+  return kStages * tiled_stage_bytes(gs, esz, ld, mode);
+}
+
+// ---- mbarrier / bulk-copy primitives (PTX) ------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t* bar, int count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+  asm volatile(
+      "{\n .reg .pred p;\n WAIT_%=:\n mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n @p bra DONE_%=;\n bra WAIT_%=;\n DONE_%=:\n}\n" ::"r"(
+          smem_u32(bar)),
+      "r"(parity)
+      : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst)),
+               "l"(src), "r"(bytes), "r"(smem_u32(bar))
+               : "memory");
+}
+
+template <int GS> __device__ __forceinline__ float gsum(float v) {
+#pragma unroll
+  for (int o = GS / 2; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+template <int GS> __device__ __forceinline__ double gsum(double v) {
+#pragma unroll
+  for (int o = GS / 2; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+
+// row held in registers, loaded from shared memory (generic loads; ldg_pack is global-only)
+template <typename T, int VEC, int GS, int NIT>
+__device__ __forceinline__ void load_row_smem(RowReg<T, VEC, GS, NIT>& x, const T* base, int lane, int nvec, int r, int exact) {
+#pragma unroll
+  for (int it = 0; it < NIT; ++it) {
+    const int vi = lane + it * GS;
+    if (vi < nvec) {
+      x.p[it] = *reinterpret_cast<const Pack<T, VEC>*>(base + vi * VEC);
+      if (VEC > 1 && !exact && vi == nvec - 1) {
+#pragma unroll
+        for (int i = 0; i < VEC; ++i) if (vi * VEC + i >= r) x.p[it].v[i] = T(0);
+      }
+    } else {
+#pragma unroll
+      for (int i = 0; i < VEC; ++i) x.p[it].v[i] = T(0);
+    }
+  }
+}
+
+template <int NST, int NW> __device__ __forceinline__ void block_reduce_store_nw(double (&st)[NST], double* out) {
+  __shared__ double sm[NST][NW];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+#pragma unroll
+  for (int s = 0; s < NST; ++s) {
+    const double v = warp_sum(st[s]);
+    if (lane == 0) sm[s][warp] = v;
+  }
+  __syncthreads();
+  if (threadIdx.x < kNStat) {
+    double v = 0.0;
+    if (threadIdx.x < NST) {
+#pragma unroll
+      for (int wv = 0; wv < NW; ++wv) v += sm[threadIdx.x][wv];
+    }
+    out[threadIdx.x] = v;
+  }
+}
+
+// Row load / store helpers with the tail handling resolved at compile time (FULL: r == VEC*GS*NIT).
+template <bool FULL, typename T, int VEC, int GS, int NIT>
+__device__ __forceinline__ void row_ldg(RowReg<T, VEC, GS, NIT>& x, const T* base, int lane, int nvec, int r, int exact) {
+  if (FULL) {
+#pragma unroll
+    for (int it = 0; it < NIT; ++it) x.p[it] = ldg_pack<T, VEC>(base + (lane + it * GS) * VEC);
+  } else {
+    x.load(base, lane, nvec, r, exact);
+  }
+}
+template <bool FULL, typename T, int VEC, int GS, int NIT>
+__device__ __forceinline__ void row_lds(RowReg<T, VEC, GS, NIT>& x, const T* base, int lane, int nvec, int r, int exact) {
+  if (FULL) {
+#pragma unroll
+    for (int it = 0; it < NIT; ++it) x.p[it] = *reinterpret_cast<const Pack<T, VEC>*>(base + (lane + it * GS) * VEC);
+  } else {
+    load_row_smem(x, base, lane, nvec, r, exact);
+  }
+}
+template <bool FULL, typename T, int VEC, int GS, int NIT>
+__device__ __forceinline__ void row_stg(const RowReg<T, VEC, GS, NIT>& x, T* base, int lane, int nvec, int r, int exact) {
+  if (FULL) {
+#pragma unroll
+    for (int it = 0; it < NIT; ++it) st_pack<T, VEC>(base + (lane + it * GS) * VEC, x.p[it]);
+  } else {
+    x.store(base, lane, nvec, r, exact);
+  }
+}
+
+// Preconditions (checked by the host, which otherwise uses k_rows): the constraints are the identity
+// diagonal ones (dcons == da == nullptr), X / X2 / y (or w) are 16-byte aligned, and the kernel is
+// given FULL tiles only: it covers rows [0, a.tiles * TR); the ragged tail goes to k_rows.
+template <typename T, int VEC, int GS, int NIT, int MODE, bool FULL>
+__global__ void __launch_bounds__(kTiledThreads) k_rows_tiled(const RowArgs<T> a) {
+  using Row = RowReg<T, VEC, GS, NIT>;
+  constexpr int TR = tile_rows(GS), CAP = tile_cap(GS), GPW = 32 / GS, NCW = kBlock / 32;
+  constexpr int NST = (MODE == ROWS_LS_FUSED) ? 12 : 6;
+  constexpr bool LS = (MODE == ROWS_LS_FUSED);
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  __shared__ uint64_t full[kStages], empty[kStages];
+  __shared__ int s_ea[kStages], s_fit[kStages];
+  const int warp = threadIdx.x >> 5, lane32 = threadIdx.x & 31;
+  const int nvec = a.nvec, r = a.r, exact = a.exact;
+  const int64_t ld = a.ld;
+  const int64_t ntiles = a.tiles;
+
+  // stage layout (must match tiled_stage_bytes)
+  const uint32_t xbytes = (uint32_t)(TR * ld * sizeof(T));
+  const uint32_t off_dc = (xbytes * (LS ? 2u : 1u) + 15u) & ~15u;
+  const uint32_t off_y = (off_dc + TR * (uint32_t)sizeof(T) + 15u) & ~15u;
+  const uint32_t off_b = off_y + TR * 8, off_rp = off_b + TR * 8, off_col = off_rp + (TR + 4) * 4;
+  const uint32_t off_val = off_col + CAP * 4;
+  const uint32_t stage_sz = (off_val + CAP * (uint32_t)sizeof(T) + 15u) & ~15u;
+
+  if (threadIdx.x == 0) {
+    for (int s = 0; s < kStages; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], NCW); }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+  }
+  __syncthreads();
+
+  double st[NST];
+#pragma unroll
+  for (int s = 0; s < NST; ++s) st[s] = 0.0;
+
+  if (warp == NCW) {
+    // ================= producer warp: lane j pre-loads the CSR bounds of the j-th upcoming tile ==========
+    const int64_t my_tiles = ntiles > blockIdx.x ? (ntiles - blockIdx.x + gridDim.x - 1) / gridDim.x : 0;
+    for (int64_t base = 0; base < my_tiles; base += 32) {
+      const int64_t tj = (int64_t)blockIdx.x + (base + lane32) * gridDim.x;
+      int e0 = 0, e1 = 0;
+      if (tj < ntiles) { e0 = __ldg(a.c_rowptr + tj * TR); e1 = __ldg(a.c_rowptr + tj * TR + TR); }
+      const int cnt = (int)min((int64_t)32, my_tiles - base);
+      for (int j = 0; j < cnt; ++j) {
+        const int e0j = __shfl_sync(0xffffffffu, e0, j), e1j = __shfl_sync(0xffffffffu, e1, j);
+        if (lane32 == 0) {
+          const int64_t it = base + j;
+          const int s = (int)(it % kStages);
+          const uint32_t ph = (uint32_t)((it / kStages) & 1);
+          const int64_t t0 = ((int64_t)blockIdx.x + it * gridDim.x) * TR;
+          mbar_wait(&empty[s], ph ^ 1u);
+          unsigned char* sb = smem_raw + (size_t)s * stage_sz;
+          const int ea = e0j & ~3, cnt4 = (e1j - ea + 3) & ~3;
+          const bool fit = cnt4 <= CAP;
+          const uint32_t cv = (fit && cnt4) ? (uint32_t)cnt4 : 0u;
+          const uint32_t rp_bytes = (TR + 4) * 4;
+          const uint32_t bytes = rp_bytes + cv * 4u + cv * (uint32_t)sizeof(T) + xbytes * (LS ? 2u : 1u) +
+                                 TR * (uint32_t)sizeof(T) + TR * 8u * (MODE == ROWS_ADJ ? 1u : 2u);
+          s_ea[s] = ea; s_fit[s] = fit;
+          mbar_expect_tx(&full[s], bytes);
+          bulk_g2s(sb, a.X + t0 * ld, xbytes, &full[s]);
+          if (LS) bulk_g2s(sb + xbytes, a.X2 + t0 * ld, xbytes, &full[s]);
+          bulk_g2s(sb + off_dc, a.dC + t0, TR * (uint32_t)sizeof(T), &full[s]);
+          bulk_g2s(sb + off_y, (MODE == ROWS_ADJ ? a.w : a.y) + t0, TR * 8u, &full[s]);
+          if (MODE != ROWS_ADJ) bulk_g2s(sb + off_b, a.b + t0, TR * 8u, &full[s]);
+          bulk_g2s(sb + off_rp, a.c_rowptr + t0, rp_bytes, &full[s]);
+          if (cv) {
+            bulk_g2s(sb + off_col, a.c_col + ea, cv * 4u, &full[s]);
+            bulk_g2s(sb + off_val, a.c_val + ea, cv * (uint32_t)sizeof(T), &full[s]);
+          }
+        }
+      }
+    }
+  } else {
+    // ================= consumer warps ======================================================================
+    const int lane = lane32 % GS;
+    const int lr = warp * GPW + lane32 / GS;           // row of the tile handled by this group
+    const uint32_t xoff = (uint32_t)(lr * ld * sizeof(T));
+    int64_t it = 0;
+    for (int64_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x, ++it) {
+      const int s = (int)(it % kStages);
+      const uint32_t ph = (uint32_t)((it / kStages) & 1);
+      const int64_t row = tile * TR + lr;
+      mbar_wait(&full[s], ph);
+      const unsigned char* sb = smem_raw + (size_t)s * stage_sz;
+      const int ea = s_ea[s];
+      const bool fit = s_fit[s] != 0;
+      Row x, d;
+      row_lds<FULL>(x, reinterpret_cast<const T*>(sb + xoff), lane, nvec, r, exact);
+      if (LS) row_lds<FULL>(d, reinterpret_cast<const T*>(sb + xbytes + xoff), lane, nvec, r, exact);
+      const T dc = reinterpret_cast<const T*>(sb + off_dc)[lr];
+      const double yv = reinterpret_cast<const double*>(sb + off_y)[lr];
+      const double bv = (MODE != ROWS_ADJ) ? reinterpret_cast<const double*>(sb + off_b)[lr] : 0.0;
+      const int* rp = reinterpret_cast<const int*>(sb + off_rp);
+      const int* colp = fit ? reinterpret_cast<const int*>(sb + off_col) - ea : a.c_col;   // indexed by absolute entry
+      const T* valp = fit ? reinterpret_cast<const T*>(sb + off_val) - ea : a.c_val;
+      const int eb = rp[lr], ee = rp[lr + 1];
+      // first kUN neighbours: missing ones become (own row, weight 0), so the gathers are unconditional
+      int ck[kUN]; T cw[kUN];
+#pragma unroll
+      for (int u = 0; u < kUN; ++u) {
+        const int e = eb + u;
+        const int k = colp[e];
+        const T v = valp[e];
+        const bool ok = LS ? (e < ee && (int64_t)k > row) : (e < ee);
+        ck[u] = ok ? k : (int)row;
+        cw[u] = ok ? v : T(0);
+      }
+      if (LS) {
+        Row xk[kUN], dk[kUN];
+#pragma unroll
+        for (int u = 0; u < kUN; ++u) {
+          row_ldg<FULL>(xk[u], a.X + (int64_t)ck[u] * ld, lane, nvec, r, exact);
+          row_ldg<FULL>(dk[u], a.X2 + (int64_t)ck[u] * ld, lane, nvec, r, exact);
+        }
+        const T rr_l = x.dot(x), rd_l = x.dot(d), dd_l = d.dot(d);
+        const double rr = (double)gsum<GS>(rr_l), rd = (double)gsum<GS>(rd_l), dd = (double)gsum<GS>(dd_l);
+        if (lane == 0) {
+          const double qv = rr - bv, q1 = 2.0 * rd, q2 = dd;
+          st[LS_YQ] += yv * qv; st[LS_YQ1] += yv * q1; st[LS_YQ2] += yv * q2;
+          st[LS_QQ] += qv * qv; st[LS_QQ1] += qv * q1; st[LS_QQ2] += qv * q2;
+          st[LS_Q11] += q1 * q1; st[LS_Q12] += q1 * q2; st[LS_Q22] += q2 * q2;
+        }
+        T sRR = T(0), sRD = T(0), sDD = T(0);
+#pragma unroll
+        for (int u = 0; u < kUN; ++u) {
+          sRR = fma(cw[u], x.dot(xk[u]), sRR);
+          sRD = fma(cw[u], x.dot(dk[u]) + d.dot(xk[u]), sRD);
+          sDD = fma(cw[u], d.dot(dk[u]), sDD);
+        }
+        for (int e = eb + kUN; e < ee; ++e) {   // rows with more than kUN neighbours
+          const int k = colp[e];
+          if ((int64_t)k > row) {
+            const T cv = valp[e];
+            Row xe, de;
+            row_ldg<FULL>(xe, a.X + (int64_t)k * ld, lane, nvec, r, exact);
+            row_ldg<FULL>(de, a.X2 + (int64_t)k * ld, lane, nvec, r, exact);
+            sRR = fma(cv, x.dot(xe), sRR);
+            sRD = fma(cv, x.dot(de) + d.dot(xe), sRD);
+            sDD = fma(cv, d.dot(de), sDD);
+          }
+        }
+        st[LS_CRR] += (double)dc * (double)rr_l + 2.0 * (double)sRR;
+        st[LS_CRD] += (double)dc * (double)rd_l + (double)sRD;
+        st[LS_CDD] += (double)dc * (double)dd_l + 2.0 * (double)sDD;
+      } else {
+        Row xn[kUN];
+#pragma unroll
+        for (int u = 0; u < kUN; ++u) row_ldg<FULL>(xn[u], a.X + (int64_t)ck[u] * ld, lane, nvec, r, exact);
+        double coef;
+        if (MODE == ROWS_FUSED_EVAL) {
+          const double z = (double)gsum<GS>(x.dot(x)), qv = z - bv, lam = yv - a.sigma * qv;
+          coef = lam;
+          if (lane == 0) {
+            if (a.z) a.z[row] = z;
+            st[ES_YQ] += yv * qv; st[ES_QQ] += qv * qv; st[ES_LZ] += lam * z;
+          }
+        } else {
+          coef = yv;   // ROWS_ADJ: the y slot holds the weight w[row]
+        }
+        Row acc;
+#pragma unroll
+        for (int i2 = 0; i2 < NIT; ++i2)
+#pragma unroll
+          for (int i = 0; i < VEC; ++i) acc.p[i2].v[i] = dc * x.p[i2].v[i];
+#pragma unroll
+        for (int u = 0; u < kUN; ++u) acc.axpy(cw[u], xn[u]);
+        for (int e = eb + kUN; e < ee; ++e) {   // rows with more than kUN neighbours
+          Row xe; row_ldg<FULL>(xe, a.X + (int64_t)colp[e] * ld, lane, nvec, r, exact);
+          acc.axpy(valp[e], xe);
+        }
+        st[ES_CX] += (double)acc.dot(x);
+        acc.axpy((T)(-coef), x);
+        const T sc = (T)a.scale;
+#pragma unroll
+        for (int i2 = 0; i2 < NIT; ++i2)
+#pragma unroll
+          for (int i = 0; i < VEC; ++i) acc.p[i2].v[i] *= sc;
+        st[ES_GG] += (double)acc.dot(acc);
+        st[ES_GR] += (double)acc.dot(x);
+        if (a.Out) row_stg<FULL>(acc, a.Out + row * ld, lane, nvec, r, exact);
+      }
+      __syncwarp();
+      if (lane32 == 0) mbar_arrive(&empty[s]);   // this warp is done with stage s
+    }
+  }
+  block_reduce_store_nw<NST, NCW + 1>(st, a.partials + (int64_t)blockIdx.x * kNStat);
+}
+
+}  // namespace alora
