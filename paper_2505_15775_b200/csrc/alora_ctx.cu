@@ -18,17 +18,25 @@ alora_status fail(alora_ctx* c, alora_status s, const std::string& msg) {
 // ---------------------------------------------------------------------------------------------
 // small kernels
 // ---------------------------------------------------------------------------------------------
-// out[s] = sum over the partial rows of up to three regions, fixed order (one block, 8 warps)
-__global__ void k_finalize(const double* p0, int n0, const double* p1, int n1, const double* p2, int n2,
-                           double* out) {
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  for (int s = warp; s < kNStat; s += kBlock / 32) {
-    double v = 0.0;
-    for (int i = lane; i < n0; i += 32) v += p0[(int64_t)i * kNStat + s];
-    for (int i = lane; i < n1; i += 32) v += p1[(int64_t)i * kNStat + s];
-    for (int i = lane; i < n2; i += 32) v += p2[(int64_t)i * kNStat + s];
-    v = warp_sum(v);
-    if (lane == 0) out[s] = v;
+// out[s] = sum over the partial rows of up to three regions, in a fixed order: thread t owns stat
+// t % 16 and the rows t / 16, t / 16 + 64, ... (coalesced 128-byte reads); the 64 row slots are then
+// summed in order through shared memory.  One block of 1024 threads.
+constexpr int kFinThreads = 1024;
+__global__ void __launch_bounds__(kFinThreads) k_finalize(const double* p0, int n0, const double* p1, int n1,
+                                                          const double* p2, int n2, double* out) {
+  __shared__ double sm[kFinThreads];
+  const int s = threadIdx.x & (kNStat - 1), slot = threadIdx.x / kNStat;
+  constexpr int NSLOT = kFinThreads / kNStat;
+  double v = 0.0;
+  for (int i = slot; i < n0; i += NSLOT) v += p0[(int64_t)i * kNStat + s];
+  for (int i = slot; i < n1; i += NSLOT) v += p1[(int64_t)i * kNStat + s];
+  for (int i = slot; i < n2; i += NSLOT) v += p2[(int64_t)i * kNStat + s];
+  sm[threadIdx.x] = v;
+  __syncthreads();
+  if (threadIdx.x < kNStat) {
+    double t = 0.0;
+    for (int k = 0; k < NSLOT; ++k) t += sm[k * kNStat + threadIdx.x];
+    out[threadIdx.x] = t;
   }
 }
 
@@ -151,7 +159,8 @@ template <typename T>
 alora_status launch_diag_rows(alora_ctx* c, int vec, int nvec, int exact, int shape, int mode, RowArgs<T>& a,
                               const void* dual, int* nparts) {
   const int gs = kShapes[shape].gs, nit = kShapes[shape].nit, tr = tile_rows(gs);
-  const int full = (nvec == gs * nit) && exact;
+  const int full = exact;   // no partially filled pack; idle lanes (nvec < gs*nit) are handled by a lane mask
+  (void)nit; (void)nvec;
   const int64_t tiles = c->n / tr;
   bool elig = !c->dcons && !c->da && tiles > 0 && !((uintptr_t)a.X % 16) && !((uintptr_t)a.X2 % 16) && !((uintptr_t)dual % 16);
   int occ = 0;
@@ -250,7 +259,7 @@ template <typename T> alora_status eval_impl(alora_ctx* c, const T* R, int32_t r
     s = launch_diag_rows<T>(c, g.vec, g.nvec, g.exact, g.shape, ROWS_FUSED_EVAL, a, c->y, &nparts);
     if (s != ALORA_OK) return s;
     time_mark(c);
-    k_finalize<<<1, kBlock, 0, c->stream>>>(c->part_rows, nparts, nullptr, 0, nullptr, 0, c->stats_dev);
+    k_finalize<<<1, kFinThreads, 0, c->stream>>>(c->part_rows, nparts, nullptr, 0, nullptr, 0, c->stats_dev);
     c->launches++;
   } else {
     if (c->pC) { s = lowrank<T>(c, R, r, ld, c->TmR, true); if (s != ALORA_OK) return s; a.pC = c->pC; }
@@ -276,7 +285,7 @@ template <typename T> alora_status eval_impl(alora_ctx* c, const T* R, int32_t r
     time_mark(c);
     ALORA_CUDA(c, launch_rows(g.vec, g.shape, ROWS_ADJ, a, grid, c->stream));
     time_mark(c);
-    k_finalize<<<1, kBlock, 0, c->stream>>>(c->part_rows, grid, c->part_cons, gc, c->part_long, c->nlong_A, c->stats_dev);
+    k_finalize<<<1, kFinThreads, 0, c->stream>>>(c->part_rows, grid, c->part_cons, gc, c->part_long, c->nlong_A, c->stats_dev);
     c->launches += 2;
   }
   ALORA_CUDA(c, cudaGetLastError());
@@ -313,7 +322,7 @@ template <typename T> alora_status ls_impl(alora_ctx* c, const T* R, const T* D,
     int nparts = 0;
     s = launch_diag_rows<T>(c, g.vec, g.nvec, g.exact, g.shape, ROWS_LS_FUSED, a, c->y, &nparts);
     if (s != ALORA_OK) return s;
-    k_finalize<<<1, kBlock, 0, c->stream>>>(c->part_rows, nparts, nullptr, 0, nullptr, 0, c->ls_dev);
+    k_finalize<<<1, kFinThreads, 0, c->stream>>>(c->part_rows, nparts, nullptr, 0, nullptr, 0, c->ls_dev);
     c->launches++;
   } else {
     if (c->pC) {
@@ -336,7 +345,7 @@ template <typename T> alora_status ls_impl(alora_ctx* c, const T* R, const T* D,
                                                            c->b, c->sigma, nullptr, nullptr, c->part_long);
       c->launches += 2;
     }
-    k_finalize<<<1, kBlock, 0, c->stream>>>(c->part_cons, gc, c->part_long, c->nlong_all, nullptr, 0, c->ls_dev);
+    k_finalize<<<1, kFinThreads, 0, c->stream>>>(c->part_cons, gc, c->part_long, c->nlong_all, nullptr, 0, c->ls_dev);
     c->launches++;
   }
   ALORA_CUDA(c, cudaGetLastError());
@@ -388,7 +397,7 @@ template <typename T> alora_status matvec_impl(alora_ctx* c, const double* mu, c
     ALORA_CUDA(c, launch_rows(g.vec, g.shape, ROWS_ADJ, a, nparts, c->stream));
     c->launches++;
   }
-  k_finalize<<<1, kBlock, 0, c->stream>>>(c->part_rows, nparts, nullptr, 0, nullptr, 0, c->mv_dev);
+  k_finalize<<<1, kFinThreads, 0, c->stream>>>(c->part_rows, nparts, nullptr, 0, nullptr, 0, c->mv_dev);
   c->launches++;
   ALORA_CUDA(c, cudaGetLastError());
   return ALORA_OK;

@@ -21,11 +21,12 @@ namespace alora {
 
 constexpr int kStages = 4;            // tiles in flight per block
 constexpr int kUN = 4;                // neighbours gathered up front per row
+constexpr int kUNL = 3;               // line search: upper-triangle neighbours gathered up front per row
 constexpr int kTiledThreads = kBlock + 32;   // 8 consumer warps + 1 producer warp
 
 __host__ __device__ constexpr int tile_rows(int gs) { return kBlock / gs; }   // one row per group per tile
 __host__ __device__ constexpr int tile_cap(int gs) {   // CSR entries staged per tile (denser tiles read global memory)
-  return tile_rows(gs) * 12 > 256 ? tile_rows(gs) * 12 : 256;
+  return tile_rows(gs) * 8 > 256 ? tile_rows(gs) * 8 : 256;
 }
 // per-stage shared memory: [X tile][D tile (line search)][dC][y|w][b][rowptr][col][val], 16-byte aligned pieces
 __host__ __device__ inline size_t tiled_stage_bytes(int gs, int esz, int64_t ld, int mode) {
@@ -52,6 +53,15 @@ __device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
 }
 __device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
   asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait_addr(uint32_t bar, uint32_t parity) {
+  asm volatile(
+      "{\n .reg .pred p;\n WAIT_%=:\n mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n @p bra DONE_%=;\n bra WAIT_%=;\n DONE_%=:\n}\n" ::"r"(bar),
+      "r"(parity)
+      : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_addr(uint32_t bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
 }
 __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
   asm volatile(
@@ -144,11 +154,30 @@ __device__ __forceinline__ void row_stg(const RowReg<T, VEC, GS, NIT>& x, T* bas
   }
 }
 
+// same, addressed as (byte pointer already offset to the lane's first pack) -- one IMAD.WIDE per row.
+// `mask` bit it says whether this lane owns pack it (lane + it*GS < nvec); it is loop-invariant.
+template <typename T, int VEC, int GS, int NIT>
+__device__ __forceinline__ void row_ldg_b(RowReg<T, VEC, GS, NIT>& x, const char* p, unsigned mask) {
+#pragma unroll
+  for (int it = 0; it < NIT; ++it) {
+    if (mask & (1u << it)) x.p[it] = ldg_pack<T, VEC>(reinterpret_cast<const T*>(p) + it * GS * VEC);
+    else {
+#pragma unroll
+      for (int i = 0; i < VEC; ++i) x.p[it].v[i] = T(0);
+    }
+  }
+}
+
+// occupancy target by the number of 32-bit registers one row vector takes per lane
+__host__ __device__ constexpr int tiled_min_blocks(int row_regs, int mode) {
+  return row_regs <= 4 ? (mode == ROWS_LS_FUSED ? 2 : 4) : row_regs <= 8 ? 2 : 1;
+}
+
 // Preconditions (checked by the host, which otherwise uses k_rows): the constraints are the identity
 // diagonal ones (dcons == da == nullptr), X / X2 / y (or w) are 16-byte aligned, and the kernel is
 // given FULL tiles only: it covers rows [0, a.tiles * TR); the ragged tail goes to k_rows.
 template <typename T, int VEC, int GS, int NIT, int MODE, bool FULL>
-__global__ void __launch_bounds__(kTiledThreads) k_rows_tiled(const RowArgs<T> a) {
+__global__ void __launch_bounds__(kTiledThreads, tiled_min_blocks(VEC * NIT * (int)sizeof(T) / 4, MODE)) k_rows_tiled(const RowArgs<T> a) {
   using Row = RowReg<T, VEC, GS, NIT>;
   constexpr int TR = tile_rows(GS), CAP = tile_cap(GS), GPW = 32 / GS, NCW = kBlock / 32;
   constexpr int NST = (MODE == ROWS_LS_FUSED) ? 12 : 6;
@@ -222,43 +251,79 @@ __global__ void __launch_bounds__(kTiledThreads) k_rows_tiled(const RowArgs<T> a
     // ================= consumer warps ======================================================================
     const int lane = lane32 % GS;
     const int lr = warp * GPW + lane32 / GS;           // row of the tile handled by this group
-    const uint32_t xoff = (uint32_t)(lr * ld * sizeof(T));
-    int64_t it = 0;
+    const uint32_t ldb = (uint32_t)(ld * sizeof(T));   // row pitch in bytes
+    const uint32_t xoff = (uint32_t)lr * ldb;
+    const uint32_t loff = (uint32_t)(lane * VEC * sizeof(T));
+    const char* Xl = reinterpret_cast<const char*>(a.X) + loff;    // lane's first pack of row 0
+    const char* X2l = LS ? reinterpret_cast<const char*>(a.X2) + loff : nullptr;
+    char* Outl = a.Out ? reinterpret_cast<char*>(a.Out) + loff : nullptr;
+    const uint32_t full0 = smem_u32(full), empty0 = smem_u32(empty);
+    unsigned lmask = 0;   // packs of a row owned by this lane
+#pragma unroll
+    for (int i2 = 0; i2 < NIT; ++i2) if (lane + i2 * GS < nvec) lmask |= 1u << i2;
+    double* const zout = a.z;
+    const double sigma = a.sigma;
+    const T sc = (T)a.scale;
+    uint32_t it = 0;
     for (int64_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x, ++it) {
-      const int s = (int)(it % kStages);
-      const uint32_t ph = (uint32_t)((it / kStages) & 1);
-      const int64_t row = tile * TR + lr;
-      mbar_wait(&full[s], ph);
-      const unsigned char* sb = smem_raw + (size_t)s * stage_sz;
-      const int ea = s_ea[s];
-      const bool fit = s_fit[s] != 0;
+      const uint32_t s = it % kStages, ph = (it / kStages) & 1u;
+      const uint32_t row = (uint32_t)(tile * TR) + (uint32_t)lr;
+      mbar_wait_addr(full0 + s * 8u, ph);
+      const unsigned char* sb = smem_raw + s * stage_sz;
       Row x, d;
-      row_lds<FULL>(x, reinterpret_cast<const T*>(sb + xoff), lane, nvec, r, exact);
-      if (LS) row_lds<FULL>(d, reinterpret_cast<const T*>(sb + xbytes + xoff), lane, nvec, r, exact);
+      if (FULL) {
+        x.zero();
+        if (LS) d.zero();
+#pragma unroll
+        for (int i2 = 0; i2 < NIT; ++i2)
+          if (lmask & (1u << i2)) {
+            x.p[i2] = *reinterpret_cast<const Pack<T, VEC>*>(sb + xoff + loff + i2 * GS * VEC * sizeof(T));
+            if (LS) d.p[i2] = *reinterpret_cast<const Pack<T, VEC>*>(sb + xbytes + xoff + loff + i2 * GS * VEC * sizeof(T));
+          }
+      } else {
+        load_row_smem(x, reinterpret_cast<const T*>(sb + xoff), lane, nvec, r, exact);
+        if (LS) load_row_smem(d, reinterpret_cast<const T*>(sb + xbytes + xoff), lane, nvec, r, exact);
+      }
       const T dc = reinterpret_cast<const T*>(sb + off_dc)[lr];
       const double yv = reinterpret_cast<const double*>(sb + off_y)[lr];
       const double bv = (MODE != ROWS_ADJ) ? reinterpret_cast<const double*>(sb + off_b)[lr] : 0.0;
       const int* rp = reinterpret_cast<const int*>(sb + off_rp);
-      const int* colp = fit ? reinterpret_cast<const int*>(sb + off_col) - ea : a.c_col;   // indexed by absolute entry
-      const T* valp = fit ? reinterpret_cast<const T*>(sb + off_val) - ea : a.c_val;
       const int eb = rp[lr], ee = rp[lr + 1];
-      // first kUN neighbours: missing ones become (own row, weight 0), so the gathers are unconditional
-      int ck[kUN]; T cw[kUN];
+      const bool fit = s_fit[s] != 0;
+      // first neighbours: missing ones become (own row, weight 0), so the gathers are unconditional.
+      // Line search walks the row's list from its END: columns ascend, so the upper triangle (col > row,
+      // each off-diagonal pair once) is the tail of the list.
+      constexpr int NU = LS ? kUNL : kUN;
+      int ck[NU]; T cw[NU];
+      if (fit) {
+        const int sh = (LS ? ee - NU : eb) - s_ea[s];
+        const int* scol = reinterpret_cast<const int*>(sb + off_col) + sh;
+        const T* sval = reinterpret_cast<const T*>(sb + off_val) + sh;
 #pragma unroll
-      for (int u = 0; u < kUN; ++u) {
-        const int e = eb + u;
-        const int k = colp[e];
-        const T v = valp[e];
-        const bool ok = LS ? (e < ee && (int64_t)k > row) : (e < ee);
-        ck[u] = ok ? k : (int)row;
-        cw[u] = ok ? v : T(0);
+        for (int u = 0; u < NU; ++u) {
+          const bool in = LS ? (ee - NU + u >= eb) : true;   // (reads below the slice start are avoided)
+          ck[u] = in ? scol[u] : 0; cw[u] = in ? sval[u] : T(0);
+        }
+      } else {
+#pragma unroll
+        for (int u = 0; u < NU; ++u) {
+          const int e = LS ? ee - NU + u : eb + u;
+          const bool in = LS ? (e >= eb) : true;
+          ck[u] = in ? __ldg(a.c_col + e) : 0; cw[u] = in ? __ldg(a.c_val + e) : T(0);
+        }
+      }
+#pragma unroll
+      for (int u = 0; u < NU; ++u) {
+        const bool ok = LS ? (ee - NU + u >= eb && (uint32_t)ck[u] > row) : (eb + u < ee);
+        ck[u] = ok ? ck[u] : (int)row;
+        cw[u] = ok ? cw[u] : T(0);
       }
       if (LS) {
-        Row xk[kUN], dk[kUN];
+        Row xk[NU], dk[NU];
 #pragma unroll
-        for (int u = 0; u < kUN; ++u) {
-          row_ldg<FULL>(xk[u], a.X + (int64_t)ck[u] * ld, lane, nvec, r, exact);
-          row_ldg<FULL>(dk[u], a.X2 + (int64_t)ck[u] * ld, lane, nvec, r, exact);
+        for (int u = 0; u < NU; ++u) {
+          if (FULL) { row_ldg_b(xk[u], Xl + (uint64_t)(uint32_t)ck[u] * ldb, lmask); row_ldg_b(dk[u], X2l + (uint64_t)(uint32_t)ck[u] * ldb, lmask); }
+          else { xk[u].load(a.X + (int64_t)ck[u] * ld, lane, nvec, r, exact); dk[u].load(a.X2 + (int64_t)ck[u] * ld, lane, nvec, r, exact); }
         }
         const T rr_l = x.dot(x), rd_l = x.dot(d), dd_l = d.dot(d);
         const double rr = (double)gsum<GS>(rr_l), rd = (double)gsum<GS>(rd_l), dd = (double)gsum<GS>(dd_l);
@@ -270,36 +335,38 @@ __global__ void __launch_bounds__(kTiledThreads) k_rows_tiled(const RowArgs<T> a
         }
         T sRR = T(0), sRD = T(0), sDD = T(0);
 #pragma unroll
-        for (int u = 0; u < kUN; ++u) {
+        for (int u = 0; u < NU; ++u) {
           sRR = fma(cw[u], x.dot(xk[u]), sRR);
           sRD = fma(cw[u], x.dot(dk[u]) + d.dot(xk[u]), sRD);
           sDD = fma(cw[u], d.dot(dk[u]), sDD);
         }
-        for (int e = eb + kUN; e < ee; ++e) {   // rows with more than kUN neighbours
-          const int k = colp[e];
-          if ((int64_t)k > row) {
-            const T cv = valp[e];
-            Row xe, de;
-            row_ldg<FULL>(xe, a.X + (int64_t)k * ld, lane, nvec, r, exact);
-            row_ldg<FULL>(de, a.X2 + (int64_t)k * ld, lane, nvec, r, exact);
-            sRR = fma(cv, x.dot(xe), sRR);
-            sRD = fma(cv, x.dot(de) + d.dot(xe), sRD);
-            sDD = fma(cv, d.dot(de), sDD);
-          }
+        for (int e = ee - NU - 1; e >= eb; --e) {   // rows with more than NU upper neighbours
+          const int k = __ldg(a.c_col + e);
+          if ((uint32_t)k <= row) break;
+          const T cv = __ldg(a.c_val + e);
+          Row xe, de;
+          xe.load(a.X + (int64_t)k * ld, lane, nvec, r, exact);
+          de.load(a.X2 + (int64_t)k * ld, lane, nvec, r, exact);
+          sRR = fma(cv, x.dot(xe), sRR);
+          sRD = fma(cv, x.dot(de) + d.dot(xe), sRD);
+          sDD = fma(cv, d.dot(de), sDD);
         }
         st[LS_CRR] += (double)dc * (double)rr_l + 2.0 * (double)sRR;
         st[LS_CRD] += (double)dc * (double)rd_l + (double)sRD;
         st[LS_CDD] += (double)dc * (double)dd_l + 2.0 * (double)sDD;
       } else {
-        Row xn[kUN];
+        Row xn[NU];
 #pragma unroll
-        for (int u = 0; u < kUN; ++u) row_ldg<FULL>(xn[u], a.X + (int64_t)ck[u] * ld, lane, nvec, r, exact);
+        for (int u = 0; u < NU; ++u) {
+          if (FULL) row_ldg_b(xn[u], Xl + (uint64_t)(uint32_t)ck[u] * ldb, lmask);
+          else xn[u].load(a.X + (int64_t)ck[u] * ld, lane, nvec, r, exact);
+        }
         double coef;
         if (MODE == ROWS_FUSED_EVAL) {
-          const double z = (double)gsum<GS>(x.dot(x)), qv = z - bv, lam = yv - a.sigma * qv;
+          const double z = (double)gsum<GS>(x.dot(x)), qv = z - bv, lam = yv - sigma * qv;
           coef = lam;
           if (lane == 0) {
-            if (a.z) a.z[row] = z;
+            if (zout) zout[row] = z;
             st[ES_YQ] += yv * qv; st[ES_QQ] += qv * qv; st[ES_LZ] += lam * z;
           }
         } else {
@@ -311,24 +378,31 @@ __global__ void __launch_bounds__(kTiledThreads) k_rows_tiled(const RowArgs<T> a
 #pragma unroll
           for (int i = 0; i < VEC; ++i) acc.p[i2].v[i] = dc * x.p[i2].v[i];
 #pragma unroll
-        for (int u = 0; u < kUN; ++u) acc.axpy(cw[u], xn[u]);
+        for (int u = 0; u < NU; ++u) acc.axpy(cw[u], xn[u]);
         for (int e = eb + kUN; e < ee; ++e) {   // rows with more than kUN neighbours
-          Row xe; row_ldg<FULL>(xe, a.X + (int64_t)colp[e] * ld, lane, nvec, r, exact);
-          acc.axpy(valp[e], xe);
+          Row xe; xe.load(a.X + (int64_t)__ldg(a.c_col + e) * ld, lane, nvec, r, exact);
+          acc.axpy(__ldg(a.c_val + e), xe);
         }
         st[ES_CX] += (double)acc.dot(x);
         acc.axpy((T)(-coef), x);
-        const T sc = (T)a.scale;
 #pragma unroll
         for (int i2 = 0; i2 < NIT; ++i2)
 #pragma unroll
           for (int i = 0; i < VEC; ++i) acc.p[i2].v[i] *= sc;
         st[ES_GG] += (double)acc.dot(acc);
         st[ES_GR] += (double)acc.dot(x);
-        if (a.Out) row_stg<FULL>(acc, a.Out + row * ld, lane, nvec, r, exact);
+        if (Outl) {
+          if (FULL) {
+#pragma unroll
+            for (int i2 = 0; i2 < NIT; ++i2)
+              if (lmask & (1u << i2)) st_pack<T, VEC>(reinterpret_cast<T*>(Outl + (uint64_t)row * ldb) + i2 * GS * VEC, acc.p[i2]);
+          } else {
+            acc.store(a.Out + (int64_t)row * ld, lane, nvec, r, exact);
+          }
+        }
       }
       __syncwarp();
-      if (lane32 == 0) mbar_arrive(&empty[s]);   // this warp is done with stage s
+      if (lane32 == 0) mbar_arrive_addr(empty0 + s * 8u);   // this warp is done with stage s
     }
   }
   block_reduce_store_nw<NST, NCW + 1>(st, a.partials + (int64_t)blockIdx.x * kNStat);
