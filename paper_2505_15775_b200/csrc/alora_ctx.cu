@@ -159,15 +159,15 @@ template <typename T>
 alora_status launch_diag_rows(alora_ctx* c, int vec, int nvec, int exact, int shape, int mode, RowArgs<T>& a,
                               const void* dual, int* nparts) {
   const int gs = kShapes[shape].gs, nit = kShapes[shape].nit, tr = tile_rows(gs);
-  const int full = exact;   // no partially filled pack; idle lanes (nvec < gs*nit) are handled by a lane mask
-  (void)nit; (void)nvec;
+  // 0: last pack partially filled (tail masks); 1: exact packs, some lanes idle (lane mask); 2: exact, all lanes busy
+  const int full = !exact ? 0 : (nvec == gs * nit ? 2 : 1);
   const int64_t tiles = c->n / tr;
   bool elig = !c->dcons && !c->da && tiles > 0 && !((uintptr_t)a.X % 16) && !((uintptr_t)a.X2 % 16) && !((uintptr_t)dual % 16);
   int occ = 0;
   if (elig) {
     int& oc = c->occ_cache[vec_slot(vec)][shape][8 + mode];
     int64_t& key = c->occ_ld[vec_slot(vec)][shape][mode];
-    const int64_t want = a.ld * 2 + full;
+    const int64_t want = a.ld * 4 + full;
     if (!oc || key != want) { oc = occ_tiled(T(), vec, shape, mode, full, a.ld); key = want; if (!oc) oc = -1; }
     occ = oc;
     elig = occ > 0;

@@ -160,7 +160,7 @@ template <typename T, int VEC, int GS, int NIT>
 __device__ __forceinline__ void row_ldg_b(RowReg<T, VEC, GS, NIT>& x, const char* p, unsigned mask) {
 #pragma unroll
   for (int it = 0; it < NIT; ++it) {
-    if (mask & (1u << it)) x.p[it] = ldg_pack<T, VEC>(reinterpret_cast<const T*>(p) + it * GS * VEC);
+    if (mask == ~0u || (mask & (1u << it))) x.p[it] = ldg_pack<T, VEC>(reinterpret_cast<const T*>(p) + it * GS * VEC);
     else {
 #pragma unroll
       for (int i = 0; i < VEC; ++i) x.p[it].v[i] = T(0);
@@ -176,7 +176,7 @@ __host__ __device__ constexpr int tiled_min_blocks(int row_regs, int mode) {
 // Preconditions (checked by the host, which otherwise uses k_rows): the constraints are the identity
 // diagonal ones (dcons == da == nullptr), X / X2 / y (or w) are 16-byte aligned, and the kernel is
 // given FULL tiles only: it covers rows [0, a.tiles * TR); the ragged tail goes to k_rows.
-template <typename T, int VEC, int GS, int NIT, int MODE, bool FULL>
+template <typename T, int VEC, int GS, int NIT, int MODE, int FULL>
 __global__ void __launch_bounds__(kTiledThreads, tiled_min_blocks(VEC * NIT * (int)sizeof(T) / 4, MODE)) k_rows_tiled(const RowArgs<T> a) {
   using Row = RowReg<T, VEC, GS, NIT>;
   constexpr int TR = tile_rows(GS), CAP = tile_cap(GS), GPW = 32 / GS, NCW = kBlock / 32;
@@ -258,9 +258,9 @@ __global__ void __launch_bounds__(kTiledThreads, tiled_min_blocks(VEC * NIT * (i
     const char* X2l = LS ? reinterpret_cast<const char*>(a.X2) + loff : nullptr;
     char* Outl = a.Out ? reinterpret_cast<char*>(a.Out) + loff : nullptr;
     const uint32_t full0 = smem_u32(full), empty0 = smem_u32(empty);
-    unsigned lmask = 0;   // packs of a row owned by this lane
+    unsigned lmask = 0;   // packs of a row owned by this lane (FULL == 2: all of them, known at compile time)
 #pragma unroll
-    for (int i2 = 0; i2 < NIT; ++i2) if (lane + i2 * GS < nvec) lmask |= 1u << i2;
+    for (int i2 = 0; i2 < NIT; ++i2) if (FULL == 2 || lane + i2 * GS < nvec) lmask |= 1u << i2;
     double* const zout = a.z;
     const double sigma = a.sigma;
     const T sc = (T)a.scale;
@@ -272,11 +272,10 @@ __global__ void __launch_bounds__(kTiledThreads, tiled_min_blocks(VEC * NIT * (i
       const unsigned char* sb = smem_raw + s * stage_sz;
       Row x, d;
       if (FULL) {
-        x.zero();
-        if (LS) d.zero();
+        if (FULL != 2) { x.zero(); if (LS) d.zero(); }
 #pragma unroll
         for (int i2 = 0; i2 < NIT; ++i2)
-          if (lmask & (1u << i2)) {
+          if (FULL == 2 || (lmask & (1u << i2))) {
             x.p[i2] = *reinterpret_cast<const Pack<T, VEC>*>(sb + xoff + loff + i2 * GS * VEC * sizeof(T));
             if (LS) d.p[i2] = *reinterpret_cast<const Pack<T, VEC>*>(sb + xbytes + xoff + loff + i2 * GS * VEC * sizeof(T));
           }
@@ -322,7 +321,7 @@ __global__ void __launch_bounds__(kTiledThreads, tiled_min_blocks(VEC * NIT * (i
         Row xk[NU], dk[NU];
 #pragma unroll
         for (int u = 0; u < NU; ++u) {
-          if (FULL) { row_ldg_b(xk[u], Xl + (uint64_t)(uint32_t)ck[u] * ldb, lmask); row_ldg_b(dk[u], X2l + (uint64_t)(uint32_t)ck[u] * ldb, lmask); }
+          if (FULL) { row_ldg_b(xk[u], Xl + (uint64_t)(uint32_t)ck[u] * ldb, FULL == 2 ? ~0u : lmask); row_ldg_b(dk[u], X2l + (uint64_t)(uint32_t)ck[u] * ldb, FULL == 2 ? ~0u : lmask); }
           else { xk[u].load(a.X + (int64_t)ck[u] * ld, lane, nvec, r, exact); dk[u].load(a.X2 + (int64_t)ck[u] * ld, lane, nvec, r, exact); }
         }
         const T rr_l = x.dot(x), rd_l = x.dot(d), dd_l = d.dot(d);
@@ -358,7 +357,7 @@ __global__ void __launch_bounds__(kTiledThreads, tiled_min_blocks(VEC * NIT * (i
         Row xn[NU];
 #pragma unroll
         for (int u = 0; u < NU; ++u) {
-          if (FULL) row_ldg_b(xn[u], Xl + (uint64_t)(uint32_t)ck[u] * ldb, lmask);
+          if (FULL) row_ldg_b(xn[u], Xl + (uint64_t)(uint32_t)ck[u] * ldb, FULL == 2 ? ~0u : lmask);
           else xn[u].load(a.X + (int64_t)ck[u] * ld, lane, nvec, r, exact);
         }
         double coef;
@@ -395,7 +394,7 @@ __global__ void __launch_bounds__(kTiledThreads, tiled_min_blocks(VEC * NIT * (i
           if (FULL) {
 #pragma unroll
             for (int i2 = 0; i2 < NIT; ++i2)
-              if (lmask & (1u << i2)) st_pack<T, VEC>(reinterpret_cast<T*>(Outl + (uint64_t)row * ldb) + i2 * GS * VEC, acc.p[i2]);
+              if (FULL == 2 || (lmask & (1u << i2))) st_pack<T, VEC>(reinterpret_cast<T*>(Outl + (uint64_t)row * ldb) + i2 * GS * VEC, acc.p[i2]);
           } else {
             acc.store(a.Out + (int64_t)row * ld, lane, nvec, r, exact);
           }
