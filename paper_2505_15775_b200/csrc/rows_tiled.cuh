@@ -170,7 +170,7 @@ __device__ __forceinline__ void row_ldg_b(RowReg<T, VEC, GS, NIT>& x, const char
 
 // occupancy target by the number of 32-bit registers one row vector takes per lane
 __host__ __device__ constexpr int tiled_min_blocks(int row_regs, int mode) {
-  return row_regs <= 4 ? (mode == ROWS_LS_FUSED ? 2 : 4) : row_regs <= 8 ? 2 : 1;
+  return row_regs <= 4 ? (mode == ROWS_LS_FUSED ? 3 : 4) : row_regs <= 8 ? 2 : 1;
 }
 
 // Preconditions (checked by the host, which otherwise uses k_rows): the constraints are the identity
@@ -182,6 +182,7 @@ __global__ void __launch_bounds__(kTiledThreads, tiled_min_blocks(VEC * NIT * (i
   constexpr int TR = tile_rows(GS), CAP = tile_cap(GS), GPW = 32 / GS, NCW = kBlock / 32;
   constexpr int NST = (MODE == ROWS_LS_FUSED) ? 12 : 6;
   constexpr bool LS = (MODE == ROWS_LS_FUSED);
+  constexpr int NSL = (LS && GS >= 4) ? 6 : NST;   // accumulators kept in the loop (line search spreads the 9 q-sums over lanes)
   extern __shared__ __align__(16) unsigned char smem_raw[];
   __shared__ uint64_t full[kStages], empty[kStages];
   __shared__ int s_ea[kStages], s_fit[kStages];
@@ -205,9 +206,9 @@ __global__ void __launch_bounds__(kTiledThreads, tiled_min_blocks(VEC * NIT * (i
   }
   __syncthreads();
 
-  double st[NST];
+  double st[NSL];
 #pragma unroll
-  for (int s = 0; s < NST; ++s) st[s] = 0.0;
+  for (int s = 0; s < NSL; ++s) st[s] = 0.0;
 
   if (warp == NCW) {
     // ================= producer warp: lane j pre-loads the CSR bounds of the j-th upcoming tile ==========
@@ -326,19 +327,25 @@ __global__ void __launch_bounds__(kTiledThreads, tiled_min_blocks(VEC * NIT * (i
         }
         const T rr_l = x.dot(x), rd_l = x.dot(d), dd_l = d.dot(d);
         const double rr = (double)gsum<GS>(rr_l), rd = (double)gsum<GS>(rd_l), dd = (double)gsum<GS>(dd_l);
-        if (lane == 0) {
-          const double qv = rr - bv, q1 = 2.0 * rd, q2 = dd;
+        const double qv = rr - bv, q1 = 2.0 * rd, q2 = dd;
+        if (GS >= 4) {
+          // every lane knows y, q, q1, q2; lanes 0, 1, 2 of the group own three of the nine sums each
+          // (lane 0: y.q y.q1 y.q2, lane 1: q.q q.q1 q.q2, lane 2: q1.q1 q1.q2 q2.q2) -> 3 accumulators per thread
+          const double A = lane == 0 ? yv : qv;
+          const double a0 = lane == 2 ? q1 : A, b0 = lane == 2 ? q1 : qv;
+          const double a1 = lane == 2 ? q1 : A, b1 = lane == 2 ? q2 : q1;
+          const double a2 = lane == 2 ? q2 : A;
+          if (lane < 3) { st[3] += a0 * b0; st[4] += a1 * b1; st[5] += a2 * q2; }
+        } else if (lane == 0) {
           st[LS_YQ] += yv * qv; st[LS_YQ1] += yv * q1; st[LS_YQ2] += yv * q2;
           st[LS_QQ] += qv * qv; st[LS_QQ1] += qv * q1; st[LS_QQ2] += qv * q2;
           st[LS_Q11] += q1 * q1; st[LS_Q12] += q1 * q2; st[LS_Q22] += q2 * q2;
         }
-        T sRR = T(0), sRD = T(0), sDD = T(0);
+        // u = sum_k c_k R_k, w = sum_k c_k D_k over the upper neighbours; then <C,.> row sums are
+        // x.u, x.w + d.u, d.w  (8 FMAs per neighbour instead of 16)
+        Row uacc, wacc; uacc.zero(); wacc.zero();
 #pragma unroll
-        for (int u = 0; u < NU; ++u) {
-          sRR = fma(cw[u], x.dot(xk[u]), sRR);
-          sRD = fma(cw[u], x.dot(dk[u]) + d.dot(xk[u]), sRD);
-          sDD = fma(cw[u], d.dot(dk[u]), sDD);
-        }
+        for (int u = 0; u < NU; ++u) { uacc.axpy(cw[u], xk[u]); wacc.axpy(cw[u], dk[u]); }
         for (int e = ee - NU - 1; e >= eb; --e) {   // rows with more than NU upper neighbours
           const int k = __ldg(a.c_col + e);
           if ((uint32_t)k <= row) break;
@@ -346,10 +353,9 @@ __global__ void __launch_bounds__(kTiledThreads, tiled_min_blocks(VEC * NIT * (i
           Row xe, de;
           xe.load(a.X + (int64_t)k * ld, lane, nvec, r, exact);
           de.load(a.X2 + (int64_t)k * ld, lane, nvec, r, exact);
-          sRR = fma(cv, x.dot(xe), sRR);
-          sRD = fma(cv, x.dot(de) + d.dot(xe), sRD);
-          sDD = fma(cv, d.dot(de), sDD);
+          uacc.axpy(cv, xe); wacc.axpy(cv, de);
         }
+        const T sRR = x.dot(uacc), sRD = x.dot(wacc) + d.dot(uacc), sDD = d.dot(wacc);
         st[LS_CRR] += (double)dc * (double)rr_l + 2.0 * (double)sRR;
         st[LS_CRD] += (double)dc * (double)rd_l + (double)sRD;
         st[LS_CDD] += (double)dc * (double)dd_l + 2.0 * (double)sDD;
@@ -404,7 +410,20 @@ __global__ void __launch_bounds__(kTiledThreads, tiled_min_blocks(VEC * NIT * (i
       if (lane32 == 0) mbar_arrive_addr(empty0 + s * 8u);   // this warp is done with stage s
     }
   }
-  block_reduce_store_nw<NST, NCW + 1>(st, a.partials + (int64_t)blockIdx.x * kNStat);
+  if (LS && GS >= 4) {
+    double full_st[NST];
+    const int gl = (threadIdx.x & 31) % GS;
+#pragma unroll
+    for (int k = 0; k < 3; ++k) full_st[k] = st[k];
+#pragma unroll
+    for (int k = 0; k < 9; ++k) full_st[3 + k] = (warp != NCW && gl == k / 3) ? st[3 + k % 3] : 0.0;
+    block_reduce_store_nw<NST, NCW + 1>(full_st, a.partials + (int64_t)blockIdx.x * kNStat);
+  } else {
+    double full_st[NST];
+#pragma unroll
+    for (int k = 0; k < NST; ++k) full_st[k] = st[k < NSL ? k : 0];
+    block_reduce_store_nw<NST, NCW + 1>(full_st, a.partials + (int64_t)blockIdx.x * kNStat);
+  }
 }
 
 }  // namespace alora
