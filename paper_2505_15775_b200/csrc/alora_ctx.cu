@@ -159,10 +159,11 @@ template <typename T>
 alora_status launch_diag_rows(alora_ctx* c, int vec, int nvec, int exact, int shape, int mode, RowArgs<T>& a,
                               const void* dual, int* nparts) {
   const int gs = kShapes[shape].gs, nit = kShapes[shape].nit, tr = tile_rows(gs);
-  // 0: last pack partially filled (tail masks); 1: exact packs, some lanes idle (lane mask); 2: exact, all lanes busy
-  const int full = !exact ? 0 : (nvec == gs * nit ? 2 : 1);
+  // 1: whole packs, some lanes of a group idle (lane mask); 2: whole packs, all lanes busy.  Rows whose last
+  // pack is partially filled (r not a multiple of the vector width) take k_rows.
+  const int full = nvec == gs * nit ? 2 : 1;
   const int64_t tiles = c->n / tr;
-  bool elig = !c->dcons && !c->da && tiles > 0 && !((uintptr_t)a.X % 16) && !((uintptr_t)a.X2 % 16) && !((uintptr_t)dual % 16);
+  bool elig = c->ell_col && exact && tiles > 0 && !((uintptr_t)a.X % 16) && !((uintptr_t)a.X2 % 16) && !((uintptr_t)dual % 16);
   int occ = 0;
   if (elig) {
     int& oc = c->occ_cache[vec_slot(vec)][shape][8 + mode];
@@ -224,6 +225,7 @@ template <typename T> void fill_rows(alora_ctx* c, RowArgs<T>& a, const Geo& g, 
   a.y = c->y; a.b = c->b; a.sigma = c->sigma; a.w = nullptr; a.z = nullptr;
   a.pC = 0; a.U = (const T*)c->U; a.Ts = c->Ts; a.scale = 1.0; a.diag_class = (c->cls == 0);
   a.partials = c->part_rows; a.row_begin = 0; a.tiles = 0;
+  a.ell_col = c->ell_col; a.ell_val = (const T*)c->ell_val; a.rem32 = c->rem32;
 }
 template <typename T> void fill_cons(alora_ctx* c, ConsArgs<T>& a, const Geo& g, const T* X, const T* X2, int r, int64_t ld) {
   a.n = c->n; a.r = r; a.ld = ld; a.nvec = g.nvec; a.exact = g.exact; a.X = X; a.X2 = X2; a.m = c->m;
@@ -319,6 +321,7 @@ template <typename T> alora_status ls_impl(alora_ctx* c, const T* R, const T* D,
     RowArgs<T> a;
     fill_rows(c, a, g, R, r, ld);
     a.X2 = D;
+    a.ell_col = c->ellu_col; a.ell_val = (const T*)c->ellu_val; a.rem32 = c->remu32;
     int nparts = 0;
     s = launch_diag_rows<T>(c, g.vec, g.nvec, g.exact, g.shape, ROWS_LS_FUSED, a, c->y, &nparts);
     if (s != ALORA_OK) return s;
@@ -427,8 +430,10 @@ extern "C" alora_status alora_get_stats(alora_ctx* c, double stats[8]) {
 }
 
 extern "C" alora_status alora_get_lambda(alora_ctx* c, double* lam_dev) {
-  if (!c || !lam_dev) return ALORA_EINVAL;
+  if (!c) return ALORA_EINVAL;
+  if (!lam_dev && c->m > 0) return fail(c, ALORA_EINVAL, "alora_get_lambda: lam_dev is NULL");
   if (!c->have_eval) return fail(c, ALORA_ESTATE, "alora_get_lambda before alora_eval");
+  if (c->m == 0) return ALORA_OK;
   const int grid = (int)std::max<int64_t>(1, std::min<int64_t>((c->m + 255) / 256, (int64_t)c->num_sms * 8));
   k_lambda<<<grid, 256, 0, c->stream>>>(c->m, c->y, c->z_last, c->b, c->sigma, lam_dev);
   c->launches++;

@@ -51,6 +51,10 @@ struct alora_ctx {
   int64_t c_nnz = 0;
   // diagonal class: constraint of row j (-1: none) and its coefficient; null = identity / ones
   int* dcons = nullptr; void* da = nullptr;
+  // identity diagonal class: padded ELL blocks (rows_tiled.cuh): kUN first neighbours per row, kUNL last
+  // upper-triangle neighbours per row, and per 32-row block a flag "some row has more"
+  int* ell_col = nullptr; void* ell_val = nullptr; unsigned char* rem32 = nullptr;
+  int* ellu_col = nullptr; void* ellu_val = nullptr; unsigned char* remu32 = nullptr;
   // general class: row-oriented full pattern of the constraints
   int* a_rowptr = nullptr; int* a_col = nullptr; void* a_val = nullptr; int* a_cons = nullptr;
   int64_t a_nnz = 0;

@@ -24,6 +24,8 @@ namespace alora {
 constexpr int kBlock = 256;
 constexpr int kLongThreshold = 128;  // constraints with more stored entries are split into chunks
 constexpr int kChunk = 64;           // entries per chunk of a long constraint
+constexpr int kUN = 4;               // diagonal class: ELL slots per row (first neighbours), see rows_tiled.cuh
+constexpr int kUNL = 3;              // diagonal class, line search: ELL slots per row (last upper-triangle neighbours)
 
 enum RowsMode { ROWS_FUSED_EVAL = 0, ROWS_ADJ = 1, ROWS_LS_FUSED = 2 };
 enum ConsMode { CONS_EVAL = 0, CONS_LS = 1 };
@@ -51,6 +53,10 @@ template <typename T> struct RowArgs {
   double* partials;  // [gridDim.x][kNStat]
   int64_t row_begin; // k_rows: first row handled (rows [row_begin, n))
   int64_t tiles;     // k_rows_tiled: number of full row tiles handled (rows [0, tiles * TR))
+  // k_rows_tiled: padded ELL block of the mode (kUN first neighbours, or kUNL last upper-triangle neighbours
+  // for the line search): slot u of row j at [j * NU + u]; rem32[j / 32] != 0: some row of that 32-row block
+  // has more neighbours than slots (walk the CSR tail)
+  const int* ell_col; const T* ell_val; const unsigned char* rem32;
 };
 
 template <typename T> struct ConsArgs {
@@ -405,6 +411,8 @@ __host__ inline int shape_index(int nvec) {
   if (nvec <= 1) return 0; if (nvec <= 2) return 1; if (nvec <= 4) return 2; if (nvec <= 8) return 3;
   if (nvec <= 16) return 4; if (nvec <= 32) return 5; if (nvec <= 64) return 6; return -1;
 }
-constexpr Shape kShapes[7] = {{1, 1}, {2, 1}, {4, 1}, {8, 1}, {8, 2}, {16, 2}, {16, 4}};
+// few lanes per row: the per-row bookkeeping (addresses, scalars, fp64 sums) is issued once per group, so
+// fewer lanes per row means fewer warp instructions per row; a lane holds up to 4 packs
+constexpr Shape kShapes[7] = {{1, 1}, {2, 1}, {4, 1}, {4, 2}, {8, 2}, {8, 4}, {16, 4}};
 
 }  // namespace alora

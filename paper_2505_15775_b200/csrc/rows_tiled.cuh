@@ -1,42 +1,44 @@
 // rows_tiled.cuh -- the row kernel of the "diagonal" constraint class (MaxCut), B200 design.
 //
-// What the first design (k_rows) got wrong on B200 (profiles/r1a_*): per row it chains three
-// dependent global loads (rowptr -> col/val -> neighbour row) and keeps too few bytes in flight, so
-// the pass is latency bound at 0.34 of the HBM roofline while moving only the algorithmic bytes.
+// History (profiles/): the first design (k_rows) chained three dependent global loads per row (rowptr ->
+// col/val -> neighbour row) and ran at 0.34 of the HBM roofline; staging the CSR slices through shared
+// memory with bulk copies brought 0.58, limited then by instruction issue: ~30 warp instructions per row,
+// most of them address arithmetic, slot-validity tests and re-derived stage offsets (profiles/r1b_*).
 //
-// Here every *streaming* input of a row tile -- the tile's rows of X (and D), its slices of dC, y, b
-// (or the weights w) and of the CSR (rowptr, col, val) -- is brought into shared memory by 1-D bulk
-// async copies (cp.async.bulk, SASS UBLKCP) issued by a dedicated producer warp into a ring of
-// kStages stages, completion signalled on mbarriers (full / empty), so tens of KB per block are in
-// flight to HBM independently of what the consumer warps are doing.  The 8 consumer warps read the
-// tile from shared memory, issue all neighbour-row gathers (the only dependent global access left;
-// they mostly hit L2) before the first FMA, write the output row with 16-byte stores and release the
-// stage per warp -- there is no block-wide barrier inside the tile loop.  Loop trip counts are
-// warp-uniform, so sub-warp reductions use full-mask shuffles.  Sums across rows are fp64, ordered,
-// two-stage as in kernels.cuh.
+// This version removes that bookkeeping from the hot loop:
+//   * the first kUN neighbours of every row (and, for the line search, its last kUNL upper-triangle ones) are
+//     kept in a padded ELL block built once in alora_create: fixed-size (col, val) slots per row, an unused
+//     slot holding (the row itself, 0).  The slots of a row tile are one contiguous slice, so they arrive by
+//     bulk copy with no alignment fix-up, and the consumer needs no rowptr, no bounds and no validity test.
+//     Rows with more neighbours than slots are flagged per 32-row block; only flagged tiles walk the CSR tail.
+//   * every *streaming* input of a row tile -- its rows of X (and D), dC, y, b (or the weights w) and the ELL
+//     slots -- is brought into shared memory by 1-D bulk async copies (cp.async.bulk, SASS UBLKCP) issued by a
+//     dedicated producer warp into a ring of kStages stages, completion signalled on mbarriers (full / empty),
+//     so tens of KB per block are in flight to HBM independently of what the consumer warps are doing.
+//   * a neighbour that is one of the tile's own rows (grid / ring neighbours j +- 1, every unused slot) is read
+//     from the staged tile; the others are gathered from global memory (mostly L2 hits), all gathers of a row
+//     issued before its first FMA.
+// The 8 consumer warps release a stage per warp -- there is no block-wide barrier inside the tile loop.
+// Loop trip counts are warp-uniform, so sub-warp reductions use full-mask shuffles.  Sums across rows are
+// fp64, ordered, two-stage as in kernels.cuh.
 #pragma once
 #include "kernels.cuh"
 
 namespace alora {
 
 constexpr int kStages = 4;            // tiles in flight per block
-constexpr int kUN = 4;                // neighbours gathered up front per row
-constexpr int kUNL = 3;               // line search: upper-triangle neighbours gathered up front per row
 constexpr int kTiledThreads = kBlock + 32;   // 8 consumer warps + 1 producer warp
 
 __host__ __device__ constexpr int tile_rows(int gs) { return kBlock / gs; }   // one row per group per tile
-__host__ __device__ constexpr int tile_cap(int gs) {   // CSR entries staged per tile (denser tiles read global memory)
-  return tile_rows(gs) * 8 > 256 ? tile_rows(gs) * 8 : 256;
-}
-// per-stage shared memory: [X tile][D tile (line search)][dC][y|w][b][rowptr][col][val], 16-byte aligned pieces
+// per-stage shared memory: [X tile][D tile (line search)][dC][y|w][b][ELL col][ELL val], 16-byte aligned pieces
 __host__ __device__ inline size_t tiled_stage_bytes(int gs, int esz, int64_t ld, int mode) {
-  const size_t tr = tile_rows(gs), cap = tile_cap(gs);
+  const size_t tr = tile_rows(gs), nu = (mode == ROWS_LS_FUSED ? kUNL : kUN);
   size_t b = tr * (size_t)ld * esz * (mode == ROWS_LS_FUSED ? 2 : 1);
   b = (b + 15) & ~(size_t)15;
   b += tr * esz;                 // dC
   b = (b + 15) & ~(size_t)15;
   b += tr * 8 * 2;               // y (or w), b
-  b += (tr + 4) * 4 + cap * 4 + cap * esz;
+  b += tr * nu * 4 + tr * nu * esz;
   return (b + 15) & ~(size_t)15;
 }
 __host__ __device__ inline size_t tiled_smem_bytes(int gs, int esz, int64_t ld, int mode) {
@@ -168,36 +170,56 @@ __device__ __forceinline__ void row_ldg_b(RowReg<T, VEC, GS, NIT>& x, const char
   }
 }
 
-// occupancy target by the number of 32-bit registers one row vector takes per lane
+
+// occupancy target by the number of 32-bit registers one row vector takes per lane: the consumer loop keeps
+// its addresses and stage offsets in registers (75 at 3 blocks / SM) instead of re-deriving them per tile
 __host__ __device__ constexpr int tiled_min_blocks(int row_regs, int mode) {
-  return row_regs <= 4 ? (mode == ROWS_LS_FUSED ? 3 : 4) : row_regs <= 8 ? 2 : 1;
+  return row_regs <= 4 ? 3 : row_regs <= 8 ? 2 : 1;
 }
 
-// Preconditions (checked by the host, which otherwise uses k_rows): the constraints are the identity
-// diagonal ones (dcons == da == nullptr), X / X2 / y (or w) are 16-byte aligned, and the kernel is
-// given FULL tiles only: it covers rows [0, a.tiles * TR); the ragged tail goes to k_rows.
+// row vector of a neighbour: from the staged tile when the neighbour is one of the tile's own rows, else gathered
+// from global memory.  sp / gp point at the lane's first pack of that row; mask: packs owned by the lane.
+template <typename T, int VEC, int GS, int NIT>
+__device__ __forceinline__ void row_nbr(RowReg<T, VEC, GS, NIT>& x, bool loc, const unsigned char* sp, const char* gp, unsigned mask) {
+#pragma unroll
+  for (int it = 0; it < NIT; ++it) {
+    if (mask == ~0u || (mask & (1u << it))) {
+      if (loc) x.p[it] = *reinterpret_cast<const Pack<T, VEC>*>(sp + it * GS * VEC * sizeof(T));
+      else x.p[it] = ldg_pack<T, VEC>(reinterpret_cast<const T*>(gp) + it * GS * VEC);
+    } else {
+#pragma unroll
+      for (int i = 0; i < VEC; ++i) x.p[it].v[i] = T(0);
+    }
+  }
+}
+
+// Preconditions (checked by the host, which otherwise uses k_rows): the constraints are the identity diagonal
+// ones (dcons == da == nullptr, ELL block present), rows are whole packs (r == nvec * VEC), X / X2 / y (or w)
+// are 16-byte aligned, and the kernel is given FULL tiles only: it covers rows [0, a.tiles * TR); the ragged
+// tail goes to k_rows.  FULL: 1 = some lanes of a group own no pack (lane mask), 2 = all lanes busy.
 template <typename T, int VEC, int GS, int NIT, int MODE, int FULL>
 __global__ void __launch_bounds__(kTiledThreads, tiled_min_blocks(VEC * NIT * (int)sizeof(T) / 4, MODE)) k_rows_tiled(const RowArgs<T> a) {
   using Row = RowReg<T, VEC, GS, NIT>;
-  constexpr int TR = tile_rows(GS), CAP = tile_cap(GS), GPW = 32 / GS, NCW = kBlock / 32;
+  constexpr int TR = tile_rows(GS), GPW = 32 / GS, NCW = kBlock / 32;
   constexpr int NST = (MODE == ROWS_LS_FUSED) ? 12 : 6;
   constexpr bool LS = (MODE == ROWS_LS_FUSED);
+  constexpr int NU = LS ? kUNL : kUN;
   constexpr int NSL = (LS && GS >= 4) ? 6 : NST;   // accumulators kept in the loop (line search spreads the 9 q-sums over lanes)
+  constexpr int ESZ = (int)sizeof(T);
   extern __shared__ __align__(16) unsigned char smem_raw[];
   __shared__ uint64_t full[kStages], empty[kStages];
-  __shared__ int s_ea[kStages], s_fit[kStages];
+  __shared__ int s_rem[kStages];
   const int warp = threadIdx.x >> 5, lane32 = threadIdx.x & 31;
   const int nvec = a.nvec, r = a.r, exact = a.exact;
   const int64_t ld = a.ld;
   const int64_t ntiles = a.tiles;
 
   // stage layout (must match tiled_stage_bytes)
-  const uint32_t xbytes = (uint32_t)(TR * ld * sizeof(T));
+  const uint32_t xbytes = (uint32_t)(TR * ld * ESZ);
   const uint32_t off_dc = (xbytes * (LS ? 2u : 1u) + 15u) & ~15u;
-  const uint32_t off_y = (off_dc + TR * (uint32_t)sizeof(T) + 15u) & ~15u;
-  const uint32_t off_b = off_y + TR * 8, off_rp = off_b + TR * 8, off_col = off_rp + (TR + 4) * 4;
-  const uint32_t off_val = off_col + CAP * 4;
-  const uint32_t stage_sz = (off_val + CAP * (uint32_t)sizeof(T) + 15u) & ~15u;
+  const uint32_t off_y = (off_dc + TR * (uint32_t)ESZ + 15u) & ~15u;
+  const uint32_t off_b = off_y + TR * 8, off_ec = off_b + TR * 8, off_ev = off_ec + TR * NU * 4;
+  const uint32_t stage_sz = (off_ev + TR * NU * (uint32_t)ESZ + 15u) & ~15u;
 
   if (threadIdx.x == 0) {
     for (int s = 0; s < kStages; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], NCW); }
@@ -211,15 +233,21 @@ __global__ void __launch_bounds__(kTiledThreads, tiled_min_blocks(VEC * NIT * (i
   for (int s = 0; s < NSL; ++s) st[s] = 0.0;
 
   if (warp == NCW) {
-    // ================= producer warp: lane j pre-loads the CSR bounds of the j-th upcoming tile ==========
+    // ================= producer warp: lane j pre-loads the remainder flags of the j-th upcoming tile ==========
     const int64_t my_tiles = ntiles > blockIdx.x ? (ntiles - blockIdx.x + gridDim.x - 1) / gridDim.x : 0;
+    const uint32_t bytes = xbytes * (LS ? 2u : 1u) + TR * (uint32_t)ESZ + TR * 8u * (MODE == ROWS_ADJ ? 1u : 2u) +
+                           TR * NU * (4u + (uint32_t)ESZ);
     for (int64_t base = 0; base < my_tiles; base += 32) {
       const int64_t tj = (int64_t)blockIdx.x + (base + lane32) * gridDim.x;
-      int e0 = 0, e1 = 0;
-      if (tj < ntiles) { e0 = __ldg(a.c_rowptr + tj * TR); e1 = __ldg(a.c_rowptr + tj * TR + TR); }
+      int rem = 0;
+      if (tj < ntiles) {
+        const int64_t b0 = (tj * TR) >> 5;
+#pragma unroll
+        for (int k = 0; k < (TR >= 32 ? TR / 32 : 1); ++k) rem |= a.rem32[b0 + k];
+      }
       const int cnt = (int)min((int64_t)32, my_tiles - base);
       for (int j = 0; j < cnt; ++j) {
-        const int e0j = __shfl_sync(0xffffffffu, e0, j), e1j = __shfl_sync(0xffffffffu, e1, j);
+        const int remj = __shfl_sync(0xffffffffu, rem, j);
         if (lane32 == 0) {
           const int64_t it = base + j;
           const int s = (int)(it % kStages);
@@ -227,103 +255,65 @@ __global__ void __launch_bounds__(kTiledThreads, tiled_min_blocks(VEC * NIT * (i
           const int64_t t0 = ((int64_t)blockIdx.x + it * gridDim.x) * TR;
           mbar_wait(&empty[s], ph ^ 1u);
           unsigned char* sb = smem_raw + (size_t)s * stage_sz;
-          const int ea = e0j & ~3, cnt4 = (e1j - ea + 3) & ~3;
-          const bool fit = cnt4 <= CAP;
-          const uint32_t cv = (fit && cnt4) ? (uint32_t)cnt4 : 0u;
-          const uint32_t rp_bytes = (TR + 4) * 4;
-          const uint32_t bytes = rp_bytes + cv * 4u + cv * (uint32_t)sizeof(T) + xbytes * (LS ? 2u : 1u) +
-                                 TR * (uint32_t)sizeof(T) + TR * 8u * (MODE == ROWS_ADJ ? 1u : 2u);
-          s_ea[s] = ea; s_fit[s] = fit;
+          s_rem[s] = remj;
           mbar_expect_tx(&full[s], bytes);
           bulk_g2s(sb, a.X + t0 * ld, xbytes, &full[s]);
           if (LS) bulk_g2s(sb + xbytes, a.X2 + t0 * ld, xbytes, &full[s]);
-          bulk_g2s(sb + off_dc, a.dC + t0, TR * (uint32_t)sizeof(T), &full[s]);
+          bulk_g2s(sb + off_dc, a.dC + t0, TR * (uint32_t)ESZ, &full[s]);
           bulk_g2s(sb + off_y, (MODE == ROWS_ADJ ? a.w : a.y) + t0, TR * 8u, &full[s]);
           if (MODE != ROWS_ADJ) bulk_g2s(sb + off_b, a.b + t0, TR * 8u, &full[s]);
-          bulk_g2s(sb + off_rp, a.c_rowptr + t0, rp_bytes, &full[s]);
-          if (cv) {
-            bulk_g2s(sb + off_col, a.c_col + ea, cv * 4u, &full[s]);
-            bulk_g2s(sb + off_val, a.c_val + ea, cv * (uint32_t)sizeof(T), &full[s]);
-          }
+          bulk_g2s(sb + off_ec, a.ell_col + t0 * NU, TR * NU * 4u, &full[s]);
+          bulk_g2s(sb + off_ev, a.ell_val + t0 * NU, TR * NU * (uint32_t)ESZ, &full[s]);
         }
       }
     }
   } else {
     // ================= consumer warps ======================================================================
+    // Loop invariants are computed once: the lane's byte offsets into a stage, the global base pointers already
+    // offset to the lane's first pack, the barrier addresses.  Stage index / parity / base advance incrementally.
     const int lane = lane32 % GS;
     const int lr = warp * GPW + lane32 / GS;           // row of the tile handled by this group
-    const uint32_t ldb = (uint32_t)(ld * sizeof(T));   // row pitch in bytes
-    const uint32_t xoff = (uint32_t)lr * ldb;
-    const uint32_t loff = (uint32_t)(lane * VEC * sizeof(T));
-    const char* Xl = reinterpret_cast<const char*>(a.X) + loff;    // lane's first pack of row 0
-    const char* X2l = LS ? reinterpret_cast<const char*>(a.X2) + loff : nullptr;
-    char* Outl = a.Out ? reinterpret_cast<char*>(a.Out) + loff : nullptr;
+    const uint32_t ldb = (uint32_t)(ld * ESZ);         // row pitch in bytes
+    const uint32_t loff = (uint32_t)(lane * VEC * ESZ);
+    const uint32_t xme = (uint32_t)lr * ldb + loff;    // this lane's first pack inside a staged X tile
+    const char* const Xl = reinterpret_cast<const char*>(a.X) + loff;    // lane's first pack of row 0
+    const char* const X2l = LS ? reinterpret_cast<const char*>(a.X2) + loff : nullptr;
+    char* const Outl = a.Out ? reinterpret_cast<char*>(a.Out) + loff : nullptr;
     const uint32_t full0 = smem_u32(full), empty0 = smem_u32(empty);
     unsigned lmask = 0;   // packs of a row owned by this lane (FULL == 2: all of them, known at compile time)
 #pragma unroll
     for (int i2 = 0; i2 < NIT; ++i2) if (FULL == 2 || lane + i2 * GS < nvec) lmask |= 1u << i2;
+    const unsigned pmask = FULL == 2 ? ~0u : lmask;
     double* const zout = a.z;
     const double sigma = a.sigma;
     const T sc = (T)a.scale;
-    uint32_t it = 0;
-    for (int64_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x, ++it) {
-      const uint32_t s = it % kStages, ph = (it / kStages) & 1u;
-      const uint32_t row = (uint32_t)(tile * TR) + (uint32_t)lr;
+    uint32_t s = 0, ph = 0;
+    const unsigned char* sb = smem_raw;
+    for (int64_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+      const uint32_t row0 = (uint32_t)(tile * TR), row = row0 + (uint32_t)lr;
       mbar_wait_addr(full0 + s * 8u, ph);
-      const unsigned char* sb = smem_raw + s * stage_sz;
       Row x, d;
-      if (FULL) {
-        if (FULL != 2) { x.zero(); if (LS) d.zero(); }
-#pragma unroll
-        for (int i2 = 0; i2 < NIT; ++i2)
-          if (FULL == 2 || (lmask & (1u << i2))) {
-            x.p[i2] = *reinterpret_cast<const Pack<T, VEC>*>(sb + xoff + loff + i2 * GS * VEC * sizeof(T));
-            if (LS) d.p[i2] = *reinterpret_cast<const Pack<T, VEC>*>(sb + xbytes + xoff + loff + i2 * GS * VEC * sizeof(T));
-          }
-      } else {
-        load_row_smem(x, reinterpret_cast<const T*>(sb + xoff), lane, nvec, r, exact);
-        if (LS) load_row_smem(d, reinterpret_cast<const T*>(sb + xbytes + xoff), lane, nvec, r, exact);
-      }
+      row_nbr(x, true, sb + xme, nullptr, pmask);
+      if (LS) row_nbr(d, true, sb + xbytes + xme, nullptr, pmask);
       const T dc = reinterpret_cast<const T*>(sb + off_dc)[lr];
       const double yv = reinterpret_cast<const double*>(sb + off_y)[lr];
       const double bv = (MODE != ROWS_ADJ) ? reinterpret_cast<const double*>(sb + off_b)[lr] : 0.0;
-      const int* rp = reinterpret_cast<const int*>(sb + off_rp);
-      const int eb = rp[lr], ee = rp[lr + 1];
-      const bool fit = s_fit[s] != 0;
-      // first neighbours: missing ones become (own row, weight 0), so the gathers are unconditional.
-      // Line search walks the row's list from its END: columns ascend, so the upper triangle (col > row,
-      // each off-diagonal pair once) is the tail of the list.
-      constexpr int NU = LS ? kUNL : kUN;
+      // ELL slots of the row: an unused slot is (the row itself, 0); an in-tile neighbour is read from the stage
       int ck[NU]; T cw[NU];
-      if (fit) {
-        const int sh = (LS ? ee - NU : eb) - s_ea[s];
-        const int* scol = reinterpret_cast<const int*>(sb + off_col) + sh;
-        const T* sval = reinterpret_cast<const T*>(sb + off_val) + sh;
-#pragma unroll
-        for (int u = 0; u < NU; ++u) {
-          const bool in = LS ? (ee - NU + u >= eb) : true;   // (reads below the slice start are avoided)
-          ck[u] = in ? scol[u] : 0; cw[u] = in ? sval[u] : T(0);
-        }
-      } else {
-#pragma unroll
-        for (int u = 0; u < NU; ++u) {
-          const int e = LS ? ee - NU + u : eb + u;
-          const bool in = LS ? (e >= eb) : true;
-          ck[u] = in ? __ldg(a.c_col + e) : 0; cw[u] = in ? __ldg(a.c_val + e) : T(0);
-        }
-      }
 #pragma unroll
       for (int u = 0; u < NU; ++u) {
-        const bool ok = LS ? (ee - NU + u >= eb && (uint32_t)ck[u] > row) : (eb + u < ee);
-        ck[u] = ok ? ck[u] : (int)row;
-        cw[u] = ok ? cw[u] : T(0);
+        ck[u] = reinterpret_cast<const int*>(sb + off_ec)[lr * NU + u];
+        cw[u] = reinterpret_cast<const T*>(sb + off_ev)[lr * NU + u];
       }
+      const bool rem = s_rem[s] != 0;   // warp-uniform: some row of the tile has more neighbours than slots
       if (LS) {
         Row xk[NU], dk[NU];
 #pragma unroll
         for (int u = 0; u < NU; ++u) {
-          if (FULL) { row_ldg_b(xk[u], Xl + (uint64_t)(uint32_t)ck[u] * ldb, FULL == 2 ? ~0u : lmask); row_ldg_b(dk[u], X2l + (uint64_t)(uint32_t)ck[u] * ldb, FULL == 2 ? ~0u : lmask); }
-          else { xk[u].load(a.X + (int64_t)ck[u] * ld, lane, nvec, r, exact); dk[u].load(a.X2 + (int64_t)ck[u] * ld, lane, nvec, r, exact); }
+          const uint32_t rel = (uint32_t)ck[u] - row0;
+          const bool loc = rel < (uint32_t)TR;
+          row_nbr(xk[u], loc, sb + rel * ldb + loff, Xl + (uint64_t)(uint32_t)ck[u] * ldb, pmask);
+          row_nbr(dk[u], loc, sb + xbytes + rel * ldb + loff, X2l + (uint64_t)(uint32_t)ck[u] * ldb, pmask);
         }
         const T rr_l = x.dot(x), rd_l = x.dot(d), dd_l = d.dot(d);
         const double rr = (double)gsum<GS>(rr_l), rd = (double)gsum<GS>(rd_l), dd = (double)gsum<GS>(dd_l);
@@ -346,14 +336,17 @@ __global__ void __launch_bounds__(kTiledThreads, tiled_min_blocks(VEC * NIT * (i
         Row uacc, wacc; uacc.zero(); wacc.zero();
 #pragma unroll
         for (int u = 0; u < NU; ++u) { uacc.axpy(cw[u], xk[u]); wacc.axpy(cw[u], dk[u]); }
-        for (int e = ee - NU - 1; e >= eb; --e) {   // rows with more than NU upper neighbours
-          const int k = __ldg(a.c_col + e);
-          if ((uint32_t)k <= row) break;
-          const T cv = __ldg(a.c_val + e);
-          Row xe, de;
-          xe.load(a.X + (int64_t)k * ld, lane, nvec, r, exact);
-          de.load(a.X2 + (int64_t)k * ld, lane, nvec, r, exact);
-          uacc.axpy(cv, xe); wacc.axpy(cv, de);
+        if (rem) {   // rows with more than NU upper neighbours: the CSR tail below the slots (columns ascend)
+          const int eb = __ldg(a.c_rowptr + row), ee = __ldg(a.c_rowptr + row + 1);
+          for (int e = ee - NU - 1; e >= eb; --e) {
+            const int k = __ldg(a.c_col + e);
+            if ((uint32_t)k <= row) break;
+            const T cv = __ldg(a.c_val + e);
+            Row xe, de;
+            xe.load(a.X + (int64_t)k * ld, lane, nvec, r, exact);
+            de.load(a.X2 + (int64_t)k * ld, lane, nvec, r, exact);
+            uacc.axpy(cv, xe); wacc.axpy(cv, de);
+          }
         }
         const T sRR = x.dot(uacc), sRD = x.dot(wacc) + d.dot(uacc), sDD = d.dot(wacc);
         st[LS_CRR] += (double)dc * (double)rr_l + 2.0 * (double)sRR;
@@ -363,8 +356,8 @@ __global__ void __launch_bounds__(kTiledThreads, tiled_min_blocks(VEC * NIT * (i
         Row xn[NU];
 #pragma unroll
         for (int u = 0; u < NU; ++u) {
-          if (FULL) row_ldg_b(xn[u], Xl + (uint64_t)(uint32_t)ck[u] * ldb, FULL == 2 ? ~0u : lmask);
-          else xn[u].load(a.X + (int64_t)ck[u] * ld, lane, nvec, r, exact);
+          const uint32_t rel = (uint32_t)ck[u] - row0;
+          row_nbr(xn[u], rel < (uint32_t)TR, sb + rel * ldb + loff, Xl + (uint64_t)(uint32_t)ck[u] * ldb, pmask);
         }
         double coef;
         if (MODE == ROWS_FUSED_EVAL) {
@@ -384,30 +377,33 @@ __global__ void __launch_bounds__(kTiledThreads, tiled_min_blocks(VEC * NIT * (i
           for (int i = 0; i < VEC; ++i) acc.p[i2].v[i] = dc * x.p[i2].v[i];
 #pragma unroll
         for (int u = 0; u < NU; ++u) acc.axpy(cw[u], xn[u]);
-        for (int e = eb + kUN; e < ee; ++e) {   // rows with more than kUN neighbours
-          Row xe; xe.load(a.X + (int64_t)__ldg(a.c_col + e) * ld, lane, nvec, r, exact);
-          acc.axpy(__ldg(a.c_val + e), xe);
+        if (rem) {   // rows with more than NU neighbours: the CSR tail beyond the slots
+          const int eb = __ldg(a.c_rowptr + row), ee = __ldg(a.c_rowptr + row + 1);
+          for (int e = eb + NU; e < ee; ++e) {
+            Row xe; xe.load(a.X + (int64_t)__ldg(a.c_col + e) * ld, lane, nvec, r, exact);
+            acc.axpy(__ldg(a.c_val + e), xe);
+          }
         }
-        st[ES_CX] += (double)acc.dot(x);
+        const T cx = acc.dot(x);
         acc.axpy((T)(-coef), x);
 #pragma unroll
         for (int i2 = 0; i2 < NIT; ++i2)
 #pragma unroll
           for (int i = 0; i < VEC; ++i) acc.p[i2].v[i] *= sc;
+        st[ES_CX] += (double)cx;
         st[ES_GG] += (double)acc.dot(acc);
         st[ES_GR] += (double)acc.dot(x);
         if (Outl) {
-          if (FULL) {
+          char* const orow = Outl + (uint64_t)row * ldb;
 #pragma unroll
-            for (int i2 = 0; i2 < NIT; ++i2)
-              if (FULL == 2 || (lmask & (1u << i2))) st_pack<T, VEC>(reinterpret_cast<T*>(Outl + (uint64_t)row * ldb) + i2 * GS * VEC, acc.p[i2]);
-          } else {
-            acc.store(a.Out + (int64_t)row * ld, lane, nvec, r, exact);
-          }
+          for (int i2 = 0; i2 < NIT; ++i2)
+            if (FULL == 2 || (lmask & (1u << i2))) st_pack<T, VEC>(reinterpret_cast<T*>(orow) + i2 * GS * VEC, acc.p[i2]);
         }
       }
       __syncwarp();
       if (lane32 == 0) mbar_arrive_addr(empty0 + s * 8u);   // this warp is done with stage s
+      ++s; sb += stage_sz;
+      if (s == kStages) { s = 0; sb = smem_raw; ph ^= 1u; }
     }
   }
   if (LS && GS >= 4) {

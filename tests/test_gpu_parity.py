@@ -37,7 +37,7 @@ def rel(a, b):
     return float(np.linalg.norm(np.asarray(a, float) - np.asarray(b, float)) / max(1e-300, np.linalg.norm(np.asarray(b, float))))
 
 
-def check_workload(torch, binding, oracle_mod, w, ld=None, label=""):
+def check_workload(torch, binding, oracle_mod, w, ld=None, label="", split_scale=False):
     P, tol = w.problem, TOL[w.dtype]
     o = oracle_mod.Oracle(P)
     dt = tdtype(torch, w)
@@ -64,9 +64,16 @@ def check_workload(torch, binding, oracle_mod, w, ld=None, label=""):
     assert abs(st[1] - parts["cx"]) <= tol * fden
     assert rel(z.cpu().numpy(), zo) <= tol, label
     Gg = G.cpu().numpy().astype(float)
-    assert rel(Gg[:, :r], Go) <= tol, label
-    assert abs(np.sqrt(st[4]) - np.linalg.norm(Go)) <= tol * np.linalg.norm(Go)
-    assert abs(st[5] - np.vdot(Go, w.R)) <= tol * (np.linalg.norm(Go) * np.linalg.norm(w.R))
+    if split_scale:
+        # tiny degenerate problems: G = 2(CR - A*(lambda)R) may cancel almost completely (one row, one
+        # constraint), so the error is measured against the two terms that are subtracted
+        CR = o.smatvec(np.zeros(P.m), w.R)
+        gden = 2.0 * (np.linalg.norm(CR) + np.linalg.norm(0.5 * Go - CR))
+        assert np.linalg.norm(Gg[:, :r] - Go) <= tol * gden, label
+    else:
+        assert rel(Gg[:, :r], Go) <= tol, label
+    assert abs(np.sqrt(st[4]) - np.linalg.norm(Go)) <= tol * (gden if split_scale else np.linalg.norm(Go))
+    assert abs(st[5] - np.vdot(Go, w.R)) <= tol * ((gden if split_scale else np.linalg.norm(Go)) * np.linalg.norm(w.R))
     if ld > r:
         assert np.all(Gg[:, r:] == 5.0), "pad columns of G must not be touched"
     # value-only call gives the same scalars
@@ -119,3 +126,58 @@ def test_ranks(torch, binding, oracle_mod, r):
     for maker in (lambda: inputs.config1(side=23, r=r), lambda: inputs.config3(n=700, m=900, nnzC=2000, r=r),
                   lambda: inputs.config2(n=300, M=900, r=r), lambda: inputs.config0(n=300, M=700, r=r)):
         check_workload(torch, binding, oracle_mod, maker(), label=f"r{r}")
+
+
+@pytest.mark.parametrize("idx", [1, 2, 3, 4])
+def test_full_configs(torch, binding, oracle_mod, idx):
+    """BASELINE.json's full sizes, ld = r as bench.py launches them; the C oracle is fast enough to check
+    every element of z, G, S(mu)v (config 4: n = 2^24, about a minute of oracle time)."""
+    check_workload(torch, binding, oracle_mod, inputs.full(idx), label=f"full{idx}")
+
+
+def _edge_problems():
+    from tests.helpers import problem_from_lists
+    out = []
+    # n = 1, one diagonal constraint, no off-diagonal cost
+    out.append(("n1", problem_from_lists(1, [(0, 0, -0.5)], [[(0, 0, 1.0)]], [1.0])))
+    # empty cost, constraints with zero entries (z_i = 0), duplicates, an isolated vertex (row 3)
+    out.append(("empty_C", problem_from_lists(5, [], [[], [(0, 1, 0.5), (0, 1, 0.25)], [(2, 2, 1.0)], []], [0.3, 0.1, 1.0, -0.2])))
+    # diagonal class with a non-identity map: constraints in reverse order, one row unconstrained, coefficients != 1
+    n = 9
+    C = [(j, j + 1, 1.0 + 0.1 * j) for j in range(n - 1)] + [(j, j, -0.3 * j) for j in range(n)]
+    A = [[(n - 1 - i, n - 1 - i, 1.0 + 0.5 * i)] for i in range(n - 1)]
+    out.append(("diag_perm", problem_from_lists(n, C, A, [1.0 + 0.1 * i for i in range(n - 1)])))
+    # one long constraint (> 128 entries) next to single-entry ones, and a dense cost row (degree n-1)
+    n = 300
+    C = [(0, k, 0.01 * k) for k in range(1, n)]
+    A = [[(j, j, 1.0) for j in range(n)] + [(j, (j + 7) % n, 0.5) if j < (j + 7) % n else ((j + 7) % n, j, 0.5) for j in range(n)]]
+    A += [[(j, j + 1, 0.5)] for j in range(0, n - 1, 3)]
+    out.append(("long_cons", problem_from_lists(n, C, A, [1.0] + [0.0] * (len(A) - 1))))
+    return out
+
+
+@pytest.mark.parametrize("dtype", [inputs.F64, inputs.F32])
+@pytest.mark.parametrize("r", [1, 4, 10])
+def test_edge_cases(torch, binding, oracle_mod, dtype, r):
+    """degenerate inputs: n = 1, empty cost, empty constraints, duplicates, permuted / weighted diagonal
+    constraints (k_rows fallback of the diagonal class), a long constraint, a dense cost row."""
+    rng = np.random.default_rng(77 + r)
+    for name, P in _edge_problems():
+        def draw(shape):
+            a = rng.standard_normal(shape)
+            return a.astype(np.float32).astype(float) if dtype == inputs.F32 else a
+        if dtype == inputs.F32:
+            P.C_val = P.C_val.astype(np.float32).astype(float); P.A_val = P.A_val.astype(np.float32).astype(float)
+        w = inputs.Workload(name=name, problem=P, dtype=dtype, r=r, R=draw((P.n, r)), y=rng.standard_normal(P.m),
+                            sigma=2.5, D=draw((P.n, r)), V=draw(P.n))
+        check_workload(torch, binding, oracle_mod, w, label=f"{name}/r{r}/{dtype}", split_scale=True)
+
+
+def test_m0_no_constraints(torch, binding, oracle_mod):
+    """m = 0: f = <C,RR^T>, G = 2CR, S = C."""
+    from tests.helpers import problem_from_lists
+    P = problem_from_lists(6, [(0, 1, 1.0), (1, 2, -2.0), (3, 3, 0.7), (4, 5, 0.5)], [], [])
+    rng = np.random.default_rng(5)
+    w = inputs.Workload(name="m0", problem=P, dtype=inputs.F64, r=3, R=rng.standard_normal((6, 3)), y=np.zeros(0),
+                        sigma=1.0, D=rng.standard_normal((6, 3)), V=rng.standard_normal(6))
+    check_workload(torch, binding, oracle_mod, w, label="m0")
