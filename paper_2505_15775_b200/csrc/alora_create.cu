@@ -359,6 +359,8 @@ extern "C" alora_status alora_create(const alora_problem* P, alora_dtype dtype, 
   A((void**)&c->stats_dev, sizeof(double) * kNStat * 4);
   A((void**)&c->z_int, sizeof(double) * std::max<int64_t>(1, c->m));
   A((void**)&c->lr_scal, sizeof(double) * 8);
+  A((void**)&c->ticket, 16);
+  if (e == cudaSuccess) e = cudaMemset(c->ticket, 0, 16);
   if (e == cudaSuccess) e = cudaHostAlloc((void**)&c->pinned, sizeof(double) * (64 + 2 * 8 * 256), cudaHostAllocDefault);
   if (e != cudaSuccess) {
     fail(c, ALORA_ECUDA, cudaGetErrorString(e));

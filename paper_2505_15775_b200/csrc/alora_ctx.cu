@@ -18,34 +18,12 @@ alora_status fail(alora_ctx* c, alora_status s, const std::string& msg) {
 // ---------------------------------------------------------------------------------------------
 // small kernels
 // ---------------------------------------------------------------------------------------------
-// out[s] = sum over the partial rows of up to three regions, in a fixed order: thread t owns stat
-// t % 16 and the rows t / 16, t / 16 + 64, ... (coalesced 128-byte reads); the 64 row slots are then
-// summed in order through shared memory.  One block of 1024 threads.
-constexpr int kFinThreads = 1024;
-__global__ void __launch_bounds__(kFinThreads) k_finalize(const double* p0, int n0, const double* p1, int n1,
-                                                          const double* p2, int n2, double* out) {
-  __shared__ double sm[kFinThreads];
-  const int s = threadIdx.x & (kNStat - 1), slot = threadIdx.x / kNStat;
-  constexpr int NSLOT = kFinThreads / kNStat;
-  double v = 0.0;
-  for (int i = slot; i < n0; i += NSLOT) v += p0[(int64_t)i * kNStat + s];
-  for (int i = slot; i < n1; i += NSLOT) v += p1[(int64_t)i * kNStat + s];
-  for (int i = slot; i < n2; i += NSLOT) v += p2[(int64_t)i * kNStat + s];
-  sm[threadIdx.x] = v;
-  __syncthreads();
-  if (threadIdx.x < kNStat) {
-    double t = 0.0;
-    for (int k = 0; k < NSLOT; ++k) t += sm[k * kNStat + threadIdx.x];
-    out[threadIdx.x] = t;
-  }
-}
-
 // one block per long slot: ordered sum of its chunk partials, then the per-constraint finish.
 // slot cons id == m denotes C's sym-upper list (line search only): its sums are <C,RR^T>,
 // <C,RD^T>+<C,DR^T> (=2<C,RD^T>, halved here) and <C,DD^T>.
 __global__ void k_long_finish(int mode, int64_t m, const int* long_cons, const int64_t* long_chptr,
                               const double* ch_out, const double* y, const double* b, double sigma,
-                              double* z, double* lam, double* partials) {
+                              double* z, double* lam, double* partials, const FinArgs fin) {
   __shared__ double sm[3][kBlock / 32];
   const int slot = blockIdx.x, lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int64_t c0 = long_chptr[slot], c1 = long_chptr[slot + 1];
@@ -72,6 +50,7 @@ __global__ void k_long_finish(int mode, int64_t m, const int* long_cons, const i
     }
     for (int s = 0; s < kNStat; ++s) partials[(int64_t)slot * kNStat + s] = st[s];
   }
+  finish_partials(fin);
 }
 
 // Low-rank cost term, stage 1: per-block partials of T = U^T X (pC x r).  blockDim.x = r * rpb.
@@ -155,10 +134,18 @@ template <typename T> int grid_rows(alora_ctx* c, int vec, int shape, int mode, 
 // Row pass of the diagonal class: the tiled kernel on the full tiles plus k_rows on the ragged tail, or
 // k_rows alone when the tiled kernel's preconditions do not hold (non-identity diagonal constraints,
 // misaligned buffers, tile too large for shared memory).  *nparts = partial rows written.
+FinArgs make_fin(const alora_ctx* c, const double* p0, int n0, const double* p1, int n1, const double* p2, int n2, double* out) {
+  FinArgs f;
+  f.p[0] = p0; f.n[0] = n0; f.p[1] = p1; f.n[1] = n1; f.p[2] = p2; f.n[2] = n2;
+  f.out = out; f.ticket = c->ticket;
+  return f;
+}
+FinArgs no_fin() { FinArgs f; f.p[0] = f.p[1] = f.p[2] = nullptr; f.n[0] = f.n[1] = f.n[2] = 0; f.out = nullptr; f.ticket = nullptr; return f; }
+
 template <typename T>
 alora_status launch_diag_rows(alora_ctx* c, int vec, int nvec, int exact, int shape, int mode, RowArgs<T>& a,
-                              const void* dual, int* nparts) {
-  const int gs = kShapes[shape].gs, nit = kShapes[shape].nit, tr = tile_rows(gs);
+                              const void* dual, double* out) {
+  const int gs = kTShapes[shape].gs, nit = kTShapes[shape].nit, tr = tile_rows(gs);
   // 1: whole packs, some lanes of a group idle (lane mask); 2: whole packs, all lanes busy.  Rows whose last
   // pack is partially filled (r not a multiple of the vector width) take k_rows.
   const int full = nvec == gs * nit ? 2 : 1;
@@ -176,25 +163,18 @@ alora_status launch_diag_rows(alora_ctx* c, int vec, int nvec, int exact, int sh
   if (!elig) {
     const int grid = grid_rows<T>(c, vec, shape, mode, c->n);
     a.row_begin = 0;
+    a.fin = make_fin(c, a.partials, grid, nullptr, 0, nullptr, 0, out);
     ALORA_CUDA(c, launch_rows(vec, shape, mode, a, grid, c->stream));
     c->launches++;
-    *nparts = grid;
     return ALORA_OK;
   }
+  // one launch: the full tiles through the staged pipeline, the ragged tail by the last block, the final sum by
+  // whichever block finishes last
   const int grid = (int)std::max<int64_t>(1, std::min<int64_t>(tiles, std::min<int64_t>((int64_t)c->num_sms * occ, c->part_cap / 2)));
   a.tiles = tiles;
+  a.fin = make_fin(c, a.partials, grid, nullptr, 0, nullptr, 0, out);
   ALORA_CUDA(c, launch_tiled(vec, shape, mode, full, a, grid, c->stream));
   c->launches++;
-  *nparts = grid;
-  if (tiles * tr < c->n) {
-    RowArgs<T> t = a;
-    t.row_begin = tiles * tr;
-    t.partials = a.partials + (int64_t)grid * kNStat;
-    const int gt = grid_rows<T>(c, vec, shape, mode, c->n - tiles * tr);
-    ALORA_CUDA(c, launch_rows(vec, shape, mode, t, gt, c->stream));
-    c->launches++;
-    *nparts = grid + gt;
-  }
   return ALORA_OK;
 }
 template <typename T> int grid_cons(alora_ctx* c, int vec, int shape, int mode, int chunked, int64_t items) {
@@ -226,12 +206,14 @@ template <typename T> void fill_rows(alora_ctx* c, RowArgs<T>& a, const Geo& g, 
   a.pC = 0; a.U = (const T*)c->U; a.Ts = c->Ts; a.scale = 1.0; a.diag_class = (c->cls == 0);
   a.partials = c->part_rows; a.row_begin = 0; a.tiles = 0;
   a.ell_col = c->ell_col; a.ell_val = (const T*)c->ell_val; a.rem32 = c->rem32;
+  a.fin = no_fin();
 }
 template <typename T> void fill_cons(alora_ctx* c, ConsArgs<T>& a, const Geo& g, const T* X, const T* X2, int r, int64_t ld) {
   a.n = c->n; a.r = r; a.ld = ld; a.nvec = g.nvec; a.exact = g.exact; a.X = X; a.X2 = X2; a.m = c->m;
   a.ptr = c->f_ptr; a.e_row = c->f_row; a.e_col = c->f_col; a.e_val = (const T*)c->f_val;
   a.y = c->y; a.b = c->b; a.sigma = c->sigma; a.z = nullptr; a.lam = c->lam;
   a.nchunk = 0; a.ch_beg = c->ch_beg; a.ch_end = c->ch_end; a.ch_out = c->ch_out; a.partials = c->part_cons;
+  a.fin = no_fin();
 }
 
 // T = U^T X (pC x r) into Tm, optionally Ts = s * Tm
@@ -256,13 +238,10 @@ template <typename T> alora_status eval_impl(alora_ctx* c, const T* R, int32_t r
   a.Out = G; a.scale = 2.0;
   if (c->cls == 0) {
     a.z = zout;
-    int nparts = 0;
     time_mark(c);
-    s = launch_diag_rows<T>(c, g.vec, g.nvec, g.exact, g.shape, ROWS_FUSED_EVAL, a, c->y, &nparts);
+    s = launch_diag_rows<T>(c, g.vec, g.nvec, g.exact, g.shape, ROWS_FUSED_EVAL, a, c->y, c->stats_dev);
     if (s != ALORA_OK) return s;
     time_mark(c);
-    k_finalize<<<1, kFinThreads, 0, c->stream>>>(c->part_rows, nparts, nullptr, 0, nullptr, 0, c->stats_dev);
-    c->launches++;
   } else {
     if (c->pC) { s = lowrank<T>(c, R, r, ld, c->TmR, true); if (s != ALORA_OK) return s; a.pC = c->pC; }
     ConsArgs<T> ca;
@@ -279,16 +258,16 @@ template <typename T> alora_status eval_impl(alora_ctx* c, const T* R, int32_t r
       const int gk = grid_cons<T>(c, g.vec, g.shape, CONS_EVAL, 1, c->nchunk_A);
       ALORA_CUDA(c, launch_cons(g.vec, g.shape, CONS_EVAL, 1, ca, gk, c->stream));
       k_long_finish<<<c->nlong_A, kBlock, 0, c->stream>>>(CONS_EVAL, c->m, c->long_cons, c->long_chptr, c->ch_out, c->y,
-                                                         c->b, c->sigma, zout, c->lam, c->part_long);
+                                                         c->b, c->sigma, zout, c->lam, c->part_long, no_fin());
       c->launches += 2;
     }
     a.w = c->lam; a.diag_class = 0;
     const int grid = grid_rows<T>(c, g.vec, g.shape, ROWS_ADJ, c->n);
+    a.fin = make_fin(c, c->part_rows, grid, c->part_cons, gc, c->part_long, c->nlong_A, c->stats_dev);   // last kernel of the call
     time_mark(c);
     ALORA_CUDA(c, launch_rows(g.vec, g.shape, ROWS_ADJ, a, grid, c->stream));
     time_mark(c);
-    k_finalize<<<1, kFinThreads, 0, c->stream>>>(c->part_rows, grid, c->part_cons, gc, c->part_long, c->nlong_A, c->stats_dev);
-    c->launches += 2;
+    c->launches++;
   }
   ALORA_CUDA(c, cudaGetLastError());
   c->z_last = zout; c->have_eval = true;
@@ -322,11 +301,8 @@ template <typename T> alora_status ls_impl(alora_ctx* c, const T* R, const T* D,
     fill_rows(c, a, g, R, r, ld);
     a.X2 = D;
     a.ell_col = c->ellu_col; a.ell_val = (const T*)c->ellu_val; a.rem32 = c->remu32;
-    int nparts = 0;
-    s = launch_diag_rows<T>(c, g.vec, g.nvec, g.exact, g.shape, ROWS_LS_FUSED, a, c->y, &nparts);
+    s = launch_diag_rows<T>(c, g.vec, g.nvec, g.exact, g.shape, ROWS_LS_FUSED, a, c->y, c->ls_dev);
     if (s != ALORA_OK) return s;
-    k_finalize<<<1, kFinThreads, 0, c->stream>>>(c->part_rows, nparts, nullptr, 0, nullptr, 0, c->ls_dev);
-    c->launches++;
   } else {
     if (c->pC) {
       s = lowrank<T>(c, R, r, ld, c->TmR, false); if (s != ALORA_OK) return s;
@@ -334,22 +310,27 @@ template <typename T> alora_status ls_impl(alora_ctx* c, const T* R, const T* D,
     }
     ConsArgs<T> ca;
     fill_cons(c, ca, g, R, D, r, ld);
+    // the last kernel of the call (k_long_finish when there are chunks, else k_cons) also does the final sum
+    const bool chunks = c->nchunk_all > 0;
     int gc = 0;
     if (c->m > 0) {
       gc = grid_cons<T>(c, g.vec, g.shape, CONS_LS, 0, c->m);
+      if (!chunks) ca.fin = make_fin(c, c->part_cons, gc, nullptr, 0, nullptr, 0, c->ls_dev);
       ALORA_CUDA(c, launch_cons(g.vec, g.shape, CONS_LS, 0, ca, gc, c->stream));
+      ca.fin = no_fin();
       c->launches++;
     }
-    if (c->nchunk_all > 0) {
+    if (chunks) {
       ca.nchunk = c->nchunk_all;
       const int gk = grid_cons<T>(c, g.vec, g.shape, CONS_LS, 1, c->nchunk_all);
       ALORA_CUDA(c, launch_cons(g.vec, g.shape, CONS_LS, 1, ca, gk, c->stream));
       k_long_finish<<<c->nlong_all, kBlock, 0, c->stream>>>(CONS_LS, c->m, c->long_cons, c->long_chptr, c->ch_out, c->y,
-                                                           c->b, c->sigma, nullptr, nullptr, c->part_long);
+                                                           c->b, c->sigma, nullptr, nullptr, c->part_long,
+                                                           make_fin(c, c->part_cons, gc, c->part_long, c->nlong_all, nullptr, 0, c->ls_dev));
       c->launches += 2;
+    } else if (c->m == 0) {
+      ALORA_CUDA(c, cudaMemsetAsync(c->ls_dev, 0, sizeof(double) * kNStat, c->stream));
     }
-    k_finalize<<<1, kFinThreads, 0, c->stream>>>(c->part_cons, gc, c->part_long, c->nlong_all, nullptr, 0, c->ls_dev);
-    c->launches++;
   }
   ALORA_CUDA(c, cudaGetLastError());
   c->have_ls = true;
@@ -391,17 +372,15 @@ template <typename T> alora_status matvec_impl(alora_ctx* c, const double* mu, c
   fill_rows(c, a, g, V, p, p);
   a.Out = W; a.scale = 1.0; a.w = mu; a.diag_class = (c->cls == 0);
   if (c->pC) { s = lowrank<T>(c, V, p, p, c->TmD, true); if (s != ALORA_OK) return s; a.pC = c->pC; }
-  int nparts = 0;
   if (c->cls == 0) {
-    s = launch_diag_rows<T>(c, g.vec, g.nvec, g.exact, g.shape, ROWS_ADJ, a, mu, &nparts);
+    s = launch_diag_rows<T>(c, g.vec, g.nvec, g.exact, g.shape, ROWS_ADJ, a, mu, c->mv_dev);
     if (s != ALORA_OK) return s;
   } else {
-    nparts = grid_rows<T>(c, g.vec, g.shape, ROWS_ADJ, c->n);
-    ALORA_CUDA(c, launch_rows(g.vec, g.shape, ROWS_ADJ, a, nparts, c->stream));
+    const int grid = grid_rows<T>(c, g.vec, g.shape, ROWS_ADJ, c->n);
+    a.fin = make_fin(c, c->part_rows, grid, nullptr, 0, nullptr, 0, c->mv_dev);
+    ALORA_CUDA(c, launch_rows(g.vec, g.shape, ROWS_ADJ, a, grid, c->stream));
     c->launches++;
   }
-  k_finalize<<<1, kFinThreads, 0, c->stream>>>(c->part_rows, nparts, nullptr, 0, nullptr, 0, c->mv_dev);
-  c->launches++;
   ALORA_CUDA(c, cudaGetLastError());
   return ALORA_OK;
 }

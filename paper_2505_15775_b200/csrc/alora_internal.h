@@ -77,6 +77,7 @@ struct alora_ctx {
   int part_cap = 0;
   double* part_rows = nullptr; double* part_cons = nullptr; double* part_long = nullptr;
   double* stats_dev = nullptr; double* ls_dev = nullptr; double* mv_dev = nullptr;
+  unsigned int* ticket = nullptr;   // FinArgs::ticket (kernels.cuh), zero between launches
   double* pinned = nullptr;  // 64 doubles
   bool have_eval = false, have_ls = false;
   int last_eval_r = 0, last_ls_r = 0;

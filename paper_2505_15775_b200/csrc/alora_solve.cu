@@ -32,7 +32,7 @@ __global__ void __launch_bounds__(kBlock) k_dots3(int64_t N, const TX* x0, const
   block_reduce_store<3>(st, part + (int64_t)blockIdx.x * kNStat);
 }
 
-__global__ void k_reduce_rows(const double* part, int nrows, double* out) {  // same order as k_finalize
+__global__ void k_reduce_rows(const double* part, int nrows, double* out) {  // ordered second stage
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   for (int s = warp; s < kNStat; s += kBlock / 32) {
     double v = 0.0;

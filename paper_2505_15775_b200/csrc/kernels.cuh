@@ -36,6 +36,16 @@ enum EvalStat { ES_CX = 0, ES_YQ = 1, ES_QQ = 2, ES_GG = 3, ES_GR = 4, ES_LZ = 5
 enum LsStat { LS_CRR = 0, LS_CRD = 1, LS_CDD = 2, LS_YQ = 3, LS_YQ1 = 4, LS_YQ2 = 5, LS_QQ = 6,
               LS_QQ1 = 7, LS_QQ2 = 8, LS_Q11 = 9, LS_Q12 = 10, LS_Q22 = 11 };
 
+// Fused final reduction: the LAST kernel of a call also sums the per-block partial rows of the call (its own
+// and those written by the kernels launched before it on the stream) into out[0..16).  Every block publishes
+// its row, takes a ticket, and the block that draws the last ticket does the sum in a fixed order, so the result
+// does not depend on which block that is.  out == nullptr: the kernel only writes its partial rows.
+struct FinArgs {
+  const double* p[3]; int n[3];   // up to three regions of partial rows ([n][kNStat])
+  double* out;                    // [kNStat]
+  unsigned int* ticket;           // zero before the launch; reset by the finishing block
+};
+
 template <typename T> struct RowArgs {
   int64_t n; int r; int64_t ld; int nvec; int exact;  // exact: r == nvec*VEC (no tail masking)
   const T* X;    // R (or V)
@@ -51,6 +61,7 @@ template <typename T> struct RowArgs {
   double scale;
   int diag_class;    // ROWS_ADJ: 1 = constraints are the per-row diagonal ones, 0 = use a_* CSR
   double* partials;  // [gridDim.x][kNStat]
+  FinArgs fin;
   int64_t row_begin; // k_rows: first row handled (rows [row_begin, n))
   int64_t tiles;     // k_rows_tiled: number of full row tiles handled (rows [0, tiles * TR))
   // k_rows_tiled: padded ELL block of the mode (kUN first neighbours, or kUNL last upper-triangle neighbours
@@ -71,6 +82,7 @@ template <typename T> struct ConsArgs {
   int64_t nchunk; const int64_t* ch_beg; const int64_t* ch_end;
   double* ch_out;                 // [nchunk][3]
   double* partials;
+  FinArgs fin;
 };
 
 // ---------------------------------------------------------------------------------------------
@@ -125,6 +137,46 @@ template <int NST> __device__ __forceinline__ void block_reduce_store(double (&s
     }
     out[threadIdx.x] = v;
   }
+}
+
+// See FinArgs.  Called by every thread of the block after the block's partial row has been written (needs
+// blockDim.x >= 256).  Thread t < 256 owns stat t % 16 and the rows t / 16, t / 16 + 16, ... of each region; the 16
+// row slots are then summed in order through shared memory.
+__device__ __forceinline__ void finish_partials(const FinArgs& f) {
+  if (!f.out) return;
+  __shared__ unsigned int s_last;
+  __shared__ double s_fin[256];
+  __threadfence();
+  __syncthreads();
+  if (threadIdx.x == 0) s_last = (atomicAdd(f.ticket, 1u) == gridDim.x - 1) ? 1u : 0u;
+  __syncthreads();
+  if (!s_last) return;
+  __threadfence();
+  if (threadIdx.x < 256) {
+    const int s = threadIdx.x & (kNStat - 1), slot = threadIdx.x / kNStat;
+    constexpr int NSLOT = 256 / kNStat;
+    double v = 0.0;
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+      const double* p = f.p[k];
+      const int n = f.n[k];
+      int i = slot;
+      for (; i + 3 * NSLOT < n; i += 4 * NSLOT) {   // four independent loads in flight
+        const double v0 = __ldcg(p + (int64_t)i * kNStat + s), v1 = __ldcg(p + (int64_t)(i + NSLOT) * kNStat + s);
+        const double v2 = __ldcg(p + (int64_t)(i + 2 * NSLOT) * kNStat + s), v3 = __ldcg(p + (int64_t)(i + 3 * NSLOT) * kNStat + s);
+        v += v0; v += v1; v += v2; v += v3;
+      }
+      for (; i < n; i += NSLOT) v += __ldcg(p + (int64_t)i * kNStat + s);
+    }
+    s_fin[threadIdx.x] = v;
+  }
+  __syncthreads();
+  if (threadIdx.x < kNStat) {
+    double t = 0.0;
+    for (int k = 0; k < 256 / kNStat; ++k) t += s_fin[k * kNStat + threadIdx.x];
+    f.out[threadIdx.x] = t;
+  }
+  if (threadIdx.x == 0) *f.ticket = 0u;
 }
 
 // Row vector held by one lane: NIT packs of VEC elements, pack index vi = lane + it*GS.
@@ -324,6 +376,7 @@ __global__ void __launch_bounds__(kBlock) k_rows(const RowArgs<T> a) {
     }
   }
   block_reduce_store<NST>(st, a.partials + (int64_t)blockIdx.x * kNStat);
+  finish_partials(a.fin);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -386,6 +439,7 @@ __global__ void __launch_bounds__(kBlock) k_cons(const ConsArgs<T> a) {
     if (lane == 0) cons_finish<MODE>(st, i, z, q1, q2, a.y, a.b, a.sigma, a.z, a.lam);
   }
   block_reduce_store<NST>(st, a.partials + (int64_t)blockIdx.x * kNStat);
+  finish_partials(a.fin);
 }
 
 // one group per chunk of <= kChunk entries of a long constraint (or of C's sym-upper list)
@@ -411,8 +465,9 @@ __host__ inline int shape_index(int nvec) {
   if (nvec <= 1) return 0; if (nvec <= 2) return 1; if (nvec <= 4) return 2; if (nvec <= 8) return 3;
   if (nvec <= 16) return 4; if (nvec <= 32) return 5; if (nvec <= 64) return 6; return -1;
 }
-// few lanes per row: the per-row bookkeeping (addresses, scalars, fp64 sums) is issued once per group, so
-// fewer lanes per row means fewer warp instructions per row; a lane holds up to 4 packs
-constexpr Shape kShapes[7] = {{1, 1}, {2, 1}, {4, 1}, {4, 2}, {8, 2}, {8, 4}, {16, 4}};
+constexpr Shape kShapes[7] = {{1, 1}, {2, 1}, {4, 1}, {8, 1}, {8, 2}, {16, 2}, {16, 4}};   // k_rows, k_cons
+// tiled row kernel: few lanes per row -- the per-row bookkeeping (addresses, scalars, fp64 sums) is issued once
+// per group, so fewer lanes per row means fewer warp instructions per row; a lane holds up to 4 packs
+constexpr Shape kTShapes[7] = {{1, 1}, {2, 1}, {4, 1}, {4, 2}, {8, 2}, {8, 4}, {16, 4}};
 
 }  // namespace alora

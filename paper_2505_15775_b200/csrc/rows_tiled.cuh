@@ -195,8 +195,8 @@ __device__ __forceinline__ void row_nbr(RowReg<T, VEC, GS, NIT>& x, bool loc, co
 
 // Preconditions (checked by the host, which otherwise uses k_rows): the constraints are the identity diagonal
 // ones (dcons == da == nullptr, ELL block present), rows are whole packs (r == nvec * VEC), X / X2 / y (or w)
-// are 16-byte aligned, and the kernel is given FULL tiles only: it covers rows [0, a.tiles * TR); the ragged
-// tail goes to k_rows.  FULL: 1 = some lanes of a group own no pack (lane mask), 2 = all lanes busy.
+// are 16-byte aligned.  Full tiles (rows [0, a.tiles * TR)) go through the staged pipeline; the ragged tail of
+// the matrix (< TR rows) is processed by the consumer warps of the last block from global memory.  FULL: 1 = some lanes of a group own no pack (lane mask), 2 = all lanes busy.
 template <typename T, int VEC, int GS, int NIT, int MODE, int FULL>
 __global__ void __launch_bounds__(kTiledThreads, tiled_min_blocks(VEC * NIT * (int)sizeof(T) / 4, MODE)) k_rows_tiled(const RowArgs<T> a) {
   using Row = RowReg<T, VEC, GS, NIT>;
@@ -287,31 +287,40 @@ __global__ void __launch_bounds__(kTiledThreads, tiled_min_blocks(VEC * NIT * (i
     double* const zout = a.z;
     const double sigma = a.sigma;
     const T sc = (T)a.scale;
-    uint32_t s = 0, ph = 0;
-    const unsigned char* sb = smem_raw;
-    for (int64_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
-      const uint32_t row0 = (uint32_t)(tile * TR), row = row0 + (uint32_t)lr;
-      mbar_wait_addr(full0 + s * 8u, ph);
+    // one row: `staged` = its streaming inputs sit in stage `sb` (tile rows [row0, row0 + TR)), else they are read
+    // from global memory (ragged tail of the matrix); live == false: padding lane of the tail, nothing is kept
+    auto do_row = [&](const bool staged, const unsigned char* sb, const uint32_t row0, const uint32_t row, const bool rem,
+                      const bool live) {
       Row x, d;
-      row_nbr(x, true, sb + xme, nullptr, pmask);
-      if (LS) row_nbr(d, true, sb + xbytes + xme, nullptr, pmask);
-      const T dc = reinterpret_cast<const T*>(sb + off_dc)[lr];
-      const double yv = reinterpret_cast<const double*>(sb + off_y)[lr];
-      const double bv = (MODE != ROWS_ADJ) ? reinterpret_cast<const double*>(sb + off_b)[lr] : 0.0;
-      // ELL slots of the row: an unused slot is (the row itself, 0); an in-tile neighbour is read from the stage
+      T dc; double yv, bv = 0.0;
       int ck[NU]; T cw[NU];
+      if (staged) {
+        row_nbr(x, true, sb + xme, nullptr, pmask);
+        if (LS) row_nbr(d, true, sb + xbytes + xme, nullptr, pmask);
+        dc = reinterpret_cast<const T*>(sb + off_dc)[lr];
+        yv = reinterpret_cast<const double*>(sb + off_y)[lr];
+        if (MODE != ROWS_ADJ) bv = reinterpret_cast<const double*>(sb + off_b)[lr];
 #pragma unroll
-      for (int u = 0; u < NU; ++u) {
-        ck[u] = reinterpret_cast<const int*>(sb + off_ec)[lr * NU + u];
-        cw[u] = reinterpret_cast<const T*>(sb + off_ev)[lr * NU + u];
+        for (int u = 0; u < NU; ++u) {
+          ck[u] = reinterpret_cast<const int*>(sb + off_ec)[lr * NU + u];
+          cw[u] = reinterpret_cast<const T*>(sb + off_ev)[lr * NU + u];
+        }
+      } else {
+        row_nbr(x, false, nullptr, Xl + (uint64_t)row * ldb, pmask);
+        if (LS) row_nbr(d, false, nullptr, X2l + (uint64_t)row * ldb, pmask);
+        dc = __ldg(a.dC + row);
+        yv = __ldg((MODE == ROWS_ADJ ? a.w : a.y) + row);
+        if (MODE != ROWS_ADJ) bv = __ldg(a.b + row);
+#pragma unroll
+        for (int u = 0; u < NU; ++u) { ck[u] = __ldg(a.ell_col + (int64_t)row * NU + u); cw[u] = __ldg(a.ell_val + (int64_t)row * NU + u); }
       }
-      const bool rem = s_rem[s] != 0;   // warp-uniform: some row of the tile has more neighbours than slots
+      // ELL slots: an unused slot is (the row itself, 0); an in-tile neighbour is read from the stage
       if (LS) {
         Row xk[NU], dk[NU];
 #pragma unroll
         for (int u = 0; u < NU; ++u) {
           const uint32_t rel = (uint32_t)ck[u] - row0;
-          const bool loc = rel < (uint32_t)TR;
+          const bool loc = staged && rel < (uint32_t)TR;
           row_nbr(xk[u], loc, sb + rel * ldb + loff, Xl + (uint64_t)(uint32_t)ck[u] * ldb, pmask);
           row_nbr(dk[u], loc, sb + xbytes + rel * ldb + loff, X2l + (uint64_t)(uint32_t)ck[u] * ldb, pmask);
         }
@@ -325,8 +334,8 @@ __global__ void __launch_bounds__(kTiledThreads, tiled_min_blocks(VEC * NIT * (i
           const double a0 = lane == 2 ? q1 : A, b0 = lane == 2 ? q1 : qv;
           const double a1 = lane == 2 ? q1 : A, b1 = lane == 2 ? q2 : q1;
           const double a2 = lane == 2 ? q2 : A;
-          if (lane < 3) { st[3] += a0 * b0; st[4] += a1 * b1; st[5] += a2 * q2; }
-        } else if (lane == 0) {
+          if (lane < 3 && live) { st[3] += a0 * b0; st[4] += a1 * b1; st[5] += a2 * q2; }
+        } else if (lane == 0 && live) {
           st[LS_YQ] += yv * qv; st[LS_YQ1] += yv * q1; st[LS_YQ2] += yv * q2;
           st[LS_QQ] += qv * qv; st[LS_QQ1] += qv * q1; st[LS_QQ2] += qv * q2;
           st[LS_Q11] += q1 * q1; st[LS_Q12] += q1 * q2; st[LS_Q22] += q2 * q2;
@@ -349,21 +358,23 @@ __global__ void __launch_bounds__(kTiledThreads, tiled_min_blocks(VEC * NIT * (i
           }
         }
         const T sRR = x.dot(uacc), sRD = x.dot(wacc) + d.dot(uacc), sDD = d.dot(wacc);
-        st[LS_CRR] += (double)dc * (double)rr_l + 2.0 * (double)sRR;
-        st[LS_CRD] += (double)dc * (double)rd_l + (double)sRD;
-        st[LS_CDD] += (double)dc * (double)dd_l + 2.0 * (double)sDD;
+        if (live) {
+          st[LS_CRR] += (double)dc * (double)rr_l + 2.0 * (double)sRR;
+          st[LS_CRD] += (double)dc * (double)rd_l + (double)sRD;
+          st[LS_CDD] += (double)dc * (double)dd_l + 2.0 * (double)sDD;
+        }
       } else {
         Row xn[NU];
 #pragma unroll
         for (int u = 0; u < NU; ++u) {
           const uint32_t rel = (uint32_t)ck[u] - row0;
-          row_nbr(xn[u], rel < (uint32_t)TR, sb + rel * ldb + loff, Xl + (uint64_t)(uint32_t)ck[u] * ldb, pmask);
+          row_nbr(xn[u], staged && rel < (uint32_t)TR, sb + rel * ldb + loff, Xl + (uint64_t)(uint32_t)ck[u] * ldb, pmask);
         }
         double coef;
         if (MODE == ROWS_FUSED_EVAL) {
           const double z = (double)gsum<GS>(x.dot(x)), qv = z - bv, lam = yv - sigma * qv;
           coef = lam;
-          if (lane == 0) {
+          if (lane == 0 && live) {
             if (zout) zout[row] = z;
             st[ES_YQ] += yv * qv; st[ES_QQ] += qv * qv; st[ES_LZ] += lam * z;
           }
@@ -390,20 +401,40 @@ __global__ void __launch_bounds__(kTiledThreads, tiled_min_blocks(VEC * NIT * (i
         for (int i2 = 0; i2 < NIT; ++i2)
 #pragma unroll
           for (int i = 0; i < VEC; ++i) acc.p[i2].v[i] *= sc;
-        st[ES_CX] += (double)cx;
-        st[ES_GG] += (double)acc.dot(acc);
-        st[ES_GR] += (double)acc.dot(x);
-        if (Outl) {
-          char* const orow = Outl + (uint64_t)row * ldb;
+        if (live) {
+          st[ES_CX] += (double)cx;
+          st[ES_GG] += (double)acc.dot(acc);
+          st[ES_GR] += (double)acc.dot(x);
+          if (Outl) {
+            char* const orow = Outl + (uint64_t)row * ldb;
 #pragma unroll
-          for (int i2 = 0; i2 < NIT; ++i2)
-            if (FULL == 2 || (lmask & (1u << i2))) st_pack<T, VEC>(reinterpret_cast<T*>(orow) + i2 * GS * VEC, acc.p[i2]);
+            for (int i2 = 0; i2 < NIT; ++i2)
+              if (FULL == 2 || (lmask & (1u << i2))) st_pack<T, VEC>(reinterpret_cast<T*>(orow) + i2 * GS * VEC, acc.p[i2]);
+          }
         }
       }
+    };
+
+    uint32_t s = 0, ph = 0;
+    const unsigned char* sb = smem_raw;
+    for (int64_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+      const uint32_t row0 = (uint32_t)(tile * TR);
+      mbar_wait_addr(full0 + s * 8u, ph);
+      do_row(true, sb, row0, row0 + (uint32_t)lr, s_rem[s] != 0, true);
       __syncwarp();
       if (lane32 == 0) mbar_arrive_addr(empty0 + s * 8u);   // this warp is done with stage s
       ++s; sb += stage_sz;
       if (s == kStages) { s = 0; sb = smem_raw; ph ^= 1u; }
+    }
+    // ragged tail of the matrix (fewer than TR rows): the last block reads them from global memory
+    if (blockIdx.x == gridDim.x - 1) {
+      const uint32_t n32 = (uint32_t)a.n;
+      for (uint32_t base = (uint32_t)(ntiles * TR); base < n32; base += TR) {
+        const uint32_t row = base + (uint32_t)lr;
+        const bool live = row < n32;
+        const uint32_t rowc = live ? row : n32 - 1;
+        do_row(false, nullptr, 0u, rowc, __ldg(a.rem32 + (rowc >> 5)) != 0, live);
+      }
     }
   }
   if (LS && GS >= 4) {
@@ -420,6 +451,7 @@ __global__ void __launch_bounds__(kTiledThreads, tiled_min_blocks(VEC * NIT * (i
     for (int k = 0; k < NST; ++k) full_st[k] = st[k < NSL ? k : 0];
     block_reduce_store_nw<NST, NCW + 1>(full_st, a.partials + (int64_t)blockIdx.x * kNStat);
   }
+  finish_partials(a.fin);
 }
 
 }  // namespace alora
