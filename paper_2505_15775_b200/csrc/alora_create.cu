@@ -229,9 +229,8 @@ template <typename T> alora_status build(alora_ctx* c, const alora_problem* P) {
     if (c->nf_C > 0) {
       const int64_t e1 = c->nf_A + c->nf_C;
       for (int64_t e = c->nf_A; e < e1; e += kChunk) { ch_beg.push_back(e); ch_end.push_back(std::min<int64_t>(e + kChunk, e1)); }
-      long_cons.push_back((int)m); long_chptr.push_back((int64_t)ch_beg.size());
     }
-    c->nchunk_all = (int64_t)ch_beg.size(); c->nlong_all = (int)long_cons.size();
+    c->nchunk_all = (int64_t)ch_beg.size();
     std::vector<T> fv(f_val.size());
     for (size_t e = 0; e < f_val.size(); ++e) fv[e] = (T)f_val[e];
     ALORA_CUDA(c, upload(c, (void**)&c->f_ptr, f_ptr));
@@ -242,8 +241,8 @@ template <typename T> alora_status build(alora_ctx* c, const alora_problem* P) {
     ALORA_CUDA(c, upload(c, (void**)&c->ch_end, ch_end));
     ALORA_CUDA(c, upload(c, (void**)&c->long_cons, long_cons));
     ALORA_CUDA(c, upload(c, (void**)&c->long_chptr, long_chptr));
-    ALORA_CUDA(c, c->pool.alloc((void**)&c->ch_out, sizeof(double) * 3 * std::max<int64_t>(1, c->nchunk_all)));
-    ALORA_CUDA(c, c->pool.alloc((void**)&c->part_long, sizeof(double) * kNStat * std::max(1, c->nlong_all)));
+    ALORA_CUDA(c, c->pool.alloc((void**)&c->ch_out, sizeof(double) * 3 * std::max<int64_t>(1, c->nchunk_A)));
+    ALORA_CUDA(c, c->pool.alloc((void**)&c->part_long, sizeof(double) * kNStat * std::max(1, c->nlong_A)));
     ALORA_CUDA(c, c->pool.alloc((void**)&c->lam, sizeof(double) * std::max<int64_t>(1, m)));
   }
   // ---- low-rank cost term --------------------------------------------------------------------
@@ -255,7 +254,7 @@ template <typename T> alora_status build(alora_ctx* c, const alora_problem* P) {
     ALORA_CUDA(c, upload(c, &c->U, U));
     c->s_host.assign(P->C_s, P->C_s + P->pC);
     ALORA_CUDA(c, upload(c, (void**)&c->s_dev, c->s_host));
-    c->lr_grid = (int)std::min<int64_t>(64, std::max<int64_t>(1, n / 64));
+    c->lr_grid = (int)std::min<int64_t>(2 * c->num_sms, std::max<int64_t>(1, n / 64));
     ALORA_CUDA(c, c->pool.alloc((void**)&c->lr_part, sizeof(double) * c->lr_grid * P->pC * c->lr_rmax));
     ALORA_CUDA(c, c->pool.alloc((void**)&c->TmR, sizeof(double) * P->pC * c->lr_rmax));
     ALORA_CUDA(c, c->pool.alloc((void**)&c->TmD, sizeof(double) * P->pC * c->lr_rmax));
@@ -356,6 +355,7 @@ extern "C" alora_status alora_create(const alora_problem* P, alora_dtype dtype, 
   auto A = [&](void** p, size_t nb) { if (e == cudaSuccess) e = c->pool.alloc(p, nb); };
   A((void**)&c->part_rows, sizeof(double) * kNStat * c->part_cap);
   A((void**)&c->part_cons, sizeof(double) * kNStat * c->part_cap);
+  A((void**)&c->part_chunk, sizeof(double) * kNStat * c->part_cap);
   A((void**)&c->stats_dev, sizeof(double) * kNStat * 4);
   A((void**)&c->z_int, sizeof(double) * std::max<int64_t>(1, c->m));
   A((void**)&c->lr_scal, sizeof(double) * 8);

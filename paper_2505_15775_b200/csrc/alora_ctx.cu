@@ -18,9 +18,7 @@ alora_status fail(alora_ctx* c, alora_status s, const std::string& msg) {
 // ---------------------------------------------------------------------------------------------
 // small kernels
 // ---------------------------------------------------------------------------------------------
-// one block per long slot: ordered sum of its chunk partials, then the per-constraint finish.
-// slot cons id == m denotes C's sym-upper list (line search only): its sums are <C,RR^T>,
-// <C,RD^T>+<C,DR^T> (=2<C,RD^T>, halved here) and <C,DD^T>.
+// one block per long constraint: ordered sum of its chunk partials, then the per-constraint finish.
 __global__ void k_long_finish(int mode, int64_t m, const int* long_cons, const int64_t* long_chptr,
                               const double* ch_out, const double* y, const double* b, double sigma,
                               double* z, double* lam, double* partials, const FinArgs fin) {
@@ -41,9 +39,7 @@ __global__ void k_long_finish(int mode, int64_t m, const int* long_cons, const i
     double st[kNStat];
     for (int s = 0; s < kNStat; ++s) st[s] = 0.0;
     const int64_t i = long_cons[slot];
-    if (i == m) {
-      st[LS_CRR] = t[0]; st[LS_CRD] = 0.5 * t[1]; st[LS_CDD] = t[2];
-    } else if (mode == CONS_EVAL) {
+    if (mode == CONS_EVAL) {
       cons_finish<CONS_EVAL>(st, i, t[0], t[1], t[2], y, b, sigma, z, lam);
     } else {
       cons_finish<CONS_LS>(st, i, t[0], t[1], t[2], y, b, sigma, z, lam);
@@ -53,10 +49,13 @@ __global__ void k_long_finish(int mode, int64_t m, const int* long_cons, const i
   finish_partials(fin);
 }
 
-// Low-rank cost term, stage 1: per-block partials of T = U^T X (pC x r).  blockDim.x = r * rpb.
+// Low-rank cost term: T = U^T X (pC x r).  Per-block partials, then the block that finishes last (ticket) sums
+// them in block order: Tm[p][c], and optionally Ts = s_p * Tm.  blockDim.x = r * rpb.
 template <typename T>
-__global__ void k_lowrank(const T* X, int64_t n, int r, int64_t ld, const T* U, int pC, double* part) {
+__global__ void k_lowrank(const T* X, int64_t n, int r, int64_t ld, const T* U, int pC, double* part, const double* s,
+                          double* Tm, double* Ts, unsigned int* ticket) {
   extern __shared__ double lsm[];  // [pC][blockDim.x]
+  __shared__ unsigned int s_last;
   const int c = threadIdx.x % r, slot = threadIdx.x / r, rpb = blockDim.x / r;
   double acc[8];
   for (int p = 0; p < 8; ++p) acc[p] = 0.0;
@@ -73,16 +72,26 @@ __global__ void k_lowrank(const T* X, int64_t n, int r, int64_t ld, const T* U, 
       part[((int64_t)blockIdx.x * pC + p) * r + c] = v;
     }
   }
-}
-// stage 2: Tm[p][c] = sum over blocks; Ts = s_p * Tm (optional)
-__global__ void k_lowrank_reduce(const double* part, int nblk, int pC, int r, const double* s, double* Tm,
-                                 double* Ts) {
-  for (int idx = threadIdx.x; idx < pC * r; idx += blockDim.x) {
+  __threadfence();
+  __syncthreads();
+  if (threadIdx.x == 0) s_last = (atomicAdd(ticket, 1u) == gridDim.x - 1) ? 1u : 0u;
+  __syncthreads();
+  if (!s_last) return;
+  __threadfence();
+  const int nblk = gridDim.x, pr = pC * r;
+  for (int idx = threadIdx.x; idx < pr; idx += blockDim.x) {
     double v = 0.0;
-    for (int bk = 0; bk < nblk; ++bk) v += part[(int64_t)bk * pC * r + idx];
+    int bk = 0;
+    for (; bk + 3 < nblk; bk += 4) {
+      const double v0 = __ldcg(part + (int64_t)bk * pr + idx), v1 = __ldcg(part + (int64_t)(bk + 1) * pr + idx);
+      const double v2 = __ldcg(part + (int64_t)(bk + 2) * pr + idx), v3 = __ldcg(part + (int64_t)(bk + 3) * pr + idx);
+      v += v0; v += v1; v += v2; v += v3;
+    }
+    for (; bk < nblk; ++bk) v += __ldcg(part + (int64_t)bk * pr + idx);
     Tm[idx] = v;
     if (Ts) Ts[idx] = s[idx / r] * v;
   }
+  if (threadIdx.x == 0) *ticket = 0u;
 }
 
 // lambda = y - sigma (z - b)
@@ -213,6 +222,7 @@ template <typename T> void fill_cons(alora_ctx* c, ConsArgs<T>& a, const Geo& g,
   a.ptr = c->f_ptr; a.e_row = c->f_row; a.e_col = c->f_col; a.e_val = (const T*)c->f_val;
   a.y = c->y; a.b = c->b; a.sigma = c->sigma; a.z = nullptr; a.lam = c->lam;
   a.nchunk = 0; a.ch_beg = c->ch_beg; a.ch_end = c->ch_end; a.ch_out = c->ch_out; a.partials = c->part_cons;
+  a.nchunk_A = c->nchunk_A; a.part_chunk = c->part_chunk;
   a.fin = no_fin();
 }
 
@@ -220,9 +230,9 @@ template <typename T> void fill_cons(alora_ctx* c, ConsArgs<T>& a, const Geo& g,
 template <typename T> alora_status lowrank(alora_ctx* c, const T* X, int r, int64_t ld, double* Tm, bool want_Ts) {
   if (r > c->lr_rmax) return fail(c, ALORA_EINVAL, "low-rank cost term supports r <= 256");
   const int rpb = std::max(1, kBlock / r), threads = r * rpb;
-  k_lowrank<T><<<c->lr_grid, threads, sizeof(double) * c->pC * threads, c->stream>>>(X, c->n, r, ld, (const T*)c->U, c->pC, c->lr_part);
-  k_lowrank_reduce<<<1, kBlock, 0, c->stream>>>(c->lr_part, c->lr_grid, c->pC, r, c->s_dev, Tm, want_Ts ? c->Ts : nullptr);
-  c->launches += 2;
+  k_lowrank<T><<<c->lr_grid, threads, sizeof(double) * c->pC * threads, c->stream>>>(X, c->n, r, ld, (const T*)c->U, c->pC, c->lr_part,
+                                                                                    c->s_dev, Tm, want_Ts ? c->Ts : nullptr, c->ticket);
+  c->launches++;
   ALORA_CUDA(c, cudaGetLastError());
   return ALORA_OK;
 }
@@ -310,9 +320,11 @@ template <typename T> alora_status ls_impl(alora_ctx* c, const T* R, const T* D,
     }
     ConsArgs<T> ca;
     fill_cons(c, ca, g, R, D, r, ld);
-    // the last kernel of the call (k_long_finish when there are chunks, else k_cons) also does the final sum
-    const bool chunks = c->nchunk_all > 0;
-    int gc = 0;
+    // launches: k_cons (short constraints), k_cons_chunk (chunks of long constraints and of C's list),
+    // k_long_finish (long constraints); whichever comes last also does the final sum
+    const bool chunks = c->nchunk_all > 0, longs = c->nlong_A > 0;
+    int gc = 0, gk = 0;
+    if (chunks) gk = grid_cons<T>(c, g.vec, g.shape, CONS_LS, 1, c->nchunk_all);
     if (c->m > 0) {
       gc = grid_cons<T>(c, g.vec, g.shape, CONS_LS, 0, c->m);
       if (!chunks) ca.fin = make_fin(c, c->part_cons, gc, nullptr, 0, nullptr, 0, c->ls_dev);
@@ -322,12 +334,15 @@ template <typename T> alora_status ls_impl(alora_ctx* c, const T* R, const T* D,
     }
     if (chunks) {
       ca.nchunk = c->nchunk_all;
-      const int gk = grid_cons<T>(c, g.vec, g.shape, CONS_LS, 1, c->nchunk_all);
+      if (!longs) ca.fin = make_fin(c, c->part_cons, gc, c->part_chunk, gk, nullptr, 0, c->ls_dev);
       ALORA_CUDA(c, launch_cons(g.vec, g.shape, CONS_LS, 1, ca, gk, c->stream));
-      k_long_finish<<<c->nlong_all, kBlock, 0, c->stream>>>(CONS_LS, c->m, c->long_cons, c->long_chptr, c->ch_out, c->y,
-                                                           c->b, c->sigma, nullptr, nullptr, c->part_long,
-                                                           make_fin(c, c->part_cons, gc, c->part_long, c->nlong_all, nullptr, 0, c->ls_dev));
-      c->launches += 2;
+      c->launches++;
+      if (longs) {
+        k_long_finish<<<c->nlong_A, kBlock, 0, c->stream>>>(CONS_LS, c->m, c->long_cons, c->long_chptr, c->ch_out, c->y,
+                                                          c->b, c->sigma, nullptr, nullptr, c->part_long,
+                                                          make_fin(c, c->part_cons, gc, c->part_chunk, gk, c->part_long, c->nlong_A, c->ls_dev));
+        c->launches++;
+      }
     } else if (c->m == 0) {
       ALORA_CUDA(c, cudaMemsetAsync(c->ls_dev, 0, sizeof(double) * kNStat, c->stream));
     }

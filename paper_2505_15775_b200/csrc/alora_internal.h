@@ -63,7 +63,7 @@ struct alora_ctx {
   int64_t nf_A = 0, nf_C = 0;
   // chunks of long constraints (first nchunk_A) and of C (the rest); slots: long constraints, then C
   int64_t* ch_beg = nullptr; int64_t* ch_end = nullptr; int64_t nchunk_A = 0, nchunk_all = 0;
-  int* long_cons = nullptr; int64_t* long_chptr = nullptr; int nlong_A = 0, nlong_all = 0;
+  int* long_cons = nullptr; int64_t* long_chptr = nullptr; int nlong_A = 0;
   double* ch_out = nullptr;
   // vectors
   double* b = nullptr; const double* y = nullptr; double sigma = 0.0; bool have_dual = false;
@@ -75,7 +75,7 @@ struct alora_ctx {
   int lr_grid = 0; int lr_rmax = 256;
   // partial sums / results
   int part_cap = 0;
-  double* part_rows = nullptr; double* part_cons = nullptr; double* part_long = nullptr;
+  double* part_rows = nullptr; double* part_cons = nullptr; double* part_long = nullptr; double* part_chunk = nullptr;
   double* stats_dev = nullptr; double* ls_dev = nullptr; double* mv_dev = nullptr;
   unsigned int* ticket = nullptr;   // FinArgs::ticket (kernels.cuh), zero between launches
   double* pinned = nullptr;  // 64 doubles

@@ -22,8 +22,8 @@
 namespace alora {
 
 constexpr int kBlock = 256;
-constexpr int kLongThreshold = 128;  // constraints with more stored entries are split into chunks
-constexpr int kChunk = 64;           // entries per chunk of a long constraint
+constexpr int kLongThreshold = 64;   // constraints with more stored entries are split into chunks
+constexpr int kChunk = 16;           // entries per chunk of a long constraint / of C's sym-upper list
 constexpr int kUN = 4;               // diagonal class: ELL slots per row (first neighbours), see rows_tiled.cuh
 constexpr int kUNL = 3;              // diagonal class, line search: ELL slots per row (last upper-triangle neighbours)
 
@@ -80,7 +80,9 @@ template <typename T> struct ConsArgs {
   double* z; double* lam;         // CONS_EVAL outputs
   // chunk kernel
   int64_t nchunk; const int64_t* ch_beg; const int64_t* ch_end;
-  double* ch_out;                 // [nchunk][3]
+  int64_t nchunk_A;               // chunks [0, nchunk_A) belong to long constraints, the rest to C's sym-upper list
+  double* ch_out;                 // [nchunk_A][3]
+  double* part_chunk;             // chunk kernel: per-block partial rows (sums over C's chunks)
   double* partials;
   FinArgs fin;
 };
@@ -432,6 +434,7 @@ __global__ void __launch_bounds__(kBlock) k_cons(const ConsArgs<T> a) {
     const int64_t e0 = __ldg(a.ptr + i), e1 = __ldg(a.ptr + i + 1);
     if (e1 - e0 > kLongThreshold) continue;  // long constraints: k_cons_chunk + k_long_finish
     T s0 = T(0), s1 = T(0), s2 = T(0);
+#pragma unroll 4
     for (int64_t e = e0; e < e1; ++e) cons_entry<T, VEC, GS, NIT, MODE>(a, e, lane, s0, s1, s2);
     const double z = group_sum<GS>((double)s0, gmask);
     double q1 = 0.0, q2 = 0.0;
@@ -442,21 +445,33 @@ __global__ void __launch_bounds__(kBlock) k_cons(const ConsArgs<T> a) {
   finish_partials(a.fin);
 }
 
-// one group per chunk of <= kChunk entries of a long constraint (or of C's sym-upper list)
+// one group per chunk of <= kChunk entries.  Chunks of a long constraint leave their three sums in ch_out
+// (k_long_finish adds them in order and finishes the constraint); chunks of C's sym-upper list (line search only)
+// go straight into the block's partial row: <C,RR^T>, <C,RD^T> (the entry sum is <C,RD^T+DR^T>, halved) and <C,DD^T>.
 template <typename T, int VEC, int GS, int NIT, int MODE>
 __global__ void __launch_bounds__(kBlock) k_cons_chunk(const ConsArgs<T> a) {
   constexpr int GPB = kBlock / GS;
+  constexpr int NST = 12;
   const int lane = threadIdx.x % GS, grp = threadIdx.x / GS;
   const unsigned gmask = group_mask<GS>();
+  double st[NST];
+#pragma unroll
+  for (int s = 0; s < NST; ++s) st[s] = 0.0;
   for (int64_t c = (int64_t)blockIdx.x * GPB + grp; c < a.nchunk; c += (int64_t)gridDim.x * GPB) {
     const int64_t e0 = __ldg(a.ch_beg + c), e1 = __ldg(a.ch_end + c);
     T s0 = T(0), s1 = T(0), s2 = T(0);
+#pragma unroll 4
     for (int64_t e = e0; e < e1; ++e) cons_entry<T, VEC, GS, NIT, MODE>(a, e, lane, s0, s1, s2);
     const double z = group_sum<GS>((double)s0, gmask);
     double q1 = 0.0, q2 = 0.0;
     if (MODE == CONS_LS) { q1 = group_sum<GS>((double)s1, gmask); q2 = group_sum<GS>((double)s2, gmask); }
-    if (lane == 0) { a.ch_out[3 * c] = z; a.ch_out[3 * c + 1] = q1; a.ch_out[3 * c + 2] = q2; }
+    if (lane == 0) {
+      if (c < a.nchunk_A) { a.ch_out[3 * c] = z; a.ch_out[3 * c + 1] = q1; a.ch_out[3 * c + 2] = q2; }
+      else { st[LS_CRR] += z; st[LS_CRD] += 0.5 * q1; st[LS_CDD] += q2; }
+    }
   }
+  block_reduce_store<NST>(st, a.part_chunk + (int64_t)blockIdx.x * kNStat);
+  finish_partials(a.fin);
 }
 
 // shapes (GS, NIT) by number of VEC-packs per row
