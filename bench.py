@@ -37,21 +37,36 @@ def workload(idx: int):
     return inputs.full(idx)
 
 
-def algorithmic_bytes(w, info) -> int:
+def algorithmic_bytes(w, info):
     """Minimum bytes of one f+grad evaluation, SURVEY.md 8(d) / DESIGN.md "Algorithmic bytes":
-    every array once (nonzeros + indices + R read + G write + y, b read + z write)."""
+    every array once (nonzeros + indices + R read + G write + y, b read + z write).
+    Returns (bytes of the whole evaluation, bytes of its dominant kernel): the diagonal class is ONE
+    kernel; in the general class the dominant kernel is the adjoint pass."""
     P = w.problem
     s = 4 if w.dtype == inputs.F32 else 8
     v = s
     n, m, r = P.n, P.m, w.r
     if info["cls"] == 0:
         full = info["c_nnz"]  # 2|E|
-        return 4 * (n + 1) + (full + n) * (4 + v) + 2 * n * r * s + 24 * n
+        b = 4 * (n + 1) + (full + n) * (4 + v) + 2 * n * r * s + 24 * n
+        return b, b
     e_up, e_full, c_full = info["nf_A"], info["a_nnz"], info["c_nnz"]
     fwd = e_up * (8 + v) + 8 * (m + 1) + n * r * s + 8 * m
     wts = 24 * m
     adj = e_full * (8 + v) + 4 * (n + 1) + (c_full + n) * (4 + v) + 4 * (n + 1) + 8 * m + 2 * n * r * s
-    return fwd + wts + adj
+    return fwd + wts + adj, adj
+
+
+def ncu_traffic(name: str):
+    """DRAM bytes per launch of the dominant kernel from the committed ncu --set full capture
+    (profiles/traffic.json, written by hand from `ncu -i ... --page raw`), or None."""
+    p = os.path.join(ROOT, "profiles", "traffic.json")
+    if not os.path.exists(p):
+        return None
+    try:
+        return json.load(open(p)).get(name, {}).get("dram_bytes_per_launch")
+    except (ValueError, OSError):
+        return None
 
 
 def peaks():
@@ -319,7 +334,7 @@ def main():
 
     if rank == 0:
         peak, peak_src = peaks()
-        B = algorithmic_bytes(w, info)
+        B_eval, B = algorithmic_bytes(w, info)
         kavg_ms = kern_ms / max(1, kern_n)
         achieved = B / (kavg_ms * 1e-3) / 1e9 if kern_n else None
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
@@ -329,12 +344,13 @@ def main():
                 "config": {"workload": w.name, "n": P.n, "m": P.m, "edges": w.meta.get("edges"), "r": r, "ld": ld,
                            "class": "diagonal (one fused pass)" if info["cls"] == 0 else "general (forward + adjoint)",
                            "parallelism": f"replicas x{world}", "l2": "no flush: per-step working set > 126 MB L2"
-                           if B > 126e6 else "no flush: working set is L2-resident (latency-bound config)"},
+                           if B_eval > 126e6 else "no flush: working set is L2-resident (latency-bound config)"},
                 "eval_only_per_s": eval_only,
-                "roofline": {"bound": "hbm", "kernel": "k_rows (fused f+grad pass)" if info["cls"] == 0 else "k_rows (adjoint pass)",
+                "roofline": {"bound": "hbm", "kernel": "k_rows_tiled (fused f+grad pass)" if info["cls"] == 0 else "k_rows (adjoint pass)",
                              "achieved": achieved, "peak": peak, "peak_source": peak_src, "unit": "GB/s",
                              "frac": (achieved / peak) if achieved else None, "algorithmic_bytes": B,
-                             "kernel_ms": kavg_ms, "kernel_launches_timed": kern_n, "traffic": None},
+                             "algorithmic_bytes_whole_eval": B_eval,
+                             "kernel_ms": kavg_ms, "kernel_launches_timed": kern_n, "traffic": ncu_traffic(w.name)},
                 "gpu_launches": int(launches), "clocks": clocks, "e2e": e2e,
                 "check": {"f": st[0], "gnorm": float(np.sqrt(st[4])), "p": [float(x) for x in pls]}}
         if not args.no_cpu_baseline and world == 1:

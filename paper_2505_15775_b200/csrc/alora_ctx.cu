@@ -78,18 +78,29 @@ __global__ void k_lowrank(const T* X, int64_t n, int r, int64_t ld, const T* U, 
   __syncthreads();
   if (!s_last) return;
   __threadfence();
-  const int nblk = gridDim.x, pr = pC * r;
-  for (int idx = threadIdx.x; idx < pr; idx += blockDim.x) {
+  // thread t sums entry t % pr over the blocks t / pr, t / pr + nsl, ... ; the nsl slices are then added in order
+  const int nblk = gridDim.x, pr = pC * r, nsl = max(1, (int)blockDim.x / pr);
+  for (int idx0 = 0; idx0 < pr; idx0 += blockDim.x) {   // one pass unless pC * r > blockDim.x
+    const int idx = idx0 + (int)threadIdx.x % pr, sl = (int)threadIdx.x / pr;
     double v = 0.0;
-    int bk = 0;
-    for (; bk + 3 < nblk; bk += 4) {
-      const double v0 = __ldcg(part + (int64_t)bk * pr + idx), v1 = __ldcg(part + (int64_t)(bk + 1) * pr + idx);
-      const double v2 = __ldcg(part + (int64_t)(bk + 2) * pr + idx), v3 = __ldcg(part + (int64_t)(bk + 3) * pr + idx);
-      v += v0; v += v1; v += v2; v += v3;
+    if (sl < nsl && idx < pr) {
+      int bk = sl;
+      for (; bk + 3 * nsl < nblk; bk += 4 * nsl) {
+        const double v0 = __ldcg(part + (int64_t)bk * pr + idx), v1 = __ldcg(part + (int64_t)(bk + nsl) * pr + idx);
+        const double v2 = __ldcg(part + (int64_t)(bk + 2 * nsl) * pr + idx), v3 = __ldcg(part + (int64_t)(bk + 3 * nsl) * pr + idx);
+        v += v0; v += v1; v += v2; v += v3;
+      }
+      for (; bk < nblk; bk += nsl) v += __ldcg(part + (int64_t)bk * pr + idx);
     }
-    for (; bk < nblk; ++bk) v += __ldcg(part + (int64_t)bk * pr + idx);
-    Tm[idx] = v;
-    if (Ts) Ts[idx] = s[idx / r] * v;
+    __syncthreads();
+    lsm[threadIdx.x] = v;
+    __syncthreads();
+    if (sl == 0 && idx < pr) {
+      double t = 0.0;
+      for (int k = 0; k < nsl; ++k) t += lsm[k * pr + (idx - idx0)];
+      Tm[idx] = t;
+      if (Ts) Ts[idx] = s[idx / r] * t;
+    }
   }
   if (threadIdx.x == 0) *ticket = 0u;
 }
@@ -120,6 +131,7 @@ namespace alora {
 namespace {
 
 int vec_slot(int vec) { return vec == 1 ? 0 : vec == 2 ? 1 : 2; }
+struct Geo { int vec, nvec, shape, exact; };
 
 // records an event on the ctx stream when kernel timing is on (pairs: before / after the dominant kernel)
 void time_mark(alora_ctx* c) {
@@ -186,6 +198,24 @@ alora_status launch_diag_rows(alora_ctx* c, int vec, int nvec, int exact, int sh
   c->launches++;
   return ALORA_OK;
 }
+// general-class adjoint pass: a group per row; single vectors (Lanczos matvec) on long rows take a warp per row
+// (measured on config 3: the warp-per-row kernel wins for p = 1, 66 vs 77 us, and loses for r = 10, 168 vs 128 us)
+template <typename T> alora_status launch_adj_general(alora_ctx* c, const Geo& g, RowArgs<T>& a, double* out) {
+  if (c->ep && g.nvec == 1) {
+    int& occ = c->occ_cache[vec_slot(g.vec)][g.shape][11];
+    if (!occ) occ = std::max(1, occ_rows_ep(T(), g.vec, g.shape));
+    const int64_t need = (c->n + kBlock / 32 - 1) / (kBlock / 32);
+    const int grid = (int)std::max<int64_t>(1, std::min<int64_t>(need, std::min<int64_t>((int64_t)c->num_sms * occ, c->part_cap)));
+    a.fin = make_fin(c, a.fin.p[0], grid, a.fin.p[1], a.fin.n[1], a.fin.p[2], a.fin.n[2], out);
+    ALORA_CUDA(c, launch_rows_ep(g.vec, g.shape, a, grid, c->stream));
+  } else {
+    const int grid = grid_rows<T>(c, g.vec, g.shape, ROWS_ADJ, c->n);
+    a.fin = make_fin(c, a.fin.p[0], grid, a.fin.p[1], a.fin.n[1], a.fin.p[2], a.fin.n[2], out);
+    ALORA_CUDA(c, launch_rows(g.vec, g.shape, ROWS_ADJ, a, grid, c->stream));
+  }
+  c->launches++;
+  return ALORA_OK;
+}
 template <typename T> int grid_cons(alora_ctx* c, int vec, int shape, int mode, int chunked, int64_t items) {
   int& occ = c->occ_cache[vec_slot(vec)][shape][3 + mode * 2 + chunked];
   if (!occ) occ = std::max(1, occ_cons(T(), vec, shape, mode, chunked));
@@ -194,7 +224,6 @@ template <typename T> int grid_cons(alora_ctx* c, int vec, int shape, int mode, 
   return (int)std::max<int64_t>(1, std::min<int64_t>(need, std::min<int64_t>((int64_t)c->num_sms * occ, c->part_cap)));
 }
 
-struct Geo { int vec, nvec, shape, exact; };
 alora_status geometry(alora_ctx* c, int32_t r, int64_t ld, const void* p0, const void* p1, const void* p2, Geo& g) {
   if (r < 1 || ld < r) return fail(c, ALORA_EINVAL, "need 1 <= r <= ld");
   if (((uintptr_t)p0 % c->esz) || ((uintptr_t)p1 % c->esz) || ((uintptr_t)p2 % c->esz)) return fail(c, ALORA_EINVAL, "misaligned pointer");
@@ -272,12 +301,11 @@ template <typename T> alora_status eval_impl(alora_ctx* c, const T* R, int32_t r
       c->launches += 2;
     }
     a.w = c->lam; a.diag_class = 0;
-    const int grid = grid_rows<T>(c, g.vec, g.shape, ROWS_ADJ, c->n);
-    a.fin = make_fin(c, c->part_rows, grid, c->part_cons, gc, c->part_long, c->nlong_A, c->stats_dev);   // last kernel of the call
+    a.fin = make_fin(c, c->part_rows, 0, c->part_cons, gc, c->part_long, c->nlong_A, nullptr);   // last kernel of the call
     time_mark(c);
-    ALORA_CUDA(c, launch_rows(g.vec, g.shape, ROWS_ADJ, a, grid, c->stream));
+    s = launch_adj_general<T>(c, g, a, c->stats_dev);
+    if (s != ALORA_OK) return s;
     time_mark(c);
-    c->launches++;
   }
   ALORA_CUDA(c, cudaGetLastError());
   c->z_last = zout; c->have_eval = true;
@@ -391,10 +419,9 @@ template <typename T> alora_status matvec_impl(alora_ctx* c, const double* mu, c
     s = launch_diag_rows<T>(c, g.vec, g.nvec, g.exact, g.shape, ROWS_ADJ, a, mu, c->mv_dev);
     if (s != ALORA_OK) return s;
   } else {
-    const int grid = grid_rows<T>(c, g.vec, g.shape, ROWS_ADJ, c->n);
-    a.fin = make_fin(c, c->part_rows, grid, nullptr, 0, nullptr, 0, c->mv_dev);
-    ALORA_CUDA(c, launch_rows(g.vec, g.shape, ROWS_ADJ, a, grid, c->stream));
-    c->launches++;
+    a.fin = make_fin(c, c->part_rows, 0, nullptr, 0, nullptr, 0, nullptr);
+    s = launch_adj_general<T>(c, g, a, c->mv_dev);
+    if (s != ALORA_OK) return s;
   }
   ALORA_CUDA(c, cudaGetLastError());
   return ALORA_OK;

@@ -12,6 +12,8 @@ namespace alora {
   cudaError_t launch_tiled_##SUF(int shape, int mode, int full, const RowArgs<T>& a, int grid, cudaStream_t s); \
   int occ_tiled_##SUF(int shape, int mode, int full, int64_t ld);                                                        \
   int occ_rows_##SUF(int shape, int mode);                                                            \
+  cudaError_t launch_rows_ep_##SUF(int shape, const RowArgs<T>& a, int grid, cudaStream_t s);         \
+  int occ_rows_ep_##SUF(int shape);                                                                   \
   int occ_cons_##SUF(int shape, int mode, int chunked);
 
 ALORA_DECL_INST(float, f32v4)
@@ -29,6 +31,17 @@ inline cudaError_t launch_rows(int vec, int shape, int mode, const RowArgs<float
 inline cudaError_t launch_rows(int vec, int shape, int mode, const RowArgs<double>& a, int grid, cudaStream_t s) {
   return vec == 2 ? launch_rows_f64v2(shape, mode, a, grid, s) : launch_rows_f64v1(shape, mode, a, grid, s);
 }
+inline cudaError_t launch_rows_ep(int vec, int shape, const RowArgs<float>& a, int grid, cudaStream_t s) {
+  return vec == 4 ? launch_rows_ep_f32v4(shape, a, grid, s)
+       : vec == 2 ? launch_rows_ep_f32v2(shape, a, grid, s) : launch_rows_ep_f32v1(shape, a, grid, s);
+}
+inline cudaError_t launch_rows_ep(int vec, int shape, const RowArgs<double>& a, int grid, cudaStream_t s) {
+  return vec == 2 ? launch_rows_ep_f64v2(shape, a, grid, s) : launch_rows_ep_f64v1(shape, a, grid, s);
+}
+inline int occ_rows_ep(float, int vec, int shape) {
+  return vec == 4 ? occ_rows_ep_f32v4(shape) : vec == 2 ? occ_rows_ep_f32v2(shape) : occ_rows_ep_f32v1(shape);
+}
+inline int occ_rows_ep(double, int vec, int shape) { return vec == 2 ? occ_rows_ep_f64v2(shape) : occ_rows_ep_f64v1(shape); }
 inline cudaError_t launch_cons(int vec, int shape, int mode, int chunked, const ConsArgs<float>& a, int grid, cudaStream_t s) {
   return vec == 4 ? launch_cons_f32v4(shape, mode, chunked, a, grid, s)
        : vec == 2 ? launch_cons_f32v2(shape, mode, chunked, a, grid, s) : launch_cons_f32v1(shape, mode, chunked, a, grid, s);

@@ -382,6 +382,90 @@ __global__ void __launch_bounds__(kBlock) k_rows(const RowArgs<T> a) {
 }
 
 // ---------------------------------------------------------------------------------------------
+// Weighted-adjoint SpMM for LONG rows (general class, tens of entries per row): one WARP per row, the 32 lanes
+// split as PL pack lanes x EL = 32 / PL entry lanes.  Entry lane el walks entries el, el + EL, ... of the row's C
+// list and of its constraint list, so a row has EL independent gather chains instead of one; the partial rows are
+// added across the entry lanes with shuffles at the end.  <C,XX^T> needs the C part alone: every lane keeps its own
+// scalar sum of c_e <X_k, X_row> over the C entries it handled (no extra reduction).  ROWS_ADJ semantics.
+template <typename T, int VEC, int PL, int NIT>
+__global__ void __launch_bounds__(kBlock) k_rows_ep(const RowArgs<T> a) {
+  using Row = RowReg<T, VEC, PL, NIT>;
+  constexpr int EL = 32 / PL, WPB = kBlock / 32, NST = 6;
+  const int lane32 = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int pl = lane32 % PL, el = lane32 / PL;
+  const int nvec = a.nvec, r = a.r, exact = a.exact;
+  const T sc = (T)a.scale;
+  double st[NST];
+#pragma unroll
+  for (int s = 0; s < NST; ++s) st[s] = 0.0;
+  for (int64_t row = (int64_t)blockIdx.x * WPB + warp; row < a.n; row += (int64_t)gridDim.x * WPB) {
+    Row x; x.load(a.X + row * a.ld, pl, nvec, r, exact);
+    Row acc; acc.zero();
+    T cxl = T(0);
+    const int cb = __ldg(a.c_rowptr + row), ce = __ldg(a.c_rowptr + row + 1);
+#pragma unroll 2
+    for (int e = cb + el; e < ce; e += EL) {
+      const int k = __ldg(a.c_col + e);
+      const T v = __ldg(a.c_val + e);
+      Row xn; xn.load(a.X + (int64_t)k * a.ld, pl, nvec, r, exact);
+      acc.axpy(v, xn);
+      cxl = fma(v, xn.dot(x), cxl);
+    }
+    double coef = 0.0;
+    if (a.diag_class) {
+      const int c = a.dcons ? __ldg(a.dcons + row) : (int)row;
+      if (c >= 0) coef = __ldg(a.w + c) * (a.da ? (double)__ldg(a.da + row) : 1.0);
+    } else {
+      const int ab = __ldg(a.a_rowptr + row), ae = __ldg(a.a_rowptr + row + 1);
+#pragma unroll 2
+      for (int e = ab + el; e < ae; e += EL) {
+        const int k = __ldg(a.a_col + e);
+        const T wv = (T)(-__ldg(a.w + __ldg(a.a_cons + e)) * (double)__ldg(a.a_val + e));
+        Row xn; xn.load(a.X + (int64_t)k * a.ld, pl, nvec, r, exact);
+        acc.axpy(wv, xn);
+      }
+    }
+#pragma unroll
+    for (int off = PL; off < 32; off <<= 1)
+#pragma unroll
+      for (int it = 0; it < NIT; ++it)
+#pragma unroll
+        for (int i = 0; i < VEC; ++i) acc.p[it].v[i] += __shfl_xor_sync(0xffffffffu, acc.p[it].v[i], off);
+    // every entry lane now holds the whole row; entry lane 0 finishes it
+    const T dc = __ldg(a.dC + row);
+    if (el == 0) cxl = fma(dc, x.dot(x), cxl);
+    acc.axpy(dc, x);
+    for (int p = 0; p < a.pC; ++p) {  // low-rank cost term: + U[row,p] * s_p (U^T X)_p
+      const T up = __ldg(a.U + row * a.pC + p);
+#pragma unroll
+      for (int it = 0; it < NIT; ++it) {
+        const int vi = pl + it * PL;
+        if (vi < nvec) {
+#pragma unroll
+          for (int i = 0; i < VEC; ++i) {
+            const int cidx = vi * VEC + i;
+            if (cidx < r) acc.p[it].v[i] = fma(up, (T)__ldg(a.Ts + p * r + cidx), acc.p[it].v[i]);
+          }
+        }
+      }
+    }
+    acc.axpy((T)(-coef), x);
+#pragma unroll
+    for (int it = 0; it < NIT; ++it)
+#pragma unroll
+      for (int i = 0; i < VEC; ++i) acc.p[it].v[i] *= sc;
+    st[ES_CX] += (double)cxl;
+    if (el == 0) {
+      st[ES_GG] += (double)acc.dot(acc);
+      st[ES_GR] += (double)acc.dot(x);
+      if (a.Out) acc.store(a.Out + row * a.ld, pl, nvec, r, exact);
+    }
+  }
+  block_reduce_store<NST>(st, a.partials + (int64_t)blockIdx.x * kNStat);
+  finish_partials(a.fin);
+}
+
+// ---------------------------------------------------------------------------------------------
 // Forward (SDDMM-style) evaluator.  One entry e = (j, k, a), j <= k, contributes
 //   w a <X_j, X_k>                 with w = 1 (j == k) or 2 (j < k)            -> z
 //   w a (<X_j,D_k> + <D_j,X_k>)    (= <A, XD^T + DX^T> restricted to the entry)  -> q1
