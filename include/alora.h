@@ -170,8 +170,8 @@ typedef struct {
 /* ALORA (Algorithm 1) on the ctx's problem.  State in/out: R_dev (DEVICE, ctx dtype, capacity
  * n*r_cap elements; on entry row-major n x *r_inout with ld = *r_inout, on exit row-major
  * n x *r_inout with ld = *r_inout), y_dev (DEVICE fp64[m], updated in place), *sigma_inout.
- * r_cap must leave room for growth (one column per outer iteration that grows, rounded up to a
- * multiple of 4); ALORA_EINVAL if growth would exceed it.  log: HOST array of log_cap records or NULL.
+ * r_cap bounds the rank: an outer iteration that would grow beyond it skips the growth step and carries on
+ * at rank r_cap (reading 27).  log: HOST array of log_cap records or NULL.
  * Returns ALORA_OK on convergence, ALORA_ENOTCONV at T_max.  (R, r, y, sigma) is the whole state of
  * Alg. 1, so a caller can checkpoint / resume with it. */
 alora_status alora_solve(alora_ctx *ctx, const alora_params *prm, void *R_dev, int32_t *r_inout,

@@ -19,7 +19,7 @@ LIB = os.path.join(CSRC, "libalora.so")
 INCLUDE = os.path.join(os.path.dirname(HERE), "include")
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
-         "-Xcompiler", "-fPIC", "-I", INCLUDE]
+         "-Xcompiler", "-fPIC", "-I", INCLUDE] + os.environ.get("ALORA_NVCC_EXTRA", "").split()   # e.g. -DALORA_KSTAGES=3
 
 
 def _sources():

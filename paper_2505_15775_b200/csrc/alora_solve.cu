@@ -67,6 +67,126 @@ __global__ void __launch_bounds__(kBlock) k_make_pair(int64_t N, double alpha, c
   }
   block_reduce_store<3>(st, part + (int64_t)blockIdx.x * kNStat);
 }
+// ---- fused L-BFGS passes ("L-BFGS in two passes") ----------------------------------------
+// The two-loop recursion only ever forms linear combinations of g, S_j, Y_j, so the direction is
+//   d = cg g + sum_j cs_j S_j + sum_j cy_j Y_j
+// with coefficients that follow from the dot products S_j.g, Y_j.g and the Gram blocks S_i.Y_j, Y_i.Y_j.  The Gram
+// blocks change by one row / column per iteration (the new pair).  So an iteration needs two passes over the
+// vectors instead of 4m + 6: k_lbfgs_dots (build the new pair, all new dot products) and k_lbfgs_combine.
+constexpr int kLbMax = 8;            // pairs the fused path handles (memory <= kLbMax - 1)
+constexpr int kLbW = 48;             // doubles per partial row (5 * kLbMax + 1 sums, padded)
+struct LbVecs { const void* S[kLbMax]; const void* Y[kLbMax]; };
+struct LbCoef { double cg; double cs[kLbMax]; double cy[kLbMax]; };
+
+// Builds S_new = alpha D, Y_new = G - Gp into the LAST listed pair (if have_new) and sums, for the np listed pairs j:
+//   [j] S_j.G   [np + j] Y_j.G   [2np + j] S_new.Y_j   [3np + j] S_j.Y_new   [4np + j] Y_new.Y_j   [5np] S_new.S_new
+// (the last four only if have_new).  Partial rows of kLbW doubles per block; the block that finishes last adds
+// them in block order into out[kLbW].
+template <typename T, int NP>
+__global__ void __launch_bounds__(kBlock) k_lbfgs_dots(int64_t N, int have_new, double alpha, const T* D, const T* G, const T* Gp,
+                                                       LbVecs v, T* Snew, T* Ynew, double* part, double* out,
+                                                       unsigned int* ticket) {
+  constexpr int VEC = 16 / (int)sizeof(T);
+  double sg[NP], yg[NP], sny[NP], syn[NP], yyn[NP], ss = 0.0;
+#pragma unroll
+  for (int j = 0; j < NP; ++j) { sg[j] = yg[j] = sny[j] = syn[j] = yyn[j] = 0.0; }
+  const int64_t nv = N / VEC;
+  for (int64_t i = (int64_t)blockIdx.x * kBlock + threadIdx.x; i < nv; i += (int64_t)gridDim.x * kBlock) {
+    const Pack<T, VEC> g = reinterpret_cast<const Pack<T, VEC>*>(G)[i];
+    Pack<T, VEC> sn, yn;
+    if (have_new) {
+      const Pack<T, VEC> d = reinterpret_cast<const Pack<T, VEC>*>(D)[i], gp = reinterpret_cast<const Pack<T, VEC>*>(Gp)[i];
+#pragma unroll
+      for (int k = 0; k < VEC; ++k) { sn.v[k] = (T)(alpha * (double)d.v[k]); yn.v[k] = (T)((double)g.v[k] - (double)gp.v[k]); }
+      reinterpret_cast<Pack<T, VEC>*>(Snew)[i] = sn;
+      reinterpret_cast<Pack<T, VEC>*>(Ynew)[i] = yn;
+    }
+#pragma unroll
+    for (int j = 0; j < NP; ++j) {
+      Pack<T, VEC> sj, yj;
+      if (have_new && j == NP - 1) { sj = sn; yj = yn; }
+      else { sj = reinterpret_cast<const Pack<T, VEC>*>(v.S[j])[i]; yj = reinterpret_cast<const Pack<T, VEC>*>(v.Y[j])[i]; }
+#pragma unroll
+      for (int k = 0; k < VEC; ++k) {
+        const double gs = (double)g.v[k], s_ = (double)sj.v[k], y_ = (double)yj.v[k];
+        sg[j] += s_ * gs; yg[j] += y_ * gs;
+        if (have_new) {
+          const double sn_ = (double)sn.v[k], yn_ = (double)yn.v[k];
+          sny[j] += sn_ * y_; syn[j] += s_ * yn_; yyn[j] += yn_ * y_;
+        }
+      }
+    }
+    if (have_new) {
+#pragma unroll
+      for (int k = 0; k < VEC; ++k) ss += (double)sn.v[k] * (double)sn.v[k];
+    }
+  }
+  __shared__ double sm[kLbW][kBlock / 32];
+  __shared__ unsigned int s_last;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  auto put = [&](int slot, double val) { const double t = warp_sum(val); if (lane == 0) sm[slot][warp] = t; };
+#pragma unroll
+  for (int j = 0; j < NP; ++j) { put(j, sg[j]); put(NP + j, yg[j]); put(2 * NP + j, sny[j]); put(3 * NP + j, syn[j]); put(4 * NP + j, yyn[j]); }
+  put(5 * NP, ss);
+  __syncthreads();
+  if (threadIdx.x < kLbW) {
+    double t = 0.0;
+    if (threadIdx.x <= 5 * NP)
+      for (int wv = 0; wv < kBlock / 32; ++wv) t += sm[threadIdx.x][wv];
+    part[(int64_t)blockIdx.x * kLbW + threadIdx.x] = t;
+  }
+  __threadfence();
+  __syncthreads();
+  if (threadIdx.x == 0) s_last = (atomicAdd(ticket, 1u) == gridDim.x - 1) ? 1u : 0u;
+  __syncthreads();
+  if (!s_last) return;
+  __threadfence();
+  // ordered final sum: thread t owns column t % kLbW and the rows t / kLbW, + 5, ... (kBlock / kLbW = 5 slices)
+  __shared__ double fin[kBlock];
+  constexpr int NSL = kBlock / kLbW;
+  const int col = threadIdx.x % kLbW, sl = threadIdx.x / kLbW;
+  double t = 0.0;
+  if (sl < NSL) {
+    int b = sl;
+    for (; b + 3 * NSL < (int)gridDim.x; b += 4 * NSL) {
+      const double v0 = __ldcg(part + (int64_t)b * kLbW + col), v1 = __ldcg(part + (int64_t)(b + NSL) * kLbW + col);
+      const double v2 = __ldcg(part + (int64_t)(b + 2 * NSL) * kLbW + col), v3 = __ldcg(part + (int64_t)(b + 3 * NSL) * kLbW + col);
+      t += v0; t += v1; t += v2; t += v3;
+    }
+    for (; b < (int)gridDim.x; b += NSL) t += __ldcg(part + (int64_t)b * kLbW + col);
+  }
+  fin[threadIdx.x] = t;
+  __syncthreads();
+  if (threadIdx.x < kLbW) {
+    double u = 0.0;
+    for (int k = 0; k < NSL; ++k) u += fin[k * kLbW + threadIdx.x];
+    out[threadIdx.x] = u;
+  }
+  if (threadIdx.x == 0) *ticket = 0u;
+}
+
+// D = cg G + sum_j cs_j S_j + cy_j Y_j   (one pass, fp64 accumulation, rounded once)
+template <typename T, int NP>
+__global__ void __launch_bounds__(kBlock) k_lbfgs_combine(int64_t N, const T* G, LbVecs v, LbCoef c, T* D) {
+  constexpr int VEC = 16 / (int)sizeof(T);
+  const int64_t nv = N / VEC;
+  for (int64_t i = (int64_t)blockIdx.x * kBlock + threadIdx.x; i < nv; i += (int64_t)gridDim.x * kBlock) {
+    const Pack<T, VEC> g = reinterpret_cast<const Pack<T, VEC>*>(G)[i];
+    double acc[VEC];
+#pragma unroll
+    for (int k = 0; k < VEC; ++k) acc[k] = c.cg * (double)g.v[k];
+#pragma unroll
+    for (int j = 0; j < NP; ++j) {
+      const Pack<T, VEC> sj = reinterpret_cast<const Pack<T, VEC>*>(v.S[j])[i], yj = reinterpret_cast<const Pack<T, VEC>*>(v.Y[j])[i];
+#pragma unroll
+      for (int k = 0; k < VEC; ++k) acc[k] += c.cs[j] * (double)sj.v[k] + c.cy[j] * (double)yj.v[k];
+    }
+    Pack<T, VEC> o;
+#pragma unroll
+    for (int k = 0; k < VEC; ++k) o.v[k] = (T)acc[k];
+    reinterpret_cast<Pack<T, VEC>*>(D)[i] = o;
+  }
+}
 // w -= a v + b u   (Lanczos three-term recurrence)
 template <typename T> __global__ void k_axpy2(int64_t N, double a, const T* v, double b, const T* u, T* w) {
   for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (int64_t)gridDim.x * blockDim.x)
@@ -176,6 +296,7 @@ struct SolveWorkspace {
   void* w = nullptr;                 // n
   double* bd_part = nullptr; double* cvec = nullptr; int bd_chunks = 0;
   double* red_part = nullptr; double* red_out = nullptr;
+  double* lb_part = nullptr; double* lb_out = nullptr;   // k_lbfgs_dots partial rows / result
   // solve
   void* buf[4 + 2 * 16] = {}; int nbuf = 0; int64_t buf_elems = 0;
   double* lam = nullptr; double* z = nullptr; double* zv = nullptr; void* ritz = nullptr;
@@ -386,6 +507,8 @@ alora_status ensure_ws(alora_ctx* c) {
   SolveWorkspace* w = c->ws;
   ALORA_CUDA(c, c->pool.alloc((void**)&w->red_part, sizeof(double) * kNStat * kRedBlocks));
   ALORA_CUDA(c, c->pool.alloc((void**)&w->red_out, sizeof(double) * kNStat));
+  ALORA_CUDA(c, c->pool.alloc((void**)&w->lb_part, sizeof(double) * kLbW * kRedBlocks));
+  ALORA_CUDA(c, c->pool.alloc((void**)&w->lb_out, sizeof(double) * kLbW));
   ALORA_CUDA(c, c->pool.alloc(&w->w, c->esz * c->n));
   ALORA_CUDA(c, c->pool.alloc(&w->ritz, c->esz * c->n));
   ALORA_CUDA(c, c->pool.alloc((void**)&w->lam, sizeof(double) * std::max<int64_t>(1, c->m)));
@@ -520,6 +643,37 @@ namespace alora {
 namespace {
 
 template <typename T>
+alora_status lbfgs_dots(alora_ctx* c, int64_t N, int np, bool have_new, double alpha, const T* D, const T* G, const T* Gp,
+                        const LbVecs& v, T* Snew, T* Ynew, double* host_out) {
+  SolveWorkspace* w = c->ws;
+  const int grid = (int)std::max<int64_t>(1, std::min<int64_t>((N / (16 / (int64_t)sizeof(T)) + kBlock - 1) / kBlock, kRedBlocks));
+  switch (np) {
+#define X(NP) case NP: k_lbfgs_dots<T, NP><<<grid, kBlock, 0, c->stream>>>(N, have_new ? 1 : 0, alpha, D, G, Gp, v, Snew, Ynew, w->lb_part, w->lb_out, c->ticket); break;
+    X(1) X(2) X(3) X(4) X(5) X(6) X(7) X(8)
+#undef X
+    default: return fail(c, ALORA_EINVAL, "lbfgs_dots: too many pairs");
+  }
+  c->launches++;
+  ALORA_CUDA(c, cudaMemcpyAsync(c->pinned + 64, w->lb_out, sizeof(double) * kLbW, cudaMemcpyDeviceToHost, c->stream));
+  ALORA_CUDA(c, cudaStreamSynchronize(c->stream));
+  for (int i = 0; i < kLbW; ++i) host_out[i] = c->pinned[64 + i];
+  return ALORA_OK;
+}
+template <typename T>
+alora_status lbfgs_combine(alora_ctx* c, int64_t N, int np, const T* G, const LbVecs& v, const LbCoef& cf, T* D) {
+  const int grid = (int)std::max<int64_t>(1, std::min<int64_t>((N / (16 / (int64_t)sizeof(T)) + kBlock - 1) / kBlock, (int64_t)c->num_sms * 8));
+  switch (np) {
+#define X(NP) case NP: k_lbfgs_combine<T, NP><<<grid, kBlock, 0, c->stream>>>(N, G, v, cf, D); break;
+    X(1) X(2) X(3) X(4) X(5) X(6) X(7) X(8)
+#undef X
+    default: return fail(c, ALORA_EINVAL, "lbfgs_combine: too many pairs");
+  }
+  c->launches++;
+  ALORA_CUDA(c, cudaGetLastError());
+  return ALORA_OK;
+}
+
+template <typename T>
 alora_status solve_impl(alora_ctx* c, const alora_params* prm, T* R_user, int32_t* r_inout, int32_t r_cap, double* y,
                         double* sigma_inout, alora_iter_record* log, int32_t log_cap, alora_result* res) {
   const auto t_start = std::chrono::steady_clock::now();
@@ -577,53 +731,123 @@ alora_status solve_impl(alora_ctx* c, const alora_params* prm, T* R_user, int32_
     std::vector<int> pairs;                 // physical slots of the stored pairs, oldest first
     int spare = 0;                          // physical slot that receives the next candidate pair
     std::vector<double> sy(nslot), yy(nslot), alp(nslot);
+    std::vector<std::vector<double>> lb_SY(nslot, std::vector<double>(nslot, 0.0)), lb_YY(nslot, std::vector<double>(nslot, 0.0));
+    std::vector<double> lb_sg(nslot, 0.0), lb_yg(nslot, 0.0);
     int it = 0; bool have_prev = false; double alpha = 0.0, gnorm = 0.0;
     while (true) {
       s = alora_eval(c, Rw, ld, ld, Gw, w->z, st); if (s != ALORA_OK) return s;
       ++rec.n_evals;
       gnorm = std::sqrt(st[4]);
       if (!std::isfinite(st[0]) || !std::isfinite(gnorm)) return fail(c, ALORA_ECUDA, "alora_solve: non-finite f or gradient");
-      if (have_prev && mem > 0) {
-        const int slot = spare;
-        const int gr = (int)std::max<int64_t>(1, std::min<int64_t>((N + kBlock - 1) / kBlock, kRedBlocks));
-        k_make_pair<T><<<gr, kBlock, 0, c->stream>>>(N, alpha, Dw, Gw, Gp, Sb[slot], Yb[slot], w->red_part);
-        k_reduce_rows<<<1, kBlock, 0, c->stream>>>(w->red_part, gr, w->red_out);
-        c->launches += 2;
-        ALORA_CUDA(c, cudaMemcpyAsync(c->pinned + 48, w->red_out, sizeof(double) * 3, cudaMemcpyDeviceToHost, c->stream));
-        ALORA_CUDA(c, cudaStreamSynchronize(c->stream));
-        const double v_sy = c->pinned[48], v_ss = c->pinned[49], v_yy = c->pinned[50];
-        if (v_sy > 1e-10 * std::sqrt(v_ss * v_yy)) {
-          sy[slot] = v_sy; yy[slot] = v_yy;
-          pairs.push_back(slot);
-          if ((int)pairs.size() > mem) { spare = pairs.front(); pairs.erase(pairs.begin()); }
-          else { spare = (int)pairs.size(); }   // slots 0..mem are handed out in order until the ring is full
+      const bool fused = mem > 0 && mem < kLbMax;
+      bool steepest = true;
+      if (fused) {
+        // ---- L-BFGS in two passes: all dot products of the iteration (and the new pair) in k_lbfgs_dots, the
+        //      coefficients of d in span{g, S_j, Y_j} on the host (same recursion as the two-loop form), one combine
+        std::vector<int> list(pairs);
+        if (have_prev) list.push_back(spare);
+        const int np = (int)list.size();
+        if (np > 0) {
+          LbVecs lv;
+          for (int j = 0; j < kLbMax; ++j) { lv.S[j] = Sb[list[j < np ? j : 0]]; lv.Y[j] = Yb[list[j < np ? j : 0]]; }
+          double h[kLbW];
+          s = lbfgs_dots<T>(c, N, np, have_prev, alpha, Dw, Gw, Gp, lv, Sb[spare], Yb[spare], h); if (s != ALORA_OK) return s;
+          for (int j = 0; j < np; ++j) { lb_sg[list[j]] = h[j]; lb_yg[list[j]] = h[np + j]; }
+          if (have_prev) {
+            const int slot = spare;
+            const double v_sy = h[2 * np + np - 1], v_yy = h[4 * np + np - 1], v_ss = h[5 * np];
+            if (v_sy > 1e-10 * std::sqrt(v_ss * v_yy)) {
+              for (int j = 0; j < np; ++j) {
+                lb_SY[slot][list[j]] = h[2 * np + j];   // S_new . Y_j
+                lb_SY[list[j]][slot] = h[3 * np + j];   // S_j . Y_new
+                lb_YY[slot][list[j]] = lb_YY[list[j]][slot] = h[4 * np + j];
+              }
+              sy[slot] = v_sy; yy[slot] = v_yy;
+              pairs.push_back(slot);
+              if ((int)pairs.size() > mem) { spare = pairs.front(); pairs.erase(pairs.begin()); }
+              else { spare = (int)pairs.size(); }
+            }
+          }
         }
-      }
-      if (gnorm / (1.0 + normC) <= tol_t || it >= prm->it_max) break;
-      // direction: two-loop recursion (reading 5); q lives in Dw
-      bool steepest = pairs.empty();
-      if (!steepest) {
-        ALORA_CUDA(c, cudaMemcpyAsync(Dw, Gw, sizeof(T) * N, cudaMemcpyDeviceToDevice, c->stream));
-        for (int i = (int)pairs.size() - 1; i >= 0; --i) {
-          const int sl = pairs[i];
-          double d; s = dot1<T>(c, N, Sb[sl], Dw, &d); if (s != ALORA_OK) return s;
-          alp[sl] = d / sy[sl];
-          k_axpy<T><<<g, 256, 0, c->stream>>>(N, -alp[sl], Yb[sl], Dw);
+        if (gnorm / (1.0 + normC) <= tol_t || it >= prm->it_max) break;
+        if (!pairs.empty()) {
+          const int k = (int)pairs.size();
+          std::vector<double> al(k), aq(k), bs(k);   // alpha_i; q = g + sum aq_j Y_j; r = gamma q + sum bs_j S_j
+          for (int i = k - 1; i >= 0; --i) {
+            const int si = pairs[i];
+            double sq = lb_sg[si];
+            for (int j = i + 1; j < k; ++j) sq += aq[j] * lb_SY[si][pairs[j]];
+            al[i] = sq / sy[si];
+            aq[i] = -al[i];
+          }
+          const int nw = pairs.back();
+          const double gamma = sy[nw] / yy[nw];
+          for (int i = 0; i < k; ++i) {
+            const int si = pairs[i];
+            double yq = lb_yg[si];
+            for (int j = 0; j < k; ++j) yq += aq[j] * lb_YY[si][pairs[j]];
+            double yr = gamma * yq;
+            for (int j = 0; j < i; ++j) yr += bs[j] * lb_SY[pairs[j]][si];
+            bs[i] = al[i] - yr / sy[si];
+          }
+          LbCoef cf; LbVecs lv;
+          cf.cg = -gamma;
+          double gd = cf.cg * st[4];
+          for (int j = 0; j < kLbMax; ++j) {
+            const int sl = pairs[j < k ? j : 0];
+            lv.S[j] = Sb[sl]; lv.Y[j] = Yb[sl];
+            cf.cs[j] = j < k ? -bs[j] : 0.0;
+            cf.cy[j] = j < k ? -gamma * aq[j] : 0.0;
+            if (j < k) gd += cf.cs[j] * lb_sg[sl] + cf.cy[j] * lb_yg[sl];
+          }
+          if (gd < 0.0) {
+            s = lbfgs_combine<T>(c, N, k, Gw, lv, cf, Dw); if (s != ALORA_OK) return s;
+            steepest = false;
+          } else { pairs.clear(); spare = 0; }   // not a descent direction: restart from -G
+        }
+      } else {
+        if (have_prev && mem > 0) {
+          const int slot = spare;
+          const int gr = (int)std::max<int64_t>(1, std::min<int64_t>((N + kBlock - 1) / kBlock, kRedBlocks));
+          k_make_pair<T><<<gr, kBlock, 0, c->stream>>>(N, alpha, Dw, Gw, Gp, Sb[slot], Yb[slot], w->red_part);
+          k_reduce_rows<<<1, kBlock, 0, c->stream>>>(w->red_part, gr, w->red_out);
+          c->launches += 2;
+          ALORA_CUDA(c, cudaMemcpyAsync(c->pinned + 48, w->red_out, sizeof(double) * 3, cudaMemcpyDeviceToHost, c->stream));
+          ALORA_CUDA(c, cudaStreamSynchronize(c->stream));
+          const double v_sy = c->pinned[48], v_ss = c->pinned[49], v_yy = c->pinned[50];
+          if (v_sy > 1e-10 * std::sqrt(v_ss * v_yy)) {
+            sy[slot] = v_sy; yy[slot] = v_yy;
+            pairs.push_back(slot);
+            if ((int)pairs.size() > mem) { spare = pairs.front(); pairs.erase(pairs.begin()); }
+            else { spare = (int)pairs.size(); }   // slots 0..mem are handed out in order until the ring is full
+          }
+        }
+        if (gnorm / (1.0 + normC) <= tol_t || it >= prm->it_max) break;
+        // direction: two-loop recursion (reading 5); q lives in Dw
+        steepest = pairs.empty();
+        if (!steepest) {
+          ALORA_CUDA(c, cudaMemcpyAsync(Dw, Gw, sizeof(T) * N, cudaMemcpyDeviceToDevice, c->stream));
+          for (int i = (int)pairs.size() - 1; i >= 0; --i) {
+            const int sl = pairs[i];
+            double d; s = dot1<T>(c, N, Sb[sl], Dw, &d); if (s != ALORA_OK) return s;
+            alp[sl] = d / sy[sl];
+            k_axpy<T><<<g, 256, 0, c->stream>>>(N, -alp[sl], Yb[sl], Dw);
+            c->launches++;
+          }
+          const int nw = pairs.back();
+          k_scale<T><<<g, 256, 0, c->stream>>>(N, sy[nw] / yy[nw], Dw);
           c->launches++;
-        }
-        const int nw = pairs.back();
-        k_scale<T><<<g, 256, 0, c->stream>>>(N, sy[nw] / yy[nw], Dw);
-        c->launches++;
-        for (size_t i = 0; i < pairs.size(); ++i) {
-          const int sl = pairs[i];
-          double d; s = dot1<T>(c, N, Yb[sl], Dw, &d); if (s != ALORA_OK) return s;
-          k_axpy<T><<<g, 256, 0, c->stream>>>(N, alp[sl] - d / sy[sl], Sb[sl], Dw);
+          for (size_t i = 0; i < pairs.size(); ++i) {
+            const int sl = pairs[i];
+            double d; s = dot1<T>(c, N, Yb[sl], Dw, &d); if (s != ALORA_OK) return s;
+            k_axpy<T><<<g, 256, 0, c->stream>>>(N, alp[sl] - d / sy[sl], Sb[sl], Dw);
+            c->launches++;
+          }
+          k_scale<T><<<g, 256, 0, c->stream>>>(N, -1.0, Dw);
           c->launches++;
+          double gd; s = dot1<T>(c, N, Gw, Dw, &gd); if (s != ALORA_OK) return s;
+          if (gd >= 0.0) { pairs.clear(); spare = 0; steepest = true; }   // not a descent direction: restart from -G
         }
-        k_scale<T><<<g, 256, 0, c->stream>>>(N, -1.0, Dw);
-        c->launches++;
-        double gd; s = dot1<T>(c, N, Gw, Dw, &gd); if (s != ALORA_OK) return s;
-        if (gd >= 0.0) { pairs.clear(); spare = 0; steepest = true; }   // not a descent direction: restart from -G
       }
       if (steepest) { k_scale_copy<T><<<g, 256, 0, c->stream>>>(N, -1.0, Gw, Dw); c->launches++; }
       double p[5];
@@ -648,9 +872,10 @@ alora_status solve_impl(alora_ctx* c, const alora_params* prm, T* R_user, int32_
     rec.theta1 = theta; rec.lanczos_steps = ksteps;
     double theta_kkt = theta;
     bool changed = false;
-    if (-theta / (1.0 + normC) > tau_neg) {
-      // -- 4. grow (Alg. 1 lines 6-8), p = 1: s* = -theta / (sigma |A(vv^T)|^2)
-      if (r + 1 > r_cap) return fail(c, ALORA_EINVAL, "alora_solve: rank growth exceeds r_cap");
+    const bool neg = -theta / (1.0 + normC) > tau_neg;
+    if (neg && r + 1 <= r_cap) {
+      // -- 4. grow (Alg. 1 lines 6-8), p = 1: s* = -theta / (sigma |A(vv^T)|^2).  At r = r_cap the
+      //       step is skipped (reading 27): the dual update and the sigma schedule carry on at rank r_cap.
       s = alora_eval(c, w->ritz, 1, 1, nullptr, w->zv, nullptr); if (s != ALORA_OK) return s;
       double avv[3]; s = dots<double, double>(c, m, 1, w->zv, w->zv, w->zv, w->zv, w->zv, w->zv, avv); if (s != ALORA_OK) return s;
       const double den = sigma * avv[0];
@@ -665,7 +890,7 @@ alora_status solve_impl(alora_ctx* c, const alora_params* prm, T* R_user, int32_
       k_set_col<T><<<ew_grid(c, n), 256, 0, c->stream>>>(n, ld, r, std::sqrt(s_star), (const T*)w->ritz, Rw);
       c->launches++;
       ++r; rec.grew = 1; changed = true;
-    } else if (r > 1) {
+    } else if (!neg && r > 1) {
       // -- 5. shrink (reading 13): drop the numerically null directions of R
       const int nblk = (int)std::max<int64_t>(1, std::min<int64_t>(64, n / 256));
       const int64_t rpb = (n + nblk - 1) / nblk;

@@ -26,7 +26,13 @@
 
 namespace alora {
 
-constexpr int kStages = 4;            // tiles in flight per block
+#ifndef ALORA_KSTAGES
+#define ALORA_KSTAGES 4
+#endif
+#ifndef ALORA_TMINB
+#define ALORA_TMINB 3
+#endif
+constexpr int kStages = ALORA_KSTAGES;   // tiles in flight per block (tuning knobs: build.py, ALORA_NVCC_EXTRA)
 constexpr int kTiledThreads = kBlock + 32;   // 8 consumer warps + 1 producer warp
 
 __host__ __device__ constexpr int tile_rows(int gs) { return kBlock / gs; }   // one row per group per tile
@@ -174,7 +180,7 @@ __device__ __forceinline__ void row_ldg_b(RowReg<T, VEC, GS, NIT>& x, const char
 // occupancy target by the number of 32-bit registers one row vector takes per lane: the consumer loop keeps
 // its addresses and stage offsets in registers (75 at 3 blocks / SM) instead of re-deriving them per tile
 __host__ __device__ constexpr int tiled_min_blocks(int row_regs, int mode) {
-  return row_regs <= 4 ? 3 : row_regs <= 8 ? 2 : 1;
+  return row_regs <= 4 ? ALORA_TMINB : row_regs <= 8 ? 2 : 1;
 }
 
 // row vector of a neighbour: from the staged tile when the neighbour is one of the tile's own rows, else gathered

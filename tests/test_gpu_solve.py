@@ -150,3 +150,17 @@ def test_solve_fp32_ring_matchings(torch, binding, oracle_mod):
     o = oracle_mod.Oracle(w.problem)
     q = o.A_op(out["R"]) - w.problem.b
     assert np.linalg.norm(q) / (1 + np.linalg.norm(w.problem.b)) <= 2e-5
+
+
+def test_rank_cap_skips_growth(torch, binding, oracle_mod):
+    """r_cap reached: the growth step is skipped instead of failing (reading 27).  K_9 from rank 1
+    with r_cap = 1 cannot reach the optimum (it needs rank >= 2 ... 8), but the call must return cleanly."""
+    n = 9
+    P = _graph_maxcut(n, [(i, j) for i in range(n) for j in range(i + 1, n)])
+    R0 = inputs._unit_rows(np.random.default_rng(3), n, 1)
+    out = gpu_solve(torch, binding, P, inputs.F64, R0, np.zeros(n), 1.0, r_cap=1, eps=1e-7, T_max=8)
+    assert all(rec.r == 1 and rec.grew == 0 for rec in out["log"])
+    # and with room to grow the same start reaches -n^2/4
+    out = gpu_solve(torch, binding, P, inputs.F64, R0, np.zeros(n), 1.0, r_cap=16, eps=1e-7)
+    o = oracle_mod.Oracle(P)
+    assert out["ok"] and abs(o.inner_C(out["R"], out["R"]) + n * n / 4) < 1e-4
