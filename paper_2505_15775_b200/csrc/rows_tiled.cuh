@@ -32,6 +32,7 @@ namespace alora {
 #ifndef ALORA_TMINB
 #define ALORA_TMINB 3
 #endif
+
 constexpr int kStages = ALORA_KSTAGES;   // tiles in flight per block (tuning knobs: build.py, ALORA_NVCC_EXTRA)
 constexpr int kTiledThreads = kBlock + 32;   // 8 consumer warps + 1 producer warp
 
