@@ -33,7 +33,10 @@ METRIC = "ALM-BM f+grad evals/sec (each step = f+grad, line-search coefficients,
 UNIT = "evals/s"
 
 
-def workload(idx: int):
+def workload(idx: int, mc: str = ""):
+    if idx == 5 and mc:   # other rows of the paper's Table 2: --mc n,r_star
+        n, rs = (int(x) for x in mc.split(","))
+        return inputs.config5(n=n, r_star=rs)
     return inputs.full(idx)
 
 
@@ -199,11 +202,16 @@ def run_solve(args, w, local, torch, binding):
     ctx = binding.Context(P, w.dtype, device=local)
     t_create = time.perf_counter() - t0
     tdt = torch.float32 if w.dtype == inputs.F32 else torch.float64
-    r_cap = args.r_cap or (64 if P.n <= 100000 else r0 + 14)
+    r_cap = args.r_cap or (64 if P.n <= 1000 else r0 + 14)
     Rbuf = torch.zeros(P.n * r_cap, dtype=tdt, device="cuda")
     Rbuf[: P.n * r0] = torch.as_tensor(w.R, dtype=tdt).cuda().reshape(-1)
-    y = torch.as_tensor(w.y, dtype=torch.float64).cuda()
-    kw = dict(eps=1e-6, stop_mode=0) if P.n <= 1000 else dict(eps=1e-5, stop_mode=1)
+    y = torch.zeros(P.m, dtype=torch.float64, device="cuda")   # Alg. 1: y0 = 0
+    # config 0: KKT <= 1e-6; config 4: relative primal infeasibility <= 1e-5 (BASELINE.json); others: the paper's
+    # rule, KKT (eq. 77) <= 1e-5
+    kw = dict(eps=1e-6, stop_mode=0) if args.config == 0 else dict(eps=1e-5, stop_mode=1) if args.config == 4 \
+        else dict(eps=1e-5, stop_mode=0)
+    if w.dtype == inputs.F32 and args.config == 5:
+        kw["stall_tol"] = 1e-9   # fp32 rounding floor of f (reading 28)
     l0 = ctx.info()["launches"]
     torch.cuda.synchronize()
     res, log, r, sg, ok = ctx.solve(binding.Params(**kw), Rbuf, r0, r_cap, y, w.sigma)
@@ -230,6 +238,7 @@ def main():
     ap.add_argument("--mode", default="path", choices=["path", "solve"],
                     help="path: the hot-path step (default, the bench contract); solve: ALM solve time of the config")
     ap.add_argument("--r-cap", type=int, default=0)
+    ap.add_argument("--mc", default="", help="config 5 only: 'n,r_star' of another row of the paper's Table 2")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
@@ -237,7 +246,7 @@ def main():
     local = int(os.environ.get("LOCAL_RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
 
-    w = workload(args.config)
+    w = workload(args.config, args.mc)
     if args.impl == "reference":
         run_reference(args, w, rank, world)
         return

@@ -154,6 +154,10 @@ typedef struct {
   double tau_shrink;   /* drop directions of R^T R with mu_j <= tau_shrink*mu_max (1e-8) */
   double s_max;        /* cap of the growth step when A(vv^T) = 0 (1e6) */
   uint64_t seed;       /* Lanczos start vectors use seed + run index (12345) */
+  double stall_tol;    /* inner loop also stops after stall_iters consecutive steps whose predicted decrease
+                          phi(0) - phi(alpha) is <= stall_tol * (1 + |f|)  (0 = off, the default; reading 28) */
+  int32_t stall_iters; /* (3) */
+  int32_t pad_;
 } alora_params;
 void alora_default_params(alora_params *p);
 

@@ -36,12 +36,14 @@ class Params:
     tau_neg: float = -1.0      # [8] growth threshold; < 0 means "use eps"
     tol_eig: float = -1.0      # [9] Lanczos residual tolerance; < 0 means eps/10
     k_max: int = 300           # [9] Lanczos steps
-    gamma: float = 2.0         # [12] sigma <- min(gamma sigma, sigma_max) if ||q|| > kappa ||q_prev||
+    gamma: float = 2.0         # [12] sigma <- min(gamma sigma, sigma_max) if ||q|| > kappa ||q_prev|| and kkt[0] > eps
     kappa: float = 0.25
     sigma_max: float = 1e8
     tau_shrink: float = 1e-8   # [13] drop directions of R^T R with mu_j <= tau_shrink * mu_max
     s_max: float = 1e6         # [7] cap of the growth step when A(vv^T) = 0
     seed: int = 12345          # Lanczos start vectors: counter_uniform(seed + run index, i)
+    stall_tol: float = 0.0     # [28] inner loop also stops after stall_iters consecutive steps whose predicted
+    stall_iters: int = 3       #      decrease phi(0) - phi(alpha) <= stall_tol (1 + |f|); 0 = off
 
 
 @dataclass
@@ -215,7 +217,7 @@ def solve(orc, R0, y0, sigma0: float, prm: Params = Params()) -> Result:
         # -- 1. inner solve: F <- argmin_F L_rho(FF^T, y)            (Alg. 1 line 4)
         tol_t = max(prm.tol_min, min(prm.tol0, prm.c_in * infeas_prev))
         S_list, Y_list = [], []
-        it, D, alpha, G_prev = 0, None, 0.0, None
+        it, D, alpha, G_prev, stalled = 0, None, 0.0, None, 0
         while True:
             G = orc.grad(y, sigma, R)
             rec.n_evals += 1
@@ -235,6 +237,11 @@ def solve(orc, R0, y0, sigma0: float, prm: Params = Params()) -> Result:
             p = orc.linesearch(y, sigma, R, D)     # quartic coefficients of f(R + alpha D)
             res.n_linesearch += 1
             alpha, _ = quartic_argmin(p)
+            if prm.stall_tol > 0.0:
+                dec = -alpha * (p[1] + alpha * (p[2] + alpha * (p[3] + alpha * p[4])))
+                stalled = stalled + 1 if dec <= prm.stall_tol * (1.0 + abs(p[0])) else 0
+                if stalled >= prm.stall_iters:
+                    break
             G_prev = G
             R = R + alpha * D
             it += 1
@@ -275,7 +282,7 @@ def solve(orc, R0, y0, sigma0: float, prm: Params = Params()) -> Result:
         rec.kkt = kkt_terms(qnorm, normb, theta_kkt, normC, cx, float(b @ y))
         rec.r, rec.cx, rec.qnorm = R.shape[1], cx, qnorm
         # -- 7. sigma schedule [12]
-        if qnorm > prm.kappa * qnorm_prev:
+        if qnorm > prm.kappa * qnorm_prev and rec.kkt[0] > prm.eps:   # no increase once the primal term is below eps
             sigma = min(prm.gamma * sigma, prm.sigma_max)
         qnorm_prev, infeas_prev = qnorm, rec.kkt[0]
         res.log.append(rec)

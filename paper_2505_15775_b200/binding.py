@@ -44,7 +44,8 @@ class Params(C.Structure):
                 ("c_in", C.c_double), ("tol_min", C.c_double), ("it_max", C.c_int32), ("lbfgs_mem", C.c_int32),
                 ("p_max", C.c_int32), ("k_max", C.c_int32), ("tau_neg", C.c_double), ("tol_eig", C.c_double),
                 ("gamma", C.c_double), ("kappa", C.c_double), ("sigma_max", C.c_double),
-                ("tau_shrink", C.c_double), ("s_max", C.c_double), ("seed", C.c_uint64)]
+                ("tau_shrink", C.c_double), ("s_max", C.c_double), ("seed", C.c_uint64),
+                ("stall_tol", C.c_double), ("stall_iters", C.c_int32), ("pad_", C.c_int32)]
 
     def __init__(self, **kw):
         super().__init__()

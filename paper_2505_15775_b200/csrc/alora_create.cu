@@ -201,6 +201,7 @@ template <typename T> alora_status build(alora_ctx* c, const alora_problem* P) {
     if (aents.size() >= (size_t)INT32_MAX) return fail(c, ALORA_EINVAL, "constraint pattern too large for int32 row pointers");
     c->a_nnz = (int64_t)aents.size();
     c->ep = (c->a_nnz + c->c_nnz) >= 8 * n;
+    c->ep_wide = (c->a_nnz + c->c_nnz) >= 96 * n;
     {
       std::vector<int> col(aents.size()), cons(aents.size());
       std::vector<T> val(aents.size());

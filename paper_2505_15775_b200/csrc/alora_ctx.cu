@@ -199,9 +199,10 @@ alora_status launch_diag_rows(alora_ctx* c, int vec, int nvec, int exact, int sh
   return ALORA_OK;
 }
 // general-class adjoint pass: a group per row; single vectors (Lanczos matvec) on long rows take a warp per row
-// (measured on config 3: the warp-per-row kernel wins for p = 1, 66 vs 77 us, and loses for r = 10, 168 vs 128 us)
+// (measured on config 3, 60 entries per row: the warp-per-row kernel wins for p = 1, 66 vs 77 us, and loses for
+// r = 10, 168 vs 128 us); rows with ~100 entries or more (matrix completion) always take a warp per row
 template <typename T> alora_status launch_adj_general(alora_ctx* c, const Geo& g, RowArgs<T>& a, double* out) {
-  if (c->ep && g.nvec == 1) {
+  if ((c->ep && g.nvec == 1) || c->ep_wide) {
     int& occ = c->occ_cache[vec_slot(g.vec)][g.shape][11];
     if (!occ) occ = std::max(1, occ_rows_ep(T(), g.vec, g.shape));
     const int64_t need = (c->n + kBlock / 32 - 1) / (kBlock / 32);

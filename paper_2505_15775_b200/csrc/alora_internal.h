@@ -58,7 +58,8 @@ struct alora_ctx {
   // general class: row-oriented full pattern of the constraints
   int* a_rowptr = nullptr; int* a_col = nullptr; void* a_val = nullptr; int* a_cons = nullptr;
   int64_t a_nnz = 0;
-  bool ep = false;   // general class with long rows (>= 8 entries per row on average): warp-per-row adjoint (k_rows_ep)
+  bool ep = false;       // general class, >= 8 entries per row on average: warp-per-row adjoint for single vectors
+  bool ep_wide = false;  // >= 96 entries per row on average (matrix completion): warp-per-row adjoint for every r
   // forward list: coalesced constraint entries [0, nf_A), then C's sym-upper entries [nf_A, nf_A+nf_C)
   int64_t* f_ptr = nullptr; int* f_row = nullptr; int* f_col = nullptr; void* f_val = nullptr;
   int64_t nf_A = 0, nf_C = 0;

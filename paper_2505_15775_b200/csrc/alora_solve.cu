@@ -622,6 +622,7 @@ extern "C" void alora_default_params(alora_params* p) {
   p->eps = 1e-5; p->stop_mode = 0; p->T_max = 100; p->tol0 = 1e-2; p->c_in = 0.1; p->tol_min = 1e-7;
   p->it_max = 500; p->lbfgs_mem = 5; p->p_max = 1; p->k_max = 300; p->tau_neg = -1.0; p->tol_eig = -1.0;
   p->gamma = 2.0; p->kappa = 0.25; p->sigma_max = 1e8; p->tau_shrink = 1e-8; p->s_max = 1e6; p->seed = 12345;
+  p->stall_tol = 0.0; p->stall_iters = 3; p->pad_ = 0;
 }
 
 extern "C" alora_status alora_lanczos(alora_ctx* c, const double* mu_dev, int32_t kmax, double tol_abs, uint64_t seed,
@@ -733,7 +734,7 @@ alora_status solve_impl(alora_ctx* c, const alora_params* prm, T* R_user, int32_
     std::vector<double> sy(nslot), yy(nslot), alp(nslot);
     std::vector<std::vector<double>> lb_SY(nslot, std::vector<double>(nslot, 0.0)), lb_YY(nslot, std::vector<double>(nslot, 0.0));
     std::vector<double> lb_sg(nslot, 0.0), lb_yg(nslot, 0.0);
-    int it = 0; bool have_prev = false; double alpha = 0.0, gnorm = 0.0;
+    int it = 0, stalled = 0; bool have_prev = false; double alpha = 0.0, gnorm = 0.0;
     while (true) {
       s = alora_eval(c, Rw, ld, ld, Gw, w->z, st); if (s != ALORA_OK) return s;
       ++rec.n_evals;
@@ -855,6 +856,11 @@ alora_status solve_impl(alora_ctx* c, const alora_params* prm, T* R_user, int32_
       ++n_ls;
       int flag;
       alpha = quartic_argmin(p, &flag);
+      if (prm->stall_tol > 0.0) {   // reading 28: the steps no longer decrease f (rounding floor of the evaluation)
+        const double dec = -alpha * (p[1] + alpha * (p[2] + alpha * (p[3] + alpha * p[4])));
+        stalled = dec <= prm->stall_tol * (1.0 + std::fabs(p[0])) ? stalled + 1 : 0;
+        if (stalled >= prm->stall_iters) break;
+      }
       std::swap(Gw, Gp);                                   // Gp <- current gradient
       k_axpy<T><<<g, 256, 0, c->stream>>>(N, alpha, Dw, Rw);   // R <- R + alpha D
       c->launches++;
@@ -937,7 +943,7 @@ alora_status solve_impl(alora_ctx* c, const alora_params* prm, T* R_user, int32_
     kkt[2] = std::fabs(cx - by[0]) / (1.0 + std::fabs(cx) + std::fabs(by[0]));
     rec.r = r; rec.cx = cx; rec.qnorm = qnorm; rec.kkt[0] = kkt[0]; rec.kkt[1] = kkt[1]; rec.kkt[2] = kkt[2];
     // -- 7. sigma schedule (reading 12)
-    if (qnorm > prm->kappa * qnorm_prev) sigma = std::min(prm->gamma * sigma, prm->sigma_max);
+    if (qnorm > prm->kappa * qnorm_prev && kkt[0] > prm->eps) sigma = std::min(prm->gamma * sigma, prm->sigma_max);
     qnorm_prev = qnorm; infeas_prev = kkt[0];
     if (log && t < log_cap) log[t] = rec;
     n_evals += rec.n_evals; outer = t + 1;

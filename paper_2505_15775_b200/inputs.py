@@ -305,7 +305,53 @@ def config4(n: int = 1 << 24, r: int = 10, seed: int = 1004) -> Workload:
                    {"edges": int(lo.shape[0])})
 
 
-CONFIGS = [config0, config1, config2, config3, config4]
+def matrix_completion_problem(rng, n1: int, n2: int, r_star: int, m: int):
+    """Matrix-completion SDP of PAPER.md:997-1008 (section 6.2):  min 1/2 tr X  s.t.
+    X = [[W1, Y], [Y^T, W2]] psd,  Y_ij = M_ij on Omega,  with M = U V^T, U (n1 x r*) and V (n2 x r*)
+    standard Gaussian and |Omega| = m entries drawn uniformly without replacement.
+
+    Constraint for (i, j) in Omega: X[i, n1 + j] = M_ij, i.e. A = (e_i e_k^T + e_k e_i^T)/2 with
+    k = n1 + j, stored sym-upper as (i, k, 1/2)  (PAPER.md:533 convention); cost C = I/2.
+    Returns (Problem, U, V)."""
+    n = n1 + n2
+    if m > n1 * n2:
+        raise ValueError("more observations than entries")
+    U, V = rng.standard_normal((n1, r_star)), rng.standard_normal((n2, r_star))
+    # m distinct flat positions in [0, n1*n2): draw with replacement, drop duplicates, top up
+    flat = np.unique(rng.integers(0, n1 * n2, size=m, dtype=np.int64))
+    while flat.shape[0] < m:
+        extra = rng.integers(0, n1 * n2, size=m - flat.shape[0], dtype=np.int64)
+        flat = np.unique(np.concatenate([flat, extra]))
+    i, j = (flat // n2).astype(np.int32), (flat % n2).astype(np.int32)
+    b = np.einsum("ec,ec->e", U[i], V[j])
+    d = np.arange(n, dtype=np.int32)
+    prob = Problem(n=n, m=m, C_row=d, C_col=d.copy(), C_val=np.full(n, 0.5),
+                   A_ptr=np.arange(m + 1, dtype=np.int64), A_row=i, A_col=(n1 + j).astype(np.int32),
+                   A_val=np.full(m, 0.5), b=b)
+    return prob, U, V
+
+
+def mc_observations(n: int, r_star: int) -> int:
+    """m = ceil(gamma r* (n - r*)), gamma = r* log n."""
+    return int(np.ceil(r_star * np.log(n) * r_star * (n - r_star)))
+
+
+def config5(n: int = 10000, r_star: int = 3, r: int = 0, seed: int = 1005, m: int = 0) -> Workload:
+    """Matrix completion (first row of the paper's Table 2 by default: r* = 3,
+    n = 10000, m = 828659), n1 = n2 = n/2, fp32 R / fp64 sums.  The paper is silent on R0, y0, sigma:
+    R ~ N(0,1) (the scale of the factors of M), y = 0, sigma = 1; the BM rank defaults to r*."""
+    rng = _rng(seed)
+    n1 = n // 2
+    m = m or mc_observations(n, r_star)
+    prob, U, V = matrix_completion_problem(rng, n1, n - n1, r_star, m)
+    r = r or r_star
+    R = rng.standard_normal((n, r))
+    y = np.zeros(m) if m > 4000000 else rng.standard_normal(m) * 0.1
+    return _finish("cfg5_matrix_completion", prob, F32, r, R, y, 1.0, rng,
+                   {"r_star": r_star, "n1": n1, "n2": n - n1, "U": U, "V": V})
+
+
+CONFIGS = [config0, config1, config2, config3, config4, config5]
 
 # scaled-down versions: several tiles plus a ragged tail, oracle finishes in well under a second
 SMALL = {
@@ -314,6 +360,7 @@ SMALL = {
     2: lambda: config2(n=701, M=5003, r=24),
     3: lambda: config3(n=3001, m=15007, nnzC=30011, r=10),
     4: lambda: config4(n=20002, r=10),
+    5: lambda: config5(n=601, r_star=3, r=4, m=20011),
 }
 
 

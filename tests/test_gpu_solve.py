@@ -164,3 +164,20 @@ def test_rank_cap_skips_growth(torch, binding, oracle_mod):
     out = gpu_solve(torch, binding, P, inputs.F64, R0, np.zeros(n), 1.0, r_cap=16, eps=1e-7)
     o = oracle_mod.Oracle(P)
     assert out["ok"] and abs(o.inner_C(out["R"], out["R"]) + n * n / 4) < 1e-4
+
+
+@pytest.mark.parametrize("dtype,tol", [(inputs.F64, 1e-5), (inputs.F32, 2e-3)])
+def test_solve_matrix_completion(torch, binding, oracle_mod, dtype, tol):
+    """Matrix completion: exact recovery of M = U V^T and optimal value = nuclear norm."""
+    rng = np.random.default_rng(11)
+    n1 = n2 = 20
+    P, U, V = inputs.matrix_completion_problem(rng, n1, n2, 2, 300)
+    M = U @ V.T
+    R0 = rng.standard_normal((P.n, 4))
+    out = gpu_solve(torch, binding, P, dtype, R0, np.zeros(P.m), 1.0, r_cap=16,
+                    eps=1e-7 if dtype == inputs.F64 else 1e-4)
+    assert out["ok"]
+    X = out["R"] @ out["R"].T
+    assert np.linalg.norm(X[:n1, n1:] - M) <= 10 * tol * np.linalg.norm(M)
+    nuc = np.linalg.svd(M, compute_uv=False).sum()
+    assert abs(0.5 * np.trace(X) - nuc) <= tol * nuc

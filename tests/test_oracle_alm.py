@@ -161,3 +161,22 @@ def test_thm1_bound_7b(alm, Oracle):
         assert np.linalg.norm(q) <= np.linalg.norm(y - ystar) / rho * (1 + 1e-6)
         # (8a) dual non-expansiveness: z = y - rho q is the updated dual
         assert np.linalg.norm(res.y - ystar) <= np.linalg.norm(y - ystar) * (1 + 1e-6)
+
+
+def test_matrix_completion_nuclear_norm(alm, Oracle):
+    """PAPER.md:997-1008 (section 6.2): with enough observations the SDP recovers M = U V^T exactly, and then
+    its optimal value 1/2 tr X equals the nuclear norm of M (textbook: ||Y||_* = min 1/2 (tr W1 + tr W2)).
+    Pins the general-class loop (single off-diagonal-entry constraints, C = I/2) against an SVD."""
+    rng = np.random.default_rng(11)
+    n1 = n2 = 20
+    P, U, V = inputs.matrix_completion_problem(rng, n1, n2, 2, 300)   # 300 of 400 entries observed
+    M = U @ V.T
+    o = Oracle(P)
+    R0 = rng.standard_normal((P.n, 4))
+    res = alm.solve(o, R0, np.zeros(P.m), 1.0, alm.Params(eps=1e-7))
+    assert res.converged
+    X = res.R @ res.R.T
+    Y = X[:n1, n1:]
+    assert np.linalg.norm(Y - M) <= 1e-4 * np.linalg.norm(M)
+    nuc = np.linalg.svd(M, compute_uv=False).sum()
+    assert abs(o.inner_C(res.R, res.R) - nuc) <= 1e-5 * nuc
