@@ -204,7 +204,9 @@ __device__ __forceinline__ void row_nbr(RowReg<T, VEC, GS, NIT>& x, bool loc, co
 // ones (dcons == da == nullptr, ELL block present), rows are whole packs (r == nvec * VEC), X / X2 / y (or w)
 // are 16-byte aligned.  Full tiles (rows [0, a.tiles * TR)) go through the staged pipeline; the ragged tail of
 // the matrix (< TR rows) is processed by the consumer warps of the last block from global memory.  FULL: 1 = some lanes of a group own no pack (lane mask), 2 = all lanes busy.
-template <typename T, int VEC, int GS, int NIT, int MODE, int FULL>
+// CLD: the leading dimension equals the row length GS * NIT * VEC (dense rows, FULL == 2), known at compile time, so
+// every stage offset and row pitch is an immediate.
+template <typename T, int VEC, int GS, int NIT, int MODE, int FULL, bool CLD = false>
 __global__ void __launch_bounds__(kTiledThreads, tiled_min_blocks(VEC * NIT * (int)sizeof(T) / 4, MODE)) k_rows_tiled(const RowArgs<T> a) {
   using Row = RowReg<T, VEC, GS, NIT>;
   constexpr int TR = tile_rows(GS), GPW = 32 / GS, NCW = kBlock / 32;
@@ -218,7 +220,7 @@ __global__ void __launch_bounds__(kTiledThreads, tiled_min_blocks(VEC * NIT * (i
   __shared__ int s_rem[kStages];
   const int warp = threadIdx.x >> 5, lane32 = threadIdx.x & 31;
   const int nvec = a.nvec, r = a.r, exact = a.exact;
-  const int64_t ld = a.ld;
+  const int64_t ld = CLD ? (int64_t)(GS * NIT * VEC) : a.ld;
   const int64_t ntiles = a.tiles;
 
   // stage layout (must match tiled_stage_bytes)
