@@ -160,6 +160,10 @@ template <typename T> alora_status build(alora_ctx* c, const alora_problem* P) {
     if (ident && ones) {
       // padded ELL blocks for the tiled row kernel: slot u of row j at [j * NU + u]; unused slot = (j, 0)
       const int64_t nb = (n + 31) / 32;
+      int64_t over4 = 0;
+      for (int64_t j = 0; j < n; ++j) over4 += (c_rowptr[j + 1] - c_rowptr[j] > 4);
+      c->ell_wide = over4 * 10 > n;
+      const int kUN = ell_slots(c->ell_wide), kUNL = ell_slots_ls(c->ell_wide);
       std::vector<int> ec((size_t)n * kUN), euc((size_t)n * kUNL);
       std::vector<T> ev((size_t)n * kUN), euv((size_t)n * kUNL);
       std::vector<unsigned char> rem(nb + 8, 0), remu(nb + 8, 0);

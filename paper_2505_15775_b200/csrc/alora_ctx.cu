@@ -177,7 +177,7 @@ alora_status launch_diag_rows(alora_ctx* c, int vec, int nvec, int exact, int sh
     int& oc = c->occ_cache[vec_slot(vec)][shape][8 + mode];
     int64_t& key = c->occ_ld[vec_slot(vec)][shape][mode];
     const int64_t want = a.ld * 4 + full;
-    if (!oc || key != want) { oc = occ_tiled(T(), vec, shape, mode, full, a.ld); key = want; if (!oc) oc = -1; }
+    if (!oc || key != want) { oc = occ_tiled(T(), vec, shape, mode, full, c->ell_wide ? 1 : 0, a.ld); key = want; if (!oc) oc = -1; }
     occ = oc;
     elig = occ > 0;
   }
@@ -194,7 +194,7 @@ alora_status launch_diag_rows(alora_ctx* c, int vec, int nvec, int exact, int sh
   const int grid = (int)std::max<int64_t>(1, std::min<int64_t>(tiles, std::min<int64_t>((int64_t)c->num_sms * occ, c->part_cap / 2)));
   a.tiles = tiles;
   a.fin = make_fin(c, a.partials, grid, nullptr, 0, nullptr, 0, out);
-  ALORA_CUDA(c, launch_tiled(vec, shape, mode, full, a, grid, c->stream));
+  ALORA_CUDA(c, launch_tiled(vec, shape, mode, full, c->ell_wide ? 1 : 0, a, grid, c->stream));
   c->launches++;
   return ALORA_OK;
 }

@@ -24,8 +24,11 @@ namespace alora {
 constexpr int kBlock = 256;
 constexpr int kLongThreshold = 64;   // constraints with more stored entries are split into chunks
 constexpr int kChunk = 16;           // entries per chunk of a long constraint / of C's sym-upper list
-constexpr int kUN = 4;               // diagonal class: ELL slots per row (first neighbours), see rows_tiled.cuh
-constexpr int kUNL = 3;              // diagonal class, line search: ELL slots per row (last upper-triangle neighbours)
+// diagonal class: ELL slots per row (first neighbours; for the line search: last upper-triangle neighbours), see
+// rows_tiled.cuh.  Two widths, chosen per problem in alora_create: narrow for degree <= 4 graphs (grids, ring +
+// matchings), wide for mesh-like graphs of degree 6..8.
+__host__ __device__ constexpr int ell_slots(bool wide) { return wide ? 8 : 4; }
+__host__ __device__ constexpr int ell_slots_ls(bool wide) { return wide ? 6 : 3; }
 
 enum RowsMode { ROWS_FUSED_EVAL = 0, ROWS_ADJ = 1, ROWS_LS_FUSED = 2 };
 enum ConsMode { CONS_EVAL = 0, CONS_LS = 1 };

@@ -6,7 +6,7 @@
 // most of them address arithmetic, slot-validity tests and re-derived stage offsets (profiles/r1b_*).
 //
 // This version removes that bookkeeping from the hot loop:
-//   * the first kUN neighbours of every row (and, for the line search, its last kUNL upper-triangle ones) are
+//   * the first 4 (or 8) neighbours of every row (and, for the line search, its last 3 (or 6) upper-triangle ones) are
 //     kept in a padded ELL block built once in alora_create: fixed-size (col, val) slots per row, an unused
 //     slot holding (the row itself, 0).  The slots of a row tile are one contiguous slice, so they arrive by
 //     bulk copy with no alignment fix-up, and the consumer needs no rowptr, no bounds and no validity test.
@@ -38,8 +38,8 @@ constexpr int kTiledThreads = kBlock + 32;   // 8 consumer warps + 1 producer wa
 
 __host__ __device__ constexpr int tile_rows(int gs) { return kBlock / gs; }   // one row per group per tile
 // per-stage shared memory: [X tile][D tile (line search)][dC][y|w][b][ELL col][ELL val], 16-byte aligned pieces
-__host__ __device__ inline size_t tiled_stage_bytes(int gs, int esz, int64_t ld, int mode) {
-  const size_t tr = tile_rows(gs), nu = (mode == ROWS_LS_FUSED ? kUNL : kUN);
+__host__ __device__ inline size_t tiled_stage_bytes(int gs, int esz, int64_t ld, int mode, bool wide) {
+  const size_t tr = tile_rows(gs), nu = (mode == ROWS_LS_FUSED ? ell_slots_ls(wide) : ell_slots(wide));
   size_t b = tr * (size_t)ld * esz * (mode == ROWS_LS_FUSED ? 2 : 1);
   b = (b + 15) & ~(size_t)15;
   b += tr * esz;                 // dC
@@ -48,8 +48,8 @@ __host__ __device__ inline size_t tiled_stage_bytes(int gs, int esz, int64_t ld,
   b += tr * nu * 4 + tr * nu * esz;
   return (b + 15) & ~(size_t)15;
 }
-__host__ __device__ inline size_t tiled_smem_bytes(int gs, int esz, int64_t ld, int mode) {
-  return kStages * tiled_stage_bytes(gs, esz, ld, mode);
+__host__ __device__ inline size_t tiled_smem_bytes(int gs, int esz, int64_t ld, int mode, bool wide) {
+  return kStages * tiled_stage_bytes(gs, esz, ld, mode, wide);
 }
 
 // ---- mbarrier / bulk-copy primitives (PTX) ------------------------------------------------------
@@ -180,8 +180,8 @@ __device__ __forceinline__ void row_ldg_b(RowReg<T, VEC, GS, NIT>& x, const char
 
 // occupancy target by the number of 32-bit registers one row vector takes per lane: the consumer loop keeps
 // its addresses and stage offsets in registers (75 at 3 blocks / SM) instead of re-deriving them per tile
-__host__ __device__ constexpr int tiled_min_blocks(int row_regs, int mode) {
-  return row_regs <= 4 ? ALORA_TMINB : row_regs <= 8 ? 2 : 1;
+__host__ __device__ constexpr int tiled_min_blocks(int row_regs, int mode, bool wide) {
+  return wide ? (row_regs <= 4 ? 2 : 1) : row_regs <= 4 ? ALORA_TMINB : row_regs <= 8 ? 2 : 1;
 }
 
 // row vector of a neighbour: from the staged tile when the neighbour is one of the tile's own rows, else gathered
@@ -206,13 +206,13 @@ __device__ __forceinline__ void row_nbr(RowReg<T, VEC, GS, NIT>& x, bool loc, co
 // the matrix (< TR rows) is processed by the consumer warps of the last block from global memory.  FULL: 1 = some lanes of a group own no pack (lane mask), 2 = all lanes busy.
 // CLD: the leading dimension equals the row length GS * NIT * VEC (dense rows, FULL == 2), known at compile time, so
 // every stage offset and row pitch is an immediate.
-template <typename T, int VEC, int GS, int NIT, int MODE, int FULL, bool CLD = false>
-__global__ void __launch_bounds__(kTiledThreads, tiled_min_blocks(VEC * NIT * (int)sizeof(T) / 4, MODE)) k_rows_tiled(const RowArgs<T> a) {
+template <typename T, int VEC, int GS, int NIT, int MODE, int FULL, bool CLD = false, bool WIDE = false>
+__global__ void __launch_bounds__(kTiledThreads, tiled_min_blocks(VEC * NIT * (int)sizeof(T) / 4, MODE, WIDE)) k_rows_tiled(const RowArgs<T> a) {
   using Row = RowReg<T, VEC, GS, NIT>;
   constexpr int TR = tile_rows(GS), GPW = 32 / GS, NCW = kBlock / 32;
   constexpr int NST = (MODE == ROWS_LS_FUSED) ? 12 : 6;
   constexpr bool LS = (MODE == ROWS_LS_FUSED);
-  constexpr int NU = LS ? kUNL : kUN;
+  constexpr int NU = LS ? ell_slots_ls(WIDE) : ell_slots(WIDE);
   constexpr int NSL = (LS && GS >= 4) ? 6 : NST;   // accumulators kept in the loop (line search spreads the 9 q-sums over lanes)
   constexpr int ESZ = (int)sizeof(T);
   extern __shared__ __align__(16) unsigned char smem_raw[];

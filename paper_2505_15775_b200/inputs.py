@@ -132,6 +132,21 @@ def torus_edges(side: int) -> tuple[np.ndarray, np.ndarray]:
     return lo.astype(np.int64), hi.astype(np.int64)
 
 
+def tri_torus_edges(side: int) -> tuple[np.ndarray, np.ndarray]:
+    """Triangulated side x side torus (degree 6): the torus edges plus the diagonal (a,c)-((a+1),(c+1)).
+    Stand-in for the mesh / Delaunay graphs of the paper's Table 1, whose vertices have
+    about six neighbours."""
+    a, c = np.meshgrid(np.arange(side), np.arange(side), indexing="ij")
+    v = (side * a + c).ravel()
+    down = (side * ((a + 1) % side) + c).ravel()
+    right = (side * a + (c + 1) % side).ravel()
+    diag = (side * ((a + 1) % side) + (c + 1) % side).ravel()
+    u = np.concatenate([v, v, v])
+    w = np.concatenate([down, right, diag])
+    lo, hi = np.minimum(u, w), np.maximum(u, w)
+    return lo.astype(np.int64), hi.astype(np.int64)
+
+
 def ring_matching_edges(rng: np.random.Generator, n: int) -> tuple[np.ndarray, np.ndarray]:
     """Ring i-(i+1) mod n plus two independent seeded random perfect matchings (n even)."""
     if n % 2:
@@ -351,7 +366,20 @@ def config5(n: int = 10000, r_star: int = 3, r: int = 0, seed: int = 1005, m: in
                    {"r_star": r_star, "n1": n1, "n2": n - n1, "U": U, "V": V})
 
 
-CONFIGS = [config0, config1, config2, config3, config4, config5]
+def config6(side: int = 1000, r: int = 16, seed: int = 1006) -> Workload:
+    """MaxCut on the triangulated torus (degree 6, mesh stand-in), unit weights as in the paper's MaxCut runs
+    (PAPER.md:969), fp32 R, y ~ N(0,1), sigma = 10.  Exercises the wide ELL variant of the tiled kernel."""
+    rng = _rng(seed)
+    lo, hi = tri_torus_edges(side)
+    lo, hi, w = coalesce_edges(lo, hi, np.ones(lo.shape[0]), side * side)
+    n = side * side
+    prob = maxcut_problem(n, lo, hi, w)
+    R = _unit_rows(rng, n, r)
+    y = rng.standard_normal(n)
+    return _finish("cfg6_maxcut_tri_torus", prob, F32, r, R, y, 10.0, rng, {"edges": int(lo.shape[0])})
+
+
+CONFIGS = [config0, config1, config2, config3, config4, config5, config6]
 
 # scaled-down versions: several tiles plus a ragged tail, oracle finishes in well under a second
 SMALL = {
@@ -361,6 +389,7 @@ SMALL = {
     3: lambda: config3(n=3001, m=15007, nnzC=30011, r=10),
     4: lambda: config4(n=20002, r=10),
     5: lambda: config5(n=601, r_star=3, r=4, m=20011),
+    6: lambda: config6(side=41, r=16),
 }
 
 

@@ -109,12 +109,12 @@ def check_workload(torch, binding, oracle_mod, w, ld=None, label="", split_scale
     ctx.close()
 
 
-@pytest.mark.parametrize("idx", [0, 1, 2, 3, 4, 5])
+@pytest.mark.parametrize("idx", [0, 1, 2, 3, 4, 5, 6])
 def test_small_configs(torch, binding, oracle_mod, idx):
     check_workload(torch, binding, oracle_mod, inputs.small(idx), label=f"small{idx}")
 
 
-@pytest.mark.parametrize("idx,ld", [(1, 20), (3, 12), (4, 11), (0, 41), (2, 26), (5, 4), (5, 8)])
+@pytest.mark.parametrize("idx,ld", [(1, 20), (3, 12), (4, 11), (0, 41), (2, 26), (5, 4), (5, 8), (6, 20), (6, 17)])
 def test_padded_leading_dimension(torch, binding, oracle_mod, idx, ld):
     """ld > r, including odd ld (element-wise path) and ld that allows wider vectors than r."""
     check_workload(torch, binding, oracle_mod, inputs.small(idx), ld=ld, label=f"small{idx}/ld{ld}")
@@ -123,12 +123,13 @@ def test_padded_leading_dimension(torch, binding, oracle_mod, idx, ld):
 @pytest.mark.parametrize("r", [1, 2, 3, 5, 7, 13, 33, 64])
 def test_ranks(torch, binding, oracle_mod, r):
     """every (GS, NIT) shape and ragged tails, both classes and dtypes."""
-    for maker in (lambda: inputs.config1(side=23, r=r), lambda: inputs.config3(n=700, m=900, nnzC=2000, r=r),
+    for maker in (lambda: inputs.config1(side=23, r=r), lambda: inputs.config6(side=19, r=r),
+                  lambda: inputs.config3(n=700, m=900, nnzC=2000, r=r),
                   lambda: inputs.config2(n=300, M=900, r=r), lambda: inputs.config0(n=300, M=700, r=r)):
         check_workload(torch, binding, oracle_mod, maker(), label=f"r{r}")
 
 
-@pytest.mark.parametrize("idx", [1, 2, 3, 4, 5])
+@pytest.mark.parametrize("idx", [1, 2, 3, 4, 5, 6])
 def test_full_configs(torch, binding, oracle_mod, idx):
     """BASELINE.json's full sizes, ld = r as bench.py launches them; the C oracle is fast enough to check
     every element of z, G, S(mu)v (config 4: n = 2^24, about a minute of oracle time)."""
