@@ -126,11 +126,13 @@ def quartic_argmin(p) -> tuple[float, int]:
     return best, 0
 
 
-def lanczos(matvec, n: int, seed: int, k_max: int, tol_abs: float):
+def lanczos(matvec, n: int, seed: int, k_max: int, tol_abs: float, p_want: int = 1):
     """Smallest Ritz pair of a symmetric operator by Lanczos with full re-orthogonalisation
     (two passes of classical Gram-Schmidt) [9].  Stops at step k when the residual estimate
     |beta_k s_k| of the smallest Ritz pair is <= tol_abs, on breakdown (beta_k ~ 0), or k = k_max.
-    Returns (theta, v, k_used, resid)."""
+    Returns (theta, v, k_used, resid); with p_want > 1 a fifth item (thetas, U): the min(p_want, k)
+    smallest Ritz values of the same k-step tridiagonal, ascending, and their unit Ritz vectors as
+    columns (the Rayleigh quotient of a Ritz vector IS its Ritz value, converged or not) [29]."""
     v = counter_uniform(seed, n)
     v /= np.sqrt(v @ v)
     V = np.zeros((min(k_max, n), n))
@@ -160,7 +162,62 @@ def lanczos(matvec, n: int, seed: int, k_max: int, tol_abs: float):
         v = w / beta
     ritz = V[:k].T @ s
     ritz /= np.sqrt(ritz @ ritz)
-    return theta, ritz, k, resid
+    if p_want <= 1:
+        return theta, ritz, k, resid
+    if k == 1:
+        return theta, ritz, k, resid, (np.array([theta]), ritz[:, None])
+    pw = min(p_want, k)
+    th, S = eigh_tridiagonal(np.array(alphas), np.array(betas[: k - 1]), select="i", select_range=(0, pw - 1))
+    U = V[:k].T @ S
+    U /= np.sqrt((U * U).sum(axis=0))
+    return theta, ritz, k, resid, (th, U)
+
+
+def psd_project(S):
+    """Nearest positive semidefinite matrix in Frobenius norm (eigenvalue clipping)."""
+    mu, Q = np.linalg.eigh(0.5 * (S + S.T))
+    return (Q * np.maximum(mu, 0.0)) @ Q.T
+
+
+def growth_sdp(theta, H, sigma: float, iters: int = 500):
+    """Alg. 1 line 7 for p negative-curvature directions U = [v_1 .. v_p] with Rayleigh
+    quotients theta (U^T S(lambda) U = diag(theta) for Ritz vectors of one Krylov space):
+        min_{S >= 0}  g(S) = sum_a theta_a S_aa + (sigma/2) || sum_{a<=b} w_ab S_ab c_ab ||^2,
+    c_ab = A((v_a v_b^T + v_b v_a^T)/2), w_ab = 1 (a = b) or 2, H[(ab),(cd)] = <c_ab, c_cd> with the pairs
+    a <= b in row-major order.  g(S) is exactly L_rho(X + U S U^T, y) - L_rho(X, y) (expand (AL)).
+    Projected gradient with step 1/L from S0 = diag(-theta_a / (sigma H[(aa),(aa)])) [10, 29].
+    Returns (S, g(S))."""
+    p = len(theta)
+    pairs = [(a, b) for a in range(p) for b in range(a, p)]
+    wgt = np.array([1.0 if a == b else 2.0 for a, b in pairs])
+    Hw = H * np.outer(wgt, wgt)
+
+    def vec(S):
+        return np.array([S[a, b] for a, b in pairs])
+
+    def g(S):
+        s = vec(S)
+        return float(theta @ np.diag(S) + 0.5 * sigma * s @ Hw @ s)
+
+    def grad(S):
+        t = sigma * (Hw @ vec(S))          # d/ds of the quadratic term
+        G = np.zeros((p, p))
+        for (a, b), tv in zip(pairs, t):
+            if a == b:
+                G[a, a] = tv
+            else:
+                G[a, b] = G[b, a] = 0.5 * tv   # s_ab stands for the two entries S_ab = S_ba
+        return G + np.diag(theta)
+
+    # Lipschitz constant of grad in the Frobenius metric of S: sigma * lambda_max of the quadratic form in S-entries
+    D = np.diag([1.0 if a == b else 1.0 / np.sqrt(2.0) for a, b in pairs])
+    L = sigma * max(np.linalg.eigvalsh(D @ Hw @ D)[-1], 1e-300)
+    S = np.diag([(-theta[a] / (sigma * H[pairs.index((a, a)), pairs.index((a, a))]))
+                 if H[pairs.index((a, a)), pairs.index((a, a))] > 0 else 0.0 for a in range(p)])
+    S = np.maximum(S, 0.0)
+    for _ in range(iters):
+        S = psd_project(S - grad(S) / L)
+    return S, g(S)
 
 
 def lbfgs_direction(G, S_list, Y_list):

@@ -113,7 +113,13 @@ template <typename T> alora_status build(alora_ctx* c, const alora_problem* P) {
   std::vector<int> f_row, f_col;
   std::vector<double> f_val;
   f_row.reserve(P->nnzA); f_col.reserve(P->nnzA); f_val.reserve(P->nnzA);
-  bool diag_class = (P->pC == 0);
+  // a single diagonal entry per constraint qualifies for the fused one-pass row kernel -- unless the graph has
+  // very heavy rows (power-law degrees): the row kernel gives a row to 1..16 lanes, so a row with tens of thousands
+  // of entries would serialise; such problems take the general path, whose adjoint pass is a warp per row and whose
+  // line search runs over C's entry list in equal chunks
+  int64_t c_maxdeg = 0;
+  for (int64_t j = 0; j < n; ++j) c_maxdeg = std::max<int64_t>(c_maxdeg, c_rowptr[j + 1] - c_rowptr[j]);
+  bool diag_class = (P->pC == 0) && c_maxdeg <= 4 * kHeavyRow;
   std::vector<int> dcons(n, -1);
   std::vector<double> da(n, 0.0);
   {
@@ -206,6 +212,23 @@ template <typename T> alora_status build(alora_ctx* c, const alora_problem* P) {
     c->a_nnz = (int64_t)aents.size();
     c->ep = (c->a_nnz + c->c_nnz) >= 8 * n;
     c->ep_wide = (c->a_nnz + c->c_nnz) >= 96 * n;
+    if (c_maxdeg > kHeavyRow) {
+      std::vector<int> seg_row, seg_beg, seg_end, heavy_rows, heavy_segptr(1, 0);
+      for (int64_t j = 0; j < n; ++j) {
+        const int e0 = c_rowptr[j], e1 = c_rowptr[j + 1];
+        if (e1 - e0 <= kHeavyRow) continue;
+        for (int e = e0; e < e1; e += kHeavyRow) { seg_row.push_back((int)j); seg_beg.push_back(e); seg_end.push_back(std::min(e + kHeavyRow, e1)); }
+        heavy_rows.push_back((int)j); heavy_segptr.push_back((int)seg_row.size());
+      }
+      c->nseg = (int)seg_row.size(); c->nheavy = (int)heavy_rows.size();
+      ALORA_CUDA(c, upload(c, (void**)&c->seg_row, seg_row));
+      ALORA_CUDA(c, upload(c, (void**)&c->seg_beg, seg_beg));
+      ALORA_CUDA(c, upload(c, (void**)&c->seg_end, seg_end));
+      ALORA_CUDA(c, upload(c, (void**)&c->heavy_rows, heavy_rows));
+      ALORA_CUDA(c, upload(c, (void**)&c->heavy_segptr, heavy_segptr));
+      ALORA_CUDA(c, c->pool.alloc(&c->seg_out, sizeof(double) * 256 * (size_t)c->nseg));
+      ALORA_CUDA(c, c->pool.alloc((void**)&c->seg_cx, sizeof(double) * (size_t)c->nseg));
+    }
     {
       std::vector<int> col(aents.size()), cons(aents.size());
       std::vector<T> val(aents.size());

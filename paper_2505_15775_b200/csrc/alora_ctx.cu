@@ -202,6 +202,12 @@ alora_status launch_diag_rows(alora_ctx* c, int vec, int nvec, int exact, int sh
 // (measured on config 3, 60 entries per row: the warp-per-row kernel wins for p = 1, 66 vs 77 us, and loses for
 // r = 10, 168 vs 128 us); rows with ~100 entries or more (matrix completion) always take a warp per row
 template <typename T> alora_status launch_adj_general(alora_ctx* c, const Geo& g, RowArgs<T>& a, double* out) {
+  if (c->nseg > 0 && g.nvec * g.vec <= 256) {   // heavy rows: their C part is summed per segment first
+    a.nseg = c->nseg;
+    const int gs = (int)std::min<int64_t>((c->nseg + kBlock / 32 - 1) / (kBlock / 32), (int64_t)c->num_sms * 8);
+    ALORA_CUDA(c, launch_rows_seg(g.vec, g.shape, a, gs, c->stream));
+    c->launches++;
+  }
   if ((c->ep && g.nvec == 1) || c->ep_wide) {
     int& occ = c->occ_cache[vec_slot(g.vec)][g.shape][11];
     if (!occ) occ = std::max(1, occ_rows_ep(T(), g.vec, g.shape));
@@ -245,6 +251,8 @@ template <typename T> void fill_rows(alora_ctx* c, RowArgs<T>& a, const Geo& g, 
   a.pC = 0; a.U = (const T*)c->U; a.Ts = c->Ts; a.scale = 1.0; a.diag_class = (c->cls == 0);
   a.partials = c->part_rows; a.row_begin = 0; a.tiles = 0;
   a.ell_col = c->ell_col; a.ell_val = (const T*)c->ell_val; a.rem32 = c->rem32;
+  a.nseg = 0; a.nheavy = c->nheavy; a.seg_row = c->seg_row; a.seg_beg = c->seg_beg; a.seg_end = c->seg_end;
+  a.heavy_rows = c->heavy_rows; a.heavy_segptr = c->heavy_segptr; a.seg_out = (T*)c->seg_out; a.seg_cx = c->seg_cx;
   a.fin = no_fin();
 }
 template <typename T> void fill_cons(alora_ctx* c, ConsArgs<T>& a, const Geo& g, const T* X, const T* X2, int r, int64_t ld) {

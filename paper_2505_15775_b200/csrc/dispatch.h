@@ -14,6 +14,7 @@ namespace alora {
   int occ_rows_##SUF(int shape, int mode);                                                            \
   cudaError_t launch_rows_ep_##SUF(int shape, const RowArgs<T>& a, int grid, cudaStream_t s);         \
   int occ_rows_ep_##SUF(int shape);                                                                   \
+  cudaError_t launch_rows_seg_##SUF(int shape, const RowArgs<T>& a, int grid, cudaStream_t s);        \
   int occ_cons_##SUF(int shape, int mode, int chunked);
 
 ALORA_DECL_INST(float, f32v4)
@@ -37,6 +38,13 @@ inline cudaError_t launch_rows_ep(int vec, int shape, const RowArgs<float>& a, i
 }
 inline cudaError_t launch_rows_ep(int vec, int shape, const RowArgs<double>& a, int grid, cudaStream_t s) {
   return vec == 2 ? launch_rows_ep_f64v2(shape, a, grid, s) : launch_rows_ep_f64v1(shape, a, grid, s);
+}
+inline cudaError_t launch_rows_seg(int vec, int shape, const RowArgs<float>& a, int grid, cudaStream_t s) {
+  return vec == 4 ? launch_rows_seg_f32v4(shape, a, grid, s)
+       : vec == 2 ? launch_rows_seg_f32v2(shape, a, grid, s) : launch_rows_seg_f32v1(shape, a, grid, s);
+}
+inline cudaError_t launch_rows_seg(int vec, int shape, const RowArgs<double>& a, int grid, cudaStream_t s) {
+  return vec == 2 ? launch_rows_seg_f64v2(shape, a, grid, s) : launch_rows_seg_f64v1(shape, a, grid, s);
 }
 inline int occ_rows_ep(float, int vec, int shape) {
   return vec == 4 ? occ_rows_ep_f32v4(shape) : vec == 2 ? occ_rows_ep_f32v2(shape) : occ_rows_ep_f32v1(shape);

@@ -22,6 +22,7 @@
 namespace alora {
 
 constexpr int kBlock = 256;
+constexpr int kHeavyRow = 128;        // a C row with more entries sends a diagonal-class problem down the general path
 constexpr int kLongThreshold = 64;   // constraints with more stored entries are split into chunks
 constexpr int kChunk = 16;           // entries per chunk of a long constraint / of C's sym-upper list
 // diagonal class: ELL slots per row (first neighbours; for the line search: last upper-triangle neighbours), see
@@ -71,6 +72,10 @@ template <typename T> struct RowArgs {
   // for the line search): slot u of row j at [j * NU + u]; rem32[j / 32] != 0: some row of that 32-row block
   // has more neighbours than slots (walk the CSR tail)
   const int* ell_col; const T* ell_val; const unsigned char* rem32;
+  // k_rows_ep: C rows with more than kHeavyRow entries are cut into segments of <= kHeavyRow entries that
+  // k_rows_seg sums first (seg_out[s][nvec * VEC], seg_cx[s]); heavy_rows (ascending) / heavy_segptr list them per row
+  int nseg, nheavy; const int* seg_row; const int* seg_beg; const int* seg_end;
+  const int* heavy_rows; const int* heavy_segptr; T* seg_out; double* seg_cx;
 };
 
 template <typename T> struct ConsArgs {
@@ -327,8 +332,21 @@ __global__ void __launch_bounds__(kBlock) k_rows(const RowArgs<T> a) {
       }
       // (C X)_row : diagonal + off-diagonal gathers
       Row acc; acc.zero(); acc.axpy(dc, x);
-      gather_axpy<T, VEC, GS, NIT>(acc, a.X, a.ld, a.c_col, a.c_val, cb, ce, lane, nvec, r, exact);
-      st[ES_CX] += (double)acc.dot(x);
+      if (MODE == ROWS_ADJ && a.nseg > 0 && ce - cb > kHeavyRow) {
+        // heavy row: its off-diagonal C part was summed per segment by k_rows_seg; add the results in order
+        int lo = 0, hi = a.nheavy - 1;
+        while (lo < hi) { const int mid = (lo + hi) >> 1; if (__ldg(a.heavy_rows + mid) < (int)row) lo = mid + 1; else hi = mid; }
+        const int s0 = __ldg(a.heavy_segptr + lo), s1 = __ldg(a.heavy_segptr + lo + 1);
+        st[ES_CX] += (double)acc.dot(x);
+        for (int sg = s0; sg < s1; ++sg) {
+          Row part; part.load(a.seg_out + (int64_t)sg * (nvec * VEC), lane, nvec, r, exact);
+          acc.axpy(T(1), part);
+          if (lane == 0) st[ES_CX] += a.seg_cx[sg];
+        }
+      } else {
+        gather_axpy<T, VEC, GS, NIT>(acc, a.X, a.ld, a.c_col, a.c_val, cb, ce, lane, nvec, r, exact);
+        st[ES_CX] += (double)acc.dot(x);
+      }
       if (MODE == ROWS_ADJ) {
         if (a.diag_class) {
           const int c = a.dcons ? __ldg(a.dcons + row) : (int)row;
@@ -406,13 +424,27 @@ __global__ void __launch_bounds__(kBlock) k_rows_ep(const RowArgs<T> a) {
     Row acc; acc.zero();
     T cxl = T(0);
     const int cb = __ldg(a.c_rowptr + row), ce = __ldg(a.c_rowptr + row + 1);
+    if (a.nseg > 0 && ce - cb > kHeavyRow) {
+      // heavy row: its C part was summed per segment by k_rows_seg; add the segment results in order
+      int lo = 0, hi = a.nheavy - 1;
+      while (lo < hi) { const int mid = (lo + hi) >> 1; if (__ldg(a.heavy_rows + mid) < (int)row) lo = mid + 1; else hi = mid; }
+      const int s0 = __ldg(a.heavy_segptr + lo), s1 = __ldg(a.heavy_segptr + lo + 1);
+      if (el == 0) {
+        for (int sg = s0; sg < s1; ++sg) {
+          Row part; part.load(a.seg_out + (int64_t)sg * (nvec * VEC), pl, nvec, r, exact);
+          acc.axpy(T(1), part);
+        }
+        if (pl == 0) { double t = 0.0; for (int sg = s0; sg < s1; ++sg) t += a.seg_cx[sg]; st[ES_CX] += t; }
+      }
+    } else {
 #pragma unroll 2
-    for (int e = cb + el; e < ce; e += EL) {
-      const int k = __ldg(a.c_col + e);
-      const T v = __ldg(a.c_val + e);
-      Row xn; xn.load(a.X + (int64_t)k * a.ld, pl, nvec, r, exact);
-      acc.axpy(v, xn);
-      cxl = fma(v, xn.dot(x), cxl);
+      for (int e = cb + el; e < ce; e += EL) {
+        const int k = __ldg(a.c_col + e);
+        const T v = __ldg(a.c_val + e);
+        Row xn; xn.load(a.X + (int64_t)k * a.ld, pl, nvec, r, exact);
+        acc.axpy(v, xn);
+        cxl = fma(v, xn.dot(x), cxl);
+      }
     }
     double coef = 0.0;
     if (a.diag_class) {
@@ -466,6 +498,41 @@ __global__ void __launch_bounds__(kBlock) k_rows_ep(const RowArgs<T> a) {
   }
   block_reduce_store<NST>(st, a.partials + (int64_t)blockIdx.x * kNStat);
   finish_partials(a.fin);
+}
+
+// Segment pass of k_rows_ep: a warp per segment (<= kHeavyRow consecutive C entries of a heavy row) leaves
+// sum_e c_e X_{k_e} in seg_out[s][0..r) and sum_e c_e <X_{k_e}, X_row> in seg_cx[s].
+template <typename T, int VEC, int PL, int NIT>
+__global__ void __launch_bounds__(kBlock) k_rows_seg(const RowArgs<T> a) {
+  using Row = RowReg<T, VEC, PL, NIT>;
+  constexpr int EL = 32 / PL, WPB = kBlock / 32;
+  const int lane32 = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int pl = lane32 % PL, el = lane32 / PL;
+  const int nvec = a.nvec, r = a.r, exact = a.exact;
+  for (int sg = blockIdx.x * WPB + warp; sg < a.nseg; sg += gridDim.x * WPB) {
+    const int64_t row = __ldg(a.seg_row + sg);
+    Row x; x.load(a.X + row * a.ld, pl, nvec, r, exact);
+    Row acc; acc.zero();
+    T cxl = T(0);
+    const int eb = __ldg(a.seg_beg + sg), ee = __ldg(a.seg_end + sg);
+#pragma unroll 2
+    for (int e = eb + el; e < ee; e += EL) {
+      const int k = __ldg(a.c_col + e);
+      const T v = __ldg(a.c_val + e);
+      Row xn; xn.load(a.X + (int64_t)k * a.ld, pl, nvec, r, exact);
+      acc.axpy(v, xn);
+      cxl = fma(v, xn.dot(x), cxl);
+    }
+#pragma unroll
+    for (int off = PL; off < 32; off <<= 1)
+#pragma unroll
+      for (int it = 0; it < NIT; ++it)
+#pragma unroll
+        for (int i = 0; i < VEC; ++i) acc.p[it].v[i] += __shfl_xor_sync(0xffffffffu, acc.p[it].v[i], off);
+    const double cx = warp_sum((double)cxl);
+    if (el == 0) acc.store(a.seg_out + (int64_t)sg * (nvec * VEC), pl, nvec, r, exact);
+    if (lane32 == 0) a.seg_cx[sg] = cx;
+  }
 }
 
 // ---------------------------------------------------------------------------------------------

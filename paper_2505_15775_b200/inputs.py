@@ -147,6 +147,22 @@ def tri_torus_edges(side: int) -> tuple[np.ndarray, np.ndarray]:
     return lo.astype(np.int64), hi.astype(np.int64)
 
 
+def rmat_edges(rng: np.random.Generator, scale: int, edge_factor: int) -> tuple[np.ndarray, np.ndarray]:
+    """R-MAT / Kronecker generator (Graph500 parameters a, b, c = 0.57, 0.19, 0.19): 2^scale vertices,
+    edge_factor * 2^scale sampled edges; power-law degrees with a few very heavy rows.  Stand-in for the
+    kron_g500 graphs, the slowest instances of the paper's Table 1."""
+    ne = edge_factor << scale
+    u = np.zeros(ne, np.int64)
+    w = np.zeros(ne, np.int64)
+    ab, c_norm, a_norm = 0.57 + 0.19, 0.19 / (1.0 - 0.76), 0.57 / 0.76
+    for bit in range(scale):
+        ii = rng.random(ne) > ab
+        jj = rng.random(ne) > np.where(ii, c_norm, a_norm)
+        u |= ii.astype(np.int64) << bit
+        w |= jj.astype(np.int64) << bit
+    return np.minimum(u, w), np.maximum(u, w)
+
+
 def ring_matching_edges(rng: np.random.Generator, n: int) -> tuple[np.ndarray, np.ndarray]:
     """Ring i-(i+1) mod n plus two independent seeded random perfect matchings (n even)."""
     if n % 2:
@@ -379,7 +395,20 @@ def config6(side: int = 1000, r: int = 16, seed: int = 1006) -> Workload:
     return _finish("cfg6_maxcut_tri_torus", prob, F32, r, R, y, 10.0, rng, {"edges": int(lo.shape[0])})
 
 
-CONFIGS = [config0, config1, config2, config3, config4, config5, config6]
+def config7(scale: int = 20, edge_factor: int = 8, r: int = 16, seed: int = 1007) -> Workload:
+    """MaxCut on an R-MAT graph (load-balance stress): unit weights, fp32 R."""
+    rng = _rng(seed)
+    lo, hi = rmat_edges(rng, scale, edge_factor)
+    n = 1 << scale
+    lo, hi, w = coalesce_edges(lo, hi, np.ones(lo.shape[0]), n)
+    w = np.ones_like(w)   # simple graph: repeated samples of an edge count once
+    prob = maxcut_problem(n, lo, hi, w)
+    R = _unit_rows(rng, n, r)
+    y = rng.standard_normal(n)
+    return _finish("cfg7_maxcut_rmat", prob, F32, r, R, y, 10.0, rng, {"edges": int(lo.shape[0])})
+
+
+CONFIGS = [config0, config1, config2, config3, config4, config5, config6, config7]
 
 # scaled-down versions: several tiles plus a ragged tail, oracle finishes in well under a second
 SMALL = {
@@ -390,6 +419,7 @@ SMALL = {
     4: lambda: config4(n=20002, r=10),
     5: lambda: config5(n=601, r_star=3, r=4, m=20011),
     6: lambda: config6(side=41, r=16),
+    7: lambda: config7(scale=11, edge_factor=8, r=16),
 }
 
 

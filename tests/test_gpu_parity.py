@@ -109,7 +109,7 @@ def check_workload(torch, binding, oracle_mod, w, ld=None, label="", split_scale
     ctx.close()
 
 
-@pytest.mark.parametrize("idx", [0, 1, 2, 3, 4, 5, 6])
+@pytest.mark.parametrize("idx", [0, 1, 2, 3, 4, 5, 6, 7])
 def test_small_configs(torch, binding, oracle_mod, idx):
     check_workload(torch, binding, oracle_mod, inputs.small(idx), label=f"small{idx}")
 
@@ -129,7 +129,7 @@ def test_ranks(torch, binding, oracle_mod, r):
         check_workload(torch, binding, oracle_mod, maker(), label=f"r{r}")
 
 
-@pytest.mark.parametrize("idx", [1, 2, 3, 4, 5, 6])
+@pytest.mark.parametrize("idx", [1, 2, 3, 4, 5, 6, 7])
 def test_full_configs(torch, binding, oracle_mod, idx):
     """BASELINE.json's full sizes, ld = r as bench.py launches them; the C oracle is fast enough to check
     every element of z, G, S(mu)v (config 4: n = 2^24, about a minute of oracle time)."""
