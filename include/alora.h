@@ -146,7 +146,8 @@ typedef struct {
   double tol0, c_in, tol_min; /* inner tolerance tol_t = max(tol_min, min(tol0, c_in*infeas_{t-1})): 1e-2, 0.1, 1e-7 */
   int32_t it_max;      /* inner iterations per outer iteration (500) */
   int32_t lbfgs_mem;   /* L-BFGS pairs (5); 0 = steepest descent with the exact step */
-  int32_t p_max;       /* eigenvectors per growth step; only 1 is implemented */
+  int32_t p_max;       /* eigenvectors per growth step, 1..4 (1: closed-form step; more: every sufficiently negative
+                          Ritz pair of the Lanczos run, small SDP of Alg. 1 line 7; reading 29) */
   int32_t k_max;       /* Lanczos steps (300) */
   double tau_neg;      /* growth threshold on -theta_1/(1+||C||_F); < 0 means eps */
   double tol_eig;      /* Lanczos residual tolerance relative to (1+||C||_F); < 0 means eps/10 */

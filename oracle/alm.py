@@ -32,7 +32,7 @@ class Params:
     tol_min: float = 1e-7
     it_max: int = 500          # [6] inner iterations per outer iteration
     lbfgs_mem: int = 5         # [5] 0 = steepest descent with exact step (the paper's GD)
-    p_max: int = 1             # [7] eigenvectors per growth step (only 1 implemented)
+    p_max: int = 1             # [7, 29] eigenvectors per growth step (1: closed form; up to 4: small SDP)
     tau_neg: float = -1.0      # [8] growth threshold; < 0 means "use eps"
     tol_eig: float = -1.0      # [9] Lanczos residual tolerance; < 0 means eps/10
     k_max: int = 300           # [9] Lanczos steps
@@ -260,12 +260,12 @@ def solve(orc, R0, y0, sigma0: float, prm: Params = Params()) -> Result:
     res = Result()
     infeas_prev, qnorm_prev, run = np.inf, np.inf, 0
 
-    def run_lanczos(w):
+    def run_lanczos(w, p_want=1):
         nonlocal run
         def mv(v):
             res.n_matvec += 1
             return orc.smatvec(w, v)
-        out = lanczos(mv, n, prm.seed + run, prm.k_max, tol_eig * (1.0 + normC))
+        out = lanczos(mv, n, prm.seed + run, prm.k_max, tol_eig * (1.0 + normC), p_want)
         run += 1
         return out
 
@@ -308,18 +308,38 @@ def solve(orc, R0, y0, sigma0: float, prm: Params = Params()) -> Result:
         lam, z = orc.lam(y, sigma, R)
         q = z - b
         # -- 3. eigenvector of nabla_X L_rho = C - A^*(lambda)         (Alg. 1 line 5)
-        theta, v, ksteps, _ = run_lanczos(lam)
+        multi = None
+        if prm.p_max > 1:
+            theta, v, ksteps, _, multi = run_lanczos(lam, prm.p_max)
+        else:
+            theta, v, ksteps, _ = run_lanczos(lam)
         rec.theta1, rec.lanczos_steps = theta, ksteps
         theta_kkt, changed = theta, False
         if -theta / (1.0 + normC) > tau_neg:
             # -- 4. grow: S <- argmin_{S>=0} L_rho(FF^T + V S V^T, y), F <- [F, V S^{1/2}]
-            #       (Alg. 1 lines 6-8); p = 1 closed form
-            #       L(X + s vv^T) - L(X) = s theta + (sigma/2) s^2 ||A(vv^T)||^2
-            av = orc.A_op(v[:, None])
-            den = sigma * float(av @ av)
-            s_star = -theta / den if den > 0.0 and -theta / den < prm.s_max else prm.s_max
-            R = np.hstack([R, np.sqrt(s_star) * v[:, None]])
-            rec.grew, changed = 1, True
+            #       (Alg. 1 lines 6-8)
+            cols = None
+            if multi is not None:
+                # [29] every Ritz pair of the run that is itself sufficiently negative joins V
+                ths, U = multi
+                sel = [j for j in range(len(ths)) if -ths[j] / (1.0 + normC) > tau_neg]
+                if len(sel) > 1:
+                    U, ths = U[:, sel], ths[sel]
+                    pairs = [(a, c) for a in range(len(sel)) for c in range(a, len(sel))]
+                    cab = np.array([orc.A_sym(U[:, [a]], U[:, [c]]) for a, c in pairs])
+                    S, gval = growth_sdp(ths, cab @ cab.T, sigma)
+                    if gval < 0.0:
+                        mu, Q = np.linalg.eigh(S)
+                        keep = mu > 1e-12 * mu[-1]
+                        cols = U @ (Q[:, keep] * np.sqrt(mu[keep]))      # [11] V S^{1/2} with S^{1/2} = Q mu^{1/2}
+            if cols is None:
+                # p = 1 closed form: L(X + s vv^T) - L(X) = s theta + (sigma/2) s^2 ||A(vv^T)||^2
+                av = orc.A_op(v[:, None])
+                den = sigma * float(av @ av)
+                s_star = -theta / den if den > 0.0 and -theta / den < prm.s_max else prm.s_max
+                cols = np.sqrt(s_star) * v[:, None]
+            R = np.hstack([R, cols])
+            rec.grew, changed = cols.shape[1], True
         elif R.shape[1] > 1:
             # -- 5. shrink [13]: drop the numerically null directions of R
             M = R.T @ R

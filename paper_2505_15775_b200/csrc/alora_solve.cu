@@ -301,6 +301,7 @@ struct SolveWorkspace {
   void* buf[4 + 2 * 16] = {}; int nbuf = 0; int64_t buf_elems = 0;
   double* lam = nullptr; double* z = nullptr; double* zv = nullptr; void* ritz = nullptr;
   double* gram_part = nullptr; double* gram = nullptr; double* Qdev = nullptr;
+  void* ritzp = nullptr; void* vtmp = nullptr; double* cab = nullptr;   // p_max > 1: Ritz vectors (4 x n), v_a + v_b, c_ab (11 x m)
 };
 
 void free_solve_workspace(alora_ctx* c) {
@@ -333,8 +334,9 @@ int sturm_count(const std::vector<double>& a, const std::vector<double>& b, int 
 
 // smallest eigenvalue (bisection) and its unit eigenvector (inverse iteration) of the k x k
 // symmetric tridiagonal with diagonal a[0..k) and off-diagonal b[0..k-1)
-void tridiag_smallest(const std::vector<double>& a, const std::vector<double>& b, int k, double& theta,
-                      std::vector<double>& s) {
+// (j+1)-th smallest eigenvalue and its unit eigenvector; `prev`: eigenvectors already found (kept orthogonal to)
+void tridiag_jth(const std::vector<double>& a, const std::vector<double>& b, int k, int j, double& theta,
+                 std::vector<double>& s, const std::vector<std::vector<double>>& prev) {
   s.assign(k, 0.0);
   if (k == 1) { theta = a[0]; s[0] = 1.0; return; }
   double lo = a[0], hi = a[0], scale = 0.0;
@@ -347,13 +349,13 @@ void tridiag_smallest(const std::vector<double>& a, const std::vector<double>& b
   for (int it = 0; it < 200 && h - l > 4e-16 * std::max(std::fabs(l), std::fabs(h)) + 1e-300; ++it) {
     const double mid = 0.5 * (l + h);
     if (mid <= l || mid >= h) break;
-    if (sturm_count(a, b, k, mid) >= 1) h = mid; else l = mid;
+    if (sturm_count(a, b, k, mid) >= j + 1) h = mid; else l = mid;
   }
   theta = 0.5 * (l + h);
   // inverse iteration: (T - shift I) x = rhs with partial pivoting (shift nudged off the eigenvalue)
   const double shift = theta - 1e-13 * std::max(scale, 1e-300) - 1e-300;
   std::vector<double> x(k), dl(k), d(k), du(k), du2(k);
-  for (int i = 0; i < k; ++i) x[i] = 1.0 + 0.01 * ((i * 7919) % 13);
+  for (int i = 0; i < k; ++i) x[i] = 1.0 + 0.01 * (((i + 31 * j) * 7919) % 13);
   for (int rep = 0; rep < 4; ++rep) {
     for (int i = 0; i < k; ++i) { d[i] = a[i] - shift; du[i] = i + 1 < k ? b[i] : 0.0; dl[i] = i + 1 < k ? b[i] : 0.0; du2[i] = 0.0; }
     // LU with partial pivoting on the tridiagonal (dgtsv style), applied to x
@@ -379,13 +381,22 @@ void tridiag_smallest(const std::vector<double>& a, const std::vector<double>& b
     x[k - 1] /= d[k - 1];
     if (k > 1) x[k - 2] = (x[k - 2] - du[k - 2] * x[k - 1]) / d[k - 2];
     for (int i = k - 3; i >= 0; --i) x[i] = (x[i] - du[i] * x[i + 1] - du2[i] * x[i + 2]) / d[i];
+    for (const auto& pv : prev) {   // close eigenvalues: stay orthogonal to the vectors already found
+      double d0 = 0.0;
+      for (int i = 0; i < k; ++i) d0 += pv[i] * x[i];
+      for (int i = 0; i < k; ++i) x[i] -= d0 * pv[i];
+    }
     double nrm = 0.0;
     for (int i = 0; i < k; ++i) nrm += x[i] * x[i];
     nrm = std::sqrt(nrm);
-    if (!(nrm > 0.0) || !std::isfinite(nrm)) { for (int i = 0; i < k; ++i) x[i] = (i == 0); nrm = 1.0; }
+    if (!(nrm > 0.0) || !std::isfinite(nrm)) { for (int i = 0; i < k; ++i) x[i] = (i == j % k); nrm = 1.0; }
     for (int i = 0; i < k; ++i) x[i] /= nrm;
   }
   s = x;
+}
+void tridiag_smallest(const std::vector<double>& a, const std::vector<double>& b, int k, double& theta,
+                      std::vector<double>& s) {
+  tridiag_jth(a, b, k, 0, theta, s, {});
 }
 
 // real roots of c3 x^3 + c2 x^2 + c1 x + c0 (c3 != 0); a complex pair whose imaginary part is below
@@ -500,6 +511,69 @@ inline int ew_grid(alora_ctx* c, int64_t N) {
 namespace alora {
 namespace {
 
+// Alg. 1 line 7 for p <= 4 directions, reading 29: minimise over S psd (p x p)
+//   g(S) = sum_a theta_a S_aa + (sigma/2) s^T Hw s,   s = (S_ab)_{a<=b} row-major, Hw = H .* (w w^T), w_ab = 1 or 2,
+// H[(ab),(cd)] = <c_ab, c_cd>, by projected gradient with step 1/L from S0 = diag(-theta_a / (sigma H[(aa),(aa)])).
+// S row-major p x p out; returns g(S).  Same iteration as oracle/alm.py::growth_sdp.
+double growth_sdp_host(int p, const double* theta, const std::vector<double>& H, double sigma, std::vector<double>& S, int iters = 500) {
+  const int np = p * (p + 1) / 2;
+  std::vector<int> pa(np), pb(np);
+  std::vector<double> wgt(np);
+  { int t = 0; for (int a = 0; a < p; ++a) for (int b = a; b < p; ++b) { pa[t] = a; pb[t] = b; wgt[t] = a == b ? 1.0 : 2.0; ++t; } }
+  auto Hw = [&](int i, int j) { return H[(size_t)i * np + j] * wgt[i] * wgt[j]; };
+  // Lipschitz constant: sigma * lambda_max(D Hw D), D = diag(1 or 1/sqrt 2)
+  std::vector<double> B((size_t)np * np), mu, Q;
+  for (int i = 0; i < np; ++i) for (int j = 0; j < np; ++j)
+    B[(size_t)i * np + j] = Hw(i, j) * (pa[i] == pb[i] ? 1.0 : M_SQRT1_2) * (pa[j] == pb[j] ? 1.0 : M_SQRT1_2);
+  jacobi_eigh(B, np, mu, Q);
+  const double L = sigma * std::max(mu[np - 1], 1e-300);
+  S.assign((size_t)p * p, 0.0);
+  for (int a = 0; a < p; ++a) {
+    int idx = 0; for (int t = 0; t < np; ++t) if (pa[t] == a && pb[t] == a) idx = t;
+    const double haa = H[(size_t)idx * np + idx];
+    S[a * p + a] = haa > 0.0 ? std::max(0.0, -theta[a] / (sigma * haa)) : 0.0;
+  }
+  std::vector<double> sv(np), tv(np), G((size_t)p * p);
+  auto gval = [&]() {
+    for (int t = 0; t < np; ++t) sv[t] = S[pa[t] * p + pb[t]];
+    double q = 0.0;
+    for (int i = 0; i < np; ++i) { double r2 = 0.0; for (int j = 0; j < np; ++j) r2 += Hw(i, j) * sv[j]; q += sv[i] * r2; }
+    double lin = 0.0;
+    for (int a = 0; a < p; ++a) lin += theta[a] * S[a * p + a];
+    return lin + 0.5 * sigma * q;
+  };
+  for (int it = 0; it < iters; ++it) {
+    for (int t = 0; t < np; ++t) sv[t] = S[pa[t] * p + pb[t]];
+    for (int i = 0; i < np; ++i) { double r2 = 0.0; for (int j = 0; j < np; ++j) r2 += Hw(i, j) * sv[j]; tv[i] = sigma * r2; }
+    std::fill(G.begin(), G.end(), 0.0);
+    for (int t = 0; t < np; ++t) {
+      if (pa[t] == pb[t]) G[pa[t] * p + pa[t]] = tv[t];
+      else G[pa[t] * p + pb[t]] = G[pb[t] * p + pa[t]] = 0.5 * tv[t];
+    }
+    for (int a = 0; a < p; ++a) G[a * p + a] += theta[a];
+    std::vector<double> Y((size_t)p * p), m2, Q2;
+    for (int i = 0; i < p * p; ++i) Y[i] = S[i] - G[i] / L;
+    for (int a = 0; a < p; ++a) for (int b = a + 1; b < p; ++b) { const double av = 0.5 * (Y[a * p + b] + Y[b * p + a]); Y[a * p + b] = Y[b * p + a] = av; }
+    jacobi_eigh(Y, p, m2, Q2);
+    for (int a = 0; a < p; ++a) for (int b = 0; b < p; ++b) {
+      double v = 0.0;
+      for (int k = 0; k < p; ++k) v += Q2[a * p + k] * std::max(m2[k], 0.0) * Q2[b * p + k];
+      S[a * p + b] = v;
+    }
+  }
+  return gval();
+}
+
+// out = 0.5 (zt - za - zb): polarisation  A((v_a v_b^T + v_b v_a^T)/2) from A((v_a+v_b)(v_a+v_b)^T), A(v_a v_a^T), A(v_b v_b^T)
+__global__ void k_polar(int64_t m, const double* zt, const double* za, const double* zb, double* out) {
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < m; i += (int64_t)gridDim.x * blockDim.x)
+    out[i] = 0.5 * (zt[i] - za[i] - zb[i]);
+}
+template <typename T> __global__ void k_add2(int64_t N, const T* x, const T* y, T* out) {   // out = x + y
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (int64_t)gridDim.x * blockDim.x)
+    out[i] = (T)((double)x[i] + (double)y[i]);
+}
+
 alora_status ensure_ws(alora_ctx* c) {
   if (c->ws) return ALORA_OK;
   c->ws = new (std::nothrow) SolveWorkspace();
@@ -540,7 +614,8 @@ template <typename T> alora_status dot1(alora_ctx* c, int64_t N, const T* x, con
 
 template <typename T>
 alora_status lanczos_impl(alora_ctx* c, const double* mu, int kmax, double tol_abs, uint64_t seed, double* theta_out,
-                          T* v_out, int* k_used, double* resid_out, int* n_matvec) {
+                          T* v_out, int* k_used, double* resid_out, int* n_matvec, int p_want = 1,
+                          std::vector<double>* thetas = nullptr, T* U_out = nullptr) {
   alora_status s = ensure_ws(c);
   if (s != ALORA_OK) return s;
   SolveWorkspace* w = c->ws;
@@ -604,6 +679,27 @@ alora_status lanczos_impl(alora_ctx* c, const double* mu, int kmax, double tol_a
     k_scale<T><<<g, 256, 0, c->stream>>>(n, 1.0 / std::sqrt(vv), v_out);
     c->launches++;
     ALORA_CUDA(c, cudaStreamSynchronize(c->stream));  // sv is about to go out of scope
+  }
+  if (p_want > 1 && thetas && U_out) {
+    // reading 29: the min(p_want, k) smallest Ritz pairs of the same k-step tridiagonal; vector j at U_out + j n
+    if (k > 1 && (int)be.size() >= k) be.resize(k - 1);
+    const int pw = std::min(p_want, k);
+    thetas->assign(pw, 0.0);
+    std::vector<std::vector<double>> found;
+    for (int j = 0; j < pw; ++j) {
+      std::vector<double> sj;
+      tridiag_jth(al, be, k, j, (*thetas)[j], sj, found);
+      found.push_back(sj);
+      ALORA_CUDA(c, cudaMemcpyAsync(w->cvec, sj.data(), sizeof(double) * k, cudaMemcpyHostToDevice, c->stream));
+      T* uj = U_out + (int64_t)j * n;
+      k_basis_combine<T><<<g, 256, 0, c->stream>>>(n, k, V, w->cvec, 0.0, 1.0, uj);
+      c->launches++;
+      double vv;
+      s = dot1<T>(c, n, uj, uj, &vv); if (s != ALORA_OK) return s;
+      k_scale<T><<<g, 256, 0, c->stream>>>(n, 1.0 / std::sqrt(vv), uj);
+      c->launches++;
+      ALORA_CUDA(c, cudaStreamSynchronize(c->stream));
+    }
   }
   ALORA_CUDA(c, cudaGetLastError());
   if (theta_out) *theta_out = theta;
@@ -687,7 +783,7 @@ alora_status solve_impl(alora_ctx* c, const alora_params* prm, T* R_user, int32_
   const int mem = std::max(0, std::min(prm->lbfgs_mem, 16));
   int r = *r_inout;
   if (r < 1 || r > r_cap) return fail(c, ALORA_EINVAL, "alora_solve: need 1 <= r <= r_cap");
-  if (prm->p_max != 1) return fail(c, ALORA_EINVAL, "alora_solve: only p_max = 1 is implemented");
+  if (prm->p_max < 1 || prm->p_max > 4) return fail(c, ALORA_EINVAL, "alora_solve: need 1 <= p_max <= 4");
   const int ldcap = pad(r_cap);
   const int64_t elems = n * (int64_t)ldcap;
   const int nslot = mem + 1;                              // one spare slot receives the candidate pair
@@ -872,7 +968,18 @@ alora_status solve_impl(alora_ctx* c, const alora_params* prm, T* R_user, int32_
     k_lambda2<<<ew_grid(c, m), 256, 0, c->stream>>>(m, y, w->z, c->b, sigma, w->lam);
     c->launches++;
     double theta = 0.0, resid = 0.0; int ksteps = 0;
-    s = lanczos_impl<T>(c, w->lam, prm->k_max, tol_eig * (1.0 + normC), prm->seed + run, &theta, (T*)w->ritz, &ksteps, &resid, &n_mv);
+    std::vector<double> thetas;
+    if (prm->p_max > 1) {
+      if (!w->ritzp) {
+        ALORA_CUDA(c, c->pool.alloc(&w->ritzp, c->esz * (size_t)n * 4));
+        ALORA_CUDA(c, c->pool.alloc(&w->vtmp, c->esz * (size_t)n));
+        ALORA_CUDA(c, c->pool.alloc((void**)&w->cab, sizeof(double) * (size_t)std::max<int64_t>(1, m) * 11));
+      }
+      s = lanczos_impl<T>(c, w->lam, prm->k_max, tol_eig * (1.0 + normC), prm->seed + run, &theta, (T*)w->ritz, &ksteps, &resid, &n_mv,
+                          prm->p_max, &thetas, (T*)w->ritzp);
+    } else {
+      s = lanczos_impl<T>(c, w->lam, prm->k_max, tol_eig * (1.0 + normC), prm->seed + run, &theta, (T*)w->ritz, &ksteps, &resid, &n_mv);
+    }
     ++run;
     if (s != ALORA_OK && s != ALORA_ENOTCONV) return s;
     rec.theta1 = theta; rec.lanczos_steps = ksteps;
@@ -882,20 +989,79 @@ alora_status solve_impl(alora_ctx* c, const alora_params* prm, T* R_user, int32_
     if (neg && r + 1 <= r_cap) {
       // -- 4. grow (Alg. 1 lines 6-8), p = 1: s* = -theta / (sigma |A(vv^T)|^2).  At r = r_cap the
       //       step is skipped (reading 27): the dual update and the sigma schedule carry on at rank r_cap.
-      s = alora_eval(c, w->ritz, 1, 1, nullptr, w->zv, nullptr); if (s != ALORA_OK) return s;
-      double avv[3]; s = dots<double, double>(c, m, 1, w->zv, w->zv, w->zv, w->zv, w->zv, w->zv, avv); if (s != ALORA_OK) return s;
-      const double den = sigma * avv[0];
-      const double s_star = (den > 0.0 && -theta / den < prm->s_max) ? -theta / den : prm->s_max;
-      const int ld2 = pad(r + 1);
-      if (ld2 != ld) {
-        k_repack<T><<<ew_grid(c, n * (int64_t)ld2), 256, 0, c->stream>>>(n, r, Rw, ld, Rtmp, ld2);
-        c->launches++;
-        std::swap(Rw, Rtmp);
-        ld = ld2;
+      // reading 29 (p_max > 1): every Ritz pair of the run that is itself sufficiently negative joins V; S from the
+      // small SDP; new columns V S^{1/2}, at most r_cap - r of them (largest eigenvalues of S first)
+      int added = 0;
+      std::vector<int> sel;
+      for (int j = 0; j < (int)thetas.size(); ++j) if (-thetas[j] / (1.0 + normC) > tau_neg) sel.push_back(j);
+      if ((int)sel.size() > 1) {
+        const int p = (int)sel.size(), np = p * (p + 1) / 2;
+        const T* U = (const T*)w->ritzp;
+        std::vector<int> pa, pb;
+        for (int a = 0; a < p; ++a) for (int b = a; b < p; ++b) { pa.push_back(a); pb.push_back(b); }
+        auto cvec = [&](int t) { return w->cab + (size_t)t * std::max<int64_t>(1, m); };
+        auto diag_idx = [&](int a) { int t = 0; for (int a2 = 0; a2 < a; ++a2) t += p - a2; return t; };
+        for (int a = 0; a < p; ++a) {   // c_aa = A(v_a v_a^T)
+          s = alora_eval(c, U + (int64_t)sel[a] * n, 1, 1, nullptr, cvec(diag_idx(a)), nullptr); if (s != ALORA_OK) return s;
+        }
+        for (int t = 0; t < np; ++t) {
+          if (pa[t] == pb[t]) continue;
+          k_add2<T><<<ew_grid(c, n), 256, 0, c->stream>>>(n, U + (int64_t)sel[pa[t]] * n, U + (int64_t)sel[pb[t]] * n, (T*)w->vtmp);
+          s = alora_eval(c, w->vtmp, 1, 1, nullptr, cvec(10), nullptr); if (s != ALORA_OK) return s;
+          k_polar<<<ew_grid(c, m), 256, 0, c->stream>>>(m, cvec(10), cvec(diag_idx(pa[t])), cvec(diag_idx(pb[t])), cvec(t));
+          c->launches += 2;
+        }
+        std::vector<double> H((size_t)np * np, 0.0);
+        for (int i = 0; i < np; ++i)
+          for (int j = i; j < np; ++j) {
+            double d3[3];
+            s = dots<double, double>(c, m, 1, cvec(i), cvec(j), cvec(i), cvec(j), cvec(i), cvec(j), d3); if (s != ALORA_OK) return s;
+            H[(size_t)i * np + j] = H[(size_t)j * np + i] = d3[0];
+          }
+        std::vector<double> th(p), S;
+        for (int a = 0; a < p; ++a) th[a] = thetas[sel[a]];
+        const double gv = growth_sdp_host(p, th.data(), H, sigma, S);
+        if (gv < 0.0) {
+          std::vector<double> mu, Q;
+          std::vector<double> S2(S);
+          jacobi_eigh(S2, p, mu, Q);
+          std::vector<int> cols;
+          for (int k2 = p - 1; k2 >= 0; --k2) if (mu[k2] > 1e-12 * mu[p - 1] && (int)cols.size() < r_cap - r) cols.push_back(k2);
+          const int ld2 = pad(r + (int)cols.size());
+          if (ld2 != ld) {
+            k_repack<T><<<ew_grid(c, n * (int64_t)ld2), 256, 0, c->stream>>>(n, r, Rw, ld, Rtmp, ld2);
+            c->launches++;
+            std::swap(Rw, Rtmp);
+            ld = ld2;
+          }
+          for (int k2 : cols) {   // column = sum_a v_a Q[a][k2] sqrt(mu_k2)
+            ALORA_CUDA(c, cudaStreamSynchronize(c->stream));
+            k_scale_copy<T><<<ew_grid(c, n), 256, 0, c->stream>>>(n, Q[0 * p + k2] * std::sqrt(mu[k2]), U + (int64_t)sel[0] * n, (T*)w->vtmp);
+            for (int a = 1; a < p; ++a)
+              k_axpy<T><<<ew_grid(c, n), 256, 0, c->stream>>>(n, Q[a * p + k2] * std::sqrt(mu[k2]), U + (int64_t)sel[a] * n, (T*)w->vtmp);
+            k_set_col<T><<<ew_grid(c, n), 256, 0, c->stream>>>(n, ld, r + added, 1.0, (const T*)w->vtmp, Rw);
+            c->launches += p + 1;
+            ++added;
+          }
+        }
       }
-      k_set_col<T><<<ew_grid(c, n), 256, 0, c->stream>>>(n, ld, r, std::sqrt(s_star), (const T*)w->ritz, Rw);
-      c->launches++;
-      ++r; rec.grew = 1; changed = true;
+      if (added == 0) {   // p = 1 closed form
+        s = alora_eval(c, w->ritz, 1, 1, nullptr, w->zv, nullptr); if (s != ALORA_OK) return s;
+        double avv[3]; s = dots<double, double>(c, m, 1, w->zv, w->zv, w->zv, w->zv, w->zv, w->zv, avv); if (s != ALORA_OK) return s;
+        const double den = sigma * avv[0];
+        const double s_star = (den > 0.0 && -theta / den < prm->s_max) ? -theta / den : prm->s_max;
+        const int ld2 = pad(r + 1);
+        if (ld2 != ld) {
+          k_repack<T><<<ew_grid(c, n * (int64_t)ld2), 256, 0, c->stream>>>(n, r, Rw, ld, Rtmp, ld2);
+          c->launches++;
+          std::swap(Rw, Rtmp);
+          ld = ld2;
+        }
+        k_set_col<T><<<ew_grid(c, n), 256, 0, c->stream>>>(n, ld, r, std::sqrt(s_star), (const T*)w->ritz, Rw);
+        c->launches++;
+        added = 1;
+      }
+      r += added; rec.grew = added; changed = true;
     } else if (!neg && r > 1) {
       // -- 5. shrink (reading 13): drop the numerically null directions of R
       const int nblk = (int)std::max<int64_t>(1, std::min<int64_t>(64, n / 256));

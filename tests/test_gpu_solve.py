@@ -181,3 +181,31 @@ def test_solve_matrix_completion(torch, binding, oracle_mod, dtype, tol):
     assert np.linalg.norm(X[:n1, n1:] - M) <= 10 * tol * np.linalg.norm(M)
     nuc = np.linalg.svd(M, compute_uv=False).sum()
     assert abs(0.5 * np.trace(X) - nuc) <= tol * nuc
+
+
+def test_solve_pmax3(torch, binding, alm, oracle_mod):
+    """p_max = 3 (reading 29): same optimum as the oracle's p_max = 3 and p_max = 1 runs on MaxCut
+    G(60,150) from rank 1, several columns added in one outer iteration, and the same growth decisions as the
+    oracle in the first outer iterations."""
+    rng = np.random.default_rng(60)
+    edges = set()
+    while len(edges) < 150:
+        i, j = sorted(int(x) for x in rng.integers(0, 60, 2))
+        if i != j:
+            edges.add((i, j))
+    P = _graph_maxcut(60, sorted(edges))
+    o = oracle_mod.Oracle(P)
+    R0 = inputs._unit_rows(np.random.default_rng(1), 60, 1)
+    ref = alm.solve(o, R0, np.zeros(60), 1.0, alm.Params(eps=1e-7, p_max=3))
+    out = gpu_solve(torch, binding, P, inputs.F64, R0, np.zeros(60), 1.0, r_cap=32, eps=1e-7, p_max=3)
+    assert out["ok"] and ref.converged
+    assert max(rec.grew for rec in out["log"]) >= 2
+    assert abs(o.inner_C(out["R"], out["R"]) - o.inner_C(ref.R, ref.R)) <= 1e-5 * abs(o.inner_C(ref.R, ref.R))
+    for a, b in list(zip(out["log"], ref.log))[:3]:
+        assert (a.r, a.grew) == (b.r, b.grew), (a.t, a.r, a.grew, b.r, b.grew)
+    # K_9 with p_max = 4 still reaches -n^2/4
+    n = 9
+    Pk = _graph_maxcut(n, [(i, j) for i in range(n) for j in range(i + 1, n)])
+    outk = gpu_solve(torch, binding, Pk, inputs.F64, inputs._unit_rows(np.random.default_rng(9), n, 1), np.zeros(n), 1.0,
+                     r_cap=32, eps=1e-7, p_max=4)
+    assert outk["ok"] and abs(oracle_mod.Oracle(Pk).inner_C(outk["R"], outk["R"]) + n * n / 4) < 1e-4

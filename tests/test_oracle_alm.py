@@ -180,3 +180,90 @@ def test_matrix_completion_nuclear_norm(alm, Oracle):
     assert np.linalg.norm(Y - M) <= 1e-4 * np.linalg.norm(M)
     nuc = np.linalg.svd(M, compute_uv=False).sum()
     assert abs(o.inner_C(res.R, res.R) - nuc) <= 1e-5 * nuc
+
+
+def test_lanczos_multi_rayleigh(alm, Oracle):
+    """[29] several Ritz pairs of one run: orthonormal vectors whose Rayleigh quotients are the Ritz values
+    (so U^T S U = diag(theta) whether or not they have converged); the converged ones match a dense solver."""
+    w = inputs.small(0)
+    o = Oracle(w.problem)
+    lam, _ = o.lam(np.random.default_rng(1).standard_normal(w.problem.m), 1.0, w.R)
+    S = o.smatvec(lam, np.eye(w.problem.n))
+    theta, v, k, resid, (ths, U) = alm.lanczos(lambda x: o.smatvec(lam, x), w.problem.n, 42, 300, 1e-8, p_want=4)
+    assert ths.shape == (4,) and U.shape == (w.problem.n, 4) and abs(ths[0] - theta) < 1e-12
+    np.testing.assert_allclose(U.T @ U, np.eye(4), atol=1e-10)
+    np.testing.assert_allclose(U.T @ S @ U, np.diag(ths), atol=1e-8)
+    ev = np.linalg.eigvalsh(S)
+    assert abs(ths[0] - ev[0]) < 1e-8 and np.all(ths >= ev[:4] - 1e-9)   # Ritz values interlace from above
+
+
+def test_growth_sdp_model_and_optimality(alm, Oracle):
+    """Alg. 1 line 7: g(S) = <U^T S(lambda) U, S> + sigma/2 ||A(U S U^T)||^2 is exactly
+    L_rho(X + U S U^T, y) - L_rho(X, y); the computed S* is feasible, satisfies the KKT conditions of the
+    small SDP (gradient psd, complementary to S*), beats random feasible points, and for p = 1 equals the
+    closed form s* = -theta / (sigma ||A(vv^T)||^2) [10]."""
+    rng = np.random.default_rng(5)
+    w = inputs.small(3)                        # general class: dense-ish A(vv^T)
+    P = w.problem
+    o = Oracle(P)
+    R, y, sigma = w.R, w.y, 0.7
+    lam, _ = o.lam(y, sigma, R)
+    n = P.n
+    # three orthonormal directions with negative curvature: bottom Ritz vectors of S(lambda)
+    _, _, _, _, (ths, U) = alm.lanczos(lambda x: o.smatvec(lam, x), n, 3, 60, 1e-10, p_want=3)
+    assert np.all(ths < 0)
+    pairs = [(a, c) for a in range(3) for c in range(a, 3)]
+    cab = np.array([o.A_sym(U[:, [a]], U[:, [c]]) for a, c in pairs])
+    H = cab @ cab.T
+    M = U.T @ o.smatvec(lam, U)
+
+    def g_model(S):
+        v = sum((1.0 if a == c else 2.0) * S[a, c] * cab[i] for i, (a, c) in enumerate(pairs))
+        return float(np.sum(M * S) + 0.5 * sigma * v @ v)
+
+    f0 = o.f(y, sigma, R)
+    for _ in range(3):
+        A = rng.standard_normal((3, 3)) * 1e-3
+        S = A @ A.T
+        mu, Q = np.linalg.eigh(S)
+        T = Q * np.sqrt(np.maximum(mu, 0))
+        df = o.f(y, sigma, np.hstack([R, U @ T])) - f0
+        assert abs(df - g_model(S)) <= 1e-9 * (abs(df) + abs(f0) * 1e-6 + 1e-12)
+    S, gval = alm.growth_sdp(ths, H, sigma)
+    assert np.linalg.eigvalsh(S)[0] >= -1e-12 and gval < 0
+    assert abs(gval - g_model(S)) <= 1e-7 * abs(gval) + 1e-7 * np.abs(M - np.diag(ths)).max()
+    # KKT of min g over the psd cone: G = dg/dS psd, <G, S> = 0
+    v = sum((1.0 if a == c else 2.0) * S[a, c] * cab[i] for i, (a, c) in enumerate(pairs))
+    G = np.diag(ths).astype(float)
+    for i, (a, c) in enumerate(pairs):
+        t = sigma * float(cab[i] @ v)
+        G[a, c] += t
+        if a != c:
+            G[c, a] += t
+    scale = np.abs(ths).max()
+    assert np.linalg.eigvalsh(G)[0] >= -1e-5 * scale and abs(np.sum(G * S)) <= 1e-5 * scale * np.trace(S)
+    for _ in range(2000):
+        A = rng.standard_normal((3, 3)) * np.sqrt(np.trace(S)) * rng.random()
+        assert g_model(A @ A.T) >= gval - 1e-9 * abs(gval)
+    # p = 1 closed form
+    S1, g1 = alm.growth_sdp(ths[:1], H[:1, :1], sigma)
+    s_star = -ths[0] / (sigma * H[0, 0])
+    assert abs(S1[0, 0] - s_star) <= 1e-12 * s_star and abs(g1 + 0.5 * ths[0] ** 2 / (sigma * H[0, 0])) <= 1e-12 * abs(g1)
+
+
+def test_solve_pmax3_same_optimum(alm, Oracle):
+    """p_max = 3 reaches the optimum that p_max = 1 reaches (MaxCut on G(60,150) from rank 1), growing by
+    several columns in at least one outer iteration."""
+    rng = np.random.default_rng(60)
+    edges = set()
+    while len(edges) < 150:
+        i, j = sorted(int(x) for x in rng.integers(0, 60, 2))
+        if i != j:
+            edges.add((i, j))
+    P = _graph_maxcut(60, sorted(edges))
+    o = Oracle(P)
+    R0 = inputs._unit_rows(np.random.default_rng(1), 60, 1)
+    r1 = alm.solve(o, R0, np.zeros(60), 1.0, alm.Params(eps=1e-7, p_max=1))
+    r3 = alm.solve(o, R0, np.zeros(60), 1.0, alm.Params(eps=1e-7, p_max=3))
+    assert r1.converged and r3.converged and max(rec.grew for rec in r3.log) >= 2
+    assert abs(o.inner_C(r1.R, r1.R) - o.inner_C(r3.R, r3.R)) <= 1e-5 * abs(o.inner_C(r1.R, r1.R))
