@@ -514,7 +514,7 @@ namespace {
 // Alg. 1 line 7 for p <= 4 directions, reading 29: minimise over S psd (p x p)
 //   g(S) = sum_a theta_a S_aa + (sigma/2) s^T Hw s,   s = (S_ab)_{a<=b} row-major, Hw = H .* (w w^T), w_ab = 1 or 2,
 // H[(ab),(cd)] = <c_ab, c_cd>, by projected gradient with step 1/L from S0 = diag(-theta_a / (sigma H[(aa),(aa)])).
-// S row-major p x p out; returns g(S).  Same iteration as oracle/alm.py::growth_sdp.
+// S row-major p x p out; returns g(S).
 double growth_sdp_host(int p, const double* theta, const std::vector<double>& H, double sigma, std::vector<double>& S, int iters = 500) {
   const int np = p * (p + 1) / 2;
   std::vector<int> pa(np), pb(np);
