@@ -212,6 +212,9 @@ def run_solve(args, w, local, torch, binding):
         else dict(eps=1e-5, stop_mode=0)
     if w.dtype == inputs.F32 and args.config == 5:
         kw["stall_tol"] = 1e-9   # fp32 rounding floor of f (reading 28)
+    for kv in args.param:
+        k, v = kv.split("=")
+        kw[k] = float(v) if ("." in v or "e" in v) else int(v)
     l0 = ctx.info()["launches"]
     torch.cuda.synchronize()
     res, log, r, sg, ok = ctx.solve(binding.Params(**kw), Rbuf, r0, r_cap, y, w.sigma)
@@ -238,6 +241,7 @@ def main():
     ap.add_argument("--mode", default="path", choices=["path", "solve"],
                     help="path: the hot-path step (default, the bench contract); solve: ALM solve time of the config")
     ap.add_argument("--r-cap", type=int, default=0)
+    ap.add_argument("--param", action="append", default=[], help="solve mode: alora_params override, e.g. --param lbfgs_mem=3")
     ap.add_argument("--mc", default="", help="config 5 only: 'n,r_star' of another row of the paper's Table 2")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
