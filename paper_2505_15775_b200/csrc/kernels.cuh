@@ -599,6 +599,40 @@ __global__ void __launch_bounds__(kBlock) k_cons(const ConsArgs<T> a) {
   finish_partials(a.fin);
 }
 
+// Forward evaluator for problems whose constraints all have exactly ONE stored entry (matrix completion, the edge
+// constraints of theta): one THREAD per constraint, so a warp instruction serves 32 constraints instead of 32 / GS.
+// The constraint streams (entry, y, b in; z, lambda out) are coalesced; the two rows are gathered pack by pack
+// (R is small and L2-resident in these workloads).  Same sums as k_cons.
+template <typename T, int VEC, int MODE>
+__global__ void __launch_bounds__(kBlock) k_cons1(const ConsArgs<T> a) {
+  constexpr int NST = (MODE == CONS_LS) ? 12 : 6;
+  double st[NST];
+#pragma unroll
+  for (int s = 0; s < NST; ++s) st[s] = 0.0;
+  const int nvec = a.nvec, r = a.r;
+  for (int64_t i = (int64_t)blockIdx.x * kBlock + threadIdx.x; i < a.m; i += (int64_t)gridDim.x * kBlock) {
+    const int j = __ldg(a.e_row + i), k = __ldg(a.e_col + i);
+    T av = __ldg(a.e_val + i);
+    if (j != k) av += av;
+    const T* xj = a.X + (int64_t)j * a.ld; const T* xk = a.X + (int64_t)k * a.ld;
+    T s0 = T(0), s1 = T(0), s2 = T(0);
+    for (int v = 0; v < nvec; ++v) {
+      Pack<T, VEC> pj = ldg_pack<T, VEC>(xj + v * VEC), pk = ldg_pack<T, VEC>(xk + v * VEC);
+      Pack<T, VEC> dj, dk;
+      if (MODE == CONS_LS) { dj = ldg_pack<T, VEC>(a.X2 + (int64_t)j * a.ld + v * VEC); dk = ldg_pack<T, VEC>(a.X2 + (int64_t)k * a.ld + v * VEC); }
+#pragma unroll
+      for (int e = 0; e < VEC; ++e) {
+        if (VEC > 1 && v * VEC + e >= r) break;   // partial last pack
+        s0 = fma(pj.v[e], pk.v[e], s0);
+        if (MODE == CONS_LS) { s1 = fma(pj.v[e], dk.v[e], fma(dj.v[e], pk.v[e], s1)); s2 = fma(dj.v[e], dk.v[e], s2); }
+      }
+    }
+    cons_finish<MODE>(st, i, (double)(av * s0), (double)(av * s1), (double)(av * s2), a.y, a.b, a.sigma, a.z, a.lam);
+  }
+  block_reduce_store<NST>(st, a.partials + (int64_t)blockIdx.x * kNStat);
+  finish_partials(a.fin);
+}
+
 // one group per chunk of <= kChunk entries.  Chunks of a long constraint leave their three sums in ch_out
 // (k_long_finish adds them in order and finishes the constraint); chunks of C's sym-upper list (line search only)
 // go straight into the block's partial row: <C,RR^T>, <C,RD^T> (the entry sum is <C,RD^T+DR^T>, halved) and <C,DD^T>.
