@@ -209,12 +209,14 @@ template <typename T> alora_status launch_adj_general(alora_ctx* c, const Geo& g
     c->launches++;
   }
   if ((c->ep && g.nvec == 1) || c->ep_wide) {
-    int& occ = c->occ_cache[vec_slot(g.vec)][g.shape][11];
-    if (!occ) occ = std::max(1, occ_rows_ep(T(), g.vec, g.shape));
+    // very long rows of thin vectors (matrix completion, r <= 8 packs): every lane owns whole rows, 32 entry lanes
+    const int eshape = (c->ep_wide && g.nvec > 1 && g.nvec <= 4) ? 7 : (c->ep_wide && g.nvec > 4 && g.nvec <= 8) ? 8 : g.shape;
+    int& occ = c->occ_cache[vec_slot(g.vec)][eshape == g.shape ? g.shape : eshape - 7][eshape == g.shape ? 11 : 7];
+    if (!occ) occ = std::max(1, occ_rows_ep(T(), g.vec, eshape));
     const int64_t need = (c->n + kBlock / 32 - 1) / (kBlock / 32);
     const int grid = (int)std::max<int64_t>(1, std::min<int64_t>(need, std::min<int64_t>((int64_t)c->num_sms * occ, c->part_cap)));
     a.fin = make_fin(c, a.fin.p[0], grid, a.fin.p[1], a.fin.n[1], a.fin.p[2], a.fin.n[2], out);
-    ALORA_CUDA(c, launch_rows_ep(g.vec, g.shape, a, grid, c->stream));
+    ALORA_CUDA(c, launch_rows_ep(g.vec, eshape, a, grid, c->stream));
   } else {
     const int grid = grid_rows<T>(c, g.vec, g.shape, ROWS_ADJ, c->n);
     a.fin = make_fin(c, a.fin.p[0], grid, a.fin.p[1], a.fin.n[1], a.fin.p[2], a.fin.n[2], out);
