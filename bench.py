@@ -34,6 +34,8 @@ UNIT = "evals/s"
 
 
 def workload(idx: int, mc: str = ""):
+    if idx in (1, 6) and mc:   # other grid sizes: --mc side
+        return (inputs.config1 if idx == 1 else inputs.config6)(side=int(mc))
     if idx == 5 and mc:   # other rows of the paper's Table 2: --mc n,r_star
         n, rs = (int(x) for x in mc.split(","))
         return inputs.config5(n=n, r_star=rs)
@@ -242,7 +244,7 @@ def main():
                     help="path: the hot-path step (default, the bench contract); solve: ALM solve time of the config")
     ap.add_argument("--r-cap", type=int, default=0)
     ap.add_argument("--param", action="append", default=[], help="solve mode: alora_params override, e.g. --param lbfgs_mem=3")
-    ap.add_argument("--mc", default="", help="config 5 only: 'n,r_star' of another row of the paper's Table 2")
+    ap.add_argument("--mc", default="", help="config 5: 'n,r_star' of another row of the paper's Table 2; configs 1 and 6: grid side")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
