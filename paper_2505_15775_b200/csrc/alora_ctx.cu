@@ -166,7 +166,7 @@ FinArgs no_fin() { FinArgs f; f.p[0] = f.p[1] = f.p[2] = nullptr; f.n[0] = f.n[1
 template <typename T>
 alora_status launch_diag_rows(alora_ctx* c, int vec, int nvec, int exact, int shape, int mode, RowArgs<T>& a,
                               const void* dual, double* out) {
-  const int gs = kTShapes[shape].gs, nit = kTShapes[shape].nit, tr = tile_rows(gs);
+  const int gs = tiled_shape(mode, shape, c->ell_wide).gs, nit = tiled_shape(mode, shape, c->ell_wide).nit, tr = tile_rows(gs);
   // 1: whole packs, some lanes of a group idle (lane mask); 2: whole packs, all lanes busy.  Rows whose last
   // pack is partially filled (r not a multiple of the vector width) take k_rows.
   const int full = nvec == gs * nit ? 2 : 1;

@@ -671,6 +671,8 @@ __host__ inline int shape_index(int nvec) {
 constexpr Shape kShapes[7] = {{1, 1}, {2, 1}, {4, 1}, {8, 1}, {8, 2}, {16, 2}, {16, 4}};   // k_rows, k_cons
 // tiled row kernel: few lanes per row -- the per-row bookkeeping (addresses, scalars, fp64 sums) is issued once
 // per group, so fewer lanes per row means fewer warp instructions per row; a lane holds up to 4 packs
-constexpr Shape kTShapes[7] = {{1, 1}, {2, 1}, {4, 1}, {4, 2}, {8, 2}, {8, 4}, {16, 4}};
+constexpr Shape kTShapes[7] = {{1, 1}, {2, 1}, {2, 2}, {4, 2}, {8, 2}, {8, 4}, {16, 4}};     // f + grad, adjoint
+constexpr Shape kTShapesLS[7] = {{1, 1}, {2, 1}, {4, 1}, {4, 2}, {8, 2}, {8, 4}, {16, 4}};   // line search (two operands per row), wide ELL
+__host__ inline Shape tiled_shape(int mode, int idx, bool wide) { return (mode == ROWS_LS_FUSED || wide) ? kTShapesLS[idx] : kTShapes[idx]; }
 
 }  // namespace alora
