@@ -62,14 +62,15 @@ def algorithmic_bytes(w, info):
     return fwd + wts + adj, adj
 
 
-def ncu_traffic(name: str):
+def ncu_traffic(name: str, n: int):
     """DRAM bytes per launch of the dominant kernel from the committed ncu --set full capture
     (profiles/traffic.json, written by hand from `ncu -i ... --page raw`), or None."""
     p = os.path.join(ROOT, "profiles", "traffic.json")
     if not os.path.exists(p):
         return None
     try:
-        return json.load(open(p)).get(name, {}).get("dram_bytes_per_launch")
+        e = json.load(open(p)).get(name, {})
+        return e.get("dram_bytes_per_launch") if e.get("n") == n else None
     except (ValueError, OSError):
         return None
 
@@ -365,7 +366,7 @@ def main():
                              "achieved": achieved, "peak": peak, "peak_source": peak_src, "unit": "GB/s",
                              "frac": (achieved / peak) if achieved else None, "algorithmic_bytes": B,
                              "algorithmic_bytes_whole_eval": B_eval,
-                             "kernel_ms": kavg_ms, "kernel_launches_timed": kern_n, "traffic": ncu_traffic(w.name)},
+                             "kernel_ms": kavg_ms, "kernel_launches_timed": kern_n, "traffic": ncu_traffic(w.name, P.n)},
                 "gpu_launches": int(launches), "clocks": clocks, "e2e": e2e,
                 "check": {"f": st[0], "gnorm": float(np.sqrt(st[4])), "p": [float(x) for x in pls]}}
         if not args.no_cpu_baseline and world == 1:
