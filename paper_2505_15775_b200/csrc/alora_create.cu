@@ -165,14 +165,12 @@ template <typename T> alora_status build(alora_ctx* c, const alora_problem* P) {
     }
     if (ident && ones) {
       // padded ELL blocks for the tiled row kernel: slot u of row j at [j * NU + u]; unused slot = (j, 0)
-      const int64_t nb = (n + 31) / 32;
       int64_t over4 = 0;
       for (int64_t j = 0; j < n; ++j) over4 += (c_rowptr[j + 1] - c_rowptr[j] > 4);
       c->ell_wide = over4 * 10 > n;
       const int kUN = ell_slots(c->ell_wide), kUNL = ell_slots_ls(c->ell_wide);
       std::vector<int> ec((size_t)n * kUN), euc((size_t)n * kUNL);
       std::vector<T> ev((size_t)n * kUN), euv((size_t)n * kUNL);
-      std::vector<unsigned char> rem(nb + 8, 0), remu(nb + 8, 0);
       for (int64_t j = 0; j < n; ++j) {
         const int e0 = c_rowptr[j], e1 = c_rowptr[j + 1];
         for (int u = 0; u < kUN; ++u) {
@@ -180,21 +178,19 @@ template <typename T> alora_status build(alora_ctx* c, const alora_problem* P) {
           ec[j * kUN + u] = e < e1 ? cents[e].col : (int)j;
           ev[j * kUN + u] = e < e1 ? (T)cents[e].val : T(0);
         }
-        if (e1 - e0 > kUN) rem[j >> 5] = 1;
+        if (e1 - e0 > kUN) ec[j * kUN] |= (int)0x80000000;   // more neighbours than slots: walk the CSR tail
         for (int u = 0; u < kUNL; ++u) {   // columns ascend: the upper triangle is the tail of the row's list
           const int e = e1 - kUNL + u;
           const bool up = e >= e0 && cents[e].col > j;
           euc[j * kUNL + u] = up ? cents[e].col : (int)j;
           euv[j * kUNL + u] = up ? (T)cents[e].val : T(0);
         }
-        if (e1 - kUNL - 1 >= e0 && cents[e1 - kUNL - 1].col > j) remu[j >> 5] = 1;
+        if (e1 - kUNL - 1 >= e0 && cents[e1 - kUNL - 1].col > j) euc[j * kUNL] |= (int)0x80000000;
       }
       ALORA_CUDA(c, upload(c, (void**)&c->ell_col, ec));
       ALORA_CUDA(c, upload(c, &c->ell_val, ev));
-      ALORA_CUDA(c, upload(c, (void**)&c->rem32, rem));
       ALORA_CUDA(c, upload(c, (void**)&c->ellu_col, euc));
       ALORA_CUDA(c, upload(c, &c->ellu_val, euv));
-      ALORA_CUDA(c, upload(c, (void**)&c->remu32, remu));
     }
   } else {
     // row-oriented full pattern with constraint ids

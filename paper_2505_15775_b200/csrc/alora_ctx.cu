@@ -252,7 +252,7 @@ template <typename T> void fill_rows(alora_ctx* c, RowArgs<T>& a, const Geo& g, 
   a.y = c->y; a.b = c->b; a.sigma = c->sigma; a.w = nullptr; a.z = nullptr;
   a.pC = 0; a.U = (const T*)c->U; a.Ts = c->Ts; a.scale = 1.0; a.diag_class = (c->cls == 0);
   a.partials = c->part_rows; a.row_begin = 0; a.tiles = 0;
-  a.ell_col = c->ell_col; a.ell_val = (const T*)c->ell_val; a.rem32 = c->rem32;
+  a.ell_col = c->ell_col; a.ell_val = (const T*)c->ell_val;
   a.nseg = 0; a.nheavy = c->nheavy; a.seg_row = c->seg_row; a.seg_beg = c->seg_beg; a.seg_end = c->seg_end;
   a.heavy_rows = c->heavy_rows; a.heavy_segptr = c->heavy_segptr; a.seg_out = (T*)c->seg_out; a.seg_cx = c->seg_cx;
   a.fin = no_fin();
@@ -354,7 +354,7 @@ template <typename T> alora_status ls_impl(alora_ctx* c, const T* R, const T* D,
     RowArgs<T> a;
     fill_rows(c, a, g, R, r, ld);
     a.X2 = D;
-    a.ell_col = c->ellu_col; a.ell_val = (const T*)c->ellu_val; a.rem32 = c->remu32;
+    a.ell_col = c->ellu_col; a.ell_val = (const T*)c->ellu_val;
     s = launch_diag_rows<T>(c, g.vec, g.nvec, g.exact, g.shape, ROWS_LS_FUSED, a, c->y, c->ls_dev);
     if (s != ALORA_OK) return s;
   } else {

@@ -54,8 +54,8 @@ struct alora_ctx {
   // identity diagonal class: padded ELL blocks (rows_tiled.cuh): kUN first neighbours per row, kUNL last
   // upper-triangle neighbours per row, and per 32-row block a flag "some row has more"
   bool ell_wide = false;   // 8 / 6 slots per row instead of 4 / 3 (more than 10 % of the rows have degree > 4)
-  int* ell_col = nullptr; void* ell_val = nullptr; unsigned char* rem32 = nullptr;
-  int* ellu_col = nullptr; void* ellu_val = nullptr; unsigned char* remu32 = nullptr;
+  int* ell_col = nullptr; void* ell_val = nullptr;
+  int* ellu_col = nullptr; void* ellu_val = nullptr;
   // general class: row-oriented full pattern of the constraints
   int* a_rowptr = nullptr; int* a_col = nullptr; void* a_val = nullptr; int* a_cons = nullptr;
   int64_t a_nnz = 0;

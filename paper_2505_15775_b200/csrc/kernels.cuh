@@ -69,9 +69,9 @@ template <typename T> struct RowArgs {
   int64_t row_begin; // k_rows: first row handled (rows [row_begin, n))
   int64_t tiles;     // k_rows_tiled: number of full row tiles handled (rows [0, tiles * TR))
   // k_rows_tiled: padded ELL block of the mode (kUN first neighbours, or kUNL last upper-triangle neighbours
-  // for the line search): slot u of row j at [j * NU + u]; rem32[j / 32] != 0: some row of that 32-row block
-  // has more neighbours than slots (walk the CSR tail)
-  const int* ell_col; const T* ell_val; const unsigned char* rem32;
+  // for the line search): slot u of row j at [j * NU + u]; sign bit of the first slot's column: the row has more
+  // neighbours than slots (walk the CSR tail)
+  const int* ell_col; const T* ell_val;
   // k_rows_ep: C rows with more than kHeavyRow entries are cut into segments of <= kHeavyRow entries that
   // k_rows_seg sums first (seg_out[s][nvec * VEC], seg_cx[s]); heavy_rows (ascending) / heavy_segptr list them per row
   int nseg, nheavy; const int* seg_row; const int* seg_beg; const int* seg_end;

@@ -10,7 +10,8 @@
 //     kept in a padded ELL block built once in alora_create: fixed-size (col, val) slots per row, an unused
 //     slot holding (the row itself, 0).  The slots of a row tile are one contiguous slice, so they arrive by
 //     bulk copy with no alignment fix-up, and the consumer needs no rowptr, no bounds and no validity test.
-//     Rows with more neighbours than slots are flagged per 32-row block; only flagged tiles walk the CSR tail.
+//     A row with more neighbours than slots carries a flag in the sign bit of its first slot's column; only such
+//     rows walk the CSR tail.
 //   * every *streaming* input of a row tile -- its rows of X (and D), dC, y, b (or the weights w) and the ELL
 //     slots -- is brought into shared memory by 1-D bulk async copies (cp.async.bulk, SASS UBLKCP) issued by a
 //     dedicated producer warp into a ring of kStages stages, completion signalled on mbarriers (full / empty),
@@ -217,7 +218,6 @@ __global__ void __launch_bounds__(kTiledThreads, tiled_min_blocks(VEC * NIT * (i
   constexpr int ESZ = (int)sizeof(T);
   extern __shared__ __align__(16) unsigned char smem_raw[];
   __shared__ uint64_t full[kStages], empty[kStages];
-  __shared__ int s_rem[kStages];
   const int warp = threadIdx.x >> 5, lane32 = threadIdx.x & 31;
   const int nvec = a.nvec, r = a.r, exact = a.exact;
   const int64_t ld = CLD ? (int64_t)(GS * NIT * VEC) : a.ld;
@@ -242,39 +242,27 @@ __global__ void __launch_bounds__(kTiledThreads, tiled_min_blocks(VEC * NIT * (i
   for (int s = 0; s < NSL; ++s) st[s] = 0.0;
 
   if (warp == NCW) {
-    // ================= producer warp: lane j pre-loads the remainder flags of the j-th upcoming tile ==========
-    const int64_t my_tiles = ntiles > blockIdx.x ? (ntiles - blockIdx.x + gridDim.x - 1) / gridDim.x : 0;
+    // ================= producer warp: streams the tiles of this block into the ring ===========================
+    // (the whole warp walks the loop, lane 0 issues: a diverged producer warp was measured 5 - 10 % slower)
     const uint32_t bytes = xbytes * (LS ? 2u : 1u) + TR * (uint32_t)ESZ + TR * 8u * (MODE == ROWS_ADJ ? 1u : 2u) +
                            TR * NU * (4u + (uint32_t)ESZ);
-    for (int64_t base = 0; base < my_tiles; base += 32) {
-      const int64_t tj = (int64_t)blockIdx.x + (base + lane32) * gridDim.x;
-      int rem = 0;
-      if (tj < ntiles) {
-        const int64_t b0 = (tj * TR) >> 5;
-#pragma unroll
-        for (int k = 0; k < (TR >= 32 ? TR / 32 : 1); ++k) rem |= a.rem32[b0 + k];
+    uint32_t s = 0, ph = 0;
+    for (int64_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+      if (lane32 == 0) {
+        const int64_t t0 = tile * TR;
+        mbar_wait(&empty[s], ph ^ 1u);
+        unsigned char* sb = smem_raw + (size_t)s * stage_sz;
+        mbar_expect_tx(&full[s], bytes);
+        bulk_g2s(sb, a.X + t0 * ld, xbytes, &full[s]);
+        if (LS) bulk_g2s(sb + xbytes, a.X2 + t0 * ld, xbytes, &full[s]);
+        bulk_g2s(sb + off_dc, a.dC + t0, TR * (uint32_t)ESZ, &full[s]);
+        bulk_g2s(sb + off_y, (MODE == ROWS_ADJ ? a.w : a.y) + t0, TR * 8u, &full[s]);
+        if (MODE != ROWS_ADJ) bulk_g2s(sb + off_b, a.b + t0, TR * 8u, &full[s]);
+        bulk_g2s(sb + off_ec, a.ell_col + t0 * NU, TR * NU * 4u, &full[s]);
+        bulk_g2s(sb + off_ev, a.ell_val + t0 * NU, TR * NU * (uint32_t)ESZ, &full[s]);
       }
-      const int cnt = (int)min((int64_t)32, my_tiles - base);
-      for (int j = 0; j < cnt; ++j) {
-        const int remj = __shfl_sync(0xffffffffu, rem, j);
-        if (lane32 == 0) {
-          const int64_t it = base + j;
-          const int s = (int)(it % kStages);
-          const uint32_t ph = (uint32_t)((it / kStages) & 1);
-          const int64_t t0 = ((int64_t)blockIdx.x + it * gridDim.x) * TR;
-          mbar_wait(&empty[s], ph ^ 1u);
-          unsigned char* sb = smem_raw + (size_t)s * stage_sz;
-          s_rem[s] = remj;
-          mbar_expect_tx(&full[s], bytes);
-          bulk_g2s(sb, a.X + t0 * ld, xbytes, &full[s]);
-          if (LS) bulk_g2s(sb + xbytes, a.X2 + t0 * ld, xbytes, &full[s]);
-          bulk_g2s(sb + off_dc, a.dC + t0, TR * (uint32_t)ESZ, &full[s]);
-          bulk_g2s(sb + off_y, (MODE == ROWS_ADJ ? a.w : a.y) + t0, TR * 8u, &full[s]);
-          if (MODE != ROWS_ADJ) bulk_g2s(sb + off_b, a.b + t0, TR * 8u, &full[s]);
-          bulk_g2s(sb + off_ec, a.ell_col + t0 * NU, TR * NU * 4u, &full[s]);
-          bulk_g2s(sb + off_ev, a.ell_val + t0 * NU, TR * NU * (uint32_t)ESZ, &full[s]);
-        }
-      }
+      __syncwarp();
+      if (++s == kStages) { s = 0; ph ^= 1u; }
     }
   } else {
     // ================= consumer warps ======================================================================
@@ -298,8 +286,7 @@ __global__ void __launch_bounds__(kTiledThreads, tiled_min_blocks(VEC * NIT * (i
     const T sc = (T)a.scale;
     // one row: `staged` = its streaming inputs sit in stage `sb` (tile rows [row0, row0 + TR)), else they are read
     // from global memory (ragged tail of the matrix); live == false: padding lane of the tail, nothing is kept
-    auto do_row = [&](const bool staged, const unsigned char* sb, const uint32_t row0, const uint32_t row, const bool rem,
-                      const bool live) {
+    auto do_row = [&](const bool staged, const unsigned char* sb, const uint32_t row0, const uint32_t row, const bool live) {
       Row x, d;
       T dc; double yv, bv = 0.0;
       int ck[NU]; T cw[NU];
@@ -323,7 +310,10 @@ __global__ void __launch_bounds__(kTiledThreads, tiled_min_blocks(VEC * NIT * (i
 #pragma unroll
         for (int u = 0; u < NU; ++u) { ck[u] = __ldg(a.ell_col + (int64_t)row * NU + u); cw[u] = __ldg(a.ell_val + (int64_t)row * NU + u); }
       }
-      // ELL slots: an unused slot is (the row itself, 0); an in-tile neighbour is read from the stage
+      // ELL slots: an unused slot is (the row itself, 0); an in-tile neighbour is read from the stage.  The sign bit
+      // of the first slot's column says that the row has more neighbours than slots (walk the CSR tail).
+      const bool rem = ck[0] < 0;
+      ck[0] &= 0x7fffffff;
       if (LS) {
         Row xk[NU], dk[NU];
 #pragma unroll
@@ -429,7 +419,7 @@ __global__ void __launch_bounds__(kTiledThreads, tiled_min_blocks(VEC * NIT * (i
     for (int64_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
       const uint32_t row0 = (uint32_t)(tile * TR);
       mbar_wait_addr(full0 + s * 8u, ph);
-      do_row(true, sb, row0, row0 + (uint32_t)lr, s_rem[s] != 0, true);
+      do_row(true, sb, row0, row0 + (uint32_t)lr, true);
       __syncwarp();
       if (lane32 == 0) mbar_arrive_addr(empty0 + s * 8u);   // this warp is done with stage s
       ++s; sb += stage_sz;
@@ -442,7 +432,7 @@ __global__ void __launch_bounds__(kTiledThreads, tiled_min_blocks(VEC * NIT * (i
         const uint32_t row = base + (uint32_t)lr;
         const bool live = row < n32;
         const uint32_t rowc = live ? row : n32 - 1;
-        do_row(false, nullptr, 0u, rowc, __ldg(a.rem32 + (rowc >> 5)) != 0, live);
+        do_row(false, nullptr, 0u, rowc, live);
       }
     }
   }
