@@ -170,13 +170,13 @@ __device__ __forceinline__ void finish_partials(const FinArgs& f) {
     for (int k = 0; k < 3; ++k) {
       const double* p = f.p[k];
       const int n = f.n[k];
-      int i = slot;
-      for (; i + 3 * NSLOT < n; i += 4 * NSLOT) {   // four independent loads in flight
-        const double v0 = __ldcg(p + (int64_t)i * kNStat + s), v1 = __ldcg(p + (int64_t)(i + NSLOT) * kNStat + s);
-        const double v2 = __ldcg(p + (int64_t)(i + 2 * NSLOT) * kNStat + s), v3 = __ldcg(p + (int64_t)(i + 3 * NSLOT) * kNStat + s);
-        v += v0; v += v1; v += v2; v += v3;
+      for (int i = slot; i < n; i += 8 * NSLOT) {   // eight independent (predicated) loads in flight per round trip
+        double t[8];
+#pragma unroll
+        for (int u = 0; u < 8; ++u) t[u] = (i + u * NSLOT < n) ? __ldcg(p + (int64_t)(i + u * NSLOT) * kNStat + s) : 0.0;
+#pragma unroll
+        for (int u = 0; u < 8; ++u) v += t[u];
       }
-      for (; i < n; i += NSLOT) v += __ldcg(p + (int64_t)i * kNStat + s);
     }
     s_fin[threadIdx.x] = v;
   }
