@@ -315,13 +315,32 @@ __global__ void __launch_bounds__(kTiledThreads, tiled_min_blocks(VEC * NIT * (i
       const bool rem = ck[0] < 0;
       ck[0] &= 0x7fffffff;
       if (LS) {
-        Row xk[NU], dk[NU];
+        // u = sum_k c_k R_k, w = sum_k c_k D_k over the upper neighbours.  Narrow rows (<= 4 registers per operand):
+        // all gathers first, then the FMAs.  Wider rows: one neighbour at a time (most upper neighbours of a grid /
+        // ring are in-tile reads from the stage, and six row vectors in flight would spill).
+        constexpr bool SEQ = VEC * NIT * (int)sizeof(T) / 4 > 4;
+        Row uacc, wacc; uacc.zero(); wacc.zero();
+        if (SEQ) {
+#pragma unroll 1
+          for (int u = 0; u < NU; ++u) {
+            const uint32_t rel = (uint32_t)ck[u] - row0;
+            const bool loc = staged && rel < (uint32_t)TR;
+            Row xk1, dk1;
+            row_nbr(xk1, loc, sb + rel * ldb + loff, Xl + (uint64_t)(uint32_t)ck[u] * ldb, pmask);
+            row_nbr(dk1, loc, sb + xbytes + rel * ldb + loff, X2l + (uint64_t)(uint32_t)ck[u] * ldb, pmask);
+            uacc.axpy(cw[u], xk1); wacc.axpy(cw[u], dk1);
+          }
+        } else {
+          Row xk[NU], dk[NU];
 #pragma unroll
-        for (int u = 0; u < NU; ++u) {
-          const uint32_t rel = (uint32_t)ck[u] - row0;
-          const bool loc = staged && rel < (uint32_t)TR;
-          row_nbr(xk[u], loc, sb + rel * ldb + loff, Xl + (uint64_t)(uint32_t)ck[u] * ldb, pmask);
-          row_nbr(dk[u], loc, sb + xbytes + rel * ldb + loff, X2l + (uint64_t)(uint32_t)ck[u] * ldb, pmask);
+          for (int u = 0; u < NU; ++u) {
+            const uint32_t rel = (uint32_t)ck[u] - row0;
+            const bool loc = staged && rel < (uint32_t)TR;
+            row_nbr(xk[u], loc, sb + rel * ldb + loff, Xl + (uint64_t)(uint32_t)ck[u] * ldb, pmask);
+            row_nbr(dk[u], loc, sb + xbytes + rel * ldb + loff, X2l + (uint64_t)(uint32_t)ck[u] * ldb, pmask);
+          }
+#pragma unroll
+          for (int u = 0; u < NU; ++u) { uacc.axpy(cw[u], xk[u]); wacc.axpy(cw[u], dk[u]); }
         }
         const T rr_l = x.dot(x), rd_l = x.dot(d), dd_l = d.dot(d);
         const double rr = (double)gsum<GS>(rr_l), rd = (double)gsum<GS>(rd_l), dd = (double)gsum<GS>(dd_l);
@@ -339,11 +358,7 @@ __global__ void __launch_bounds__(kTiledThreads, tiled_min_blocks(VEC * NIT * (i
           st[LS_QQ] += qv * qv; st[LS_QQ1] += qv * q1; st[LS_QQ2] += qv * q2;
           st[LS_Q11] += q1 * q1; st[LS_Q12] += q1 * q2; st[LS_Q22] += q2 * q2;
         }
-        // u = sum_k c_k R_k, w = sum_k c_k D_k over the upper neighbours; then <C,.> row sums are
-        // x.u, x.w + d.u, d.w  (8 FMAs per neighbour instead of 16)
-        Row uacc, wacc; uacc.zero(); wacc.zero();
-#pragma unroll
-        for (int u = 0; u < NU; ++u) { uacc.axpy(cw[u], xk[u]); wacc.axpy(cw[u], dk[u]); }
+        // the <C,.> row sums are x.u, x.w + d.u, d.w  (8 FMAs per neighbour instead of 16)
         if (rem) {   // rows with more than NU upper neighbours: the CSR tail below the slots (columns ascend)
           const int eb = __ldg(a.c_rowptr + row), ee = __ldg(a.c_rowptr + row + 1);
           for (int e = ee - NU - 1; e >= eb; --e) {
