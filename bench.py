@@ -213,6 +213,8 @@ def run_solve(args, w, local, torch, binding):
     # rule, KKT (eq. 77) <= 1e-5
     kw = dict(eps=1e-6, stop_mode=0) if args.config == 0 else dict(eps=1e-5, stop_mode=1) if args.config == 4 \
         else dict(eps=1e-5, stop_mode=0)
+    if args.config == 4:
+        kw["it_max"] = 100   # inexact inner solves; measured 17 s against 95 s with the default 500
     if w.dtype == inputs.F32 and args.config == 5:
         kw["stall_tol"] = 1e-9   # fp32 rounding floor of f (reading 28)
     for kv in args.param:

@@ -42,17 +42,30 @@ __global__ void k_reduce_rows(const double* part, int nrows, double* out) {  // 
   }
 }
 
+// Element-wise passes: 16-byte packs over the aligned bulk (when both arrays are 16-byte aligned), scalars for the tail.
+template <typename T, bool READ_Y, typename F> __device__ __forceinline__ void ew2(int64_t N, const T* x, T* y, F f) {   // y[i] = f(x[i], y[i])
+  constexpr int VEC = 16 / (int)sizeof(T);
+  const bool al = (((uintptr_t)x | (uintptr_t)y) & 15) == 0;
+  const int64_t nv = al ? N / VEC : 0;
+  const int64_t tid = (int64_t)blockIdx.x * blockDim.x + threadIdx.x, nth = (int64_t)gridDim.x * blockDim.x;
+  for (int64_t i = tid; i < nv; i += nth) {
+    const Pack<T, VEC> xv = reinterpret_cast<const Pack<T, VEC>*>(x)[i];
+    Pack<T, VEC> yv;
+    if (READ_Y) yv = reinterpret_cast<Pack<T, VEC>*>(y)[i];
+#pragma unroll
+    for (int k = 0; k < VEC; ++k) yv.v[k] = f(xv.v[k], READ_Y ? yv.v[k] : T(0));
+    reinterpret_cast<Pack<T, VEC>*>(y)[i] = yv;
+  }
+  for (int64_t i = nv * VEC + tid; i < N; i += nth) y[i] = f(x[i], READ_Y ? y[i] : T(0));
+}
 template <typename T> __global__ void k_axpy(int64_t N, double a, const T* x, T* y) {  // y += a x
-  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (int64_t)gridDim.x * blockDim.x)
-    y[i] = (T)((double)y[i] + a * (double)x[i]);
+  ew2<T, true>(N, x, y, [a](T xv, T yv) { return (T)((double)yv + a * (double)xv); });
 }
 template <typename T> __global__ void k_scale_copy(int64_t N, double a, const T* x, T* y) {  // y = a x
-  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (int64_t)gridDim.x * blockDim.x)
-    y[i] = (T)(a * (double)x[i]);
+  ew2<T, false>(N, x, y, [a](T xv, T) { return (T)(a * (double)xv); });
 }
 template <typename T> __global__ void k_scale(int64_t N, double a, T* y) {  // y *= a
-  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (int64_t)gridDim.x * blockDim.x)
-    y[i] = (T)(a * (double)y[i]);
+  ew2<T, false>(N, y, y, [a](T xv, T) { return (T)(a * (double)xv); });
 }
 // L-BFGS pair: S = alpha D, Y = G - Gprev, and the sums S.Y, S.S, Y.Y in the same pass
 template <typename T>
