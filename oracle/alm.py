@@ -12,7 +12,9 @@ Library primitives used as steps: numpy dot/matmul, ``numpy.roots`` (cubic), ``n
 parity unpinned (by the paper): the L-BFGS / sigma-schedule / shrink constants are free parameters
 (readings 5, 6, 12, 13); they are pinned only oracle-vs-GPU.  What *is* pinned against the paper
 and mathematics (tests/test_oracle_alm.py): closed-form MaxCut / theta optima, Prop. 6 escape,
-Lanczos against a dense eigen-solver, exact line search against a brute-force scan.
+Lanczos against a dense eigen-solver, exact line search against a brute-force scan, the matrix-completion
+optimum against the nuclear norm (SVD), the p_max > 1 growth step against its model identity (exact decrease
+of the augmented Lagrangian), the KKT conditions of the small SDP and the p = 1 closed form.
 """
 from __future__ import annotations
 
