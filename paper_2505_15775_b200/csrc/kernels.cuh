@@ -672,7 +672,7 @@ constexpr Shape kShapes[7] = {{1, 1}, {2, 1}, {4, 1}, {8, 1}, {8, 2}, {16, 2}, {
 // tiled row kernel: few lanes per row -- the per-row bookkeeping (addresses, scalars, fp64 sums) is issued once
 // per group, so fewer lanes per row means fewer warp instructions per row; a lane holds up to 4 packs
 constexpr Shape kTShapes[7] = {{1, 1}, {2, 1}, {2, 2}, {4, 2}, {8, 2}, {8, 4}, {16, 4}};     // f + grad, adjoint
-constexpr Shape kTShapesLS[7] = {{1, 1}, {2, 1}, {4, 1}, {4, 2}, {8, 2}, {8, 4}, {16, 4}};   // line search (two operands per row; measured: 2 lanes per row is slower there, 58.8 vs 52 us), wide ELL
+constexpr Shape kTShapesLS[7] = {{1, 1}, {2, 1}, {4, 1}, {4, 2}, {8, 2}, {8, 4}, {16, 4}};   // line search (two operands per row; measured: 2 lanes per row is slower there, 50.7 vs 48.4 us), wide ELL
 __host__ inline Shape tiled_shape(int mode, int idx, bool wide) { return (mode == ROWS_LS_FUSED || wide) ? kTShapesLS[idx] : kTShapes[idx]; }
 
 }  // namespace alora

@@ -316,19 +316,31 @@ __global__ void __launch_bounds__(kTiledThreads, tiled_min_blocks(VEC * NIT * (i
       ck[0] &= 0x7fffffff;
       if (LS) {
         // u = sum_k c_k R_k, w = sum_k c_k D_k over the upper neighbours.  Narrow rows (<= 4 registers per operand):
-        // all gathers first, then the FMAs.  Wider rows: one neighbour at a time (most upper neighbours of a grid /
-        // ring are in-tile reads from the stage, and six row vectors in flight would spill).
+        // all gathers first, then the FMAs.  Wider rows: the R operand of all slots, then the D operand (2 NU row
+        // vectors in flight would spill).
         constexpr bool SEQ = VEC * NIT * (int)sizeof(T) / 4 > 4;
         Row uacc, wacc; uacc.zero(); wacc.zero();
         if (SEQ) {
-#pragma unroll 1
-          for (int u = 0; u < NU; ++u) {
-            const uint32_t rel = (uint32_t)ck[u] - row0;
-            const bool loc = staged && rel < (uint32_t)TR;
-            Row xk1, dk1;
-            row_nbr(xk1, loc, sb + rel * ldb + loff, Xl + (uint64_t)(uint32_t)ck[u] * ldb, pmask);
-            row_nbr(dk1, loc, sb + xbytes + rel * ldb + loff, X2l + (uint64_t)(uint32_t)ck[u] * ldb, pmask);
-            uacc.axpy(cw[u], xk1); wacc.axpy(cw[u], dk1);
+          // two phases (R operand, then D operand): NU row vectors in flight instead of 2 NU
+          {
+            Row xk[NU];
+#pragma unroll
+            for (int u = 0; u < NU; ++u) {
+              const uint32_t rel = (uint32_t)ck[u] - row0;
+              row_nbr(xk[u], staged && rel < (uint32_t)TR, sb + rel * ldb + loff, Xl + (uint64_t)(uint32_t)ck[u] * ldb, pmask);
+            }
+#pragma unroll
+            for (int u = 0; u < NU; ++u) uacc.axpy(cw[u], xk[u]);
+          }
+          {
+            Row dk[NU];
+#pragma unroll
+            for (int u = 0; u < NU; ++u) {
+              const uint32_t rel = (uint32_t)ck[u] - row0;
+              row_nbr(dk[u], staged && rel < (uint32_t)TR, sb + xbytes + rel * ldb + loff, X2l + (uint64_t)(uint32_t)ck[u] * ldb, pmask);
+            }
+#pragma unroll
+            for (int u = 0; u < NU; ++u) wacc.axpy(cw[u], dk[u]);
           }
         } else {
           Row xk[NU], dk[NU];
