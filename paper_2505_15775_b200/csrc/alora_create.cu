@@ -246,6 +246,7 @@ template <typename T> alora_status build(alora_ctx* c, const alora_problem* P) {
     c->nchunk_A = (int64_t)ch_beg.size(); c->nlong_A = (int)long_cons.size();
     c->single_entry = m > 0;
     for (int64_t i = 0; i < m && c->single_entry; ++i) c->single_entry = (f_ptr[i + 1] - f_ptr[i] == 1);
+    c->short_cons = m > 0 && c->nf_A <= 8 * m;
     // forward list continues with C's sym-upper entries (diagonal, then upper triangle of the CSR)
     for (int64_t j = 0; j < n; ++j)
       if (dC[j] != 0.0) { f_row.push_back((int)j); f_col.push_back((int)j); f_val.push_back(dC[j]); }

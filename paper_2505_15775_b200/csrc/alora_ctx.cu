@@ -299,9 +299,9 @@ template <typename T> alora_status eval_impl(alora_ctx* c, const T* R, int32_t r
     ca.z = zout;
     int gc = 0;
     if (c->m > 0) {
-      if (c->single_entry) {
+      if (c->single_entry || c->short_cons) {
         gc = (int)std::min<int64_t>((c->m + kBlock - 1) / kBlock, std::min<int64_t>((int64_t)c->num_sms * 8, c->part_cap));
-        ALORA_CUDA(c, launch_cons1(g.vec, CONS_EVAL, ca, gc, c->stream));
+        ALORA_CUDA(c, launch_cons1(g.vec, CONS_EVAL, c->single_entry ? 1 : 0, ca, gc, c->stream));
       } else {
         gc = grid_cons<T>(c, g.vec, g.shape, CONS_EVAL, 0, c->m);
         ALORA_CUDA(c, launch_cons(g.vec, g.shape, CONS_EVAL, 0, ca, gc, c->stream));
@@ -370,10 +370,10 @@ template <typename T> alora_status ls_impl(alora_ctx* c, const T* R, const T* D,
     int gc = 0, gk = 0;
     if (chunks) gk = grid_cons<T>(c, g.vec, g.shape, CONS_LS, 1, c->nchunk_all);
     if (c->m > 0) {
-      gc = c->single_entry ? (int)std::min<int64_t>((c->m + kBlock - 1) / kBlock, std::min<int64_t>((int64_t)c->num_sms * 8, c->part_cap))
+      gc = (c->single_entry || c->short_cons) ? (int)std::min<int64_t>((c->m + kBlock - 1) / kBlock, std::min<int64_t>((int64_t)c->num_sms * 8, c->part_cap))
                            : grid_cons<T>(c, g.vec, g.shape, CONS_LS, 0, c->m);
       if (!chunks) ca.fin = make_fin(c, c->part_cons, gc, nullptr, 0, nullptr, 0, c->ls_dev);
-      if (c->single_entry) ALORA_CUDA(c, launch_cons1(g.vec, CONS_LS, ca, gc, c->stream));
+      if (c->single_entry || c->short_cons) ALORA_CUDA(c, launch_cons1(g.vec, CONS_LS, c->single_entry ? 1 : 0, ca, gc, c->stream));
       else ALORA_CUDA(c, launch_cons(g.vec, g.shape, CONS_LS, 0, ca, gc, c->stream));
       ca.fin = no_fin();
       c->launches++;

@@ -63,6 +63,7 @@ struct alora_ctx {
   int nseg = 0, nheavy = 0; int* seg_row = nullptr; int* seg_beg = nullptr; int* seg_end = nullptr;
   int* heavy_rows = nullptr; int* heavy_segptr = nullptr; void* seg_out = nullptr; double* seg_cx = nullptr;
   bool single_entry = false;   // every constraint has exactly one stored entry: thread-per-constraint forward (k_cons1)
+  bool short_cons = false;     // at most 8 stored entries per constraint on average: thread-per-constraint forward too
   bool ep = false;       // general class, >= 8 entries per row on average: warp-per-row adjoint for single vectors
   bool ep_wide = false;  // >= 96 entries per row on average (matrix completion): warp-per-row adjoint for every r
   // forward list: coalesced constraint entries [0, nf_A), then C's sym-upper entries [nf_A, nf_A+nf_C)

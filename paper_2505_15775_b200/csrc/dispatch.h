@@ -7,7 +7,7 @@ namespace alora {
 
 #define ALORA_DECL_INST(T, SUF)                                                                       \
   cudaError_t launch_rows_##SUF(int shape, int mode, const RowArgs<T>& a, int grid, cudaStream_t s);  \
-  cudaError_t launch_cons1_##SUF(int mode, const ConsArgs<T>& a, int grid, cudaStream_t s);           \
+  cudaError_t launch_cons1_##SUF(int mode, int single, const ConsArgs<T>& a, int grid, cudaStream_t s); \
   cudaError_t launch_cons_##SUF(int shape, int mode, int chunked, const ConsArgs<T>& a, int grid,     \
                                 cudaStream_t s);                                                      \
   cudaError_t launch_tiled_##SUF(int shape, int mode, int full, int wide, const RowArgs<T>& a, int grid, cudaStream_t s); \
@@ -51,11 +51,12 @@ inline int occ_rows_ep(float, int vec, int shape) {
   return vec == 4 ? occ_rows_ep_f32v4(shape) : vec == 2 ? occ_rows_ep_f32v2(shape) : occ_rows_ep_f32v1(shape);
 }
 inline int occ_rows_ep(double, int vec, int shape) { return vec == 2 ? occ_rows_ep_f64v2(shape) : occ_rows_ep_f64v1(shape); }
-inline cudaError_t launch_cons1(int vec, int mode, const ConsArgs<float>& a, int grid, cudaStream_t s) {
-  return vec == 4 ? launch_cons1_f32v4(mode, a, grid, s) : vec == 2 ? launch_cons1_f32v2(mode, a, grid, s) : launch_cons1_f32v1(mode, a, grid, s);
+inline cudaError_t launch_cons1(int vec, int mode, int single, const ConsArgs<float>& a, int grid, cudaStream_t s) {
+  return vec == 4 ? launch_cons1_f32v4(mode, single, a, grid, s)
+       : vec == 2 ? launch_cons1_f32v2(mode, single, a, grid, s) : launch_cons1_f32v1(mode, single, a, grid, s);
 }
-inline cudaError_t launch_cons1(int vec, int mode, const ConsArgs<double>& a, int grid, cudaStream_t s) {
-  return vec == 2 ? launch_cons1_f64v2(mode, a, grid, s) : launch_cons1_f64v1(mode, a, grid, s);
+inline cudaError_t launch_cons1(int vec, int mode, int single, const ConsArgs<double>& a, int grid, cudaStream_t s) {
+  return vec == 2 ? launch_cons1_f64v2(mode, single, a, grid, s) : launch_cons1_f64v1(mode, single, a, grid, s);
 }
 inline cudaError_t launch_cons(int vec, int shape, int mode, int chunked, const ConsArgs<float>& a, int grid, cudaStream_t s) {
   return vec == 4 ? launch_cons_f32v4(shape, mode, chunked, a, grid, s)

@@ -599,11 +599,13 @@ __global__ void __launch_bounds__(kBlock) k_cons(const ConsArgs<T> a) {
   finish_partials(a.fin);
 }
 
-// Forward evaluator for problems whose constraints all have exactly ONE stored entry (matrix completion, the edge
-// constraints of theta): one THREAD per constraint, so a warp instruction serves 32 constraints instead of 32 / GS.
-// The constraint streams (entry, y, b in; z, lambda out) are coalesced; the two rows are gathered pack by pack
-// (R is small and L2-resident in these workloads).  Same sums as k_cons.
-template <typename T, int VEC, int MODE>
+// Forward evaluator with one THREAD per constraint, for constraints with few stored entries (SINGLE: exactly one
+// each -- matrix completion, the edge constraints of theta; otherwise a short list via ptr -- random sparse
+// constraints): a warp instruction serves 32 constraints instead of 32 / GS.  The constraint streams (entries, y, b
+// in; z, lambda out) are coalesced; the rows are gathered pack by pack (R is small and L2-resident in these
+// workloads).  Constraints with more than kLongThreshold entries are skipped (chunk kernels), as in k_cons.  Same
+// sums as k_cons.
+template <typename T, int VEC, int MODE, bool SINGLE>
 __global__ void __launch_bounds__(kBlock) k_cons1(const ConsArgs<T> a) {
   constexpr int NST = (MODE == CONS_LS) ? 12 : 6;
   double st[NST];
@@ -611,23 +613,29 @@ __global__ void __launch_bounds__(kBlock) k_cons1(const ConsArgs<T> a) {
   for (int s = 0; s < NST; ++s) st[s] = 0.0;
   const int nvec = a.nvec, r = a.r;
   for (int64_t i = (int64_t)blockIdx.x * kBlock + threadIdx.x; i < a.m; i += (int64_t)gridDim.x * kBlock) {
-    const int j = __ldg(a.e_row + i), k = __ldg(a.e_col + i);
-    T av = __ldg(a.e_val + i);
-    if (j != k) av += av;
-    const T* xj = a.X + (int64_t)j * a.ld; const T* xk = a.X + (int64_t)k * a.ld;
-    T s0 = T(0), s1 = T(0), s2 = T(0);
-    for (int v = 0; v < nvec; ++v) {
-      Pack<T, VEC> pj = ldg_pack<T, VEC>(xj + v * VEC), pk = ldg_pack<T, VEC>(xk + v * VEC);
-      Pack<T, VEC> dj, dk;
-      if (MODE == CONS_LS) { dj = ldg_pack<T, VEC>(a.X2 + (int64_t)j * a.ld + v * VEC); dk = ldg_pack<T, VEC>(a.X2 + (int64_t)k * a.ld + v * VEC); }
+    const int64_t e0 = SINGLE ? i : __ldg(a.ptr + i), e1 = SINGLE ? i + 1 : __ldg(a.ptr + i + 1);
+    if (!SINGLE && e1 - e0 > kLongThreshold) continue;
+    T t0 = T(0), t1 = T(0), t2 = T(0);
+    for (int64_t e = e0; e < e1; ++e) {
+      const int j = __ldg(a.e_row + e), k = __ldg(a.e_col + e);
+      T av = __ldg(a.e_val + e);
+      if (j != k) av += av;
+      const T* xj = a.X + (int64_t)j * a.ld; const T* xk = a.X + (int64_t)k * a.ld;
+      T s0 = T(0), s1 = T(0), s2 = T(0);
+      for (int v = 0; v < nvec; ++v) {
+        Pack<T, VEC> pj = ldg_pack<T, VEC>(xj + v * VEC), pk = ldg_pack<T, VEC>(xk + v * VEC);
+        Pack<T, VEC> dj, dk;
+        if (MODE == CONS_LS) { dj = ldg_pack<T, VEC>(a.X2 + (int64_t)j * a.ld + v * VEC); dk = ldg_pack<T, VEC>(a.X2 + (int64_t)k * a.ld + v * VEC); }
 #pragma unroll
-      for (int e = 0; e < VEC; ++e) {
-        if (VEC > 1 && v * VEC + e >= r) break;   // partial last pack
-        s0 = fma(pj.v[e], pk.v[e], s0);
-        if (MODE == CONS_LS) { s1 = fma(pj.v[e], dk.v[e], fma(dj.v[e], pk.v[e], s1)); s2 = fma(dj.v[e], dk.v[e], s2); }
+        for (int q = 0; q < VEC; ++q) {
+          if (VEC > 1 && v * VEC + q >= r) break;   // partial last pack
+          s0 = fma(pj.v[q], pk.v[q], s0);
+          if (MODE == CONS_LS) { s1 = fma(pj.v[q], dk.v[q], fma(dj.v[q], pk.v[q], s1)); s2 = fma(dj.v[q], dk.v[q], s2); }
+        }
       }
+      t0 = fma(av, s0, t0); t1 = fma(av, s1, t1); t2 = fma(av, s2, t2);
     }
-    cons_finish<MODE>(st, i, (double)(av * s0), (double)(av * s1), (double)(av * s2), a.y, a.b, a.sigma, a.z, a.lam);
+    cons_finish<MODE>(st, i, (double)t0, (double)t1, (double)t2, a.y, a.b, a.sigma, a.z, a.lam);
   }
   block_reduce_store<NST>(st, a.partials + (int64_t)blockIdx.x * kNStat);
   finish_partials(a.fin);
