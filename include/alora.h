@@ -125,7 +125,8 @@ alora_status alora_smatvec(alora_ctx *ctx, const double *mu_dev, const void *V, 
 /* Measurement hook (bench.py): when enabled, alora_eval brackets its dominant kernel (the fused
  * row pass of the diagonal class, the adjoint pass of the general class) with CUDA events on the ctx
  * stream; alora_kernel_timing_read synchronises, returns the summed kernel time and the number of
- * launches timed since the last read (at most 8192 between reads), and resets. */
+ * launches timed since the last read (at most 8192 between reads), and resets.  enable = k > 1 brackets every
+ * k-th evaluation only (two event records cost about 5 us of stream time per evaluation). */
 alora_status alora_kernel_timing(alora_ctx *ctx, int enable);
 alora_status alora_kernel_timing_read(alora_ctx *ctx, double *total_ms, int64_t *count);
 

@@ -199,7 +199,8 @@ class Context:
         self._chk(_lib.alora_smatvec(self._h, _ptr(mu), _ptr(V), p, _ptr(W), _ptr(out)))
         return None if out is None else float(out[0])
 
-    def kernel_timing(self, enable: bool):
+    def kernel_timing(self, enable):
+        """False / True, or an int k > 1: bracket every k-th evaluation only."""
         self._chk(_lib.alora_kernel_timing(self._h, int(enable)))
 
     def kernel_timing_read(self):

@@ -136,6 +136,8 @@ struct Geo { int vec, nvec, shape, exact; };
 // records an event on the ctx stream when kernel timing is on (pairs: before / after the dominant kernel)
 void time_mark(alora_ctx* c) {
   if (!c->timing) return;
+  // every `timing_every`-th evaluation is bracketed (the two marks of one evaluation share the decision)
+  if (c->timing_every > 1 && ((c->timing_calls++ >> 1) % c->timing_every) != 0) return;
   if (c->ev_used == c->ev.size()) {
     if (c->ev.size() >= 16384) return;
     cudaEvent_t e;
@@ -534,7 +536,7 @@ extern "C" alora_status alora_smatvec(alora_ctx* c, const double* mu_dev, const 
 
 extern "C" alora_status alora_kernel_timing(alora_ctx* c, int enable) {
   if (!c) return ALORA_EINVAL;
-  c->timing = enable != 0; c->ev_used = 0;
+  c->timing = enable != 0; c->timing_every = enable > 1 ? enable : 1; c->timing_calls = 0; c->ev_used = 0;
   return ALORA_OK;
 }
 

@@ -98,7 +98,7 @@ struct alora_ctx {
   int64_t occ_ld[3][7][4];   // ld for which the tiled-kernel occupancy was computed
   alora::SolveWorkspace* ws = nullptr;
   // optional CUDA-event timing of the dominant kernel of alora_eval (bench.py roofline)
-  bool timing = false; std::vector<cudaEvent_t> ev; size_t ev_used = 0;
+  bool timing = false; int timing_every = 1; int64_t timing_calls = 0; std::vector<cudaEvent_t> ev; size_t ev_used = 0;
 };
 
 namespace alora {
