@@ -122,6 +122,11 @@ alora_status alora_get_linesearch(alora_ctx *ctx, double p[5]);
 alora_status alora_smatvec(alora_ctx *ctx, const double *mu_dev, const void *V, int32_t p, void *W,
                            double *vw);
 
+/* CUDA graphs: alora_eval (stats == NULL), alora_linesearch (p == NULL) and alora_smatvec (vw == NULL) only enqueue
+ * kernels on the ctx stream -- no synchronisation, no allocation after the first call with the same shapes -- so a
+ * sequence of them can be captured into a CUDA graph on that stream and replayed; alora_get_stats /
+ * alora_get_linesearch read the results of the last replay. */
+
 /* Measurement hook (bench.py): when enabled, alora_eval brackets its dominant kernel (the fused
  * row pass of the diagonal class, the adjoint pass of the general class) with CUDA events on the ctx
  * stream; alora_kernel_timing_read synchronises, returns the summed kernel time and the number of

@@ -182,3 +182,37 @@ def test_m0_no_constraints(torch, binding, oracle_mod):
     w = inputs.Workload(name="m0", problem=P, dtype=inputs.F64, r=3, R=rng.standard_normal((6, 3)), y=np.zeros(0),
                         sigma=1.0, D=rng.standard_normal((6, 3)), V=rng.standard_normal(6))
     check_workload(torch, binding, oracle_mod, w, label="m0")
+
+
+def test_cuda_graph_capture_of_a_step(torch, binding, oracle_mod):
+    """The three hot-path calls enqueue kernels only (no synchronisation, no allocation) when no host output is
+    requested, so a step can be captured into a CUDA graph on the ctx stream and replayed; the replay gives the
+    same scalars and arrays as the direct calls."""
+    w = inputs.small(1)
+    P, r = w.problem, w.r
+    s = torch.cuda.Stream()
+    s.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(s):
+        ctx = binding.Context(P, w.dtype, stream=s.cuda_stream)
+        R = dev(torch, w.R, torch.float32); D = dev(torch, w.D, torch.float32); V = dev(torch, w.V, torch.float32)
+        G = torch.zeros_like(R); W = torch.zeros_like(V)
+        y = dev(torch, w.y, torch.float64)
+        z = torch.zeros(P.m, dtype=torch.float64, device="cuda"); lam = torch.zeros_like(z)
+        ctx.set_dual(y, w.sigma)
+        st0 = ctx.eval(R, r, r, G, z); ctx.get_lambda(lam)
+        p0 = ctx.linesearch(R, D, r, r)
+        ctx.smatvec(lam, V, 1, W, fetch=False)
+        torch.cuda.synchronize()
+        G0, W0 = G.clone(), W.clone()
+        G.zero_(); W.zero_()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=s):
+            ctx.eval(R, r, r, G, z, stats=False)
+            ctx.linesearch(R, D, r, r, fetch=False)
+            ctx.smatvec(lam, V, 1, W, fetch=False)
+        G.zero_(); W.zero_()
+        g.replay(); g.replay()
+        torch.cuda.synchronize()
+        assert torch.equal(G, G0) and torch.equal(W, W0)
+        assert np.array_equal(ctx.get_stats(), st0) and np.array_equal(ctx.get_linesearch(), p0)
+        ctx.close()
