@@ -119,7 +119,7 @@ template <typename T> alora_status build(alora_ctx* c, const alora_problem* P) {
   // line search runs over C's entry list in equal chunks
   int64_t c_maxdeg = 0;
   for (int64_t j = 0; j < n; ++j) c_maxdeg = std::max<int64_t>(c_maxdeg, c_rowptr[j + 1] - c_rowptr[j]);
-  bool diag_class = (P->pC == 0) && c_maxdeg <= 4 * kHeavyRow;
+  bool diag_class = (P->pC == 0) && c_maxdeg <= kGeneralRow;
   std::vector<int> dcons(n, -1);
   std::vector<double> da(n, 0.0);
   {
@@ -208,7 +208,7 @@ template <typename T> alora_status build(alora_ctx* c, const alora_problem* P) {
     c->a_nnz = (int64_t)aents.size();
     c->ep = (c->a_nnz + c->c_nnz) >= 8 * n;
     c->ep_wide = (c->a_nnz + c->c_nnz) >= 96 * n;
-    if (c_maxdeg > kHeavyRow) {
+    if (c_maxdeg > kGeneralRow) {   // power-law graphs: every C row longer than kHeavyRow is segmented
       std::vector<int> seg_row, seg_beg, seg_end, heavy_rows, heavy_segptr(1, 0);
       for (int64_t j = 0; j < n; ++j) {
         const int e0 = c_rowptr[j], e1 = c_rowptr[j + 1];
@@ -222,7 +222,6 @@ template <typename T> alora_status build(alora_ctx* c, const alora_problem* P) {
       ALORA_CUDA(c, upload(c, (void**)&c->seg_end, seg_end));
       ALORA_CUDA(c, upload(c, (void**)&c->heavy_rows, heavy_rows));
       ALORA_CUDA(c, upload(c, (void**)&c->heavy_segptr, heavy_segptr));
-      ALORA_CUDA(c, c->pool.alloc(&c->seg_out, sizeof(double) * 256 * (size_t)c->nseg));
       ALORA_CUDA(c, c->pool.alloc((void**)&c->seg_cx, sizeof(double) * (size_t)c->nseg));
     }
     {

@@ -204,7 +204,14 @@ alora_status launch_diag_rows(alora_ctx* c, int vec, int nvec, int exact, int sh
 // (measured on config 3, 60 entries per row: the warp-per-row kernel wins for p = 1, 66 vs 77 us, and loses for
 // r = 10, 168 vs 128 us); rows with ~100 entries or more (matrix completion) always take a warp per row
 template <typename T> alora_status launch_adj_general(alora_ctx* c, const Geo& g, RowArgs<T>& a, double* out) {
-  if (c->nseg > 0 && g.nvec * g.vec <= 256) {   // heavy rows: their C part is summed per segment first
+  if (c->nseg > 0) {   // heavy rows: their C part is summed per segment first
+    const size_t need = (size_t)c->nseg * (size_t)(g.nvec * g.vec) * c->esz;
+    if (need > c->seg_out_bytes) {
+      if (c->seg_out) c->pool.release(c->seg_out);
+      ALORA_CUDA(c, c->pool.alloc(&c->seg_out, need));
+      c->seg_out_bytes = need;
+    }
+    a.seg_out = (T*)c->seg_out;
     a.nseg = c->nseg;
     const int gs = (int)std::min<int64_t>((c->nseg + kBlock / 32 - 1) / (kBlock / 32), (int64_t)c->num_sms * 8);
     ALORA_CUDA(c, launch_rows_seg(g.vec, g.shape, a, gs, c->stream));

@@ -62,6 +62,7 @@ struct alora_ctx {
   // heavy C rows (> kHeavyRow entries) cut into segments for k_rows_seg / k_rows_ep
   int nseg = 0, nheavy = 0; int* seg_row = nullptr; int* seg_beg = nullptr; int* seg_end = nullptr;
   int* heavy_rows = nullptr; int* heavy_segptr = nullptr; void* seg_out = nullptr; double* seg_cx = nullptr;
+  size_t seg_out_bytes = 0;   // seg_out is sized on first use for the row length in use (nseg * pitch elements)
   bool single_entry = false;   // every constraint has exactly one stored entry: thread-per-constraint forward (k_cons1)
   bool short_cons = false;     // at most 8 stored entries per constraint on average: thread-per-constraint forward too
   bool ep = false;       // general class, >= 8 entries per row on average: warp-per-row adjoint for single vectors

@@ -22,7 +22,8 @@
 namespace alora {
 
 constexpr int kBlock = 256;
-constexpr int kHeavyRow = 128;        // a C row with more entries sends a diagonal-class problem down the general path
+constexpr int kGeneralRow = 512;      // a C row with more entries sends a diagonal-class problem down the general path
+constexpr int kHeavyRow = 128;        // general path: C rows with more entries are cut into segments of this many entries
 constexpr int kLongThreshold = 64;   // constraints with more stored entries are split into chunks
 constexpr int kChunk = 16;           // entries per chunk of a long constraint / of C's sym-upper list
 // diagonal class: ELL slots per row (first neighbours; for the line search: last upper-triangle neighbours), see
