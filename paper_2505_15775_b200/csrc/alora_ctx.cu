@@ -246,6 +246,8 @@ alora_status geometry(alora_ctx* c, int32_t r, int64_t ld, const void* p0, const
   if (r < 1 || ld < r) return fail(c, ALORA_EINVAL, "need 1 <= r <= ld");
   if (((uintptr_t)p0 % c->esz) || ((uintptr_t)p1 % c->esz) || ((uintptr_t)p2 % c->esz)) return fail(c, ALORA_EINVAL, "misaligned pointer");
   g.vec = pick_vec(c, ld, p0, p1, p2);
+  // padded rows (ld > r) on the staged-tile path: a narrower pack that divides r keeps that path eligible
+  if (c->cls == 0 && c->ell_col) while (g.vec > 1 && r % g.vec) g.vec /= 2;
   g.nvec = (r + g.vec - 1) / g.vec;
   g.shape = shape_index(g.nvec);
   g.exact = (g.nvec * g.vec == r);

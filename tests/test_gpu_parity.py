@@ -174,6 +174,55 @@ def test_edge_cases(torch, binding, oracle_mod, dtype, r):
         check_workload(torch, binding, oracle_mod, w, label=f"{name}/r{r}/{dtype}", split_scale=True)
 
 
+def _fuzz_problem(rng, kind):
+    """Random structures that walk the dispatch: `general` = random constraints (0..150 entries: short lists,
+    single entries, chunked long ones), optional low-rank cost term; `diag` = one unit diagonal constraint per
+    row with random row degrees around the ELL slot counts (overflow rows); `hub` = the same with one row of
+    degree > 512 (general path, heavy-row segments)."""
+    from tests.helpers import problem_from_lists, random_problem
+    if kind == "general":
+        n = int(rng.integers(2, 1500)); m = int(rng.integers(1, 2 * n))
+        return random_problem(rng, n, m, max_nnz=int(rng.choice([1, 3, 8, 150])), nnzC=int(rng.integers(0, 6 * n)),
+                              pC=int(rng.choice([0, 0, 1, 3])))
+    n = int(rng.integers(130, 2500))
+    C = {}
+    for j in range(n):
+        for _ in range(int(rng.integers(0, 7 if kind == "diag" else 4))):
+            k = int(rng.integers(n))
+            if k != j:
+                C[(min(j, k), max(j, k))] = float(rng.standard_normal())
+        if rng.random() < 0.3:
+            C[(j, j)] = float(rng.standard_normal())
+    if kind == "hub":
+        h = int(rng.integers(n))
+        for k in rng.choice(n, size=min(n - 1, 700), replace=False):
+            if int(k) != h:
+                C[(min(h, int(k)), max(h, int(k)))] = float(rng.standard_normal())
+    Cl = sorted((j, k, v) for (j, k), v in C.items())
+    return problem_from_lists(n, Cl, [[(j, j, 1.0)] for j in range(n)], [1.0] * n)
+
+
+@pytest.mark.parametrize("seed", range(12))
+def test_random_structures(torch, binding, oracle_mod, seed):
+    rng = np.random.default_rng(9000 + seed)
+    kind = ["general", "diag", "hub"][seed % 3]
+    dtype = inputs.F32 if (seed // 3) % 2 else inputs.F64
+    P = _fuzz_problem(rng, kind)
+    r = int(rng.choice([1, 2, 4, 6, 10, 16, 24]))
+    ld = r + int(rng.choice([0, 0, 1, 2, 4]))
+
+    def draw(shape):
+        a = rng.standard_normal(shape)
+        return a.astype(np.float32).astype(float) if dtype == inputs.F32 else a
+    if dtype == inputs.F32:
+        P.C_val = P.C_val.astype(np.float32).astype(float); P.A_val = P.A_val.astype(np.float32).astype(float)
+        if P.pC:
+            P.C_U = P.C_U.astype(np.float32).astype(float)
+    w = inputs.Workload(name=f"fuzz{seed}", problem=P, dtype=dtype, r=r, R=draw((P.n, r)), y=rng.standard_normal(P.m),
+                        sigma=float(rng.uniform(0.1, 10.0)), D=draw((P.n, r)), V=draw(P.n))
+    check_workload(torch, binding, oracle_mod, w, ld=ld, label=f"fuzz{seed}/{kind}/r{r}/ld{ld}/{dtype}", split_scale=True)
+
+
 def test_m0_no_constraints(torch, binding, oracle_mod):
     """m = 0: f = <C,RR^T>, G = 2CR, S = C."""
     from tests.helpers import problem_from_lists
