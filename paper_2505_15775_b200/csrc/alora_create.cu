@@ -9,6 +9,7 @@
 //                C's sym-upper entries, and the chunk tables of the "long" constraints and of C.
 #include <algorithm>
 #include <cmath>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 
@@ -208,6 +209,26 @@ template <typename T> alora_status build(alora_ctx* c, const alora_problem* P) {
     c->a_nnz = (int64_t)aents.size();
     c->ep = (c->a_nnz + c->c_nnz) >= 8 * n;
     c->ep_wide = (c->a_nnz + c->c_nnz) >= 96 * n;
+    {
+      // skewed row lengths (power-law graphs): k_rows walks the rows by decreasing work, so the groups of a warp
+      // (and the blocks of a wave) get rows of nearly equal length; counting sort, stable in the row index
+      const int64_t mean = (c->a_nnz + c->c_nnz) / std::max<int64_t>(1, n);
+      int64_t wmax = 0;
+      std::vector<int> work(n);
+      for (int64_t j = 0; j < n; ++j) {
+        const int cd = c_rowptr[j + 1] - c_rowptr[j];
+        const int w = (cd > kHeavyRow ? (cd + kHeavyRow - 1) / kHeavyRow : cd) + (a_rowptr[j + 1] - a_rowptr[j]);
+        work[j] = w; wmax = std::max<int64_t>(wmax, w);
+      }
+      if (!c->ep_wide && wmax > 4 * mean + 16 && !std::getenv("ALORA_NO_ROW_ORDER")) {
+        std::vector<int64_t> cnt((size_t)wmax + 2, 0);
+        for (int64_t j = 0; j < n; ++j) cnt[(size_t)(wmax - work[j]) + 1]++;
+        for (size_t k = 1; k < cnt.size(); ++k) cnt[k] += cnt[k - 1];
+        std::vector<int> perm(n);
+        for (int64_t j = 0; j < n; ++j) perm[(size_t)cnt[(size_t)(wmax - work[j])]++] = (int)j;
+        ALORA_CUDA(c, upload(c, (void**)&c->row_perm, perm));
+      }
+    }
     if (c_maxdeg > kGeneralRow) {   // power-law graphs: every C row longer than kHeavyRow is segmented
       std::vector<int> seg_row, seg_beg, seg_end, heavy_rows, heavy_segptr(1, 0);
       for (int64_t j = 0; j < n; ++j) {

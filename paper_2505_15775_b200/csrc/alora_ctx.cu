@@ -217,7 +217,7 @@ template <typename T> alora_status launch_adj_general(alora_ctx* c, const Geo& g
     ALORA_CUDA(c, launch_rows_seg(g.vec, g.shape, a, gs, c->stream));
     c->launches++;
   }
-  if ((c->ep && g.nvec == 1) || c->ep_wide) {
+  if ((c->ep && g.nvec == 1 && !c->row_perm) || c->ep_wide) {
     // very long rows of thin vectors (matrix completion, r <= 8 packs): every lane owns whole rows, 32 entry lanes
     const int eshape = (c->ep_wide && g.nvec > 1 && g.nvec <= 4) ? 7 : (c->ep_wide && g.nvec > 4 && g.nvec <= 8) ? 8 : g.shape;
     int& occ = c->occ_cache[vec_slot(g.vec)][eshape == g.shape ? g.shape : eshape - 7][eshape == g.shape ? 11 : 7];
@@ -228,6 +228,7 @@ template <typename T> alora_status launch_adj_general(alora_ctx* c, const Geo& g
     ALORA_CUDA(c, launch_rows_ep(g.vec, eshape, a, grid, c->stream));
   } else {
     const int grid = grid_rows<T>(c, g.vec, g.shape, ROWS_ADJ, c->n);
+    a.perm = c->row_perm;
     a.fin = make_fin(c, a.fin.p[0], grid, a.fin.p[1], a.fin.n[1], a.fin.p[2], a.fin.n[2], out);
     ALORA_CUDA(c, launch_rows(g.vec, g.shape, ROWS_ADJ, a, grid, c->stream));
   }
@@ -257,6 +258,7 @@ alora_status geometry(alora_ctx* c, int32_t r, int64_t ld, const void* p0, const
 
 template <typename T> void fill_rows(alora_ctx* c, RowArgs<T>& a, const Geo& g, const T* X, int r, int64_t ld) {
   a.n = c->n; a.r = r; a.ld = ld; a.nvec = g.nvec; a.exact = g.exact; a.X = X; a.X2 = nullptr; a.Out = nullptr;
+  a.perm = nullptr;
   a.c_rowptr = c->c_rowptr; a.c_col = c->c_col; a.c_val = (const T*)c->c_val; a.dC = (const T*)c->dC;
   a.dcons = c->dcons; a.da = (const T*)c->da;
   a.a_rowptr = c->a_rowptr; a.a_col = c->a_col; a.a_val = (const T*)c->a_val; a.a_cons = c->a_cons;

@@ -66,6 +66,7 @@ struct alora_ctx {
   bool single_entry = false;   // every constraint has exactly one stored entry: thread-per-constraint forward (k_cons1)
   bool short_cons = false;     // at most 8 stored entries per constraint on average: thread-per-constraint forward too
   bool ep = false;       // general class, >= 8 entries per row on average: warp-per-row adjoint for single vectors
+  int* row_perm = nullptr;  // general class, skewed row lengths: rows by decreasing work (k_rows walks this order)
   bool ep_wide = false;  // >= 96 entries per row on average (matrix completion): warp-per-row adjoint for every r
   // forward list: coalesced constraint entries [0, nf_A), then C's sym-upper entries [nf_A, nf_A+nf_C)
   int64_t* f_ptr = nullptr; int* f_row = nullptr; int* f_col = nullptr; void* f_val = nullptr;

@@ -77,6 +77,8 @@ template <typename T> struct RowArgs {
   // k_rows_seg sums first (seg_out[s][nvec * VEC], seg_cx[s]); heavy_rows (ascending) / heavy_segptr list them per row
   int nseg, nheavy; const int* seg_row; const int* seg_beg; const int* seg_end;
   const int* heavy_rows; const int* heavy_segptr; T* seg_out; double* seg_cx;
+  // optional processing order of the rows (general class, skewed degrees): position -> row, heaviest rows first
+  const int* perm;
 };
 
 template <typename T> struct ConsArgs {
@@ -281,7 +283,8 @@ __global__ void __launch_bounds__(kBlock) k_rows(const RowArgs<T> a) {
 #pragma unroll
   for (int s = 0; s < NST; ++s) st[s] = 0.0;
 
-  for (int64_t row = a.row_begin + (int64_t)blockIdx.x * GPB + grp; row < a.n; row += (int64_t)gridDim.x * GPB) {
+  for (int64_t pos = a.row_begin + (int64_t)blockIdx.x * GPB + grp; pos < a.n; pos += (int64_t)gridDim.x * GPB) {
+    const int64_t row = a.perm ? (int64_t)__ldg(a.perm + pos) : pos;
     Row x; x.load(a.X + row * a.ld, lane, nvec, r, exact);
     const int cb = __ldg(a.c_rowptr + row), ce = __ldg(a.c_rowptr + row + 1);
     const T dc = __ldg(a.dC + row);
