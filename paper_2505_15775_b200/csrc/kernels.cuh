@@ -271,8 +271,14 @@ __device__ __forceinline__ void gather_axpy(RowReg<T, VEC, GS, NIT>& acc, const 
   }
 }
 
+// The adjoint pass is a chain of dependent gathers per row (pointers -> columns -> rows); it is bound by the number
+// of warps that hide that latency, so its registers are capped for 6 blocks per SM (measured, min blocks 1 / 4 / 5 /
+// 6 / 8: config 3 175 / 174 / 146 / 135 / 128 us, config 7 506 / 446 / 404 / 439 / 427 us, config 2 55 / 45 / 39 / 39 / 43 us)
+#ifndef ALORA_ROWS_MINB
+#define ALORA_ROWS_MINB 6
+#endif
 template <typename T, int VEC, int GS, int NIT, int MODE>
-__global__ void __launch_bounds__(kBlock) k_rows(const RowArgs<T> a) {
+__global__ void __launch_bounds__(kBlock, (MODE == ROWS_ADJ && NIT <= 2) ? ALORA_ROWS_MINB : 1) k_rows(const RowArgs<T> a) {
   using Row = RowReg<T, VEC, GS, NIT>;
   constexpr int GPB = kBlock / GS;
   constexpr int NST = (MODE == ROWS_LS_FUSED) ? 12 : 6;
