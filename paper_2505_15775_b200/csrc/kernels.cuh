@@ -101,17 +101,38 @@ template <typename T> struct ConsArgs {
 // ---------------------------------------------------------------------------------------------
 template <typename T, int VEC> struct alignas(sizeof(T) * VEC) Pack { T v[VEC]; };
 
+// Read-only row loads.  ALORA_LD_L2HINT (default on): ld.global.nc with the L2::64B prefetch-size hint -- measured on
+// config 4 (random 40-byte row gathers from a 671 MB R): 1 150 -> 1 109 us for the f + grad kernel; plain
+// ld.global.nc (__ldg), .L1::no_allocate, .cg and .cs were equal or slower (profiles/r1t_README.md).
+#ifndef ALORA_LD_L2HINT
+#define ALORA_LD_L2HINT 1
+#endif
+#if ALORA_LD_L2HINT
+#define ALORA_LD_NC "ld.global.nc.L2::64B"
+#else
+#define ALORA_LD_NC "ld.global.nc"
+#endif
 template <typename T, int VEC> __device__ __forceinline__ Pack<T, VEC> ldg_pack(const T* p);
 template <> __device__ __forceinline__ Pack<float, 4> ldg_pack<float, 4>(const float* p) {
-  float4 t = __ldg(reinterpret_cast<const float4*>(p)); Pack<float, 4> o; o.v[0] = t.x; o.v[1] = t.y; o.v[2] = t.z; o.v[3] = t.w; return o; }
+  Pack<float, 4> o;
+  asm(ALORA_LD_NC ".v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(o.v[0]), "=f"(o.v[1]), "=f"(o.v[2]), "=f"(o.v[3]) : "l"(p));
+  return o; }
 template <> __device__ __forceinline__ Pack<float, 2> ldg_pack<float, 2>(const float* p) {
-  float2 t = __ldg(reinterpret_cast<const float2*>(p)); Pack<float, 2> o; o.v[0] = t.x; o.v[1] = t.y; return o; }
+  Pack<float, 2> o;
+  asm(ALORA_LD_NC ".v2.f32 {%0,%1}, [%2];" : "=f"(o.v[0]), "=f"(o.v[1]) : "l"(p));
+  return o; }
 template <> __device__ __forceinline__ Pack<float, 1> ldg_pack<float, 1>(const float* p) {
-  Pack<float, 1> o; o.v[0] = __ldg(p); return o; }
+  Pack<float, 1> o;
+  asm(ALORA_LD_NC ".f32 %0, [%1];" : "=f"(o.v[0]) : "l"(p));
+  return o; }
 template <> __device__ __forceinline__ Pack<double, 2> ldg_pack<double, 2>(const double* p) {
-  double2 t = __ldg(reinterpret_cast<const double2*>(p)); Pack<double, 2> o; o.v[0] = t.x; o.v[1] = t.y; return o; }
+  Pack<double, 2> o;
+  asm(ALORA_LD_NC ".v2.f64 {%0,%1}, [%2];" : "=d"(o.v[0]), "=d"(o.v[1]) : "l"(p));
+  return o; }
 template <> __device__ __forceinline__ Pack<double, 1> ldg_pack<double, 1>(const double* p) {
-  Pack<double, 1> o; o.v[0] = __ldg(p); return o; }
+  Pack<double, 1> o;
+  asm(ALORA_LD_NC ".f64 %0, [%1];" : "=d"(o.v[0]) : "l"(p));
+  return o; }
 
 template <typename T, int VEC> __device__ __forceinline__ void st_pack(T* p, const Pack<T, VEC>& x) {
   *reinterpret_cast<Pack<T, VEC>*>(p) = x;
