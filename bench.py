@@ -91,10 +91,24 @@ class ClockSampler:
         self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
         try:
             self.p = subprocess.Popen(["nvidia-smi", "-i", str(gpu), f"--query-gpu={self.Q}",
-                                       "--format=csv,noheader,nounits", "-lms", "100"],
+                                       "--format=csv,noheader,nounits", "-lms", "20"],
                                       stdout=self.f, stderr=subprocess.DEVNULL)
         except OSError:
             self.p = None
+
+    def wait_first(self, keep_busy, timeout_s: float = 4.0):
+        """nvidia-smi needs a few hundred ms to print its first line, longer than a short timed region: keep the GPU
+        under the same load (`keep_busy` = one untimed step + sync) until the first sample is there."""
+        if self.p is None:
+            return
+        t0 = time.perf_counter()
+        while time.perf_counter() - t0 < timeout_s:
+            keep_busy()
+            try:
+                if os.path.getsize(self.f.name) > 0:
+                    return
+            except OSError:
+                return
 
     def stop(self):
         out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": []}
@@ -238,7 +252,7 @@ def run_solve(args, w, local, torch, binding):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--steps", type=int, default=1000)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=1, help="BASELINE.json config index (default 1: torus MaxCut)")
@@ -307,6 +321,8 @@ def main():
         step()
     barrier()
     sampler = ClockSampler(local) if rank == 0 else None
+    if sampler:   # untimed steps of the same load until nvidia-smi has produced its first sample
+        sampler.wait_first(lambda: (step(), torch.cuda.synchronize()))
     l0 = ctx.info()["launches"]
     ctx.kernel_timing(8 if args.steps >= 64 else True)   # every 8th evaluation of the timed region is bracketed by events
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
