@@ -6,6 +6,7 @@ import os
 import re
 import subprocess
 import sys
+import time
 
 import numpy as np
 import pytest
@@ -103,3 +104,20 @@ def test_replica_aggregation_gloo_world2(tmp_path):
     for p in procs:
         out, err = p.communicate(timeout=120)
         assert p.returncode == 0 and "ok" in out, err[-2000:]
+
+
+def test_clock_sampler_parses_samples_and_waits_for_the_first(tmp_path, monkeypatch):
+    """bench.ClockSampler with a stand-in for nvidia-smi: wait_first keeps calling the load until the
+    first line is there, stop() reports the median clock and the active throttle reasons."""
+    import bench
+    fake = tmp_path / "nvidia-smi"
+    fake.write_text("#!/bin/bash\nsleep 0.3\nfor i in 1 2 3 4 5 6 7 8 9 10; do echo '1965, 1965, Not Active, Not Active, Not Active, Active'; sleep 0.02; done\nsleep 30\n")
+    fake.chmod(0o755)
+    monkeypatch.setenv("PATH", str(tmp_path) + os.pathsep + os.environ["PATH"])
+    s = bench.ClockSampler(0)
+    calls = []
+    s.wait_first(lambda: (calls.append(1), time.sleep(0.01)), timeout_s=5.0)
+    assert len(calls) >= 5          # the first line took 0.3 s
+    time.sleep(0.1)
+    out = s.stop()
+    assert out["sm_mhz"] == 1965.0 and out["sm_max_mhz"] == 1965.0 and out["reasons"] == ["sw_power_cap"]
