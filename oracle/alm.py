@@ -48,6 +48,14 @@ class Params:
     stall_iters: int = 3       #      decrease phi(0) - phi(alpha) <= stall_tol (1 + |f|); 0 = off
 
 
+def preset_params(f32: bool, **kw) -> Params:
+    """Same preset as alora_preset_params (include/alora.h): fp32 storage -> bounded inexact inner solves
+    (it_max = 100) with the stall rule [28] on."""
+    base = dict(it_max=100, stall_tol=1e-9, stall_iters=3) if f32 else {}
+    base.update(kw)
+    return Params(**base)
+
+
 @dataclass
 class IterRecord:
     t: int = 0
@@ -248,6 +256,28 @@ def kkt_terms(qnorm, normb, theta_min, normC, cx, by):
             abs(cx - by) / (1.0 + abs(cx) + abs(by)))
 
 
+def kkt_at(orc, R, y, theta_min):
+    """KKT(X, y) of eq. 77 at X = RR^T, from the definitions: ||A(X) - b||_2, ||b||_2,
+    ||C||_F, <C,X>, b^T y (l2 norms); theta_min = lambda_min(C - A^*(y)) is passed in
+    (the loop has it from Lanczos [16], the pins from a dense eigen-solver)."""
+    b = orc.b
+    q = orc.A_op(R) - b
+    return kkt_terms(float(np.sqrt(q @ q)), float(np.sqrt(b @ b)), theta_min, orc.normC(),
+                     orc.inner_C(R, R), float(b @ y))
+
+
+def shrink_rank(R, tau_shrink: float):
+    """Rank shrink [13]: eigen-decompose R^T R = Q M Q^T and drop the directions with
+    mu_j <= tau_shrink * mu_max, R <- R Q_keep.  X = RR^T loses only the dropped directions' mu_j, so with
+    exact null directions X (hence f, A(X), ||G||_F) is unchanged.  Returns (R_new, number dropped);
+    never drops everything."""
+    mu, Q = np.linalg.eigh(R.T @ R)
+    keep = mu > tau_shrink * mu[-1]
+    if not keep.all() and keep.any():
+        return R @ Q[:, keep], int((~keep).sum())
+    return R, 0
+
+
 def solve(orc, R0, y0, sigma0: float, prm: Params = Params()) -> Result:
     """ALORA (Algorithm 1) with readings 5-13, 17, 20 of DESIGN.md.
 
@@ -344,12 +374,9 @@ def solve(orc, R0, y0, sigma0: float, prm: Params = Params()) -> Result:
             rec.grew, changed = cols.shape[1], True
         elif R.shape[1] > 1:
             # -- 5. shrink [13]: drop the numerically null directions of R
-            M = R.T @ R
-            mu, Q = np.linalg.eigh(M)
-            keep = mu > prm.tau_shrink * mu[-1]
-            if not keep.all() and keep.any():
-                R = R @ Q[:, keep]
-                rec.shrank, changed = int((~keep).sum()), True
+            R, dropped = shrink_rank(R, prm.tau_shrink)
+            if dropped:
+                rec.shrank, changed = dropped, True
         if changed:
             q = orc.A_op(R) - b
         qnorm = float(np.sqrt(q @ q))
@@ -358,7 +385,7 @@ def solve(orc, R0, y0, sigma0: float, prm: Params = Params()) -> Result:
         if changed:                       # [17] S(lambda) != S(y_new) once R changed: recompute
             theta_kkt, _, _, _ = run_lanczos(y)
         cx = orc.inner_C(R, R)
-        rec.kkt = kkt_terms(qnorm, normb, theta_kkt, normC, cx, float(b @ y))
+        rec.kkt = kkt_at(orc, R, y, theta_kkt)        # eq. 77 at (RR^T, y_new)
         rec.r, rec.cx, rec.qnorm = R.shape[1], cx, qnorm
         # -- 7. sigma schedule [12]
         if qnorm > prm.kappa * qnorm_prev and rec.kkt[0] > prm.eps:   # no increase once the primal term is below eps

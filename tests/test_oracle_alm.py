@@ -26,10 +26,127 @@ def alm():
 
 
 def test_counter_uniform(alm):
+    """Start-vector generator [9] against literal values computed with exact Python integers
+    (tests/golden/make_counter_uniform.py, which imports nothing from this repo) and against its statistics."""
+    for c in GOLD["counter_uniform"]["cases"]:
+        v = alm.counter_uniform(c["seed"], c["i"] + 1)
+        assert v[c["i"]] == c["v"], c
     v = alm.counter_uniform(7, 100000)
     assert np.all(np.abs(v) < 1) and abs(v.mean()) < 0.01 and abs(v.var() - 1 / 3) < 0.01
-    np.testing.assert_array_equal(v, inputs.counter_uniform(7, 100000))
     assert not np.array_equal(v[:100], alm.counter_uniform(8, 100))
+
+
+def _dense_bfgs_inverse(S_list, Y_list, n):
+    """Textbook BFGS inverse-Hessian recursion H <- (I - rho s y^T) H (I - rho y s^T) + rho s s^T applied to the
+    pairs oldest first, from H_0 = (s^T y / y^T y) I of the NEWEST pair (Nocedal & Wright, eq. 6.17 / 7.20)."""
+    s, y = S_list[-1], Y_list[-1]
+    H = (s @ y) / (y @ y) * np.eye(n)
+    for s, y in zip(S_list, Y_list):
+        rho = 1.0 / (y @ s)
+        V = np.eye(n) - rho * np.outer(y, s)
+        H = V.T @ H @ V + rho * np.outer(s, s)
+    return H
+
+
+@pytest.mark.parametrize("npairs", [1, 2, 3, 5])
+def test_lbfgs_direction_equals_dense_bfgs(alm, npairs):
+    """The two-loop recursion [5] must give D = -H g with H the dense BFGS inverse Hessian built from the same
+    pairs (a wrong sign of rho, a wrong loop order, or the scaling of the oldest pair all fail here)."""
+    rng = np.random.default_rng(100 + npairs)
+    n = 12
+    A = rng.standard_normal((n, n)); A = A @ A.T + n * np.eye(n)      # pairs from a convex quadratic: s^T y > 0
+    S_list = [rng.standard_normal(n) for _ in range(npairs)]
+    Y_list = [A @ s for s in S_list]
+    g = rng.standard_normal(n)
+    D = alm.lbfgs_direction(g, S_list, Y_list)
+    ref = -_dense_bfgs_inverse(S_list, Y_list, n) @ g
+    assert np.linalg.norm(D - ref) <= 1e-12 * np.linalg.norm(ref)
+    # matrix-shaped arguments (the loop hands over n x r arrays): same numbers
+    D2 = alm.lbfgs_direction(g.reshape(4, 3), [s.reshape(4, 3) for s in S_list], [y.reshape(4, 3) for y in Y_list])
+    np.testing.assert_allclose(D2.ravel(), D, rtol=1e-13, atol=1e-15)
+    assert np.array_equal(alm.lbfgs_direction(g, [], []), -g)
+
+
+def test_lbfgs_exact_steps_terminate_like_cg(alm):
+    """On a strictly convex quadratic with exact steps and memory >= n, the L-BFGS iterates coincide with those
+    of conjugate gradients (textbook: BFGS with exact line searches generates conjugate directions), so the
+    gradient vanishes after at most n steps."""
+    rng = np.random.default_rng(5)
+    n = 10
+    A = rng.standard_normal((n, n)); A = A @ A.T + np.eye(n)
+    b = rng.standard_normal(n)
+    x = np.zeros(n); g = A @ x - b
+    xc = np.zeros(n); rc = b - A @ xc; pc = rc.copy()               # CG (Hestenes-Stiefel)
+    S_list, Y_list = [], []
+    for it in range(n):
+        d = alm.lbfgs_direction(g, S_list, Y_list)
+        alpha = -(g @ d) / (d @ A @ d)
+        x_new = x + alpha * d; g_new = A @ x_new - b
+        S_list.append(x_new - x); Y_list.append(g_new - g)
+        x, g = x_new, g_new
+        ac = (rc @ rc) / (pc @ A @ pc); xc = xc + ac * pc
+        rn = rc - ac * (A @ pc); pc = rn + (rn @ rn) / (rc @ rc) * pc; rc = rn
+        assert np.linalg.norm(x - xc) <= 1e-8 * (1 + np.linalg.norm(xc)), it
+    assert np.linalg.norm(g) <= 1e-8 * np.linalg.norm(b)
+
+
+def _sqrtf(expr):
+    return float(eval(expr, {"sqrt": np.sqrt}))
+
+
+def test_kkt_terms_hand_computed(alm, Oracle):
+    """eq. 77 on the data of eq. 36, values worked out by hand in
+    tests/golden/paper_examples.json["eq36_kkt"]; and exact zeros at the K_n primal-dual certificate."""
+    from tests.helpers import problem_from_lists
+    P = problem_from_lists(2, [], [[(0, 0, 1.0)], [(0, 1, 0.5)], [(0, 0, 1.0), (1, 1, 1.0)]], GOLD["eq36"]["b"])
+    o = Oracle(P)
+    for c in GOLD["eq36_kkt"]["cases"]:
+        R = np.diag(np.sqrt(c["X_diag"])); y = np.array(c["y"])
+        lam_min = np.linalg.eigvalsh(o.smatvec(y, np.eye(2)))[0]
+        got = alm.kkt_at(o, R, y, lam_min)
+        want = [_sqrtf(e) for e in c["kkt"]]
+        np.testing.assert_allclose(got, want, rtol=1e-14, atol=1e-15)
+    # the scalar form used inside the loop: l2 norms, the three "1 +" denominators, min{0, .}
+    assert alm.kkt_terms(3.0, 1.0, -0.5, 3.0, 2.0, -1.0) == (1.5, 0.125, 0.75)
+    assert alm.kkt_terms(0.0, 5.0, +0.7, 3.0, 2.0, 2.0) == (0.0, 0.0, 0.0)
+    for n in (5, 9):
+        Pk = _graph_maxcut(n, [(i, j) for i in range(n) for j in range(i + 1, n)])
+        ok = Oracle(Pk)
+        X = (n * np.eye(n) - np.ones((n, n))) / (n - 1)
+        mu, Q = np.linalg.eigh(X)
+        R = Q[:, 1:] * np.sqrt(mu[1:])
+        ystar = np.full(n, -n / 4)
+        lam_min = np.linalg.eigvalsh(ok.smatvec(ystar, np.eye(n)))[0]
+        assert max(alm.kkt_at(ok, R, ystar, lam_min)) < 1e-13
+
+
+def test_shrink_keeps_X_when_directions_are_null(alm, Oracle):
+    """[13] R <- R Q_keep drops only null directions of R: X = RR^T, hence f, z = A(X) and ||G||_F, are unchanged
+    to rounding, G(R Q) = G(R) Q, and the rank is the true rank; a full-rank R is left alone."""
+    w = inputs.small(3)
+    o = Oracle(w.problem)
+    rng = np.random.default_rng(8)
+    n, r1, r = w.problem.n, 4, 9
+    Q0, _ = np.linalg.qr(rng.standard_normal((r, r)))
+    R = np.hstack([rng.standard_normal((n, r1)) / np.sqrt(n), np.zeros((n, r - r1))]) @ Q0   # rank 4 inside 9 columns
+    R2, dropped = alm.shrink_rank(R, 1e-8)
+    assert dropped == r - r1 and R2.shape == (n, r1)
+    np.testing.assert_allclose(R2 @ R2.T, R @ R.T, atol=1e-15)
+    y, sg = w.y, w.sigma
+    f1, f2 = o.f(y, sg, R), o.f(y, sg, R2)
+    assert abs(f1 - f2) <= 1e-12 * (1 + abs(f1))
+    np.testing.assert_allclose(o.A_op(R2), o.A_op(R), rtol=0, atol=1e-14 * (1 + np.abs(o.A_op(R)).max()))
+    G1, G2 = o.grad(y, sg, R), o.grad(y, sg, R2)
+    assert abs(np.linalg.norm(G1) - np.linalg.norm(G2)) <= 1e-12 * np.linalg.norm(G1)
+    Qk = np.linalg.lstsq(R, R2, rcond=None)[0]                     # R2 = R Qk
+    np.testing.assert_allclose(G1 @ Qk, G2, atol=1e-12 * np.abs(G1).max())
+    R3, d3 = alm.shrink_rank(rng.standard_normal((50, 5)), 1e-8)
+    assert d3 == 0 and R3.shape == (50, 5)
+    # threshold is relative to the largest eigenvalue of R^T R: a direction at 1e-5 of the largest singular value
+    # (mu ratio 1e-10) goes, one at 1e-3 (ratio 1e-6) stays, whatever the scale of R
+    U, _ = np.linalg.qr(rng.standard_normal((50, 3)))
+    R4, d4 = alm.shrink_rank(U * np.array([100.0, 0.1, 1e-3]), 1e-8)
+    assert d4 == 1 and R4.shape == (50, 2)
 
 
 def test_quartic_argmin_bruteforce(alm):
