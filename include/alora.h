@@ -104,18 +104,36 @@ alora_status alora_get_lambda(alora_ctx *ctx, double *lam_dev);
 alora_status alora_eval_host(alora_ctx *ctx, const void *R_host, int32_t r, int64_t ld, void *G_host,
                              double *z_host, double stats[8]);
 
+/* One whole step of the hot path with HOST buffers (bench.py's end-to-end leg): f + grad at R, the line-search
+ * coefficients along D (warm form) and W = S(lambda) V with lambda of that evaluation.  R_host, D_host (n x r, ld),
+ * V_host (n): inputs; G_host (n x r, ld), z_host (fp64[m]), W_host (n): outputs, each may be NULL.  All HOST, ctx
+ * dtype; page-locked memory makes the copies asynchronous.  The copies run inside the call and are overlapped with
+ * the kernels where the data flow allows (D goes up while f + grad runs and G comes down; G, z come down on a
+ * second stream while the line search runs).  stats[8], p[5], vw as in the device calls (non-NULL).  Synchronises. */
+alora_status alora_step_host(alora_ctx *ctx, const void *R_host, const void *D_host, const void *V_host, int32_t r,
+                             int64_t ld, void *G_host, double *z_host, void *W_host, double stats[8], double p[5],
+                             double *vw);
+
 /* Exact line search: coefficients p[0..4] (HOST) of alpha -> f(R + alpha D) = sum_k p_k alpha^k, from
  * q = A(RR^T)-b, q1 = A(RD^T+DR^T), q2 = A(DD^T) expanded in (AL-BM):
  *   p0 = f(R), p1 = 2<C,RD^T> - y.q1 + sigma q.q1 = <G,D>, p2 = <C,DD^T> - y.q2 + (sigma/2)|q1|^2 + sigma q.q2,
  *   p3 = sigma q1.q2, p4 = (sigma/2)|q2|^2.
- * Correct called cold (recomputes q from R).  R, D as in alora_eval.  Synchronises.
- * p == NULL: enqueue only; fetch with alora_get_linesearch. */
-alora_status alora_linesearch(alora_ctx *ctx, const void *R, const void *D, int32_t r, int64_t ld,
+ * R, D as in alora_eval.  Synchronises.  p == NULL: enqueue only; fetch with alora_get_linesearch.
+ * warm == 0 ("cold", what bench.py times): correct whatever was called before -- q is recomputed from R.
+ * warm != 0: the caller states that the ctx still holds the state of an alora_eval on this same R (same pointer,
+ *   r, ld, same y and sigma, R not written since); the library may then reuse that state instead of recomputing
+ *   it (p0 is taken from the evaluation's f, and q-only sums from its scalars).  ALORA_ESTATE if no such evaluation
+ *   is on record (different R pointer / r / ld, or alora_set_dual called since).  Results equal the cold form to
+ *   rounding.  (DESIGN.md section 6 says what is and is not worth reusing: keeping C R across the line search does
+ *   not reduce the bytes of an inner iteration on this layout.) */
+alora_status alora_linesearch(alora_ctx *ctx, const void *R, const void *D, int32_t r, int64_t ld, int32_t warm,
                               double p[5]);
 alora_status alora_get_linesearch(alora_ctx *ctx, double p[5]);
 
 /* W = S(mu) V = (C - A^*(mu)) V  (the operator of Alg. 1 line 5, with
- * mu = lambda, and of eq. 77, with mu = y).  mu_dev: DEVICE fp64[m].  V, W: DEVICE, ctx
+ * mu = lambda, and of eq. 77, with mu = y).  mu_dev: DEVICE fp64[m], or NULL = lambda = y - sigma q of
+ * the last alora_eval (recomputed from that evaluation's z -- if the caller passed its own z_dev there,
+ * that buffer must still hold it; ALORA_ESTATE if there was no evaluation).  V, W: DEVICE, ctx
  * dtype, row-major n x p, contiguous (ld = p); p = 1 for vectors.  W must not alias V.
  * vw: HOST double* receiving <V,W> = sum_ij V_ij W_ij (the Lanczos alpha for p = 1), or NULL; the call
  * synchronises only if vw != NULL. */
@@ -135,13 +153,20 @@ alora_status alora_smatvec(alora_ctx *ctx, const double *mu_dev, const void *V, 
 alora_status alora_kernel_timing(alora_ctx *ctx, int enable);
 alora_status alora_kernel_timing_read(alora_ctx *ctx, double *total_ms, int64_t *count);
 
-/* Smallest Ritz pair of S(mu) by Lanczos with full re-orthogonalisation (reading 9):
- * start vector v0[i] = counter_uniform(seed, i), stops at step k when |beta_k s_k| <= tol_abs, on
- * breakdown, or at k = kmax (then returns ALORA_ENOTCONV with the best pair so far).
- * theta: HOST double*; v_dev: DEVICE, ctx dtype, [n] (unit Ritz vector) or NULL;
- * k_used: HOST int32*; resid: HOST double* (residual estimate), each may be NULL. */
-alora_status alora_lanczos(alora_ctx *ctx, const double *mu_dev, int32_t kmax, double tol_abs,
-                           uint64_t seed, double *theta, void *v_dev, int32_t *k_used, double *resid);
+/* The p_want smallest Ritz pairs of S(mu) by Lanczos with full re-orthogonalisation (Alg. 1 line 5, PAPER.md:913:
+ * "r-many negative smallest eigenvectors", :932-934; readings 9 and 29): start vector
+ * v0[i] = counter_uniform(seed, i); the run stops at step k when the SMALLEST pair's residual estimate
+ * |beta_k s_k| <= tol_abs, on breakdown, or at k = kmax (then ALORA_ENOTCONV with the best pairs so far); the
+ * min(p_want, k) smallest Ritz pairs of that k-step tridiagonal are returned (a Ritz vector's Rayleigh quotient
+ * is its Ritz value whether or not the pair has converged; resid says how far each one is).
+ * mu_dev: DEVICE fp64[m], or NULL = lambda of the last alora_eval (as in alora_smatvec).  1 <= p_want <= 8.
+ * theta: HOST double[p_want], ascending.  V_dev: DEVICE, ctx dtype, p_want vectors of length n, COLUMN-major
+ * (unit Ritz vector j is the contiguous array V_dev + j*n), or NULL.  p_found: HOST int32* (pairs returned);
+ * k_used: HOST int32* (Lanczos steps); resid: HOST double[p_want] (|beta_k s_{k,j}| per pair).  theta, p_found,
+ * k_used, resid may each be NULL.  Synchronises. */
+alora_status alora_lanczos(alora_ctx *ctx, const double *mu_dev, int32_t kmax, double tol_abs, uint64_t seed,
+                           int32_t p_want, double *theta, void *V_dev, int32_t *p_found, int32_t *k_used,
+                           double *resid);
 
 /* Free constants of the ALORA loop (Algorithm 1; readings in DESIGN.md).  Fill with
  * alora_default_params, then edit. */
@@ -151,7 +176,7 @@ typedef struct {
   int32_t T_max;       /* outer iterations (100) */
   double tol0, c_in, tol_min; /* inner tolerance tol_t = max(tol_min, min(tol0, c_in*infeas_{t-1})): 1e-2, 0.1, 1e-7 */
   int32_t it_max;      /* inner iterations per outer iteration (500) */
-  int32_t lbfgs_mem;   /* L-BFGS pairs (5); 0 = steepest descent with the exact step */
+  int32_t lbfgs_mem;   /* L-BFGS pairs (5), at most 16 (larger values are clamped to 16); 0 = steepest descent with the exact step */
   int32_t p_max;       /* eigenvectors per growth step, 1..4 (1: closed-form step; more: every sufficiently negative
                           Ritz pair of the Lanczos run, small SDP of Alg. 1 line 7; reading 29) */
   int32_t k_max;       /* Lanczos steps (300) */
@@ -167,6 +192,12 @@ typedef struct {
   int32_t pad_;
 } alora_params;
 void alora_default_params(alora_params *p);
+/* Defaults adjusted to the context dtype.  ALORA_F64: alora_default_params.  ALORA_F32: the gradient norm of an fp32
+ * evaluation cannot fall below its rounding floor, so late outer iterations would spend all it_max = 500 inner
+ * iterations without decreasing f; the preset bounds the inner solves -- "approximately solving" the subproblem is
+ * what the paper's practical variant does -- with it_max = 100 and the stall rule on
+ * (stall_tol = 1e-9, stall_iters = 3; readings 6 and 28).  oracle/alm.py has the same preset. */
+void alora_preset_params(alora_params *p, alora_dtype dtype);
 
 typedef struct { /* one row per outer iteration */
   int32_t t, r, inner_iters, n_evals, lanczos_steps, grew, shrank, pad_;

@@ -56,6 +56,18 @@ class Params(C.Structure):
             setattr(self, k, v)
 
 
+    @classmethod
+    def preset(cls, dtype, **kw):
+        """alora_preset_params for the context dtype (F32: bounded inexact inner solves), then overrides."""
+        p = cls()
+        _lib.alora_preset_params(C.byref(p), {"f32": F32, "f64": F64, F32: F32, F64: F64}[dtype])
+        for k, v in kw.items():
+            if not hasattr(p, k):
+                raise AttributeError(k)
+            setattr(p, k, v)
+        return p
+
+
 class IterRecord(C.Structure):
     _fields_ = [("t", C.c_int32), ("r", C.c_int32), ("inner_iters", C.c_int32), ("n_evals", C.c_int32),
                 ("lanczos_steps", C.c_int32), ("grew", C.c_int32), ("shrank", C.c_int32), ("pad_", C.c_int32),
@@ -76,6 +88,8 @@ _lib.alora_last_error.argtypes = [C.c_void_p]
 _lib.alora_destroy.restype = None
 _lib.alora_destroy.argtypes = [C.c_void_p]
 _lib.alora_default_params.restype = None
+_lib.alora_preset_params.restype = None
+_lib.alora_preset_params.argtypes = [C.c_void_p, C.c_int]
 _vp, _i32, _i64, _dbl = C.c_void_p, C.c_int32, C.c_int64, C.c_double
 _lib.alora_create.argtypes = [C.POINTER(_Problem), C.c_int, C.c_int, _vp, C.POINTER(_vp)]
 _lib.alora_info.argtypes = [_vp, _vp]
@@ -84,12 +98,13 @@ _lib.alora_eval.argtypes = [_vp, _vp, _i32, _i64, _vp, _vp, _vp]
 _lib.alora_get_stats.argtypes = [_vp, _vp]
 _lib.alora_get_lambda.argtypes = [_vp, _vp]
 _lib.alora_eval_host.argtypes = [_vp, _vp, _i32, _i64, _vp, _vp, _vp]
-_lib.alora_linesearch.argtypes = [_vp, _vp, _vp, _i32, _i64, _vp]
+_lib.alora_step_host.argtypes = [_vp, _vp, _vp, _vp, _i32, _i64, _vp, _vp, _vp, _vp, _vp, _vp]
+_lib.alora_linesearch.argtypes = [_vp, _vp, _vp, _i32, _i64, _i32, _vp]
 _lib.alora_get_linesearch.argtypes = [_vp, _vp]
 _lib.alora_smatvec.argtypes = [_vp, _vp, _vp, _i32, _vp, _vp]
 _lib.alora_kernel_timing.argtypes = [_vp, C.c_int]
 _lib.alora_kernel_timing_read.argtypes = [_vp, _vp, _vp]
-_lib.alora_lanczos.argtypes = [_vp, _vp, _i32, _dbl, C.c_uint64, _vp, _vp, _vp, _vp]
+_lib.alora_lanczos.argtypes = [_vp, _vp, _i32, _dbl, C.c_uint64, _i32, _vp, _vp, _vp, _vp, _vp]
 _lib.alora_solve.argtypes = [_vp, C.POINTER(Params), _vp, _vp, _i32, _vp, _vp, _vp, _i32, _vp]
 
 
@@ -184,9 +199,18 @@ class Context:
         self._chk(_lib.alora_eval_host(self._h, _ptr(R_host), r, ld, _ptr(G_host), _ptr(z_host), out.ctypes.data))
         return out
 
-    def linesearch(self, R, D, r: int, ld: int, fetch: bool = True):
+    def step_host(self, R_host, D_host, V_host, r: int, ld: int, G_host=None, z_host=None, W_host=None):
+        """One whole step (f + grad, line-search coefficients, S(lambda) V) through HOST buffers.
+        Returns (stats[8], p[5], <V,W>)."""
+        st, p, vw = np.zeros(8), np.zeros(5), C.c_double()
+        self._chk(_lib.alora_step_host(self._h, _ptr(R_host), _ptr(D_host), _ptr(V_host), r, ld, _ptr(G_host), _ptr(z_host),
+                                       _ptr(W_host), st.ctypes.data, p.ctypes.data, C.addressof(vw)))
+        return st, p, vw.value
+
+    def linesearch(self, R, D, r: int, ld: int, fetch: bool = True, warm: bool = False):
+        """warm=True: the ctx still holds an alora_eval of this same R (same tensor, r, ld, dual)."""
         out = np.zeros(5) if fetch else None
-        self._chk(_lib.alora_linesearch(self._h, _ptr(R), _ptr(D), r, ld, _ptr(out)))
+        self._chk(_lib.alora_linesearch(self._h, _ptr(R), _ptr(D), r, ld, 1 if warm else 0, _ptr(out)))
         return out
 
     def get_linesearch(self):
@@ -208,12 +232,18 @@ class Context:
         self._chk(_lib.alora_kernel_timing_read(self._h, C.addressof(ms), C.addressof(cnt)))
         return ms.value, cnt.value
 
-    def lanczos(self, mu, kmax: int, tol_abs: float, seed: int, v=None):
-        theta, resid, k = C.c_double(), C.c_double(), C.c_int32()
-        st = self._chk(_lib.alora_lanczos(self._h, _ptr(mu), kmax, float(tol_abs), C.c_uint64(seed),
-                                          C.addressof(theta), _ptr(v), C.addressof(k), C.addressof(resid)),
+    def lanczos(self, mu, kmax: int, tol_abs: float, seed: int, v=None, p_want: int = 1):
+        """p_want == 1: returns (theta, k_used, resid, converged); v: device [n] or None.
+        p_want > 1: returns (theta[p_found], k_used, resid[p_found], converged); v: device buffer of p_want * n
+        elements (Ritz vector j at v[j*n:(j+1)*n]) or None.  mu=None: lambda of the last eval."""
+        theta, resid = np.zeros(p_want), np.zeros(p_want)
+        k, pf = C.c_int32(), C.c_int32()
+        st = self._chk(_lib.alora_lanczos(self._h, _ptr(mu), kmax, float(tol_abs), C.c_uint64(seed), p_want,
+                                          theta.ctypes.data, _ptr(v), C.addressof(pf), C.addressof(k), resid.ctypes.data),
                        allow=(ENOTCONV,))
-        return theta.value, k.value, resid.value, st == OK
+        if p_want == 1:
+            return float(theta[0]), k.value, float(resid[0]), st == OK
+        return theta[: pf.value].copy(), k.value, resid[: pf.value].copy(), st == OK
 
     def solve(self, params: Params, R, r: int, r_cap: int, y, sigma: float, log_cap: int = 256):
         """Returns (Result, [IterRecord], r_final, sigma_final, converged)."""

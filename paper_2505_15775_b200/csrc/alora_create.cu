@@ -361,6 +361,9 @@ extern "C" void alora_destroy(alora_ctx* c) {
   cudaSetDevice(c->device);
   free_solve_workspace(c);
   for (cudaEvent_t e : c->ev) cudaEventDestroy(e);
+  if (c->ev_eval) cudaEventDestroy(c->ev_eval);
+  if (c->ev_down) cudaEventDestroy(c->ev_down);
+  if (c->stream2) cudaStreamDestroy(c->stream2);
   c->pool.free_all();
   if (c->pinned) cudaFreeHost(c->pinned);
   if (c->pinR) cudaFreeHost(c->pinR);
@@ -386,6 +389,7 @@ extern "C" alora_status alora_create(const alora_problem* P, alora_dtype dtype, 
   if (!c) return ALORA_ENOMEM;
   c->device = device; c->stream = (cudaStream_t)cuda_stream; c->dtype = dtype;
   c->esz = dtype == ALORA_F32 ? 4 : 8; c->n = P->n; c->m = P->m;
+  if (const char* e = std::getenv("ALORA_CW")) c->cw = std::atoi(e) != 0;   // measurement switch
   std::memset(c->occ_cache, 0, sizeof(c->occ_cache));
   std::memset(c->occ_ld, 0, sizeof(c->occ_ld));
   cudaDeviceProp prop;
@@ -416,6 +420,9 @@ extern "C" alora_status alora_create(const alora_problem* P, alora_dtype dtype, 
   }
   c->ls_dev = c->stats_dev + kNStat;
   c->mv_dev = c->stats_dev + 2 * kNStat;
+  // the uploads and memsets above ran on the legacy default stream; the ctx stream may be a non-blocking one that
+  // is not ordered against it, so everything is made complete before the first call can enqueue work
+  if (cudaDeviceSynchronize() != cudaSuccess) { fail(c, ALORA_ECUDA, "cudaDeviceSynchronize failed at the end of alora_create"); return bail(ALORA_ECUDA); }
   *out = c;
   return ALORA_OK;
 }
@@ -433,6 +440,6 @@ extern "C" alora_status alora_set_dual(alora_ctx* c, const double* y_dev, double
   if (!c) return ALORA_EINVAL;
   if ((!y_dev && c->m > 0) || !(sigma > 0.0) || !std::isfinite(sigma))
     return fail(c, ALORA_EINVAL, "alora_set_dual: need y_dev != NULL and finite sigma > 0");
-  c->y = y_dev; c->sigma = sigma; c->have_dual = true; c->have_eval = false;
+  c->y = y_dev; c->sigma = sigma; c->have_dual = true; c->have_eval = false; c->last_eval_R = nullptr;
   return ALORA_OK;
 }

@@ -122,6 +122,22 @@ int pick_vec(const alora_ctx* c, int64_t ld, const void* p0, const void* p1, con
   return 1;
 }
 
+// mu_dev == NULL in alora_smatvec / alora_lanczos: lambda = y - sigma (z - b) of the last alora_eval.
+// The general class wrote it during that evaluation (c->lam); the diagonal class never stores it (it is formed and
+// consumed inside the fused pass), so it is recomputed here from that evaluation's z.
+alora_status resolve_mu(alora_ctx* c, const double** mu, const char* who) {
+  if (*mu || c->m == 0) return ALORA_OK;
+  if (!c->have_eval) return fail(c, ALORA_ESTATE, std::string(who) + ": mu_dev == NULL needs a preceding alora_eval");
+  if (c->cls == 1) { *mu = c->lam; return ALORA_OK; }
+  if (!c->lam_auto) ALORA_CUDA(c, c->pool.alloc((void**)&c->lam_auto, sizeof(double) * c->m));
+  const int grid = (int)std::max<int64_t>(1, std::min<int64_t>((c->m + 255) / 256, (int64_t)c->num_sms * 8));
+  k_lambda<<<grid, 256, 0, c->stream>>>(c->m, c->y, c->z_last, c->b, c->sigma, c->lam_auto);
+  c->launches++;
+  ALORA_CUDA(c, cudaGetLastError());
+  *mu = c->lam_auto;
+  return ALORA_OK;
+}
+
 }  // namespace alora
 
 // ---------------------------------------------------------------------------------------------
@@ -196,7 +212,14 @@ alora_status launch_diag_rows(alora_ctx* c, int vec, int nvec, int exact, int sh
   const int grid = (int)std::max<int64_t>(1, std::min<int64_t>(tiles, std::min<int64_t>((int64_t)c->num_sms * occ, c->part_cap / 2)));
   a.tiles = tiles;
   a.fin = make_fin(c, a.partials, grid, nullptr, 0, nullptr, 0, out);
-  ALORA_CUDA(c, launch_tiled(vec, shape, mode, full, c->ell_wide ? 1 : 0, a, grid, c->stream));
+  {
+    const cudaError_t e = launch_tiled(vec, shape, mode, full, c->ell_wide ? 1 : 0, a, grid, c->stream, c->device);
+    if (e != cudaSuccess)
+      return fail(c, ALORA_ECUDA, std::string("tiled row kernel launch: ") + cudaGetErrorString(e) + " (vec " + std::to_string(vec) +
+                  ", shape " + std::to_string(shape) + ", mode " + std::to_string(mode) + ", full " + std::to_string(full) +
+                  ", grid " + std::to_string(grid) + ", blocks/SM " + std::to_string(occ) + ", smem " +
+                  std::to_string(tiled_smem_bytes(gs, (int)c->esz, a.ld, mode, c->ell_wide)) + ")");
+  }
   c->launches++;
   return ALORA_OK;
 }
@@ -217,7 +240,17 @@ template <typename T> alora_status launch_adj_general(alora_ctx* c, const Geo& g
     ALORA_CUDA(c, launch_rows_seg(g.vec, g.shape, a, gs, c->stream));
     c->launches++;
   }
-  if ((c->ep && g.nvec == 1 && !c->row_perm) || c->ep_wide) {
+  if (c->cw && g.nvec <= 32) {
+    // cooperative warp per row (k_rows_cw): coalesced entry metadata, one request per gathered row
+    int pl2 = 0; while ((1 << pl2) < g.nvec) ++pl2;
+    int& occ = c->occ_cw[vec_slot(g.vec)][pl2];
+    if (!occ) occ = std::max(1, occ_rows_cw(T(), g.vec, g.nvec));
+    const int64_t need = (c->n + kBlock / 32 - 1) / (kBlock / 32);
+    const int grid = (int)std::max<int64_t>(1, std::min<int64_t>(need, std::min<int64_t>((int64_t)c->num_sms * occ, c->part_cap)));
+    a.perm = c->row_perm;
+    a.fin = make_fin(c, a.fin.p[0], grid, a.fin.p[1], a.fin.n[1], a.fin.p[2], a.fin.n[2], out);
+    ALORA_CUDA(c, launch_rows_cw(g.vec, a, grid, c->stream));
+  } else if ((c->ep && g.nvec == 1 && !c->row_perm) || c->ep_wide) {
     // very long rows of thin vectors (matrix completion, r <= 8 packs): every lane owns whole rows, 32 entry lanes
     const int eshape = (c->ep_wide && g.nvec > 1 && g.nvec <= 4) ? 7 : (c->ep_wide && g.nvec > 4 && g.nvec <= 8) ? 8 : g.shape;
     int& occ = c->occ_cache[vec_slot(g.vec)][eshape == g.shape ? g.shape : eshape - 7][eshape == g.shape ? 11 : 7];
@@ -290,6 +323,42 @@ template <typename T> alora_status lowrank(alora_ctx* c, const T* X, int r, int6
   return ALORA_OK;
 }
 
+// Forward pass of the general class with the cooperative entry kernel: k_ent_cw over the entries, then (unless every
+// constraint is a single entry) k_cons_fin per short constraint and k_long_fin_e per long one.  `nent` entries are
+// walked (the constraint entries; for the line search C's sym-upper list as well).  The partial rows land in
+// part_cons (*ge rows), part_chunk (*gf rows) and part_long (nlong_A rows); `last_fin`, if given, is attached to the
+// last kernel launched (the line search ends here; an evaluation ends with the adjoint pass).
+template <typename T>
+alora_status forward_cw(alora_ctx* c, const Geo& g, int mode, ConsArgs<T>& ca, int64_t nent, int* ge, int* gf, double* last_out) {
+  const int K = 3;
+  const size_t need = (size_t)std::max<int64_t>(1, c->nf_A) * K * c->esz;
+  if (!c->e_out) ALORA_CUDA(c, c->pool.alloc(&c->e_out, need));
+  ca.nent = nent; ca.nf_A = c->nf_A; ca.e_out = (T*)c->e_out; ca.long_cons = c->long_cons;
+  const bool single = c->single_entry, fin_k = !single && c->m > 0, longs = fin_k && c->nlong_A > 0;
+  *ge = (int)std::max<int64_t>(1, std::min<int64_t>((nent + kBlock - 1) / kBlock, std::min<int64_t>((int64_t)c->num_sms * 8, c->part_cap)));
+  *gf = fin_k ? (int)std::max<int64_t>(1, std::min<int64_t>((c->m + kBlock - 1) / kBlock, std::min<int64_t>((int64_t)c->num_sms * 8, c->part_cap))) : 0;
+  auto fin_all = [&]() { return make_fin(c, c->part_cons, *ge, c->part_chunk, *gf, c->part_long, longs ? c->nlong_A : 0, last_out); };
+  ca.partials = c->part_cons; ca.part_chunk = c->part_chunk;
+  ca.fin = (last_out && !fin_k) ? fin_all() : no_fin();
+  ALORA_CUDA(c, launch_ent_cw(g.vec, mode, single ? 1 : 0, ca, *ge, c->stream));
+  c->launches++;
+  if (fin_k) {
+    ca.fin = (last_out && !longs) ? fin_all() : no_fin();
+    if (mode == CONS_EVAL) k_cons_fin<T, CONS_EVAL><<<*gf, kBlock, 0, c->stream>>>(ca);
+    else k_cons_fin<T, CONS_LS><<<*gf, kBlock, 0, c->stream>>>(ca);
+    c->launches++;
+    if (longs) {
+      ca.fin = last_out ? fin_all() : no_fin();
+      if (mode == CONS_EVAL) k_long_fin_e<T, CONS_EVAL><<<c->nlong_A, kBlock, 0, c->stream>>>(ca, c->part_long);
+      else k_long_fin_e<T, CONS_LS><<<c->nlong_A, kBlock, 0, c->stream>>>(ca, c->part_long);
+      c->launches++;
+    }
+  }
+  ca.fin = no_fin();
+  ALORA_CUDA(c, cudaGetLastError());
+  return ALORA_OK;
+}
+
 template <typename T> alora_status eval_impl(alora_ctx* c, const T* R, int32_t r, int64_t ld, T* G, double* z_dev) {
   Geo g;
   alora_status s = geometry(c, r, ld, R, G, nullptr, g);
@@ -311,6 +380,22 @@ template <typename T> alora_status eval_impl(alora_ctx* c, const T* R, int32_t r
     fill_cons(c, ca, g, R, (const T*)nullptr, r, ld);
     ca.z = zout;
     int gc = 0;
+    if (c->cw && g.nvec <= 32 && c->m > 0) {
+      int ge = 0, gf = 0;
+      s = forward_cw<T>(c, g, CONS_EVAL, ca, c->nf_A, &ge, &gf, nullptr);
+      if (s != ALORA_OK) return s;
+      a.w = c->lam; a.diag_class = 0;
+      const bool fin_k = !c->single_entry;
+      a.fin = make_fin(c, c->part_rows, 0, fin_k ? c->part_chunk : c->part_cons, fin_k ? gf : ge, c->part_long,
+                       (fin_k && c->nlong_A > 0) ? c->nlong_A : 0, nullptr);   // last kernel of the call
+      time_mark(c);
+      s = launch_adj_general<T>(c, g, a, c->stats_dev);
+      if (s != ALORA_OK) return s;
+      time_mark(c);
+      ALORA_CUDA(c, cudaGetLastError());
+      c->z_last = zout; c->have_eval = true;
+      return ALORA_OK;
+    }
     if (c->m > 0) {
       if (c->single_entry || c->short_cons) {
         gc = (int)std::min<int64_t>((c->m + kBlock - 1) / kBlock, std::min<int64_t>((int64_t)c->num_sms * 8, c->part_cap));
@@ -377,6 +462,13 @@ template <typename T> alora_status ls_impl(alora_ctx* c, const T* R, const T* D,
     }
     ConsArgs<T> ca;
     fill_cons(c, ca, g, R, D, r, ld);
+    if (c->cw && g.nvec <= 32 && c->nf_A + c->nf_C > 0) {
+      int ge = 0, gf = 0;
+      s = forward_cw<T>(c, g, CONS_LS, ca, c->nf_A + c->nf_C, &ge, &gf, c->ls_dev);
+      if (s != ALORA_OK) return s;
+      c->have_ls = true;
+      return ALORA_OK;
+    }
     // launches: k_cons (short constraints), k_cons_chunk (chunks of long constraints and of C's list),
     // k_long_finish (long constraints); whichever comes last also does the final sum
     const bool chunks = c->nchunk_all > 0, longs = c->nlong_A > 0;
@@ -414,6 +506,7 @@ template <typename T> alora_status ls_impl(alora_ctx* c, const T* R, const T* D,
 
 alora_status fetch_ls(alora_ctx* c, int r, double p[5]) {
   ALORA_CUDA(c, cudaMemcpyAsync(c->pinned, c->ls_dev, sizeof(double) * kNStat, cudaMemcpyDeviceToHost, c->stream));
+  if (c->ls_warm) ALORA_CUDA(c, cudaMemcpyAsync(c->pinned + 16, c->ls_warm_stats, sizeof(double) * kNStat, cudaMemcpyDeviceToHost, c->stream));
   const bool lr = c->pC && c->cls == 1;
   if (lr) {
     ALORA_CUDA(c, cudaMemcpyAsync(c->pinned + 64, c->TmR, sizeof(double) * c->pC * r, cudaMemcpyDeviceToHost, c->stream));
@@ -431,6 +524,12 @@ alora_status fetch_ls(alora_ctx* c, int r, double p[5]) {
     }
   const double sg = c->sigma;
   p[0] = cRR - s[LS_YQ] + 0.5 * sg * s[LS_QQ];
+  if (c->ls_warm) {   // p0 = f(R) of the evaluation the caller vouched for (its <C,RR^T> already holds the low-rank term)
+    const double* e = c->pinned + 16;
+    double cx = e[ES_CX];
+    if (lr) for (int q = 0; q < c->pC; ++q) { const double* tr = s + 64 + q * r; double rr = 0; for (int k = 0; k < r; ++k) rr += tr[k] * tr[k]; cx += c->s_host[q] * rr; }
+    p[0] = cx - e[ES_YQ] + 0.5 * sg * e[ES_QQ];
+  }
   p[1] = 2.0 * cRD - s[LS_YQ1] + sg * s[LS_QQ1];
   p[2] = cDD - s[LS_YQ2] + 0.5 * sg * s[LS_Q11] + sg * s[LS_QQ2];
   p[3] = sg * s[LS_Q12];
@@ -471,7 +570,7 @@ extern "C" alora_status alora_eval(alora_ctx* c, const void* R, int32_t r, int64
   alora_status s = c->dtype == ALORA_F32 ? eval_impl<float>(c, (const float*)R, r, ld, (float*)G, z_dev)
                                          : eval_impl<double>(c, (const double*)R, r, ld, (double*)G, z_dev);
   if (s != ALORA_OK) return s;
-  c->last_eval_r = r;
+  c->last_eval_r = r; c->last_eval_R = R; c->last_eval_ld = ld;
   return stats ? fetch_stats(c, r, stats) : ALORA_OK;
 }
 
@@ -513,14 +612,73 @@ extern "C" alora_status alora_eval_host(alora_ctx* c, const void* R_host, int32_
   return fetch_stats(c, r, stats);
 }
 
-extern "C" alora_status alora_linesearch(alora_ctx* c, const void* R, const void* D, int32_t r, int64_t ld, double p[5]) {
+extern "C" alora_status alora_step_host(alora_ctx* c, const void* R_host, const void* D_host, const void* V_host, int32_t r,
+                                        int64_t ld, void* G_host, double* z_host, void* W_host, double stats[8], double p[5],
+                                        double* vw) {
+  if (!c || !R_host || !D_host || !V_host || !stats || !p || !vw) return c ? fail(c, ALORA_EINVAL, "alora_step_host: NULL argument") : ALORA_EINVAL;
+  if (r < 1 || ld < r) return fail(c, ALORA_EINVAL, "need 1 <= r <= ld");
+  if (!c->have_dual) return fail(c, ALORA_ESTATE, "alora_step_host before alora_set_dual");
+  ALORA_CUDA(c, cudaSetDevice(c->device));
+  const size_t nb = (size_t)c->n * (size_t)ld * c->esz, nv = (size_t)c->n * c->esz;
+  if (nb > c->stage_bytes) {
+    if (c->stageR) { c->pool.release(c->stageR); c->pool.release(c->stageG); }
+    ALORA_CUDA(c, c->pool.alloc(&c->stageR, nb));
+    ALORA_CUDA(c, c->pool.alloc(&c->stageG, nb));
+    c->stage_bytes = nb;
+  }
+  if (nb > c->stage2_bytes) {
+    if (c->stageD) { c->pool.release(c->stageD); c->pool.release(c->stageV); c->pool.release(c->stageW); }
+    ALORA_CUDA(c, c->pool.alloc(&c->stageD, nb));
+    ALORA_CUDA(c, c->pool.alloc(&c->stageV, nv));
+    ALORA_CUDA(c, c->pool.alloc(&c->stageW, nv));
+    c->stage2_bytes = nb;
+  }
+  if (!c->stream2) {
+    ALORA_CUDA(c, cudaStreamCreateWithFlags(&c->stream2, cudaStreamNonBlocking));
+    ALORA_CUDA(c, cudaEventCreateWithFlags(&c->ev_eval, cudaEventDisableTiming));
+    ALORA_CUDA(c, cudaEventCreateWithFlags(&c->ev_down, cudaEventDisableTiming));
+  }
+  // ctx stream: R up, f + grad, D and V up (the host-to-device engine is free again while G comes down), line search,
+  // matvec, W down.  stream2: G and z down as soon as f + grad is done.
+  ALORA_CUDA(c, cudaMemcpyAsync(c->stageR, R_host, nb, cudaMemcpyHostToDevice, c->stream));
+  alora_status s = alora_eval(c, c->stageR, r, ld, G_host ? c->stageG : nullptr, nullptr, nullptr);
+  if (s != ALORA_OK) return s;
+  ALORA_CUDA(c, cudaEventRecord(c->ev_eval, c->stream));
+  ALORA_CUDA(c, cudaStreamWaitEvent(c->stream2, c->ev_eval, 0));
+  if (G_host) ALORA_CUDA(c, cudaMemcpyAsync(G_host, c->stageG, nb, cudaMemcpyDeviceToHost, c->stream2));
+  if (z_host) ALORA_CUDA(c, cudaMemcpyAsync(z_host, c->z_int, sizeof(double) * c->m, cudaMemcpyDeviceToHost, c->stream2));
+  ALORA_CUDA(c, cudaEventRecord(c->ev_down, c->stream2));
+  ALORA_CUDA(c, cudaMemcpyAsync(c->stageD, D_host, nb, cudaMemcpyHostToDevice, c->stream));
+  ALORA_CUDA(c, cudaMemcpyAsync(c->stageV, V_host, nv, cudaMemcpyHostToDevice, c->stream));
+  s = alora_linesearch(c, c->stageR, c->stageD, r, ld, 1, nullptr);
+  if (s != ALORA_OK) return s;
+  s = alora_smatvec(c, nullptr, c->stageV, 1, c->stageW, nullptr);
+  if (s != ALORA_OK) return s;
+  if (W_host) ALORA_CUDA(c, cudaMemcpyAsync(W_host, c->stageW, nv, cudaMemcpyDeviceToHost, c->stream));
+  ALORA_CUDA(c, cudaMemcpyAsync(c->pinned + 32, c->mv_dev, sizeof(double) * kNStat, cudaMemcpyDeviceToHost, c->stream));
+  ALORA_CUDA(c, cudaStreamWaitEvent(c->stream, c->ev_down, 0));   // the call's results are complete when the ctx stream is
+  s = fetch_stats(c, r, stats);            // synchronises the ctx stream
+  if (s != ALORA_OK) return s;
+  *vw = c->pinned[32 + ES_GR];
+  return fetch_ls(c, r, p);
+}
+
+extern "C" alora_status alora_linesearch(alora_ctx* c, const void* R, const void* D, int32_t r, int64_t ld, int32_t warm,
+                                         double p[5]) {
   if (!c || !R || !D) return c ? fail(c, ALORA_EINVAL, "alora_linesearch: NULL argument") : ALORA_EINVAL;
   if (!c->have_dual) return fail(c, ALORA_ESTATE, "alora_linesearch before alora_set_dual");
+  if (warm && !(c->have_eval && c->last_eval_R == R && c->last_eval_r == r && c->last_eval_ld == ld))
+    return fail(c, ALORA_ESTATE, "alora_linesearch(warm): no alora_eval of this R (same pointer, r, ld, dual) is on record");
   ALORA_CUDA(c, cudaSetDevice(c->device));
   alora_status s = c->dtype == ALORA_F32 ? ls_impl<float>(c, (const float*)R, (const float*)D, r, ld)
                                          : ls_impl<double>(c, (const double*)R, (const double*)D, r, ld);
   if (s != ALORA_OK) return s;
   c->last_ls_r = r;
+  c->ls_warm = warm != 0;
+  if (warm) {   // the evaluation's scalars, taken now (a later alora_eval overwrites stats_dev); device-to-device, capturable
+    if (!c->ls_warm_stats) ALORA_CUDA(c, c->pool.alloc((void**)&c->ls_warm_stats, sizeof(double) * kNStat));
+    ALORA_CUDA(c, cudaMemcpyAsync(c->ls_warm_stats, c->stats_dev, sizeof(double) * kNStat, cudaMemcpyDeviceToDevice, c->stream));
+  }
   return p ? fetch_ls(c, r, p) : ALORA_OK;
 }
 
@@ -531,10 +689,12 @@ extern "C" alora_status alora_get_linesearch(alora_ctx* c, double p[5]) {
 }
 
 extern "C" alora_status alora_smatvec(alora_ctx* c, const double* mu_dev, const void* V, int32_t p, void* W, double* vw) {
-  if (!c || !V || !W || (!mu_dev && c->m > 0)) return c ? fail(c, ALORA_EINVAL, "alora_smatvec: NULL argument") : ALORA_EINVAL;
+  if (!c || !V || !W) return c ? fail(c, ALORA_EINVAL, "alora_smatvec: NULL argument") : ALORA_EINVAL;
   if (V == W) return fail(c, ALORA_EINVAL, "W must not alias V");
   ALORA_CUDA(c, cudaSetDevice(c->device));
-  alora_status s = c->dtype == ALORA_F32 ? matvec_impl<float>(c, mu_dev, (const float*)V, p, (float*)W)
+  alora_status s = resolve_mu(c, &mu_dev, "alora_smatvec");
+  if (s != ALORA_OK) return s;
+  s = c->dtype == ALORA_F32 ? matvec_impl<float>(c, mu_dev, (const float*)V, p, (float*)W)
                                          : matvec_impl<double>(c, mu_dev, (const double*)V, p, (double*)W);
   if (s != ALORA_OK) return s;
   if (vw) {

@@ -14,20 +14,23 @@ namespace alora {
 // device array with byte accounting
 struct DevPool {
   std::vector<void*> ptrs;
+  std::vector<size_t> sizes;
   size_t bytes = 0;
   cudaError_t alloc(void** p, size_t nbytes) {
     *p = nullptr;
     if (nbytes == 0) nbytes = 16;
     cudaError_t e = cudaMalloc(p, nbytes);
-    if (e == cudaSuccess) { ptrs.push_back(*p); bytes += nbytes; }
+    if (e == cudaSuccess) { ptrs.push_back(*p); sizes.push_back(nbytes); bytes += nbytes; }
     return e;
   }
   void release(void* p) {
-    for (auto& q : ptrs) if (q == p) { cudaFree(q); q = nullptr; }
+    if (!p) return;
+    for (size_t i = 0; i < ptrs.size(); ++i)
+      if (ptrs[i] == p) { cudaFree(p); bytes -= sizes[i]; ptrs[i] = nullptr; sizes[i] = 0; }
   }
   void free_all() {
     for (void* p : ptrs) if (p) cudaFree(p);
-    ptrs.clear();
+    ptrs.clear(); sizes.clear(); bytes = 0;
   }
 };
 
@@ -53,6 +56,8 @@ struct alora_ctx {
   int* dcons = nullptr; void* da = nullptr;
   // identity diagonal class: padded ELL blocks (rows_tiled.cuh): kUN first neighbours per row, kUNL last
   // upper-triangle neighbours per row, and per 32-row block a flag "some row has more"
+  bool cw = false;         // general class: cooperative entry / row kernels (k_ent_cw, k_rows_cw); ALORA_CW=1 turns them on
+  int occ_cw[3][6] = {};
   bool ell_wide = false;   // 8 / 6 slots per row instead of 4 / 3 (more than 10 % of the rows have degree > 4)
   int* ell_col = nullptr; void* ell_val = nullptr;
   int* ellu_col = nullptr; void* ellu_val = nullptr;
@@ -75,6 +80,7 @@ struct alora_ctx {
   int64_t* ch_beg = nullptr; int64_t* ch_end = nullptr; int64_t nchunk_A = 0, nchunk_all = 0;
   int* long_cons = nullptr; int64_t* long_chptr = nullptr; int nlong_A = 0;
   double* ch_out = nullptr;
+  void* e_out = nullptr;      // per-entry sums of the cooperative forward evaluator (nf_A x 3, ctx dtype), on first use
   // vectors
   double* b = nullptr; const double* y = nullptr; double sigma = 0.0; bool have_dual = false;
   double* z_int = nullptr; double* lam = nullptr; const double* z_last = nullptr;
@@ -91,9 +97,14 @@ struct alora_ctx {
   double* pinned = nullptr;  // 64 doubles
   bool have_eval = false, have_ls = false;
   int last_eval_r = 0, last_ls_r = 0;
+  const void* last_eval_R = nullptr; int64_t last_eval_ld = 0;   // what a warm alora_linesearch must match
+  bool ls_warm = false; double* ls_warm_stats = nullptr;          // copy of the evaluation's scalars taken by a warm call
+  double* lam_auto = nullptr;   // diagonal class: lambda of the last evaluation, formed on demand (mu_dev == NULL)
   int64_t launches = 0;
   // staging for alora_eval_host
   void* stageR = nullptr; void* stageG = nullptr; size_t stage_bytes = 0;
+  void* stageD = nullptr; void* stageV = nullptr; void* stageW = nullptr; size_t stage2_bytes = 0;   // alora_step_host
+  cudaStream_t stream2 = nullptr; cudaEvent_t ev_eval = nullptr, ev_down = nullptr;                  // second copy stream
   void* pinR = nullptr; size_t pin_bytes = 0;
   // occupancy cache [vec idx][shape][kind]
   int occ_cache[3][7][12];
@@ -115,6 +126,7 @@ alora_status fail(alora_ctx* c, alora_status s, const std::string& msg);
   } while (0)
 
 // alora_ctx.cu
+alora_status resolve_mu(alora_ctx* c, const double** mu, const char* who);   // NULL -> lambda of the last alora_eval
 int pick_vec(const alora_ctx* c, int64_t ld, const void* p0, const void* p1, const void* p2);
 void free_solve_workspace(alora_ctx* c);
 

@@ -87,6 +87,7 @@ __global__ void __launch_bounds__(kBlock) k_make_pair(int64_t N, double alpha, c
 // blocks change by one row / column per iteration (the new pair).  So an iteration needs two passes over the
 // vectors instead of 4m + 6: k_lbfgs_dots (build the new pair, all new dot products) and k_lbfgs_combine.
 constexpr int kLbMax = 8;            // pairs the fused path handles (memory <= kLbMax - 1)
+constexpr int kMemMax = 16;          // largest lbfgs_mem (larger values are clamped); sizes SolveWorkspace::buf
 constexpr int kLbW = 48;             // doubles per partial row (5 * kLbMax + 1 sums, padded)
 struct LbVecs { const void* S[kLbMax]; const void* Y[kLbMax]; };
 struct LbCoef { double cg; double cs[kLbMax]; double cy[kLbMax]; };
@@ -311,7 +312,8 @@ struct SolveWorkspace {
   double* red_part = nullptr; double* red_out = nullptr;
   double* lb_part = nullptr; double* lb_out = nullptr;   // k_lbfgs_dots partial rows / result
   // solve
-  void* buf[4 + 2 * 16] = {}; int nbuf = 0; int64_t buf_elems = 0;
+  static constexpr int kNBuf = 5 + 2 * (kMemMax + 1);   // R, G, D, Gprev, Rtmp + (mem + 1) slots each of S and Y
+  void* buf[kNBuf] = {}; int nbuf = 0; int64_t buf_elems = 0;
   double* lam = nullptr; double* z = nullptr; double* zv = nullptr; void* ritz = nullptr;
   double* gram_part = nullptr; double* gram = nullptr; double* Qdev = nullptr;
   void* ritzp = nullptr; void* vtmp = nullptr; double* cab = nullptr;   // p_max > 1: Ritz vectors (4 x n), v_a + v_b, c_ab (11 x m)
@@ -628,7 +630,7 @@ template <typename T> alora_status dot1(alora_ctx* c, int64_t N, const T* x, con
 template <typename T>
 alora_status lanczos_impl(alora_ctx* c, const double* mu, int kmax, double tol_abs, uint64_t seed, double* theta_out,
                           T* v_out, int* k_used, double* resid_out, int* n_matvec, int p_want = 1,
-                          std::vector<double>* thetas = nullptr, T* U_out = nullptr) {
+                          std::vector<double>* thetas = nullptr, T* U_out = nullptr, std::vector<double>* resids = nullptr) {
   alora_status s = ensure_ws(c);
   if (s != ALORA_OK) return s;
   SolveWorkspace* w = c->ws;
@@ -651,7 +653,7 @@ alora_status lanczos_impl(alora_ctx* c, const double* mu, int kmax, double tol_a
   k_scale<T><<<g, 256, 0, c->stream>>>(n, 1.0 / std::sqrt(nrm2), V);
   c->launches++;
   std::vector<double> al, be, sv;
-  double theta = 0.0, resid = INFINITY;
+  double theta = 0.0, resid = INFINITY, beta_last = 0.0;
   int k = 0;
   bool conv = false;
   while (true) {
@@ -671,6 +673,7 @@ alora_status lanczos_impl(alora_ctx* c, const double* mu, int kmax, double tol_a
     double b2;
     s = dot1<T>(c, n, wv, wv, &b2); if (s != ALORA_OK) return s;
     const double beta = std::sqrt(b2);
+    beta_last = beta;
     ++k;
     tridiag_smallest(al, be, k, theta, sv);
     resid = std::fabs(beta * sv[k - 1]);
@@ -693,16 +696,20 @@ alora_status lanczos_impl(alora_ctx* c, const double* mu, int kmax, double tol_a
     c->launches++;
     ALORA_CUDA(c, cudaStreamSynchronize(c->stream));  // sv is about to go out of scope
   }
-  if (p_want > 1 && thetas && U_out) {
+  if (p_want > 1 && thetas) {
     // reading 29: the min(p_want, k) smallest Ritz pairs of the same k-step tridiagonal; vector j at U_out + j n
+    // (U_out == nullptr: values and residual estimates only)
     if (k > 1 && (int)be.size() >= k) be.resize(k - 1);
     const int pw = std::min(p_want, k);
     thetas->assign(pw, 0.0);
+    if (resids) resids->assign(pw, 0.0);
     std::vector<std::vector<double>> found;
     for (int j = 0; j < pw; ++j) {
       std::vector<double> sj;
       tridiag_jth(al, be, k, j, (*thetas)[j], sj, found);
       found.push_back(sj);
+      if (resids) (*resids)[j] = std::fabs(beta_last * sj[k - 1]);
+      if (!U_out) continue;
       ALORA_CUDA(c, cudaMemcpyAsync(w->cvec, sj.data(), sizeof(double) * k, cudaMemcpyHostToDevice, c->stream));
       T* uj = U_out + (int64_t)j * n;
       k_basis_combine<T><<<g, 256, 0, c->stream>>>(n, k, V, w->cvec, 0.0, 1.0, uj);
@@ -734,14 +741,35 @@ extern "C" void alora_default_params(alora_params* p) {
   p->stall_tol = 0.0; p->stall_iters = 3; p->pad_ = 0;
 }
 
+extern "C" void alora_preset_params(alora_params* p, alora_dtype dtype) {
+  if (!p) return;
+  alora_default_params(p);
+  if (dtype == ALORA_F32) { p->it_max = 100; p->stall_tol = 1e-9; p->stall_iters = 3; }
+}
+
 extern "C" alora_status alora_lanczos(alora_ctx* c, const double* mu_dev, int32_t kmax, double tol_abs, uint64_t seed,
-                                      double* theta, void* v_dev, int32_t* k_used, double* resid) {
-  if (!c || (!mu_dev && c->m > 0) || kmax < 1) return c ? fail(c, ALORA_EINVAL, "alora_lanczos: bad argument") : ALORA_EINVAL;
+                                      int32_t p_want, double* theta, void* V_dev, int32_t* p_found, int32_t* k_used,
+                                      double* resid) {
+  if (!c || kmax < 1 || p_want < 1 || p_want > 8) return c ? fail(c, ALORA_EINVAL, "alora_lanczos: need kmax >= 1 and 1 <= p_want <= 8") : ALORA_EINVAL;
   ALORA_CUDA(c, cudaSetDevice(c->device));
+  alora_status s = resolve_mu(c, &mu_dev, "alora_lanczos");
+  if (s != ALORA_OK) return s;
   int k = 0;
-  alora_status s = c->dtype == ALORA_F32
-      ? lanczos_impl<float>(c, mu_dev, kmax, tol_abs, seed, theta, (float*)v_dev, &k, resid, nullptr)
-      : lanczos_impl<double>(c, mu_dev, kmax, tol_abs, seed, theta, (double*)v_dev, &k, resid, nullptr);
+  double th0 = 0.0, res0 = 0.0;
+  std::vector<double> ths, rss;
+  if (p_want == 1) {
+    s = c->dtype == ALORA_F32
+        ? lanczos_impl<float>(c, mu_dev, kmax, tol_abs, seed, &th0, (float*)V_dev, &k, &res0, nullptr)
+        : lanczos_impl<double>(c, mu_dev, kmax, tol_abs, seed, &th0, (double*)V_dev, &k, &res0, nullptr);
+    ths.assign(1, th0); rss.assign(1, res0);
+  } else {
+    s = c->dtype == ALORA_F32
+        ? lanczos_impl<float>(c, mu_dev, kmax, tol_abs, seed, &th0, (float*)nullptr, &k, &res0, nullptr, p_want, &ths, (float*)V_dev, &rss)
+        : lanczos_impl<double>(c, mu_dev, kmax, tol_abs, seed, &th0, (double*)nullptr, &k, &res0, nullptr, p_want, &ths, (double*)V_dev, &rss);
+  }
+  if (s != ALORA_OK && s != ALORA_ENOTCONV) return s;
+  for (size_t j = 0; j < ths.size(); ++j) { if (theta) theta[j] = ths[j]; if (resid) resid[j] = rss[j]; }
+  if (p_found) *p_found = (int32_t)ths.size();
   if (k_used) *k_used = k;
   return s;
 }
@@ -793,7 +821,7 @@ alora_status solve_impl(alora_ctx* c, const alora_params* prm, T* R_user, int32_
   const int64_t n = c->n, m = c->m;
   const int A = (int)(16 / sizeof(T));                    // columns are padded (with zeros) to 16-byte rows
   auto pad = [&](int r) { return (r + A - 1) / A * A; };
-  const int mem = std::max(0, std::min(prm->lbfgs_mem, 16));
+  const int mem = std::max(0, std::min(prm->lbfgs_mem, kMemMax));
   int r = *r_inout;
   if (r < 1 || r > r_cap) return fail(c, ALORA_EINVAL, "alora_solve: need 1 <= r <= r_cap");
   if (prm->p_max < 1 || prm->p_max > 4) return fail(c, ALORA_EINVAL, "alora_solve: need 1 <= p_max <= 4");
@@ -801,10 +829,15 @@ alora_status solve_impl(alora_ctx* c, const alora_params* prm, T* R_user, int32_
   const int64_t elems = n * (int64_t)ldcap;
   const int nslot = mem + 1;                              // one spare slot receives the candidate pair
   const int nbuf = 5 + 2 * nslot;
+  static_assert(5 + 2 * (kMemMax + 1) <= SolveWorkspace::kNBuf, "SolveWorkspace::buf too small");
   if (w->buf_elems < elems || w->nbuf < nbuf) {
-    for (int i = 0; i < w->nbuf; ++i) c->pool.release(w->buf[i]);
-    for (int i = 0; i < nbuf; ++i) ALORA_CUDA(c, c->pool.alloc(&w->buf[i], sizeof(T) * elems));
-    w->nbuf = nbuf; w->buf_elems = elems;
+    for (int i = 0; i < w->nbuf; ++i) { c->pool.release(w->buf[i]); w->buf[i] = nullptr; }
+    w->nbuf = 0; w->buf_elems = 0;          // an allocation failure below leaves a consistent (empty) workspace
+    for (int i = 0; i < nbuf; ++i) {
+      ALORA_CUDA(c, c->pool.alloc(&w->buf[i], sizeof(T) * elems));
+      w->nbuf = i + 1;
+    }
+    w->buf_elems = elems;
   }
   if (!w->gram) {
     ALORA_CUDA(c, c->pool.alloc((void**)&w->gram_part, sizeof(double) * 256 * 256 * 64));
@@ -961,7 +994,7 @@ alora_status solve_impl(alora_ctx* c, const alora_params* prm, T* R_user, int32_
       }
       if (steepest) { k_scale_copy<T><<<g, 256, 0, c->stream>>>(N, -1.0, Gw, Dw); c->launches++; }
       double p[5];
-      s = alora_linesearch(c, Rw, Dw, ld, ld, p); if (s != ALORA_OK) return s;
+      s = alora_linesearch(c, Rw, Dw, ld, ld, 1, p); if (s != ALORA_OK) return s;   // warm: Rw was just evaluated
       ++n_ls;
       int flag;
       alpha = quartic_argmin(p, &flag);

@@ -96,6 +96,10 @@ template <typename T> struct ConsArgs {
   double* part_chunk;             // chunk kernel: per-block partial rows (sums over C's chunks)
   double* partials;
   FinArgs fin;
+  // cooperative forward evaluator (k_ent_cw / k_cons_fin / k_long_fin_e): entries [0, nent) are walked, the first nf_A
+  // of them belong to constraints (their per-entry sums go to e_out[e][K], K = 1 or 3), the rest to C's sym-upper list
+  int64_t nent, nf_A; T* e_out;
+  const int* long_cons;           // ids of the constraints with more than kLongThreshold entries (one block each)
 };
 
 // ---------------------------------------------------------------------------------------------
@@ -531,6 +535,146 @@ __global__ void __launch_bounds__(kBlock) k_rows_ep(const RowArgs<T> a) {
   finish_partials(a.fin);
 }
 
+// ---------------------------------------------------------------------------------------------
+// Weighted-adjoint SpMM of the general class, cooperative warp per row ("cw").  The thread-per-item kernels of this
+// path are bound by the L1 request pipeline, not by bytes (profiles/r2b_README.md: k_cons1 runs at 85 % of the L1
+// throughput with 9 % of the issue slots used) -- a request is one 128-byte line touched by one warp instruction.  So
+//   * the entry metadata of a row (column, value, constraint id) is read 32 entries at a time, one entry per lane
+//     (coalesced: one request per array per 32 entries instead of one per entry), the weight lambda[cons] is
+//     gathered by the lane that owns the entry, and the lane forms the entry's coefficient c_e or -lambda_i a_e;
+//   * the neighbour rows are then gathered EL = 32 / PL entries per instruction: PL (a power of two >= the packs of
+//     a row) consecutive lanes take the consecutive packs of one row, column and coefficient arriving by shuffle --
+//     one request per gathered row;
+//   * every lane accumulates one pack; the EL partial rows are added by a butterfly once per row.
+// ROWS_ADJ semantics (Out = scale * (C - sum_i w_i A_i) X, <C,XX^T>, |Out|^2, <Out,X>), nvec <= PL.
+template <typename T, int VEC, int PL, int UNR>
+__global__ void __launch_bounds__(kBlock) k_rows_cw(const RowArgs<T> a) {
+  constexpr int WPB = kBlock / 32, NST = 6, EL = 32 / PL;
+  using P = Pack<T, VEC>;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int nvec = a.nvec, r = a.r;
+  const int pl = lane & (PL - 1), el = lane / PL;
+  const bool pok = pl < nvec;                    // this lane owns a pack of the row
+  const bool tailmask = VEC > 1 && !a.exact && pl == nvec - 1;
+  const int64_t ld = a.ld;
+  const T* const Xp = a.X + pl * VEC;            // lane's pack of row 0
+  const T sc = (T)a.scale;
+  double st[NST];
+#pragma unroll
+  for (int s = 0; s < NST; ++s) st[s] = 0.0;
+  auto zero = [] { P z;
+#pragma unroll
+    for (int i = 0; i < VEC; ++i) z.v[i] = T(0);
+    return z; };
+  auto load_pack = [&](const T* p) {   // p points at the lane's pack; elements beyond r zeroed (partial last pack)
+    if (!pok) return zero();
+    P v = ldg_pack<T, VEC>(p);
+    if (tailmask) {
+#pragma unroll
+      for (int i = 0; i < VEC; ++i) if (pl * VEC + i >= r) v.v[i] = T(0);
+    }
+    return v;
+  };
+  for (int64_t pos = (int64_t)blockIdx.x * WPB + warp; pos < a.n; pos += (int64_t)gridDim.x * WPB) {
+    const int64_t row = a.perm ? (int64_t)__ldg(a.perm + pos) : pos;
+    const P x = load_pack(Xp + row * ld);
+    P acc = zero();
+    // one list of entries [beg, end): coefficients val[e] (cons == nullptr) or -w[cons[e]] * val[e]
+    auto walk = [&](const int* __restrict__ col, const T* __restrict__ val, const int* __restrict__ cons, int beg, int end) {
+      for (int base = beg; base < end; base += 32) {
+        const int e = base + lane;
+        int col_l = (int)row; T cf_l = T(0);       // padding entries: the row itself with coefficient 0
+        if (e < end) {
+          col_l = __ldg(col + e);
+          const T v = __ldg(val + e);
+          cf_l = cons ? (T)(-__ldg(a.w + __ldg(cons + e)) * (double)v) : v;
+        }
+        const int cnt = min(32, end - base);
+        for (int j = 0; j < cnt; j += EL * UNR) {
+          P pk[UNR]; T cf[UNR];
+#pragma unroll
+          for (int u = 0; u < UNR; ++u) {
+            const int src = (j + u * EL + el) & 31;
+            const int cu = __shfl_sync(0xffffffffu, col_l, src);
+            cf[u] = __shfl_sync(0xffffffffu, cf_l, src);
+            pk[u] = load_pack(Xp + (int64_t)cu * ld);
+          }
+#pragma unroll
+          for (int u = 0; u < UNR; ++u)
+#pragma unroll
+            for (int i = 0; i < VEC; ++i) acc.v[i] = fma(cf[u], pk[u].v[i], acc.v[i]);
+        }
+      }
+    };
+    const int cb = __ldg(a.c_rowptr + row), ce = __ldg(a.c_rowptr + row + 1);
+    if (a.nseg > 0 && ce - cb > kHeavyRow) {
+      // heavy row: its C part was summed per segment by k_rows_seg; entry lane 0 adds the segment results in order
+      int lo = 0, hi = a.nheavy - 1;
+      while (lo < hi) { const int mid = (lo + hi) >> 1; if (__ldg(a.heavy_rows + mid) < (int)row) lo = mid + 1; else hi = mid; }
+      const int s0 = __ldg(a.heavy_segptr + lo), s1 = __ldg(a.heavy_segptr + lo + 1);
+      if (el == 0) {
+        for (int sg = s0; sg < s1; ++sg) {
+          const P part = load_pack(a.seg_out + (int64_t)sg * (nvec * VEC) + pl * VEC);
+#pragma unroll
+          for (int i = 0; i < VEC; ++i) acc.v[i] += part.v[i];
+        }
+        if (lane == 0) { double t = 0.0; for (int sg = s0; sg < s1; ++sg) t += a.seg_cx[sg]; st[ES_CX] += t; }
+      }
+    } else {
+      walk(a.c_col, a.c_val, nullptr, cb, ce);
+      T cxl = T(0);   // lane-partial <(C_offdiag X)_row, X_row>: every lane holds part of the row sum of its pack
+#pragma unroll
+      for (int i = 0; i < VEC; ++i) cxl = fma(acc.v[i], x.v[i], cxl);
+      st[ES_CX] += (double)cxl;
+    }
+    double coef = 0.0;
+    if (a.diag_class) {
+      const int c = a.dcons ? __ldg(a.dcons + row) : (int)row;
+      if (c >= 0) coef = __ldg(a.w + c) * (a.da ? (double)__ldg(a.da + row) : 1.0);
+    } else {
+      walk(a.a_col, a.a_val, a.a_cons, __ldg(a.a_rowptr + row), __ldg(a.a_rowptr + row + 1));
+    }
+    // add the EL partial rows (lanes with the same pl): butterfly over the entry-lane bits
+#pragma unroll
+    for (int off = PL; off < 32; off <<= 1)
+#pragma unroll
+      for (int i = 0; i < VEC; ++i) acc.v[i] += __shfl_xor_sync(0xffffffffu, acc.v[i], off);
+    if (el == 0 && pok) {
+      const T dc = __ldg(a.dC + row);
+      T xx = T(0);
+#pragma unroll
+      for (int i = 0; i < VEC; ++i) { xx = fma(x.v[i], x.v[i], xx); acc.v[i] = fma(dc, x.v[i], acc.v[i]); }
+      st[ES_CX] += (double)(dc * xx);
+      for (int p = 0; p < a.pC; ++p) {  // low-rank cost term: + U[row,p] * s_p (U^T X)_p
+        const T up = __ldg(a.U + row * a.pC + p);
+#pragma unroll
+        for (int i = 0; i < VEC; ++i) {
+          const int cidx = pl * VEC + i;
+          if (cidx < r) acc.v[i] = fma(up, (T)__ldg(a.Ts + p * r + cidx), acc.v[i]);
+        }
+      }
+      T gg = T(0), gr = T(0);
+#pragma unroll
+      for (int i = 0; i < VEC; ++i) {
+        acc.v[i] = fma((T)(-coef), x.v[i], acc.v[i]) * sc;
+        gg = fma(acc.v[i], acc.v[i], gg); gr = fma(acc.v[i], x.v[i], gr);
+      }
+      st[ES_GG] += (double)gg; st[ES_GR] += (double)gr;
+      if (a.Out) {
+        T* o = a.Out + row * ld + pl * VEC;
+        if (tailmask) {
+#pragma unroll
+          for (int i = 0; i < VEC; ++i) if (pl * VEC + i < r) o[i] = acc.v[i];
+        } else {
+          st_pack<T, VEC>(o, acc);
+        }
+      }
+    }
+  }
+  block_reduce_store<NST>(st, a.partials + (int64_t)blockIdx.x * kNStat);
+  finish_partials(a.fin);
+}
+
 // Segment pass of k_rows_ep: a warp per segment (<= kHeavyRow consecutive C entries of a heavy row) leaves
 // sum_e c_e X_{k_e} in seg_out[s][0..r) and sum_e c_e <X_{k_e}, X_row> in seg_cx[s].
 template <typename T, int VEC, int PL, int NIT>
@@ -669,6 +813,144 @@ __global__ void __launch_bounds__(kBlock) k_cons1(const ConsArgs<T> a) {
     cons_finish<MODE>(st, i, (double)t0, (double)t1, (double)t2, a.y, a.b, a.sigma, a.z, a.lam);
   }
   block_reduce_store<NST>(st, a.partials + (int64_t)blockIdx.x * kNStat);
+  finish_partials(a.fin);
+}
+
+// ---------------------------------------------------------------------------------------------
+// Cooperative forward evaluator ("cw", same idea as k_rows_cw): a warp takes 32 consecutive forward entries, reads
+// their (row, col, value) one entry per lane (coalesced), then gathers the two rows of EL = 32 / PL entries per
+// instruction with PL consecutive lanes on the consecutive packs of a row (one request per row instead of one per
+// pack), forms the lane-partial dot products, adds them over the PL lanes of an entry by a butterfly, and the entry's
+// first lane scales by w a.  SINGLE (every constraint is one entry): that lane finishes the constraint in place.
+// Otherwise the per-entry sums go to e_out and k_cons_fin / k_long_fin_e add them per constraint in a fixed order.
+// Entries beyond nf_A are C's sym-upper list (line search): <C,RR^T>, <C,RD^T>, <C,DD^T> straight into the stats.
+template <typename T, int VEC, int PL, int MODE, bool SINGLE, int UNR>
+__global__ void __launch_bounds__(kBlock) k_ent_cw(const ConsArgs<T> a) {
+  constexpr int WPB = kBlock / 32, NST = (MODE == CONS_LS) ? 12 : 6, K = (MODE == CONS_LS) ? 3 : 1, EL = 32 / PL;
+  constexpr bool LS = (MODE == CONS_LS);
+  using P = Pack<T, VEC>;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int nvec = a.nvec, r = a.r;
+  const int pl = lane & (PL - 1), el = lane / PL;
+  const bool pok = pl < nvec;
+  const bool tailmask = VEC > 1 && !a.exact && pl == nvec - 1;
+  const int64_t ld = a.ld;
+  const T* const Xp = a.X + pl * VEC;
+  const T* const Dp = LS ? a.X2 + pl * VEC : nullptr;
+  double st[NST];
+#pragma unroll
+  for (int s = 0; s < NST; ++s) st[s] = 0.0;
+  auto zero = [] { P z;
+#pragma unroll
+    for (int i = 0; i < VEC; ++i) z.v[i] = T(0);
+    return z; };
+  auto load_pack = [&](const T* p) {
+    if (!pok) return zero();
+    P v = ldg_pack<T, VEC>(p);
+    if (tailmask) {
+#pragma unroll
+      for (int i = 0; i < VEC; ++i) if (pl * VEC + i >= r) v.v[i] = T(0);
+    }
+    return v;
+  };
+  auto dotp = [](const P& x, const P& y) { T t = T(0);
+#pragma unroll
+    for (int i = 0; i < VEC; ++i) t = fma(x.v[i], y.v[i], t);
+    return t; };
+  auto seg = [](T v) {   // sum over the PL lanes of an entry (every lane gets it)
+#pragma unroll
+    for (int off = PL / 2; off > 0; off >>= 1) v += __shfl_xor_sync(0xffffffffu, v, off);
+    return v; };
+  for (int64_t base = ((int64_t)blockIdx.x * WPB + warp) * 32; base < a.nent; base += (int64_t)gridDim.x * WPB * 32) {
+    const int64_t e = base + lane;
+    int jr = 0, kc = 0; T av = T(0);     // padding entries of the last batch: row 0 with itself, coefficient 0
+    if (e < a.nent) { jr = __ldg(a.e_row + e); kc = __ldg(a.e_col + e); av = __ldg(a.e_val + e); if (jr != kc) av += av; }
+    const int cnt = (int)min((int64_t)32, a.nent - base);
+    for (int j = 0; j < cnt; j += EL * UNR) {
+      P xj[UNR], xk[UNR], dj[UNR], dk[UNR];
+      T au[UNR];
+#pragma unroll
+      for (int u = 0; u < UNR; ++u) {
+        const int src = (j + u * EL + el) & 31;
+        const int ju = __shfl_sync(0xffffffffu, jr, src), ku = __shfl_sync(0xffffffffu, kc, src);
+        au[u] = __shfl_sync(0xffffffffu, av, src);
+        xj[u] = load_pack(Xp + (int64_t)ju * ld);
+        xk[u] = ku != ju ? load_pack(Xp + (int64_t)ku * ld) : xj[u];
+        if (LS) {
+          dj[u] = load_pack(Dp + (int64_t)ju * ld);
+          dk[u] = ku != ju ? load_pack(Dp + (int64_t)ku * ld) : dj[u];
+        }
+      }
+#pragma unroll
+      for (int u = 0; u < UNR; ++u) {
+        const T s0 = seg(dotp(xj[u], xk[u]));
+        T s1 = T(0), s2 = T(0);
+        if (LS) { s1 = seg(dotp(xj[u], dk[u]) + dotp(dj[u], xk[u])); s2 = seg(dotp(dj[u], dk[u])); }
+        const int64_t ei = base + j + u * EL + el;
+        if (pl == 0 && j + u * EL + el < cnt) {
+          const T v0 = au[u] * s0, v1 = au[u] * s1, v2 = au[u] * s2;
+          if (ei < a.nf_A) {
+            if (SINGLE) {
+              cons_finish<MODE>(st, ei, (double)v0, (double)v1, (double)v2, a.y, a.b, a.sigma, a.z, a.lam);
+            } else {
+              a.e_out[ei * K] = v0;
+              if (LS) { a.e_out[ei * K + 1] = v1; a.e_out[ei * K + 2] = v2; }
+            }
+          } else if (LS) {   // C's sym-upper list: the entry sums are <C,RR^T>, <C,RD^T + DR^T>, <C,DD^T> restricted to the entry
+            st[LS_CRR] += (double)v0; st[LS_CRD] += 0.5 * (double)v1; st[LS_CDD] += (double)v2;
+          }
+        }
+      }
+    }
+  }
+  block_reduce_store<NST>(st, a.partials + (int64_t)blockIdx.x * kNStat);
+  finish_partials(a.fin);
+}
+
+// per-constraint sums of the entry results of k_ent_cw (constraints with at most kLongThreshold entries), a thread
+// per constraint, entries added in list order, then the per-constraint finish (a2)
+template <typename T, int MODE>
+__global__ void __launch_bounds__(kBlock) k_cons_fin(const ConsArgs<T> a) {
+  constexpr int NST = (MODE == CONS_LS) ? 12 : 6, K = (MODE == CONS_LS) ? 3 : 1;
+  double st[NST];
+#pragma unroll
+  for (int s = 0; s < NST; ++s) st[s] = 0.0;
+  for (int64_t i = (int64_t)blockIdx.x * kBlock + threadIdx.x; i < a.m; i += (int64_t)gridDim.x * kBlock) {
+    const int64_t e0 = __ldg(a.ptr + i), e1 = __ldg(a.ptr + i + 1);
+    if (e1 - e0 > kLongThreshold) continue;
+    double t0 = 0.0, t1 = 0.0, t2 = 0.0;
+    for (int64_t e = e0; e < e1; ++e) {
+      t0 += (double)a.e_out[e * K];
+      if (MODE == CONS_LS) { t1 += (double)a.e_out[e * K + 1]; t2 += (double)a.e_out[e * K + 2]; }
+    }
+    cons_finish<MODE>(st, i, t0, t1, t2, a.y, a.b, a.sigma, a.z, a.lam);
+  }
+  block_reduce_store<NST>(st, a.part_chunk + (int64_t)blockIdx.x * kNStat);
+  finish_partials(a.fin);
+}
+
+// the same for one long constraint per block: thread t adds entries t, t + 256, ... in order, then an ordered block sum
+template <typename T, int MODE>
+__global__ void __launch_bounds__(kBlock) k_long_fin_e(const ConsArgs<T> a, double* part_long) {
+  constexpr int K = (MODE == CONS_LS) ? 3 : 1;
+  __shared__ double sm[3][kBlock / 32];
+  const int slot = blockIdx.x, lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int64_t i = a.long_cons[slot], e0 = a.ptr[i], e1 = a.ptr[i + 1];
+  double v[3] = {0.0, 0.0, 0.0};
+  for (int64_t e = e0 + threadIdx.x; e < e1; e += kBlock) {
+    v[0] += (double)a.e_out[e * K];
+    if (MODE == CONS_LS) { v[1] += (double)a.e_out[e * K + 1]; v[2] += (double)a.e_out[e * K + 2]; }
+  }
+  for (int k = 0; k < 3; ++k) { const double t = warp_sum(v[k]); if (lane == 0) sm[k][warp] = t; }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    double t[3] = {0.0, 0.0, 0.0};
+    for (int k = 0; k < 3; ++k) for (int wv = 0; wv < kBlock / 32; ++wv) t[k] += sm[k][wv];
+    double st[kNStat];
+    for (int s = 0; s < kNStat; ++s) st[s] = 0.0;
+    cons_finish<MODE>(st, i, t[0], t[1], t[2], a.y, a.b, a.sigma, a.z, a.lam);
+    for (int s = 0; s < kNStat; ++s) part_long[(int64_t)slot * kNStat + s] = st[s];
+  }
   finish_partials(a.fin);
 }
 

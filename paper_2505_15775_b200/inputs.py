@@ -2,9 +2,12 @@
 
 This module only *constructs problem data*: graphs, the MaxCut cost C = -L/4 built from the
 Laplacian formula (section 6.1), constraint patterns, right-hand sides and random
-starting points.  It holds none of the method's arithmetic (no f, no gradient, no line search, no
-matvec) and imports neither ``oracle/`` nor the CUDA binding.  Both sides consume the arrays it
-returns.
+starting points.  It holds none of the solver's arithmetic (no f, no gradient, no line search, no
+matvec, no random numbers the method draws) and imports neither ``oracle/`` nor the CUDA binding.
+Both sides consume the arrays it returns.  One piece of data construction restates a definition of the
+paper: ``planted_rhs`` forms b_i = <A_i, R0 R0^T> for BASELINE.json's config 3 with numpy,
+because b IS the workload there; it feeds neither side's results, and tests/test_inputs.py and
+tests/test_oracle_pins.py check it against the oracle's own A(.).
 
 Storage convention: **sym-upper COO** -- an entry ``(j, k, a)`` with
 ``j <= k`` means ``A[j,k] = A[k,j] = a``.  Constraints are stacked: entries
@@ -243,9 +246,11 @@ def _random_sym_entries(rng, n: int, count: int):
 
 
 def planted_rhs(p_ptr, row, col, val, R0) -> np.ndarray:
-    """Right-hand side of the planted instance, b_i = <A_i, R0 R0^T>  (BASELINE.json config 3).
+    """Right-hand side of the planted instance, b_i = <A_i, R0 R0^T>  (BASELINE.json config 3; PAPER.md:91).
 
-    Data construction only (fp64): diagonal entries count once, off-diagonal stored entries twice.
+    Data construction (fp64, numpy): diagonal entries count once, off-diagonal stored entries twice.  This is the
+    one place where the generator restates a formula of the method (module docstring); it is checked against the
+    oracle's A(.) in tests/test_inputs.py, and neither the oracle nor the CUDA path calls it.
     """
     w = np.where(row == col, 1.0, 2.0) * val * np.einsum("ec,ec->e", R0[row], R0[col])
     cons = np.repeat(np.arange(p_ptr.shape[0] - 1), np.diff(p_ptr))
@@ -429,18 +434,3 @@ def small(idx: int) -> Workload:
 
 def full(idx: int) -> Workload:
     return CONFIGS[idx]()
-
-
-# ----------------------------------------------------------------------------------------------
-# counter-based uniform generator used for the Lanczos start vector (reading 9):
-# v0[i] = u(seed, i) in (-1, 1).  Integer arithmetic only, so the CUDA kernel and the oracle
-# (which each implement it on their own) produce bit-identical vectors.  This copy exists for
-# tests that want to look at the vector; neither side imports it.
-# ----------------------------------------------------------------------------------------------
-def counter_uniform(seed: int, count: int) -> np.ndarray:
-    with np.errstate(over="ignore"):
-        x = (np.arange(count, dtype=np.uint64) + np.uint64(seed) * np.uint64(0x9E3779B97F4A7C15))
-        x = (x ^ (x >> np.uint64(30))) * np.uint64(0xBF58476D1CE4E5B9)
-        x = (x ^ (x >> np.uint64(27))) * np.uint64(0x94D049BB133111EB)
-        x = x ^ (x >> np.uint64(31))
-    return ((x >> np.uint64(11)).astype(np.float64) + 0.5) * (2.0 / 9007199254740992.0) - 1.0

@@ -51,6 +51,16 @@ def test_params_struct_layout_matches_binding(lib):
         assert getattr(p, f) == getattr(q, f), f
 
 
+def test_preset_matches_oracle_preset(lib):
+    from paper_2505_15775_b200 import binding
+    from oracle import alm
+    for dt, f32 in (("f32", True), ("f64", False)):
+        p, q = binding.Params.preset(dt), alm.preset_params(f32)
+        for f in ("eps", "it_max", "lbfgs_mem", "stall_tol", "stall_iters", "tol0", "c_in", "tol_min", "gamma", "kappa"):
+            assert getattr(p, f) == getattr(q, f), (dt, f)
+    assert binding.Params.preset("f32").it_max == 100 and binding.Params.preset("f64").it_max == 500
+
+
 def test_create_validates_and_has_no_cpu_fallback():
     import torch
     from paper_2505_15775_b200 import binding, inputs

@@ -37,6 +37,17 @@ def rel(a, b):
     return float(np.linalg.norm(np.asarray(a, float) - np.asarray(b, float)) / max(1e-300, np.linalg.norm(np.asarray(b, float))))
 
 
+def worst_row(got, ref, extra=0.0):
+    """max over rows j of ||got_j - ref_j|| / (||ref_j|| + ||ref||_F / sqrt(n) + extra_j): a single bad row (a ragged
+    tail, a heavy row, a mis-staged tile) shows up here at full size, where it moves the whole-array ratio by only
+    1 / sqrt(n).  The floor ||ref||_F / sqrt(n) is the typical row norm (rows that cancel are measured against it)."""
+    got = np.asarray(got, float).reshape(len(ref), -1); ref = np.asarray(ref, float).reshape(len(ref), -1)
+    err = np.linalg.norm(got - ref, axis=1)
+    den = np.linalg.norm(ref, axis=1) + np.linalg.norm(ref) / np.sqrt(max(1, len(ref))) + extra
+    j = int(np.argmax(err / np.maximum(den, 1e-300)))
+    return float(err[j] / max(den[j], 1e-300)), j
+
+
 def check_workload(torch, binding, oracle_mod, w, ld=None, label="", split_scale=False):
     P, tol = w.problem, TOL[w.dtype]
     o = oracle_mod.Oracle(P)
@@ -62,16 +73,32 @@ def check_workload(torch, binding, oracle_mod, w, ld=None, label="", split_scale
     fden = abs(parts["cx"]) + abs(parts["yq"]) + 0.5 * w.sigma * parts["qq"]
     assert abs(st[0] - parts["f"]) <= tol * fden, (label, st[0], parts["f"])
     assert abs(st[1] - parts["cx"]) <= tol * fden
-    assert rel(z.cpu().numpy(), zo) <= tol, label
+    zg = z.cpu().numpy()
+    assert rel(zg, zo) <= tol, label
+    # per constraint: |dz_i| against |z_i|, the typical |z| and -- for constraints whose terms cancel -- the sum of
+    # the absolute values of the terms (|A|(|R||R|^T), from the oracle run on |A|, |R|)
+    zabs = oracle_mod.Oracle(_abs_problem(P)).A_op(np.abs(w.R)) if P.m else np.zeros(0)
+    if P.m:
+        ez, iz = worst_row(zg, zo, extra=zabs if split_scale else 0.0)
+        assert ez <= tol, (label, "worst constraint", iz, ez)
     Gg = G.cpu().numpy().astype(float)
+    # per row of G: the error a row inherits from lambda_i = y_i - sigma (z_i - b_i) is sigma |dz_i| <= sigma tol |z|_i
+    # times the rows it multiplies ("Precision"); rowext carries that term
+    lam_scale = w.sigma * tol * (zabs if split_scale else np.abs(zo))
+    rowext = _adjoint_abs(P, lam_scale, np.abs(w.R)) / tol if P.m else 0.0
     if split_scale:
         # tiny degenerate problems: G = 2(CR - A*(lambda)R) may cancel almost completely (one row, one
         # constraint), so the error is measured against the two terms that are subtracted
         CR = o.smatvec(np.zeros(P.m), w.R)
         gden = 2.0 * (np.linalg.norm(CR) + np.linalg.norm(0.5 * Go - CR))
         assert np.linalg.norm(Gg[:, :r] - Go) <= tol * gden, label
+        rows_split = 2.0 * (np.linalg.norm(CR, axis=1) + np.linalg.norm(0.5 * Go - CR, axis=1))
+        eg, jg = worst_row(Gg[:, :r], Go, extra=rows_split + rowext)
+        assert eg <= tol, (label, "worst row of G", jg, eg)
     else:
         assert rel(Gg[:, :r], Go) <= tol, label
+        eg, jg = worst_row(Gg[:, :r], Go, extra=rowext)
+        assert eg <= tol, (label, "worst row of G", jg, eg)
     assert abs(np.sqrt(st[4]) - np.linalg.norm(Go)) <= tol * (gden if split_scale else np.linalg.norm(Go))
     assert abs(st[5] - np.vdot(Go, w.R)) <= tol * ((gden if split_scale else np.linalg.norm(Go)) * np.linalg.norm(w.R))
     if ld > r:
@@ -86,10 +113,15 @@ def check_workload(torch, binding, oracle_mod, w, ld=None, label="", split_scale
     lamo, _ = o.lam(w.y, w.sigma, w.R)
     torch.cuda.synchronize()
     assert np.linalg.norm(lam.cpu().numpy() - lamo) <= tol * (np.linalg.norm(w.y) + w.sigma * np.linalg.norm(zo)), label
-    # line search
+    # line search: cold, then warm (the ctx holds the evaluation of this same R)
     p = ctx.linesearch(R, D, r, ld)
     po = o.linesearch(w.y, w.sigma, w.R, w.D)
     assert np.abs(p - po).max() <= tol * np.abs(po).sum(), (label, p, po)
+    pw = ctx.linesearch(R, D, r, ld, warm=True)
+    assert np.abs(pw - po).max() <= tol * np.abs(po).sum(), (label, pw, po)
+    with pytest.raises(binding.AloraError) as e:          # no evaluation of D on record
+        ctx.linesearch(D, R, r, ld, warm=True)
+    assert e.value.status == binding.ESTATE
     # matvec
     mu = dev(torch, lamo, torch.float64)
     V = dev(torch, w.V, dt)
@@ -97,7 +129,16 @@ def check_workload(torch, binding, oracle_mod, w, ld=None, label="", split_scale
     vw = ctx.smatvec(mu, V, 1, W)
     Wo = o.smatvec(lamo, w.V)
     assert rel(W.cpu().numpy(), Wo) <= tol, label
+    ew, jw = worst_row(W.cpu().numpy(), Wo, extra=_smat_abs(P, lamo, np.abs(w.V)) if split_scale else 0.0)
+    assert ew <= tol, (label, "worst row of S(mu)v", jw, ew)
     assert abs(vw - w.V @ Wo) <= tol * np.linalg.norm(w.V) * np.linalg.norm(Wo)
+    # mu = NULL: lambda of the last evaluation (the ctx still holds the evaluation of R above)
+    W0 = torch.zeros_like(V)
+    ctx.smatvec(None, V, 1, W0)
+    # the library's lambda carries sigma |dz_i| <= lam_scale_i per constraint; that perturbs S(lambda) v by at most
+    # sum_i lam_scale_i |A_i| |v|
+    dW = 0.5 * np.linalg.norm(_adjoint_abs(P, lam_scale, np.abs(w.V).reshape(-1, 1))) if P.m else 0.0
+    assert np.linalg.norm(W0.cpu().numpy().astype(float) - Wo) <= tol * np.linalg.norm(Wo) + dW, label
     # block matvec with p = 3 columns
     V3h = np.stack([w.V, np.roll(w.V, 1), w.V ** 2], axis=1)
     if w.dtype == inputs.F32:
@@ -107,6 +148,36 @@ def check_workload(torch, binding, oracle_mod, w, ld=None, label="", split_scale
     torch.cuda.synchronize()
     assert rel(W3.cpu().numpy(), o.smatvec(lamo, V3h)) <= tol, label
     ctx.close()
+
+
+def _abs_problem(P):
+    """the same problem with |a_e| for every stored constraint entry (inputs for an error scale, not a result)"""
+    return inputs.Problem(**{**P.__dict__, "A_val": np.abs(P.A_val), "C_val": np.abs(P.C_val),
+                             "C_U": None if P.C_U is None else np.abs(P.C_U), "C_s": None if P.C_s is None else np.abs(P.C_s)})
+
+
+def _adjoint_abs(P, wts, Rabs):
+    """row norms of sum_i wts_i |A_i| Rabs  (scale of the error that a perturbation wts of lambda causes in G / 2)"""
+    n = P.n
+    out = np.zeros_like(Rabs)
+    cons = np.repeat(np.arange(P.m), np.diff(P.A_ptr))
+    wv = wts[cons] * np.abs(P.A_val)
+    np.add.at(out, P.A_row, wv[:, None] * Rabs[P.A_col])
+    off = P.A_row != P.A_col
+    np.add.at(out, P.A_col[off], wv[off, None] * Rabs[P.A_row[off]])
+    return 2.0 * np.linalg.norm(out, axis=1)
+
+
+def _smat_abs(P, mu, Vabs):
+    """row scale of S(mu) v when its terms cancel: (|C| + sum |mu_i| |A_i|) |v| (low-rank cost term included)"""
+    Vabs = Vabs.reshape(P.n, -1)
+    out = np.zeros_like(Vabs)
+    np.add.at(out, P.C_row, np.abs(P.C_val)[:, None] * Vabs[P.C_col])
+    off = P.C_row != P.C_col
+    np.add.at(out, P.C_col[off], np.abs(P.C_val)[off, None] * Vabs[P.C_row[off]])
+    if P.pC:
+        out += np.abs(P.C_U) @ (np.abs(P.C_s)[:, None] * (np.abs(P.C_U).T @ Vabs))
+    return np.linalg.norm(out, axis=1) + _adjoint_abs(P, np.abs(mu), Vabs) / 2.0
 
 
 @pytest.mark.parametrize("idx", [0, 1, 2, 3, 4, 5, 6, 7])

@@ -72,6 +72,42 @@ def test_lanczos_matches_oracle_and_dense(torch, binding, alm, oracle_mod):
     ctx.close()
 
 
+def test_lanczos_multi_pair_abi(torch, binding, alm, oracle_mod):
+    """alora_lanczos with p_want = 4 (Alg. 1 line 5): theta ascending, column-major unit Ritz vectors
+    with Rayleigh quotients theta (V^T S V = diag(theta)), residual estimates, same values as the oracle's run;
+    mu = NULL takes lambda of the last evaluation."""
+    w = inputs.small(0)
+    P = w.problem
+    o = oracle_mod.Oracle(P)
+    y = np.random.default_rng(1).standard_normal(P.m)
+    lam, _ = o.lam(y, 1.0, w.R)
+    S = o.smatvec(lam, np.eye(P.n))
+    th_o, v_o, k_o, res_o, (ths_o, U_o) = alm.lanczos(lambda x: o.smatvec(lam, x), P.n, 42, 300, 1e-8, p_want=4)
+    ctx = binding.Context(P, inputs.F64)
+    Vd = torch.zeros(4 * P.n, dtype=torch.float64, device="cuda")
+    ths, k, resid, ok = ctx.lanczos(torch.as_tensor(lam).cuda(), 300, 1e-8, 42, Vd, p_want=4)
+    assert ok and ths.shape == (4,) and resid.shape == (4,) and abs(k - k_o) <= 2
+    assert np.all(np.diff(ths) >= 0) and np.abs(ths - ths_o).max() < 1e-8 and resid[0] <= 1e-8
+    U = Vd.cpu().numpy().reshape(4, P.n).T
+    np.testing.assert_allclose(U.T @ U, np.eye(4), atol=1e-9)
+    np.testing.assert_allclose(U.T @ S @ U, np.diag(ths), atol=1e-7)
+    for j in range(4):     # the residual estimate |beta_k s_kj| is the true residual norm of the Ritz pair
+        assert abs(np.linalg.norm(S @ U[:, j] - ths[j] * U[:, j]) - resid[j]) <= 1e-6 * (1 + resid[j])
+    # mu = NULL after an evaluation with the same (y, sigma): same operator
+    R = torch.as_tensor(w.R).cuda(); yd = torch.as_tensor(y).cuda()
+    ctx.set_dual(yd, 1.0)
+    with pytest.raises(binding.AloraError) as e:
+        ctx.lanczos(None, 300, 1e-8, 42, None)
+    assert e.value.status == binding.ESTATE
+    ctx.eval(R, w.r, w.r, None, None)
+    th1, k1, _, ok1 = ctx.lanczos(None, 300, 1e-8, 42, None)
+    assert ok1 and abs(th1 - ths[0]) < 1e-9
+    # values only (no vectors), fewer steps than pairs asked for
+    th2, k2, r2, ok2 = ctx.lanczos(None, 3, 1e-14, 42, None, p_want=8)
+    assert k2 == 3 and th2.shape == (3,) and not ok2
+    ctx.close()
+
+
 def test_lanczos_fp32(torch, binding, oracle_mod):
     w = inputs.small(4)
     P = w.problem
@@ -150,6 +186,41 @@ def test_solve_fp32_ring_matchings(torch, binding, oracle_mod):
     o = oracle_mod.Oracle(w.problem)
     q = o.A_op(out["R"]) - w.problem.b
     assert np.linalg.norm(q) / (1 + np.linalg.norm(w.problem.b)) <= 2e-5
+
+
+def test_solve_lbfgs_memory_bounds(torch, binding, oracle_mod):
+    """lbfgs_mem = 16 (the documented maximum; the two-loop path, mem >= 8) and a value above it (clamped) reach
+    the K_9 optimum; the workspace holds 5 + 2 (16 + 1) arrays."""
+    n = 9
+    P = _graph_maxcut(n, [(i, j) for i in range(n) for j in range(i + 1, n)])
+    R0 = inputs._unit_rows(np.random.default_rng(4), n, 4)
+    o = oracle_mod.Oracle(P)
+    for mem in (16, 40, 0):
+        out = gpu_solve(torch, binding, P, inputs.F64, R0, np.zeros(n), 1.0, r_cap=16, eps=1e-7, lbfgs_mem=mem)
+        assert out["ok"] and abs(o.inner_C(out["R"], out["R"]) + n * n / 4) < 1e-4, mem
+
+
+def test_config4_full_solve(torch, binding, oracle_mod):
+    """BASELINE.json's target: the full rank-adaptive ALM solve of the n = 2^24 MaxCut config reaches relative primal
+    infeasibility <= 1e-5 (first term of eq. 77) on one B200, with the library's preset for fp32
+    contexts (alora_preset_params).  The residual A(RR^T) - b of the returned R is recomputed by the oracle."""
+    w = inputs.full(4)
+    P = w.problem
+    r_cap = w.r + 14
+    ctx = binding.Context(P, w.dtype)
+    Rbuf = torch.zeros(P.n * r_cap, dtype=torch.float32, device="cuda")
+    Rbuf[: P.n * w.r] = torch.as_tensor(w.R, dtype=torch.float32).cuda().reshape(-1)
+    y = torch.zeros(P.m, dtype=torch.float64, device="cuda")
+    prm = binding.Params.preset(w.dtype, eps=1e-5, stop_mode=1)
+    res, log, r, sg, ok = ctx.solve(prm, Rbuf, w.r, r_cap, y, w.sigma)
+    assert ok and res.kkt[0] <= 1e-5, (res.kkt[0], res.outer_iters)
+    R = Rbuf[: P.n * r].reshape(P.n, r).cpu().numpy().astype(float)
+    ctx.close()
+    del Rbuf
+    o = oracle_mod.Oracle(P)
+    q = o.A_op(R) - P.b
+    assert np.linalg.norm(q) / (1 + np.linalg.norm(P.b)) <= 1.05e-5
+    assert res.seconds < 120.0
 
 
 def test_rank_cap_skips_growth(torch, binding, oracle_mod):
