@@ -267,6 +267,12 @@ template <typename T> alora_status build(alora_ctx* c, const alora_problem* P) {
     c->single_entry = m > 0;
     for (int64_t i = 0; i < m && c->single_entry; ++i) c->single_entry = (f_ptr[i + 1] - f_ptr[i] == 1);
     c->short_cons = m > 0 && c->nf_A <= 8 * m;
+    if (m > 0 && !c->single_entry) {   // uniform constraints: k_ent_cw finishes them in its own pass
+      const int64_t npc = f_ptr[1] - f_ptr[0];
+      bool uni = npc > 1 && npc <= 32 && 32 % npc == 0;
+      for (int64_t i = 0; i < m && uni; ++i) uni = (f_ptr[i + 1] - f_ptr[i] == npc);
+      c->uniform_npc = uni ? (int)npc : 0;
+    }
     // forward list continues with C's sym-upper entries (diagonal, then upper triangle of the CSR)
     for (int64_t j = 0; j < n; ++j)
       if (dC[j] != 0.0) { f_row.push_back((int)j); f_col.push_back((int)j); f_val.push_back(dC[j]); }
@@ -389,7 +395,7 @@ extern "C" alora_status alora_create(const alora_problem* P, alora_dtype dtype, 
   if (!c) return ALORA_ENOMEM;
   c->device = device; c->stream = (cudaStream_t)cuda_stream; c->dtype = dtype;
   c->esz = dtype == ALORA_F32 ? 4 : 8; c->n = P->n; c->m = P->m;
-  if (const char* e = std::getenv("ALORA_CW")) c->cw = std::atoi(e) != 0;   // measurement switch
+  if (const char* e = std::getenv("ALORA_CW")) c->cw = std::atoi(e);   // measurement switch: 0 never, 1 default, 2 always
   std::memset(c->occ_cache, 0, sizeof(c->occ_cache));
   std::memset(c->occ_ld, 0, sizeof(c->occ_ld));
   cudaDeviceProp prop;

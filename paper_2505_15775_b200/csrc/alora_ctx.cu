@@ -223,6 +223,14 @@ alora_status launch_diag_rows(alora_ctx* c, int vec, int nvec, int exact, int sh
   c->launches++;
   return ALORA_OK;
 }
+// The cooperative kernels (k_ent_cw, k_rows_cw) pay when a gathered row is more than one pack (otherwise a thread per
+// item already makes one request per row) and the rows do not sit in L1 (measured, profiles/r2b_README.md: config 3
+// 466 -> 352 us per step, config 2 adjoint 39 -> 28 us; config 5, n r = 120 KB: 84 -> 96 us).  ALORA_CW=0 / 2: never / always.
+inline bool use_cw(const alora_ctx* c, const Geo& g, int r) {
+  if (c->cw == 0 || g.nvec > 32) return false;
+  if (c->cw == 2) return true;
+  return g.nvec >= 2 && (size_t)c->n * (size_t)r * c->esz >= ((size_t)1 << 20);
+}
 // general-class adjoint pass: a group per row; single vectors (Lanczos matvec) on long rows take a warp per row
 // (measured on config 3, 60 entries per row: the warp-per-row kernel wins for p = 1, 66 vs 77 us, and loses for
 // r = 10, 168 vs 128 us); rows with ~100 entries or more (matrix completion) always take a warp per row
@@ -240,8 +248,9 @@ template <typename T> alora_status launch_adj_general(alora_ctx* c, const Geo& g
     ALORA_CUDA(c, launch_rows_seg(g.vec, g.shape, a, gs, c->stream));
     c->launches++;
   }
-  if (c->cw && g.nvec <= 32) {
-    // cooperative warp per row (k_rows_cw): coalesced entry metadata, one request per gathered row
+  if (use_cw(c, g, a.r) && !c->row_perm && !c->ep_wide) {
+    // cooperative warp per row (k_rows_cw): coalesced entry metadata, one request per gathered row; not for skewed row
+    // lengths (config 7: 769 against 474 us) nor for very long rows of thin vectors (k_rows_ep is as fast there)
     int pl2 = 0; while ((1 << pl2) < g.nvec) ++pl2;
     int& occ = c->occ_cw[vec_slot(g.vec)][pl2];
     if (!occ) occ = std::max(1, occ_rows_cw(T(), g.vec, g.nvec));
@@ -334,7 +343,8 @@ alora_status forward_cw(alora_ctx* c, const Geo& g, int mode, ConsArgs<T>& ca, i
   const size_t need = (size_t)std::max<int64_t>(1, c->nf_A) * K * c->esz;
   if (!c->e_out) ALORA_CUDA(c, c->pool.alloc(&c->e_out, need));
   ca.nent = nent; ca.nf_A = c->nf_A; ca.e_out = (T*)c->e_out; ca.long_cons = c->long_cons;
-  const bool single = c->single_entry, fin_k = !single && c->m > 0, longs = fin_k && c->nlong_A > 0;
+  ca.npc = c->uniform_npc;
+  const bool single = c->single_entry, fin_k = !single && c->uniform_npc <= 1 && c->m > 0, longs = fin_k && c->nlong_A > 0;
   *ge = (int)std::max<int64_t>(1, std::min<int64_t>((nent + kBlock - 1) / kBlock, std::min<int64_t>((int64_t)c->num_sms * 8, c->part_cap)));
   *gf = fin_k ? (int)std::max<int64_t>(1, std::min<int64_t>((c->m + kBlock - 1) / kBlock, std::min<int64_t>((int64_t)c->num_sms * 8, c->part_cap))) : 0;
   auto fin_all = [&]() { return make_fin(c, c->part_cons, *ge, c->part_chunk, *gf, c->part_long, longs ? c->nlong_A : 0, last_out); };
@@ -380,12 +390,12 @@ template <typename T> alora_status eval_impl(alora_ctx* c, const T* R, int32_t r
     fill_cons(c, ca, g, R, (const T*)nullptr, r, ld);
     ca.z = zout;
     int gc = 0;
-    if (c->cw && g.nvec <= 32 && c->m > 0) {
+    if (use_cw(c, g, r) && c->m > 0) {
       int ge = 0, gf = 0;
       s = forward_cw<T>(c, g, CONS_EVAL, ca, c->nf_A, &ge, &gf, nullptr);
       if (s != ALORA_OK) return s;
       a.w = c->lam; a.diag_class = 0;
-      const bool fin_k = !c->single_entry;
+      const bool fin_k = !c->single_entry && c->uniform_npc <= 1;
       a.fin = make_fin(c, c->part_rows, 0, fin_k ? c->part_chunk : c->part_cons, fin_k ? gf : ge, c->part_long,
                        (fin_k && c->nlong_A > 0) ? c->nlong_A : 0, nullptr);   // last kernel of the call
       time_mark(c);
@@ -462,7 +472,7 @@ template <typename T> alora_status ls_impl(alora_ctx* c, const T* R, const T* D,
     }
     ConsArgs<T> ca;
     fill_cons(c, ca, g, R, D, r, ld);
-    if (c->cw && g.nvec <= 32 && c->nf_A + c->nf_C > 0) {
+    if (use_cw(c, g, r) && c->nf_A + c->nf_C > 0) {
       int ge = 0, gf = 0;
       s = forward_cw<T>(c, g, CONS_LS, ca, c->nf_A + c->nf_C, &ge, &gf, c->ls_dev);
       if (s != ALORA_OK) return s;

@@ -56,7 +56,7 @@ struct alora_ctx {
   int* dcons = nullptr; void* da = nullptr;
   // identity diagonal class: padded ELL blocks (rows_tiled.cuh): kUN first neighbours per row, kUNL last
   // upper-triangle neighbours per row, and per 32-row block a flag "some row has more"
-  bool cw = false;         // general class: cooperative entry / row kernels (k_ent_cw, k_rows_cw); ALORA_CW=1 turns them on
+  int cw = 1;              // general class, cooperative entry / row kernels (k_ent_cw, k_rows_cw): 1 = where they pay (use_cw), 0 = never, 2 = always (ALORA_CW)
   int occ_cw[3][6] = {};
   bool ell_wide = false;   // 8 / 6 slots per row instead of 4 / 3 (more than 10 % of the rows have degree > 4)
   int* ell_col = nullptr; void* ell_val = nullptr;
@@ -68,6 +68,7 @@ struct alora_ctx {
   int nseg = 0, nheavy = 0; int* seg_row = nullptr; int* seg_beg = nullptr; int* seg_end = nullptr;
   int* heavy_rows = nullptr; int* heavy_segptr = nullptr; void* seg_out = nullptr; double* seg_cx = nullptr;
   size_t seg_out_bytes = 0;   // seg_out is sized on first use for the row length in use (nseg * pitch elements)
+  int uniform_npc = 0;         // > 1: every constraint has exactly this many stored entries and it divides 32
   bool single_entry = false;   // every constraint has exactly one stored entry: thread-per-constraint forward (k_cons1)
   bool short_cons = false;     // at most 8 stored entries per constraint on average: thread-per-constraint forward too
   bool ep = false;       // general class, >= 8 entries per row on average: warp-per-row adjoint for single vectors

@@ -99,6 +99,7 @@ template <typename T> struct ConsArgs {
   // cooperative forward evaluator (k_ent_cw / k_cons_fin / k_long_fin_e): entries [0, nent) are walked, the first nf_A
   // of them belong to constraints (their per-entry sums go to e_out[e][K], K = 1 or 3), the rest to C's sym-upper list
   int64_t nent, nf_A; T* e_out;
+  int npc;                        // > 1: every constraint has exactly npc entries (npc divides 32): k_ent_cw finishes them itself
   const int* long_cons;           // ids of the constraints with more than kLongThreshold entries (one block each)
 };
 
@@ -180,6 +181,10 @@ template <int NST> __device__ __forceinline__ void block_reduce_store(double (&s
 // See FinArgs.  Called by every thread of the block after the block's partial row has been written (needs
 // blockDim.x >= 256).  Thread t < 256 owns stat t % 16 and the rows t / 16, t / 16 + 16, ... of each region; the 16
 // row slots are then summed in order through shared memory.
+#ifndef ALORA_FIN_LOADS
+#define ALORA_FIN_LOADS 16
+#endif
+constexpr int kFinLoads = ALORA_FIN_LOADS;   // 444 partial rows / 16 row slots = 28 loads per thread: two round trips instead of four
 __device__ __forceinline__ void finish_partials(const FinArgs& f) {
   if (!f.out) return;
   __shared__ unsigned int s_last;
@@ -198,12 +203,12 @@ __device__ __forceinline__ void finish_partials(const FinArgs& f) {
     for (int k = 0; k < 3; ++k) {
       const double* p = f.p[k];
       const int n = f.n[k];
-      for (int i = slot; i < n; i += 8 * NSLOT) {   // eight independent (predicated) loads in flight per round trip
-        double t[8];
+      for (int i = slot; i < n; i += kFinLoads * NSLOT) {   // kFinLoads independent (predicated) loads in flight per round trip
+        double t[kFinLoads];
 #pragma unroll
-        for (int u = 0; u < 8; ++u) t[u] = (i + u * NSLOT < n) ? __ldcg(p + (int64_t)(i + u * NSLOT) * kNStat + s) : 0.0;
+        for (int u = 0; u < kFinLoads; ++u) t[u] = (i + u * NSLOT < n) ? __ldcg(p + (int64_t)(i + u * NSLOT) * kNStat + s) : 0.0;
 #pragma unroll
-        for (int u = 0; u < 8; ++u) v += t[u];
+        for (int u = 0; u < kFinLoads; ++u) v += t[u];
       }
     }
     s_fin[threadIdx.x] = v;
@@ -557,7 +562,8 @@ __global__ void __launch_bounds__(kBlock) k_rows_cw(const RowArgs<T> a) {
   const bool pok = pl < nvec;                    // this lane owns a pack of the row
   const bool tailmask = VEC > 1 && !a.exact && pl == nvec - 1;
   const int64_t ld = a.ld;
-  const T* const Xp = a.X + pl * VEC;            // lane's pack of row 0
+  const int plc = min(pl, nvec - 1);             // lanes beyond the row read its last pack (same request) and drop it
+  const T* const Xp = a.X + plc * VEC;           // lane's pack of row 0
   const T sc = (T)a.scale;
   double st[NST];
 #pragma unroll
@@ -566,15 +572,21 @@ __global__ void __launch_bounds__(kBlock) k_rows_cw(const RowArgs<T> a) {
 #pragma unroll
     for (int i = 0; i < VEC; ++i) z.v[i] = T(0);
     return z; };
-  auto load_pack = [&](const T* p) {   // p points at the lane's pack; elements beyond r zeroed (partial last pack)
-    if (!pok) return zero();
+  // p points at the lane's pack.  The load is unconditional (a branch around it costs a convergence barrier per load);
+  // lanes that own no pack and the elements beyond r (partial last pack) are zeroed by selects.
+  const int nkeep = !pok ? 0 : (tailmask ? r - pl * VEC : VEC);
+  auto load_pack = [&](const T* p) {
     P v = ldg_pack<T, VEC>(p);
-    if (tailmask) {
 #pragma unroll
-      for (int i = 0; i < VEC; ++i) if (pl * VEC + i >= r) v.v[i] = T(0);
-    }
+    for (int i = 0; i < VEC; ++i) v.v[i] = i < nkeep ? v.v[i] : T(0);
     return v;
   };
+  // the 32 (column, coefficient) pairs of a batch pass from the lanes that loaded them to the lanes that use them
+  // through a warp-private piece of shared memory (a shuffle inside this data-dependent loop would cost a
+  // convergence barrier each)
+  __shared__ int s_col[WPB][32];
+  __shared__ T s_cf[WPB][32];
+  int* const colS = s_col[warp]; T* const cfS = s_cf[warp];
   for (int64_t pos = (int64_t)blockIdx.x * WPB + warp; pos < a.n; pos += (int64_t)gridDim.x * WPB) {
     const int64_t row = a.perm ? (int64_t)__ldg(a.perm + pos) : pos;
     const P x = load_pack(Xp + row * ld);
@@ -589,21 +601,23 @@ __global__ void __launch_bounds__(kBlock) k_rows_cw(const RowArgs<T> a) {
           const T v = __ldg(val + e);
           cf_l = cons ? (T)(-__ldg(a.w + __ldg(cons + e)) * (double)v) : v;
         }
+        colS[lane] = col_l; cfS[lane] = cf_l;
+        __syncwarp();
         const int cnt = min(32, end - base);
-        for (int j = 0; j < cnt; j += EL * UNR) {
+        for (int j = el; j < cnt; j += EL * UNR) {
           P pk[UNR]; T cf[UNR];
 #pragma unroll
           for (int u = 0; u < UNR; ++u) {
-            const int src = (j + u * EL + el) & 31;
-            const int cu = __shfl_sync(0xffffffffu, col_l, src);
-            cf[u] = __shfl_sync(0xffffffffu, cf_l, src);
-            pk[u] = load_pack(Xp + (int64_t)cu * ld);
+            const int src = j + u * EL;          // < 32: EL * UNR <= 32 and j - el is a multiple of EL * UNR
+            cf[u] = cfS[src];
+            pk[u] = load_pack(Xp + (int64_t)colS[src] * ld);
           }
 #pragma unroll
           for (int u = 0; u < UNR; ++u)
 #pragma unroll
             for (int i = 0; i < VEC; ++i) acc.v[i] = fma(cf[u], pk[u].v[i], acc.v[i]);
         }
+        __syncwarp();
       }
     };
     const int cb = __ldg(a.c_rowptr + row), ce = __ldg(a.c_rowptr + row + 1);
@@ -614,7 +628,7 @@ __global__ void __launch_bounds__(kBlock) k_rows_cw(const RowArgs<T> a) {
       const int s0 = __ldg(a.heavy_segptr + lo), s1 = __ldg(a.heavy_segptr + lo + 1);
       if (el == 0) {
         for (int sg = s0; sg < s1; ++sg) {
-          const P part = load_pack(a.seg_out + (int64_t)sg * (nvec * VEC) + pl * VEC);
+          const P part = load_pack(a.seg_out + (int64_t)sg * (nvec * VEC) + plc * VEC);
 #pragma unroll
           for (int i = 0; i < VEC; ++i) acc.v[i] += part.v[i];
         }
@@ -835,8 +849,9 @@ __global__ void __launch_bounds__(kBlock) k_ent_cw(const ConsArgs<T> a) {
   const bool pok = pl < nvec;
   const bool tailmask = VEC > 1 && !a.exact && pl == nvec - 1;
   const int64_t ld = a.ld;
-  const T* const Xp = a.X + pl * VEC;
-  const T* const Dp = LS ? a.X2 + pl * VEC : nullptr;
+  const int plc = min(pl, nvec - 1);
+  const T* const Xp = a.X + plc * VEC;
+  const T* const Dp = LS ? a.X2 + plc * VEC : nullptr;
   double st[NST];
 #pragma unroll
   for (int s = 0; s < NST; ++s) st[s] = 0.0;
@@ -844,13 +859,11 @@ __global__ void __launch_bounds__(kBlock) k_ent_cw(const ConsArgs<T> a) {
 #pragma unroll
     for (int i = 0; i < VEC; ++i) z.v[i] = T(0);
     return z; };
-  auto load_pack = [&](const T* p) {
-    if (!pok) return zero();
+  const int nkeep = !pok ? 0 : (tailmask ? r - pl * VEC : VEC);   // elements of the lane's pack that exist
+  auto load_pack = [&](const T* p) {   // unconditional load, lanes without a pack / elements beyond r zeroed by selects
     P v = ldg_pack<T, VEC>(p);
-    if (tailmask) {
 #pragma unroll
-      for (int i = 0; i < VEC; ++i) if (pl * VEC + i >= r) v.v[i] = T(0);
-    }
+    for (int i = 0; i < VEC; ++i) v.v[i] = i < nkeep ? v.v[i] : T(0);
     return v;
   };
   auto dotp = [](const P& x, const P& y) { T t = T(0);
@@ -861,17 +874,26 @@ __global__ void __launch_bounds__(kBlock) k_ent_cw(const ConsArgs<T> a) {
 #pragma unroll
     for (int off = PL / 2; off > 0; off >>= 1) v += __shfl_xor_sync(0xffffffffu, v, off);
     return v; };
-  for (int64_t base = ((int64_t)blockIdx.x * WPB + warp) * 32; base < a.nent; base += (int64_t)gridDim.x * WPB * 32) {
+  // uniform constraints (a.npc > 1 entries each, npc | 32): the entry sums of a batch meet in shared memory and the
+  // first 32 / npc lanes finish the batch's constraints -- no e_out, no second kernel
+  __shared__ T s_ev[SINGLE ? 1 : WPB][SINGLE ? 1 : 32 * K];
+  T* const evS = s_ev[SINGLE ? 0 : warp];
+  const int npc = SINGLE ? 1 : a.npc;
+  // Every loop below has a block-uniform or compile-time trip count, so the shuffles need no convergence barriers:
+  // a block takes WPB batches at a time, warps whose batch starts beyond the list run on padding entries (row 0 with
+  // itself, coefficient 0) and write nothing.
+  for (int64_t cbk = blockIdx.x; cbk * (WPB * 32) < a.nent; cbk += gridDim.x) {
+    const int64_t base = (cbk * WPB + warp) * 32;
     const int64_t e = base + lane;
-    int jr = 0, kc = 0; T av = T(0);     // padding entries of the last batch: row 0 with itself, coefficient 0
+    int jr = 0, kc = 0; T av = T(0);
     if (e < a.nent) { jr = __ldg(a.e_row + e); kc = __ldg(a.e_col + e); av = __ldg(a.e_val + e); if (jr != kc) av += av; }
-    const int cnt = (int)min((int64_t)32, a.nent - base);
-    for (int j = 0; j < cnt; j += EL * UNR) {
+#pragma unroll
+    for (int j = 0; j < 32; j += EL * UNR) {
       P xj[UNR], xk[UNR], dj[UNR], dk[UNR];
       T au[UNR];
 #pragma unroll
       for (int u = 0; u < UNR; ++u) {
-        const int src = (j + u * EL + el) & 31;
+        const int src = j + u * EL + el;
         const int ju = __shfl_sync(0xffffffffu, jr, src), ku = __shfl_sync(0xffffffffu, kc, src);
         au[u] = __shfl_sync(0xffffffffu, av, src);
         xj[u] = load_pack(Xp + (int64_t)ju * ld);
@@ -887,11 +909,15 @@ __global__ void __launch_bounds__(kBlock) k_ent_cw(const ConsArgs<T> a) {
         T s1 = T(0), s2 = T(0);
         if (LS) { s1 = seg(dotp(xj[u], dk[u]) + dotp(dj[u], xk[u])); s2 = seg(dotp(dj[u], dk[u])); }
         const int64_t ei = base + j + u * EL + el;
-        if (pl == 0 && j + u * EL + el < cnt) {
+        if (pl == 0 && ei < a.nent) {
           const T v0 = au[u] * s0, v1 = au[u] * s1, v2 = au[u] * s2;
           if (ei < a.nf_A) {
             if (SINGLE) {
               cons_finish<MODE>(st, ei, (double)v0, (double)v1, (double)v2, a.y, a.b, a.sigma, a.z, a.lam);
+            } else if (npc > 1) {
+              const int sl = (j + u * EL + el) * K;
+              evS[sl] = v0;
+              if (LS) { evS[sl + 1] = v1; evS[sl + 2] = v2; }
             } else {
               a.e_out[ei * K] = v0;
               if (LS) { a.e_out[ei * K + 1] = v1; a.e_out[ei * K + 2] = v2; }
@@ -901,6 +927,20 @@ __global__ void __launch_bounds__(kBlock) k_ent_cw(const ConsArgs<T> a) {
           }
         }
       }
+    }
+    if (!SINGLE && npc > 1) {   // block-uniform condition
+      __syncwarp();
+      const int64_t ci = base / npc + lane;          // base is a multiple of 32, hence of npc
+      if (lane < 32 / npc && ci < a.m) {
+        double t0 = 0.0, t1 = 0.0, t2 = 0.0;
+        for (int t = 0; t < npc; ++t) {
+          const int sl = (lane * npc + t) * K;
+          t0 += (double)evS[sl];
+          if (LS) { t1 += (double)evS[sl + 1]; t2 += (double)evS[sl + 2]; }
+        }
+        cons_finish<MODE>(st, ci, t0, t1, t2, a.y, a.b, a.sigma, a.z, a.lam);
+      }
+      __syncwarp();
     }
   }
   block_reduce_store<NST>(st, a.partials + (int64_t)blockIdx.x * kNStat);
