@@ -99,6 +99,19 @@ alora_status alora_get_stats(alora_ctx *ctx, double stats[8]); /* of the last al
  * Enqueues only. */
 alora_status alora_get_lambda(alora_ctx *ctx, double *lam_dev);
 
+/* Helpers for callers that assemble z = A(RR^T) themselves -- the row-sharded evaluation of
+ * paper_2505_15775_b200/sharded.py, where z is the sum over ranks of the partial z of each rank's entries and a rank
+ * owns a block of rows.
+ * alora_dual_terms: q = z - b, lambda = y - sigma q with the (y, sigma) of alora_set_dual, for the
+ *   caller's z_dev (DEVICE fp64[m]); lam_dev (DEVICE fp64[m]) receives lambda or is NULL; out: HOST double[3] =
+ *   {y.q, ||q||^2, lambda.z}.
+ * alora_rowdots: out (HOST double[2]) = {sum X_ij^2, sum X_ij Y_ij} over the first n_rows rows of X, Y (DEVICE, ctx
+ *   dtype, row-major with r columns and leading dimension ld).
+ * Both synchronise. */
+alora_status alora_dual_terms(alora_ctx *ctx, const double *z_dev, double *lam_dev, double out[3]);
+alora_status alora_rowdots(alora_ctx *ctx, const void *X, const void *Y, int64_t n_rows, int32_t r, int64_t ld,
+                           double out[2]);
+
 /* Same as alora_eval but R, G, z are HOST buffers (G, z may be NULL): copies R to the device,
  * evaluates, copies G and z back, inside the call.  stats as above (must be non-NULL). */
 alora_status alora_eval_host(alora_ctx *ctx, const void *R_host, int32_t r, int64_t ld, void *G_host,

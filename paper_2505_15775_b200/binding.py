@@ -97,6 +97,8 @@ _lib.alora_set_dual.argtypes = [_vp, _vp, _dbl]
 _lib.alora_eval.argtypes = [_vp, _vp, _i32, _i64, _vp, _vp, _vp]
 _lib.alora_get_stats.argtypes = [_vp, _vp]
 _lib.alora_get_lambda.argtypes = [_vp, _vp]
+_lib.alora_dual_terms.argtypes = [_vp, _vp, _vp, _vp]
+_lib.alora_rowdots.argtypes = [_vp, _vp, _vp, _i64, _i32, _i64, _vp]
 _lib.alora_eval_host.argtypes = [_vp, _vp, _i32, _i64, _vp, _vp, _vp]
 _lib.alora_step_host.argtypes = [_vp, _vp, _vp, _vp, _i32, _i64, _vp, _vp, _vp, _vp, _vp, _vp]
 _lib.alora_linesearch.argtypes = [_vp, _vp, _vp, _i32, _i64, _i32, _vp]
@@ -193,6 +195,18 @@ class Context:
 
     def get_lambda(self, lam):
         self._chk(_lib.alora_get_lambda(self._h, _ptr(lam)))
+
+    def dual_terms(self, z, lam=None):
+        """(y.q, ||q||^2, lambda.z) for a caller-supplied device z (q = z - b); lam (device, m) receives lambda."""
+        out = np.zeros(3)
+        self._chk(_lib.alora_dual_terms(self._h, _ptr(z), _ptr(lam), out.ctypes.data))
+        return out
+
+    def rowdots(self, X, Y, n_rows: int, r: int, ld: int):
+        """(sum X^2, sum X Y) over the first n_rows rows."""
+        out = np.zeros(2)
+        self._chk(_lib.alora_rowdots(self._h, _ptr(X), _ptr(Y), n_rows, r, ld, out.ctypes.data))
+        return out
 
     def eval_host(self, R_host, r: int, ld: int, G_host=None, z_host=None):
         out = np.zeros(8)

@@ -138,6 +138,27 @@ alora_status resolve_mu(alora_ctx* c, const double** mu, const char* who) {
   return ALORA_OK;
 }
 
+// the scalars of the last evaluation: device-to-host copies into the pinned block (no synchronisation), and their
+// assembly into stats[8] once the stream has been synchronised
+alora_status stats_enqueue(alora_ctx* c, int r_lowrank) {
+  ALORA_CUDA(c, cudaMemcpyAsync(c->pinned, c->stats_dev, sizeof(double) * kNStat, cudaMemcpyDeviceToHost, c->stream));
+  if (c->pC && c->cls == 1)
+    ALORA_CUDA(c, cudaMemcpyAsync(c->pinned + 64, c->TmR, sizeof(double) * c->pC * r_lowrank, cudaMemcpyDeviceToHost, c->stream));
+  return ALORA_OK;
+}
+void stats_finish(alora_ctx* c, int r_lowrank, double stats[8]) {
+  const double* p = c->pinned;
+  double cx = p[ES_CX];
+  if (c->pC && c->cls == 1)
+    for (int q = 0; q < c->pC; ++q) {
+      double t = 0.0;
+      for (int k = 0; k < r_lowrank; ++k) t += p[64 + q * r_lowrank + k] * p[64 + q * r_lowrank + k];
+      cx += c->s_host[q] * t;
+    }
+  stats[1] = cx; stats[2] = p[ES_YQ]; stats[3] = p[ES_QQ]; stats[4] = p[ES_GG]; stats[5] = p[ES_GR]; stats[6] = p[ES_LZ]; stats[7] = 0.0;
+  stats[0] = cx - p[ES_YQ] + 0.5 * c->sigma * p[ES_QQ];
+}
+
 }  // namespace alora
 
 // ---------------------------------------------------------------------------------------------
@@ -226,8 +247,8 @@ alora_status launch_diag_rows(alora_ctx* c, int vec, int nvec, int exact, int sh
 // The cooperative kernels (k_ent_cw, k_rows_cw) pay when a gathered row is more than one pack (otherwise a thread per
 // item already makes one request per row) and the rows do not sit in L1 (measured, profiles/r2b_README.md: config 3
 // 466 -> 352 us per step, config 2 adjoint 39 -> 28 us; config 5, n r = 120 KB: 84 -> 96 us).  ALORA_CW=0 / 2: never / always.
-inline bool use_cw(const alora_ctx* c, const Geo& g, int r) {
-  if (c->cw == 0 || g.nvec > 32) return false;
+inline bool use_cw(const alora_ctx* c, const Geo& g, int r, int64_t ld) {
+  if (c->cw == 0 || g.nvec > 32 || (uint64_t)c->n * (uint64_t)ld >= ((uint64_t)1 << 32)) return false;   // 32-bit element offsets
   if (c->cw == 2) return true;
   return g.nvec >= 2 && (size_t)c->n * (size_t)r * c->esz >= ((size_t)1 << 20);
 }
@@ -248,7 +269,7 @@ template <typename T> alora_status launch_adj_general(alora_ctx* c, const Geo& g
     ALORA_CUDA(c, launch_rows_seg(g.vec, g.shape, a, gs, c->stream));
     c->launches++;
   }
-  if (use_cw(c, g, a.r) && !c->row_perm && !c->ep_wide) {
+  if (use_cw(c, g, a.r, a.ld) && !c->row_perm && !c->ep_wide) {
     // cooperative warp per row (k_rows_cw): coalesced entry metadata, one request per gathered row; not for skewed row
     // lengths (config 7: 769 against 474 us) nor for very long rows of thin vectors (k_rows_ep is as fast there)
     int pl2 = 0; while ((1 << pl2) < g.nvec) ++pl2;
@@ -390,7 +411,7 @@ template <typename T> alora_status eval_impl(alora_ctx* c, const T* R, int32_t r
     fill_cons(c, ca, g, R, (const T*)nullptr, r, ld);
     ca.z = zout;
     int gc = 0;
-    if (use_cw(c, g, r) && c->m > 0) {
+    if (use_cw(c, g, r, ld) && c->m > 0) {
       int ge = 0, gf = 0;
       s = forward_cw<T>(c, g, CONS_EVAL, ca, c->nf_A, &ge, &gf, nullptr);
       if (s != ALORA_OK) return s;
@@ -437,20 +458,10 @@ template <typename T> alora_status eval_impl(alora_ctx* c, const T* R, int32_t r
 }
 
 alora_status fetch_stats(alora_ctx* c, int r_lowrank, double stats[8]) {
-  ALORA_CUDA(c, cudaMemcpyAsync(c->pinned, c->stats_dev, sizeof(double) * kNStat, cudaMemcpyDeviceToHost, c->stream));
-  if (c->pC && c->cls == 1)
-    ALORA_CUDA(c, cudaMemcpyAsync(c->pinned + 64, c->TmR, sizeof(double) * c->pC * r_lowrank, cudaMemcpyDeviceToHost, c->stream));
+  alora_status s = stats_enqueue(c, r_lowrank);
+  if (s != ALORA_OK) return s;
   ALORA_CUDA(c, cudaStreamSynchronize(c->stream));
-  const double* p = c->pinned;
-  double cx = p[ES_CX];
-  if (c->pC && c->cls == 1)
-    for (int q = 0; q < c->pC; ++q) {
-      double t = 0.0;
-      for (int k = 0; k < r_lowrank; ++k) t += p[64 + q * r_lowrank + k] * p[64 + q * r_lowrank + k];
-      cx += c->s_host[q] * t;
-    }
-  stats[1] = cx; stats[2] = p[ES_YQ]; stats[3] = p[ES_QQ]; stats[4] = p[ES_GG]; stats[5] = p[ES_GR]; stats[6] = p[ES_LZ]; stats[7] = 0.0;
-  stats[0] = cx - p[ES_YQ] + 0.5 * c->sigma * p[ES_QQ];
+  stats_finish(c, r_lowrank, stats);
   return ALORA_OK;
 }
 
@@ -472,7 +483,7 @@ template <typename T> alora_status ls_impl(alora_ctx* c, const T* R, const T* D,
     }
     ConsArgs<T> ca;
     fill_cons(c, ca, g, R, D, r, ld);
-    if (use_cw(c, g, r) && c->nf_A + c->nf_C > 0) {
+    if (use_cw(c, g, r, ld) && c->nf_A + c->nf_C > 0) {
       int ge = 0, gf = 0;
       s = forward_cw<T>(c, g, CONS_LS, ca, c->nf_A + c->nf_C, &ge, &gf, c->ls_dev);
       if (s != ALORA_OK) return s;

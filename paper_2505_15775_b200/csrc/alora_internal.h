@@ -127,6 +127,8 @@ alora_status fail(alora_ctx* c, alora_status s, const std::string& msg);
   } while (0)
 
 // alora_ctx.cu
+alora_status stats_enqueue(alora_ctx* c, int r_lowrank);                    // scalars of the last evaluation: enqueue the copies ...
+void stats_finish(alora_ctx* c, int r_lowrank, double stats[8]);          // ... and assemble them after a synchronise
 alora_status resolve_mu(alora_ctx* c, const double** mu, const char* who);   // NULL -> lambda of the last alora_eval
 int pick_vec(const alora_ctx* c, int64_t ld, const void* p0, const void* p1, const void* p2);
 void free_solve_workspace(alora_ctx* c);

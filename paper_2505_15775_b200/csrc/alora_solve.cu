@@ -201,20 +201,24 @@ __global__ void __launch_bounds__(kBlock) k_lbfgs_combine(int64_t N, const T* G,
     reinterpret_cast<Pack<T, VEC>*>(D)[i] = o;
   }
 }
-// w -= a v + b u   (Lanczos three-term recurrence)
-template <typename T> __global__ void k_axpy2(int64_t N, double a, const T* v, double b, const T* u, T* w) {
+// w -= a v + b u   (Lanczos three-term recurrence); a = *a_dev is <v, S v> left on the device by the matvec
+template <typename T> __global__ void k_axpy2(int64_t N, const double* a_dev, const T* v, double b, const T* u, T* w) {
+  const double a = *a_dev;
   for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (int64_t)gridDim.x * blockDim.x)
     w[i] = (T)((double)w[i] - a * (double)v[i] - (u ? b * (double)u[i] : 0.0));
 }
-// c[j] partials for j < k: V is k x N (row j contiguous);  blockIdx.y = j
+// c[j] = <V_j, w> for j < k: V is k x N (row j contiguous), blockIdx.y = j, nchunk blocks per j leave partial sums;
+// the block that draws the last ticket adds the chunks of every j in order (no separate reduction launch)
 template <typename T>
-__global__ void __launch_bounds__(kBlock) k_basis_dots(int64_t N, const T* V, const T* w, double* part, int nchunk) {
+__global__ void __launch_bounds__(kBlock) k_basis_dots(int64_t N, const T* V, const T* w, double* part, int nchunk, int k,
+                                                       double* c, unsigned int* ticket) {
   const int j = blockIdx.y;
   const T* vj = V + (int64_t)j * N;
   double st[1] = {0.0};
   for (int64_t i = (int64_t)blockIdx.x * kBlock + threadIdx.x; i < N; i += (int64_t)gridDim.x * kBlock)
     st[0] += (double)vj[i] * (double)w[i];
   __shared__ double sm[kBlock / 32];
+  __shared__ unsigned int s_last;
   const double v = warp_sum(st[0]);
   if ((threadIdx.x & 31) == 0) sm[threadIdx.x >> 5] = v;
   __syncthreads();
@@ -222,23 +226,53 @@ __global__ void __launch_bounds__(kBlock) k_basis_dots(int64_t N, const T* V, co
     double t = 0.0;
     for (int wv = 0; wv < kBlock / 32; ++wv) t += sm[wv];
     part[(int64_t)j * nchunk + blockIdx.x] = t;
+    __threadfence();
+    s_last = (atomicAdd(ticket, 1u) == gridDim.x * gridDim.y - 1) ? 1u : 0u;
   }
-}
-__global__ void k_basis_dots_reduce(const double* part, int nchunk, int k, double* c) {
-  const int j = blockIdx.x * blockDim.x + threadIdx.x;
-  if (j < k) {
+  __syncthreads();
+  if (!s_last) return;
+  __threadfence();
+  for (int jj = threadIdx.x; jj < k; jj += kBlock) {
     double t = 0.0;
-    for (int i = 0; i < nchunk; ++i) t += part[(int64_t)j * nchunk + i];
-    c[j] = t;
+    for (int i = 0; i < nchunk; ++i) t += __ldcg(part + (int64_t)jj * nchunk + i);
+    c[jj] = t;
   }
+  if (threadIdx.x == 0) *ticket = 0u;
 }
-// out[i] = beta*out[i] + sign * sum_j c[j] V[j][i]    (c on the device)
+// out[i] = beta*out[i] + sign * sum_j c[j] V[j][i]    (c on the device); nrm != nullptr: also ||out||^2 (ordered
+// two-stage sum, the block that finishes last adds the per-block partials)
 template <typename T>
-__global__ void k_basis_combine(int64_t N, int k, const T* V, const double* c, double beta, double sign, T* out) {
+__global__ void __launch_bounds__(kBlock) k_basis_combine(int64_t N, int k, const T* V, const double* c, double beta, double sign, T* out,
+                                                          double* part, double* nrm, unsigned int* ticket) {
+  double st[1] = {0.0};
   for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (int64_t)gridDim.x * blockDim.x) {
     double t = 0.0;
     for (int j = 0; j < k; ++j) t += c[j] * (double)V[(int64_t)j * N + i];
-    out[i] = (T)((beta != 0.0 ? beta * (double)out[i] : 0.0) + sign * t);
+    const T o = (T)((beta != 0.0 ? beta * (double)out[i] : 0.0) + sign * t);
+    out[i] = o;
+    st[0] += (double)o * (double)o;
+  }
+  if (!nrm) return;
+  __shared__ double sm[kBlock / 32];
+  __shared__ unsigned int s_last;
+  const double v = warp_sum(st[0]);
+  if ((threadIdx.x & 31) == 0) sm[threadIdx.x >> 5] = v;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    double t = 0.0;
+    for (int wv = 0; wv < kBlock / 32; ++wv) t += sm[wv];
+    part[blockIdx.x] = t;
+    __threadfence();
+    s_last = (atomicAdd(ticket, 1u) == gridDim.x - 1) ? 1u : 0u;
+  }
+  __syncthreads();
+  if (!s_last) return;
+  __threadfence();
+  if (threadIdx.x < 32) {
+    double t = 0.0;
+    for (int i = threadIdx.x; i < (int)gridDim.x; i += 32) t += __ldcg(part + i);   // lane-strided, then an ordered warp sum
+    t = warp_sum(t);
+    if (threadIdx.x == 0) { *nrm = t; *ticket = 0u; }
   }
 }
 // v0[i] = counter_uniform(seed, i) in (-1,1): splitmix64-style hash, integer arithmetic only
@@ -657,21 +691,24 @@ alora_status lanczos_impl(alora_ctx* c, const double* mu, int kmax, double tol_a
   int k = 0;
   bool conv = false;
   while (true) {
+    // one step = 6 launches and ONE synchronisation: matvec (leaves alpha = <v, S v> on the device), three-term
+    // recurrence reading alpha there, two classical Gram-Schmidt passes (dots with their reduction fused, combine; the
+    // second combine also forms ||w||^2), then alpha and ||w||^2 come back together
     T* vk = V + (int64_t)k * n;
-    double a;
-    s = alora_smatvec(c, mu, vk, 1, wv, &a); if (s != ALORA_OK) return s;
+    s = alora_smatvec(c, mu, vk, 1, wv, nullptr); if (s != ALORA_OK) return s;
     if (n_matvec) ++*n_matvec;
-    al.push_back(a);
-    k_axpy2<T><<<g, 256, 0, c->stream>>>(n, a, vk, k ? be.back() : 0.0, k ? vk - n : (const T*)nullptr, wv);
+    k_axpy2<T><<<g, 256, 0, c->stream>>>(n, c->mv_dev + ES_GR, vk, k ? be.back() : 0.0, k ? vk - n : (const T*)nullptr, wv);
     c->launches++;
     for (int pass = 0; pass < 2; ++pass) {  // classical Gram-Schmidt against V[0..k], twice
-      k_basis_dots<T><<<dim3(w->bd_chunks, k + 1), kBlock, 0, c->stream>>>(n, V, wv, w->bd_part, w->bd_chunks);
-      k_basis_dots_reduce<<<(k + 1 + 127) / 128, 128, 0, c->stream>>>(w->bd_part, w->bd_chunks, k + 1, w->cvec);
-      k_basis_combine<T><<<g, 256, 0, c->stream>>>(n, k + 1, V, w->cvec, 1.0, -1.0, wv);
-      c->launches += 3;
+      k_basis_dots<T><<<dim3(w->bd_chunks, k + 1), kBlock, 0, c->stream>>>(n, V, wv, w->bd_part, w->bd_chunks, k + 1, w->cvec, c->ticket);
+      k_basis_combine<T><<<g, kBlock, 0, c->stream>>>(n, k + 1, V, w->cvec, 1.0, -1.0, wv, w->red_part, pass ? w->red_out : nullptr, c->ticket);
+      c->launches += 2;
     }
-    double b2;
-    s = dot1<T>(c, n, wv, wv, &b2); if (s != ALORA_OK) return s;
+    ALORA_CUDA(c, cudaMemcpyAsync(c->pinned + 48, w->red_out, sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    ALORA_CUDA(c, cudaMemcpyAsync(c->pinned + 49, c->mv_dev + ES_GR, sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    ALORA_CUDA(c, cudaStreamSynchronize(c->stream));
+    const double b2 = c->pinned[48], a = c->pinned[49];
+    al.push_back(a);
     const double beta = std::sqrt(b2);
     beta_last = beta;
     ++k;
@@ -688,7 +725,7 @@ alora_status lanczos_impl(alora_ctx* c, const double* mu, int kmax, double tol_a
   }
   if (v_out) {  // Ritz vector V_k s, normalised
     ALORA_CUDA(c, cudaMemcpyAsync(w->cvec, sv.data(), sizeof(double) * k, cudaMemcpyHostToDevice, c->stream));
-    k_basis_combine<T><<<g, 256, 0, c->stream>>>(n, k, V, w->cvec, 0.0, 1.0, v_out);
+    k_basis_combine<T><<<g, kBlock, 0, c->stream>>>(n, k, V, w->cvec, 0.0, 1.0, v_out, nullptr, nullptr, nullptr);
     c->launches++;
     double vv;
     s = dot1<T>(c, n, v_out, v_out, &vv); if (s != ALORA_OK) return s;
@@ -712,7 +749,7 @@ alora_status lanczos_impl(alora_ctx* c, const double* mu, int kmax, double tol_a
       if (!U_out) continue;
       ALORA_CUDA(c, cudaMemcpyAsync(w->cvec, sj.data(), sizeof(double) * k, cudaMemcpyHostToDevice, c->stream));
       T* uj = U_out + (int64_t)j * n;
-      k_basis_combine<T><<<g, 256, 0, c->stream>>>(n, k, V, w->cvec, 0.0, 1.0, uj);
+      k_basis_combine<T><<<g, kBlock, 0, c->stream>>>(n, k, V, w->cvec, 0.0, 1.0, uj, nullptr, nullptr, nullptr);
       c->launches++;
       double vv;
       s = dot1<T>(c, n, uj, uj, &vv); if (s != ALORA_OK) return s;
@@ -739,6 +776,71 @@ extern "C" void alora_default_params(alora_params* p) {
   p->it_max = 500; p->lbfgs_mem = 5; p->p_max = 1; p->k_max = 300; p->tau_neg = -1.0; p->tol_eig = -1.0;
   p->gamma = 2.0; p->kappa = 0.25; p->sigma_max = 1e8; p->tau_shrink = 1e-8; p->s_max = 1e6; p->seed = 12345;
   p->stall_tol = 0.0; p->stall_iters = 3; p->pad_ = 0;
+}
+
+namespace alora {
+__global__ void __launch_bounds__(kBlock) k_dual_terms(int64_t m, const double* y, const double* z, const double* b, double sigma,
+                                                       double* lam, double* part) {
+  double st[3] = {0.0, 0.0, 0.0};
+  for (int64_t i = (int64_t)blockIdx.x * kBlock + threadIdx.x; i < m; i += (int64_t)gridDim.x * kBlock) {
+    const double q = z[i] - b[i], yv = y[i], l = yv - sigma * q;
+    if (lam) lam[i] = l;
+    st[0] += yv * q; st[1] += q * q; st[2] += l * z[i];
+  }
+  block_reduce_store<3>(st, part + (int64_t)blockIdx.x * kNStat);
+}
+// sums over the first n_rows rows of row-major X, Y (r columns, leading dimension ld): X.X and X.Y
+template <typename T>
+__global__ void __launch_bounds__(kBlock) k_rowdots(int64_t n_rows, int r, int64_t ld, const T* X, const T* Y, double* part) {
+  double st[3] = {0.0, 0.0, 0.0};
+  const int64_t N = n_rows * r;
+  for (int64_t i = (int64_t)blockIdx.x * kBlock + threadIdx.x; i < N; i += (int64_t)gridDim.x * kBlock) {
+    const int64_t row = i / r, idx = row * ld + (i - row * r);
+    const double x = (double)X[idx];
+    st[0] += x * x; st[1] += x * (double)Y[idx];
+  }
+  block_reduce_store<3>(st, part + (int64_t)blockIdx.x * kNStat);
+}
+}  // namespace alora
+
+namespace {
+alora_status fetch_red(alora_ctx* c, int grid, int cnt, double* out) {
+  alora::SolveWorkspace* w = c->ws;
+  alora::k_reduce_rows<<<1, alora::kBlock, 0, c->stream>>>(w->red_part, grid, w->red_out);
+  c->launches++;
+  ALORA_CUDA(c, cudaMemcpyAsync(c->pinned + 48, w->red_out, sizeof(double) * 3, cudaMemcpyDeviceToHost, c->stream));
+  ALORA_CUDA(c, cudaStreamSynchronize(c->stream));
+  for (int i = 0; i < cnt; ++i) out[i] = c->pinned[48 + i];
+  return ALORA_OK;
+}
+}  // namespace
+
+extern "C" alora_status alora_dual_terms(alora_ctx* c, const double* z_dev, double* lam_dev, double out[3]) {
+  if (!c || !out || (!z_dev && c->m > 0)) return c ? fail(c, ALORA_EINVAL, "alora_dual_terms: NULL argument") : ALORA_EINVAL;
+  if (!c->have_dual) return fail(c, ALORA_ESTATE, "alora_dual_terms before alora_set_dual");
+  ALORA_CUDA(c, cudaSetDevice(c->device));
+  alora_status s = ensure_ws(c);
+  if (s != ALORA_OK) return s;
+  out[0] = out[1] = out[2] = 0.0;
+  if (c->m == 0) return ALORA_OK;
+  const int grid = (int)std::max<int64_t>(1, std::min<int64_t>((c->m + kBlock - 1) / kBlock, kRedBlocks));
+  k_dual_terms<<<grid, kBlock, 0, c->stream>>>(c->m, c->y, z_dev, c->b, c->sigma, lam_dev, c->ws->red_part);
+  c->launches++;
+  return fetch_red(c, grid, 3, out);
+}
+
+extern "C" alora_status alora_rowdots(alora_ctx* c, const void* X, const void* Y, int64_t n_rows, int32_t r, int64_t ld, double out[2]) {
+  if (!c || !X || !Y || !out || n_rows < 0 || r < 1 || ld < r) return c ? fail(c, ALORA_EINVAL, "alora_rowdots: bad argument") : ALORA_EINVAL;
+  ALORA_CUDA(c, cudaSetDevice(c->device));
+  alora_status s = ensure_ws(c);
+  if (s != ALORA_OK) return s;
+  out[0] = out[1] = 0.0;
+  if (n_rows == 0) return ALORA_OK;
+  const int grid = (int)std::max<int64_t>(1, std::min<int64_t>((n_rows * r + kBlock - 1) / kBlock, kRedBlocks));
+  if (c->dtype == ALORA_F32) k_rowdots<float><<<grid, kBlock, 0, c->stream>>>(n_rows, r, ld, (const float*)X, (const float*)Y, c->ws->red_part);
+  else k_rowdots<double><<<grid, kBlock, 0, c->stream>>>(n_rows, r, ld, (const double*)X, (const double*)Y, c->ws->red_part);
+  c->launches++;
+  return fetch_red(c, grid, 2, out);
 }
 
 extern "C" void alora_preset_params(alora_params* p, alora_dtype dtype) {
@@ -780,9 +882,11 @@ extern "C" alora_status alora_lanczos(alora_ctx* c, const double* mu_dev, int32_
 namespace alora {
 namespace {
 
+// launches k_lbfgs_dots and the copy of its sums into the pinned block (offset kLbPinned); no synchronisation
+constexpr int kLbPinned = 64 + 8 * 256;
 template <typename T>
-alora_status lbfgs_dots(alora_ctx* c, int64_t N, int np, bool have_new, double alpha, const T* D, const T* G, const T* Gp,
-                        const LbVecs& v, T* Snew, T* Ynew, double* host_out) {
+alora_status lbfgs_dots_enqueue(alora_ctx* c, int64_t N, int np, bool have_new, double alpha, const T* D, const T* G, const T* Gp,
+                                const LbVecs& v, T* Snew, T* Ynew) {
   SolveWorkspace* w = c->ws;
   const int grid = (int)std::max<int64_t>(1, std::min<int64_t>((N / (16 / (int64_t)sizeof(T)) + kBlock - 1) / kBlock, kRedBlocks));
   switch (np) {
@@ -792,9 +896,7 @@ alora_status lbfgs_dots(alora_ctx* c, int64_t N, int np, bool have_new, double a
     default: return fail(c, ALORA_EINVAL, "lbfgs_dots: too many pairs");
   }
   c->launches++;
-  ALORA_CUDA(c, cudaMemcpyAsync(c->pinned + 64, w->lb_out, sizeof(double) * kLbW, cudaMemcpyDeviceToHost, c->stream));
-  ALORA_CUDA(c, cudaStreamSynchronize(c->stream));
-  for (int i = 0; i < kLbW; ++i) host_out[i] = c->pinned[64 + i];
+  ALORA_CUDA(c, cudaMemcpyAsync(c->pinned + kLbPinned, w->lb_out, sizeof(double) * kLbW, cudaMemcpyDeviceToHost, c->stream));
   return ALORA_OK;
 }
 template <typename T>
@@ -878,23 +980,30 @@ alora_status solve_impl(alora_ctx* c, const alora_params* prm, T* R_user, int32_
     std::vector<double> lb_sg(nslot, 0.0), lb_yg(nslot, 0.0);
     int it = 0, stalled = 0; bool have_prev = false; double alpha = 0.0, gnorm = 0.0;
     while (true) {
-      s = alora_eval(c, Rw, ld, ld, Gw, w->z, st); if (s != ALORA_OK) return s;
+      // the evaluation and -- on the fused L-BFGS path -- the dots pass of the iteration are enqueued back to back and
+      // their scalars come back with ONE synchronisation (the dots pass needs nothing the host learns from the evaluation)
+      const bool fused = mem > 0 && mem < kLbMax;
+      std::vector<int> list;
+      if (fused) { list = pairs; if (have_prev) list.push_back(spare); }
+      const int np = (int)list.size();
+      s = alora_eval(c, Rw, ld, ld, Gw, w->z, nullptr); if (s != ALORA_OK) return s;
+      s = stats_enqueue(c, ld); if (s != ALORA_OK) return s;
+      if (np > 0) {
+        LbVecs lv;
+        for (int j = 0; j < kLbMax; ++j) { lv.S[j] = Sb[list[j < np ? j : 0]]; lv.Y[j] = Yb[list[j < np ? j : 0]]; }
+        s = lbfgs_dots_enqueue<T>(c, N, np, have_prev, alpha, Dw, Gw, Gp, lv, Sb[spare], Yb[spare]); if (s != ALORA_OK) return s;
+      }
+      ALORA_CUDA(c, cudaStreamSynchronize(c->stream));
+      stats_finish(c, ld, st);
       ++rec.n_evals;
       gnorm = std::sqrt(st[4]);
       if (!std::isfinite(st[0]) || !std::isfinite(gnorm)) return fail(c, ALORA_ECUDA, "alora_solve: non-finite f or gradient");
-      const bool fused = mem > 0 && mem < kLbMax;
       bool steepest = true;
       if (fused) {
         // ---- L-BFGS in two passes: all dot products of the iteration (and the new pair) in k_lbfgs_dots, the
         //      coefficients of d in span{g, S_j, Y_j} on the host (same recursion as the two-loop form), one combine
-        std::vector<int> list(pairs);
-        if (have_prev) list.push_back(spare);
-        const int np = (int)list.size();
         if (np > 0) {
-          LbVecs lv;
-          for (int j = 0; j < kLbMax; ++j) { lv.S[j] = Sb[list[j < np ? j : 0]]; lv.Y[j] = Yb[list[j < np ? j : 0]]; }
-          double h[kLbW];
-          s = lbfgs_dots<T>(c, N, np, have_prev, alpha, Dw, Gw, Gp, lv, Sb[spare], Yb[spare], h); if (s != ALORA_OK) return s;
+          const double* h = c->pinned + kLbPinned;
           for (int j = 0; j < np; ++j) { lb_sg[list[j]] = h[j]; lb_yg[list[j]] = h[np + j]; }
           if (have_prev) {
             const int slot = spare;

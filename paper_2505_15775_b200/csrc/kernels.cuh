@@ -562,6 +562,7 @@ __global__ void __launch_bounds__(kBlock) k_rows_cw(const RowArgs<T> a) {
   const bool pok = pl < nvec;                    // this lane owns a pack of the row
   const bool tailmask = VEC > 1 && !a.exact && pl == nvec - 1;
   const int64_t ld = a.ld;
+  const uint32_t ld32 = (uint32_t)a.ld;          // the host selects this kernel only when n * ld < 2^32 elements
   const int plc = min(pl, nvec - 1);             // lanes beyond the row read its last pack (same request) and drop it
   const T* const Xp = a.X + plc * VEC;           // lane's pack of row 0
   const T sc = (T)a.scale;
@@ -610,7 +611,7 @@ __global__ void __launch_bounds__(kBlock) k_rows_cw(const RowArgs<T> a) {
           for (int u = 0; u < UNR; ++u) {
             const int src = j + u * EL;          // < 32: EL * UNR <= 32 and j - el is a multiple of EL * UNR
             cf[u] = cfS[src];
-            pk[u] = load_pack(Xp + (int64_t)colS[src] * ld);
+            pk[u] = load_pack(Xp + (uint32_t)colS[src] * ld32);   // 32-bit element offset: two instructions instead of seven
           }
 #pragma unroll
           for (int u = 0; u < UNR; ++u)
@@ -848,7 +849,7 @@ __global__ void __launch_bounds__(kBlock) k_ent_cw(const ConsArgs<T> a) {
   const int pl = lane & (PL - 1), el = lane / PL;
   const bool pok = pl < nvec;
   const bool tailmask = VEC > 1 && !a.exact && pl == nvec - 1;
-  const int64_t ld = a.ld;
+  const uint32_t ld32 = (uint32_t)a.ld;          // the host selects this kernel only when n * ld < 2^32 elements
   const int plc = min(pl, nvec - 1);
   const T* const Xp = a.X + plc * VEC;
   const T* const Dp = LS ? a.X2 + plc * VEC : nullptr;
@@ -887,6 +888,9 @@ __global__ void __launch_bounds__(kBlock) k_ent_cw(const ConsArgs<T> a) {
     const int64_t e = base + lane;
     int jr = 0, kc = 0; T av = T(0);
     if (e < a.nent) { jr = __ldg(a.e_row + e); kc = __ldg(a.e_col + e); av = __ldg(a.e_val + e); if (jr != kc) av += av; }
+    // slots [0, lim_A) of the batch are constraint entries, [lim_A, lim_ent) entries of C's list (32-bit compares below)
+    const int lim_ent = (int)max((int64_t)0, min((int64_t)32, a.nent - base));
+    const int lim_A = (int)max((int64_t)0, min((int64_t)32, a.nf_A - base));
 #pragma unroll
     for (int j = 0; j < 32; j += EL * UNR) {
       P xj[UNR], xk[UNR], dj[UNR], dk[UNR];
@@ -896,11 +900,12 @@ __global__ void __launch_bounds__(kBlock) k_ent_cw(const ConsArgs<T> a) {
         const int src = j + u * EL + el;
         const int ju = __shfl_sync(0xffffffffu, jr, src), ku = __shfl_sync(0xffffffffu, kc, src);
         au[u] = __shfl_sync(0xffffffffu, av, src);
-        xj[u] = load_pack(Xp + (int64_t)ju * ld);
-        xk[u] = ku != ju ? load_pack(Xp + (int64_t)ku * ld) : xj[u];
+        const uint32_t oj = (uint32_t)ju * ld32, ok = (uint32_t)ku * ld32;   // 32-bit element offsets
+        xj[u] = load_pack(Xp + oj);
+        xk[u] = ku != ju ? load_pack(Xp + ok) : xj[u];
         if (LS) {
-          dj[u] = load_pack(Dp + (int64_t)ju * ld);
-          dk[u] = ku != ju ? load_pack(Dp + (int64_t)ku * ld) : dj[u];
+          dj[u] = load_pack(Dp + oj);
+          dk[u] = ku != ju ? load_pack(Dp + ok) : dj[u];
         }
       }
 #pragma unroll
@@ -908,14 +913,15 @@ __global__ void __launch_bounds__(kBlock) k_ent_cw(const ConsArgs<T> a) {
         const T s0 = seg(dotp(xj[u], xk[u]));
         T s1 = T(0), s2 = T(0);
         if (LS) { s1 = seg(dotp(xj[u], dk[u]) + dotp(dj[u], xk[u])); s2 = seg(dotp(dj[u], dk[u])); }
-        const int64_t ei = base + j + u * EL + el;
-        if (pl == 0 && ei < a.nent) {
+        const int slot = j + u * EL + el;
+        const int64_t ei = base + slot;
+        if (pl == 0 && slot < lim_ent) {
           const T v0 = au[u] * s0, v1 = au[u] * s1, v2 = au[u] * s2;
-          if (ei < a.nf_A) {
+          if (slot < lim_A) {
             if (SINGLE) {
               cons_finish<MODE>(st, ei, (double)v0, (double)v1, (double)v2, a.y, a.b, a.sigma, a.z, a.lam);
             } else if (npc > 1) {
-              const int sl = (j + u * EL + el) * K;
+              const int sl = slot * K;
               evS[sl] = v0;
               if (LS) { evS[sl + 1] = v1; evS[sl + 2] = v2; }
             } else {
@@ -977,9 +983,19 @@ __global__ void __launch_bounds__(kBlock) k_long_fin_e(const ConsArgs<T> a, doub
   const int slot = blockIdx.x, lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int64_t i = a.long_cons[slot], e0 = a.ptr[i], e1 = a.ptr[i + 1];
   double v[3] = {0.0, 0.0, 0.0};
-  for (int64_t e = e0 + threadIdx.x; e < e1; e += kBlock) {
-    v[0] += (double)a.e_out[e * K];
-    if (MODE == CONS_LS) { v[1] += (double)a.e_out[e * K + 1]; v[2] += (double)a.e_out[e * K + 2]; }
+  constexpr int U = 8;   // loads in flight per thread (the sums stay in entry order)
+  for (int64_t eb = e0 + threadIdx.x; eb < e1; eb += (int64_t)kBlock * U) {
+    T t[U][K];
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+      const int64_t e = eb + (int64_t)u * kBlock;
+#pragma unroll
+      for (int k = 0; k < K; ++k) t[u][k] = e < e1 ? __ldcg(a.e_out + e * K + k) : T(0);
+    }
+#pragma unroll
+    for (int u = 0; u < U; ++u)
+#pragma unroll
+      for (int k = 0; k < K; ++k) v[k] += (double)t[u][k];
   }
   for (int k = 0; k < 3; ++k) { const double t = warp_sum(v[k]); if (lane == 0) sm[k][warp] = t; }
   __syncthreads();
