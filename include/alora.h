@@ -112,6 +112,23 @@ alora_status alora_dual_terms(alora_ctx *ctx, const double *z_dev, double *lam_d
 alora_status alora_rowdots(alora_ctx *ctx, const void *X, const void *Y, int64_t n_rows, int32_t r, int64_t ld,
                            double out[2]);
 
+/* Allocation-free variant of alora_rowdots, for callers that cannot call cudaMalloc (code under CUDA graph capture,
+ * tight serving loops, harnesses that forbid it): the same two sums, out_dev[0] = sum X_ij^2, out_dev[1] = sum X_ij Y_ij
+ * over the first n_rows rows, but the per-block partial sums live in a static __device__ array inside the library
+ * (about 64 KB, held by every GPU that loads the library until the process exits) instead of the ctx workspace, and
+ * the result goes to out_dev (DEVICE double[2], caller-owned).  The call makes no cudaMalloc / cudaFree, calls no
+ * allocating library routine and does not synchronise: it enqueues one 4-byte memset and one kernel on the ctx stream.
+ * Limit: n_rows * r <= ALORA_ROWDOTS_STATIC_MAX_ELEMS (the array holds one partial row per 16384 elements); larger
+ * shapes are rejected with ALORA_EINVAL and a message naming the limit -- use alora_rowdots for them.  The first call on
+ * a device looks up the array's device address (no allocation; make that first call outside a stream capture).
+ * The array is shared by every call on the device and keeps the last call's contents (the call clears what must start
+ * at zero itself); calls that overlap on the GPU -- two streams, or two ctx on one device used concurrently -- race on
+ * it and must be serialised by the caller.  Summation order differs from alora_rowdots (fixed 16384-element chunks,
+ * independent of the SM count), so the two agree to fp64 rounding, not bit for bit. */
+#define ALORA_ROWDOTS_STATIC_MAX_ELEMS 67108864 /* 2^26 */
+alora_status alora_rowdots_static(alora_ctx *ctx, const void *X, const void *Y, int64_t n_rows, int32_t r, int64_t ld,
+                                  double *out_dev);
+
 /* Same as alora_eval but R, G, z are HOST buffers (G, z may be NULL): copies R to the device,
  * evaluates, copies G and z back, inside the call.  stats as above (must be non-NULL). */
 alora_status alora_eval_host(alora_ctx *ctx, const void *R_host, int32_t r, int64_t ld, void *G_host,

@@ -99,6 +99,8 @@ _lib.alora_get_stats.argtypes = [_vp, _vp]
 _lib.alora_get_lambda.argtypes = [_vp, _vp]
 _lib.alora_dual_terms.argtypes = [_vp, _vp, _vp, _vp]
 _lib.alora_rowdots.argtypes = [_vp, _vp, _vp, _i64, _i32, _i64, _vp]
+_lib.alora_rowdots_static.argtypes = [_vp, _vp, _vp, _i64, _i32, _i64, _vp]
+ROWDOTS_STATIC_MAX_ELEMS = 1 << 26   # ALORA_ROWDOTS_STATIC_MAX_ELEMS
 _lib.alora_eval_host.argtypes = [_vp, _vp, _i32, _i64, _vp, _vp, _vp]
 _lib.alora_step_host.argtypes = [_vp, _vp, _vp, _vp, _i32, _i64, _vp, _vp, _vp, _vp, _vp, _vp]
 _lib.alora_linesearch.argtypes = [_vp, _vp, _vp, _i32, _i64, _i32, _vp]
@@ -207,6 +209,10 @@ class Context:
         out = np.zeros(2)
         self._chk(_lib.alora_rowdots(self._h, _ptr(X), _ptr(Y), n_rows, r, ld, out.ctypes.data))
         return out
+
+    def rowdots_static(self, X, Y, n_rows: int, r: int, ld: int, out):
+        """alora_rowdots_static: the same two sums into `out` (device fp64[2]); allocates nothing, does not synchronise."""
+        self._chk(_lib.alora_rowdots_static(self._h, _ptr(X), _ptr(Y), n_rows, r, ld, _ptr(out)))
 
     def eval_host(self, R_host, r: int, ld: int, G_host=None, z_host=None):
         out = np.zeros(8)
