@@ -172,6 +172,22 @@ template <typename T> alora_status build(alora_ctx* c, const alora_problem* P) {
       const int kUN = ell_slots(c->ell_wide), kUNL = ell_slots_ls(c->ell_wide);
       std::vector<int> ec((size_t)n * kUN), euc((size_t)n * kUNL);
       std::vector<T> ev((size_t)n * kUN), euv((size_t)n * kUNL);
+      // Wide block (meshes): within a row the slots are ordered nearest neighbour first (|col - j| ascending, unused
+      // slots last), so that slot u is an in-tile neighbour (read from the staged tile) or a farther one (gathered) for
+      // most rows of a warp alike and the kernel's in-tile / gather branch per slot rarely diverges (config 6: f + grad
+      // 55.3 -> 53.5 us, line search 63.4 -> 61.6 us).  The narrow block's kernels use predicated load pairs; there the
+      // order changes nothing or costs (config 4 line search 1 108 -> 1 140 us), so it keeps the CSR order.
+      const char* env_sort = std::getenv("ALORA_ELL_SORT");
+      const bool sort_slots = env_sort ? std::atoi(env_sort) != 0 : c->ell_wide;   // pays on the wide block (meshes) only: measured
+      auto order_slots = [&](int* col, T* val, int cnt, int64_t j) {
+        for (int a = 1; a < cnt; ++a) {   // insertion sort, cnt <= 8
+          const int cc = col[a]; const T vv = val[a];
+          auto key = [&](int cl, T vl) { return (vl == T(0) && cl == (int)j) ? (int64_t)1 << 40 : std::llabs((long long)cl - (long long)j); };
+          int b = a - 1;
+          while (b >= 0 && key(col[b], val[b]) > key(cc, vv)) { col[b + 1] = col[b]; val[b + 1] = val[b]; --b; }
+          col[b + 1] = cc; val[b + 1] = vv;
+        }
+      };
       for (int64_t j = 0; j < n; ++j) {
         const int e0 = c_rowptr[j], e1 = c_rowptr[j + 1];
         for (int u = 0; u < kUN; ++u) {
@@ -179,6 +195,7 @@ template <typename T> alora_status build(alora_ctx* c, const alora_problem* P) {
           ec[j * kUN + u] = e < e1 ? cents[e].col : (int)j;
           ev[j * kUN + u] = e < e1 ? (T)cents[e].val : T(0);
         }
+        if (sort_slots) order_slots(&ec[j * kUN], &ev[j * kUN], kUN, j);
         if (e1 - e0 > kUN) ec[j * kUN] |= (int)0x80000000;   // more neighbours than slots: walk the CSR tail
         for (int u = 0; u < kUNL; ++u) {   // columns ascend: the upper triangle is the tail of the row's list
           const int e = e1 - kUNL + u;
@@ -186,7 +203,11 @@ template <typename T> alora_status build(alora_ctx* c, const alora_problem* P) {
           euc[j * kUNL + u] = up ? cents[e].col : (int)j;
           euv[j * kUNL + u] = up ? (T)cents[e].val : T(0);
         }
+        if (sort_slots) order_slots(&euc[j * kUNL], &euv[j * kUNL], kUNL, j);
         if (e1 - kUNL - 1 >= e0 && cents[e1 - kUNL - 1].col > j) euc[j * kUNL] |= (int)0x80000000;
+        auto bits = [](int64_t d) { int b = 0; while (d) { ++b; d >>= 1; } return b; };
+        for (int u = 0; u < kUN; ++u) { const int cl = ec[j * kUN + u] & 0x7fffffff; if (cl != (int)j) c->ell_hist[0][bits(std::llabs((long long)cl - (long long)j))]++; }
+        for (int u = 0; u < kUNL; ++u) { const int cl = euc[j * kUNL + u] & 0x7fffffff; if (cl != (int)j) c->ell_hist[1][bits(std::llabs((long long)cl - (long long)j))]++; }
       }
       ALORA_CUDA(c, upload(c, (void**)&c->ell_col, ec));
       ALORA_CUDA(c, upload(c, &c->ell_val, ev));
@@ -396,10 +417,12 @@ extern "C" alora_status alora_create(const alora_problem* P, alora_dtype dtype, 
   c->device = device; c->stream = (cudaStream_t)cuda_stream; c->dtype = dtype;
   c->esz = dtype == ALORA_F32 ? 4 : 8; c->n = P->n; c->m = P->m;
   if (const char* e = std::getenv("ALORA_CW")) c->cw = std::atoi(e);   // measurement switch: 0 never, 1 default, 2 always
+  if (const char* e = std::getenv("ALORA_SEL")) c->sel = std::atoi(e);       // measurement switch: dense line-search variant, 0 branches, 1 predicated loads, -1 by far share
+  if (const char* e = std::getenv("ALORA_L2POL")) c->l2pol = std::atoi(e);   // measurement switch: L2 policies of the tiled kernel (RowArgs::l2pol), -1 = by size
   std::memset(c->occ_cache, 0, sizeof(c->occ_cache));
   std::memset(c->occ_ld, 0, sizeof(c->occ_ld));
   cudaDeviceProp prop;
-  if (cudaGetDeviceProperties(&prop, device) == cudaSuccess) c->num_sms = prop.multiProcessorCount;
+  if (cudaGetDeviceProperties(&prop, device) == cudaSuccess) { c->num_sms = prop.multiProcessorCount; if (prop.l2CacheSize > 0) c->l2_bytes = (size_t)prop.l2CacheSize; }
   alora_status s;
   try {
     s = dtype == ALORA_F32 ? build<float>(c, P) : build<double>(c, P);

@@ -212,11 +212,30 @@ alora_status launch_diag_rows(alora_ctx* c, int vec, int nvec, int exact, int sh
   const int64_t tiles = c->n / tr;
   bool elig = c->ell_col && exact && tiles > 0 && !((uintptr_t)a.X % 16) && !((uintptr_t)a.X2 % 16) && !((uintptr_t)dual % 16);
   int occ = 0;
+  // Share of a row's neighbours that are far (beyond a quarter of L2 in rows of this width): the gathers of such a
+  // problem miss L2, their latency is what the pass waits for, and issuing them as predicated load pairs instead of
+  // a branch per neighbour pays (config 4: line search 1 283 -> 1 108 us); the dense line-search variant of an
+  // L2-resident grid is 4 % faster with branches (config 1), so that variant exists in both forms.
+  bool sel = c->sel > 0;
+  if (c->sel < 0) {
+    const int64_t far_rows = std::max<int64_t>(1, (int64_t)(c->l2_bytes / 4) / std::max<int64_t>(1, a.ld * (int64_t)c->esz));
+    const int64_t* h = c->ell_hist[mode == ROWS_LS_FUSED ? 1 : 0];
+    int64_t tot = 0, far = 0;
+    for (int b = 0; b < 34; ++b) { tot += h[b]; if (b > 0 && ((int64_t)1 << (b - 1)) >= far_rows) far += h[b]; }
+    sel = far * 20 > tot;
+  }
+  const int flags = (c->ell_wide ? 1 : 0) | (sel ? 2 : 0);
+  // L2 policies (RowArgs::l2pol) by size: the single-vector matvec whose streamed slots exceed L2 while its vector
+  // fits keeps the vector resident (gathers evict_last, streamed data and output evict_first; config 4: 429 -> 325 us;
+  // config 1, all L2-resident: 12.4 -> 14.8 us, so not there); f + grad and line search: no effect measured
+  if (c->l2pol < 0)
+    a.l2pol = (mode == ROWS_ADJ && (size_t)c->n * (size_t)(ell_slots(c->ell_wide) * (4 + c->esz)) > c->l2_bytes &&
+               (size_t)c->n * (size_t)a.ld * c->esz * 2 <= c->l2_bytes * 3) ? 13 : 0;
   if (elig) {
     int& oc = c->occ_cache[vec_slot(vec)][shape][8 + mode];
     int64_t& key = c->occ_ld[vec_slot(vec)][shape][mode];
-    const int64_t want = a.ld * 4 + full;
-    if (!oc || key != want) { oc = occ_tiled(T(), vec, shape, mode, full, c->ell_wide ? 1 : 0, a.ld); key = want; if (!oc) oc = -1; }
+    const int64_t want = (a.ld * 4 + full) * 2 + (sel ? 1 : 0);
+    if (!oc || key != want) { oc = occ_tiled(T(), vec, shape, mode, full, flags, a.ld); key = want; if (!oc) oc = -1; }
     occ = oc;
     elig = occ > 0;
   }
@@ -234,7 +253,7 @@ alora_status launch_diag_rows(alora_ctx* c, int vec, int nvec, int exact, int sh
   a.tiles = tiles;
   a.fin = make_fin(c, a.partials, grid, nullptr, 0, nullptr, 0, out);
   {
-    const cudaError_t e = launch_tiled(vec, shape, mode, full, c->ell_wide ? 1 : 0, a, grid, c->stream, c->device);
+    const cudaError_t e = launch_tiled(vec, shape, mode, full, flags, a, grid, c->stream, c->device);
     if (e != cudaSuccess)
       return fail(c, ALORA_ECUDA, std::string("tiled row kernel launch: ") + cudaGetErrorString(e) + " (vec " + std::to_string(vec) +
                   ", shape " + std::to_string(shape) + ", mode " + std::to_string(mode) + ", full " + std::to_string(full) +
@@ -321,7 +340,7 @@ alora_status geometry(alora_ctx* c, int32_t r, int64_t ld, const void* p0, const
 
 template <typename T> void fill_rows(alora_ctx* c, RowArgs<T>& a, const Geo& g, const T* X, int r, int64_t ld) {
   a.n = c->n; a.r = r; a.ld = ld; a.nvec = g.nvec; a.exact = g.exact; a.X = X; a.X2 = nullptr; a.Out = nullptr;
-  a.perm = nullptr;
+  a.perm = nullptr; a.l2pol = c->l2pol < 0 ? 0 : c->l2pol;
   a.c_rowptr = c->c_rowptr; a.c_col = c->c_col; a.c_val = (const T*)c->c_val; a.dC = (const T*)c->dC;
   a.dcons = c->dcons; a.da = (const T*)c->da;
   a.a_rowptr = c->a_rowptr; a.a_col = c->a_col; a.a_val = (const T*)c->a_val; a.a_cons = c->a_cons;

@@ -11,8 +11,8 @@ namespace alora {
   cudaError_t launch_ent_cw_##SUF(int mode, int single, const ConsArgs<T>& a, int grid, cudaStream_t s); \
   cudaError_t launch_cons_##SUF(int shape, int mode, int chunked, const ConsArgs<T>& a, int grid,     \
                                 cudaStream_t s);                                                      \
-  cudaError_t launch_tiled_##SUF(int shape, int mode, int full, int wide, const RowArgs<T>& a, int grid, cudaStream_t s, int dev); \
-  int occ_tiled_##SUF(int shape, int mode, int full, int wide, int64_t ld);                                                      \
+  cudaError_t launch_tiled_##SUF(int shape, int mode, int full, int flags, const RowArgs<T>& a, int grid, cudaStream_t s, int dev); \
+  int occ_tiled_##SUF(int shape, int mode, int full, int flags, int64_t ld);                                                      \
   int occ_rows_##SUF(int shape, int mode);                                                            \
   cudaError_t launch_rows_ep_##SUF(int shape, const RowArgs<T>& a, int grid, cudaStream_t s);         \
   cudaError_t launch_rows_cw_##SUF(const RowArgs<T>& a, int grid, cudaStream_t s);                    \
@@ -83,18 +83,18 @@ inline cudaError_t launch_cons(int vec, int shape, int mode, int chunked, const 
 inline cudaError_t launch_cons(int vec, int shape, int mode, int chunked, const ConsArgs<double>& a, int grid, cudaStream_t s) {
   return vec == 2 ? launch_cons_f64v2(shape, mode, chunked, a, grid, s) : launch_cons_f64v1(shape, mode, chunked, a, grid, s);
 }
-inline cudaError_t launch_tiled(int vec, int shape, int mode, int full, int wide, const RowArgs<float>& a, int grid, cudaStream_t s, int dev) {
-  return vec == 4 ? launch_tiled_f32v4(shape, mode, full, wide, a, grid, s, dev)
-       : vec == 2 ? launch_tiled_f32v2(shape, mode, full, wide, a, grid, s, dev) : launch_tiled_f32v1(shape, mode, full, wide, a, grid, s, dev);
+inline cudaError_t launch_tiled(int vec, int shape, int mode, int full, int flags, const RowArgs<float>& a, int grid, cudaStream_t s, int dev) {
+  return vec == 4 ? launch_tiled_f32v4(shape, mode, full, flags, a, grid, s, dev)
+       : vec == 2 ? launch_tiled_f32v2(shape, mode, full, flags, a, grid, s, dev) : launch_tiled_f32v1(shape, mode, full, flags, a, grid, s, dev);
 }
-inline cudaError_t launch_tiled(int vec, int shape, int mode, int full, int wide, const RowArgs<double>& a, int grid, cudaStream_t s, int dev) {
-  return vec == 2 ? launch_tiled_f64v2(shape, mode, full, wide, a, grid, s, dev) : launch_tiled_f64v1(shape, mode, full, wide, a, grid, s, dev);
+inline cudaError_t launch_tiled(int vec, int shape, int mode, int full, int flags, const RowArgs<double>& a, int grid, cudaStream_t s, int dev) {
+  return vec == 2 ? launch_tiled_f64v2(shape, mode, full, flags, a, grid, s, dev) : launch_tiled_f64v1(shape, mode, full, flags, a, grid, s, dev);
 }
-inline int occ_tiled(float, int vec, int shape, int mode, int full, int wide, int64_t ld) {
-  return vec == 4 ? occ_tiled_f32v4(shape, mode, full, wide, ld) : vec == 2 ? occ_tiled_f32v2(shape, mode, full, wide, ld) : occ_tiled_f32v1(shape, mode, full, wide, ld);
+inline int occ_tiled(float, int vec, int shape, int mode, int full, int flags, int64_t ld) {
+  return vec == 4 ? occ_tiled_f32v4(shape, mode, full, flags, ld) : vec == 2 ? occ_tiled_f32v2(shape, mode, full, flags, ld) : occ_tiled_f32v1(shape, mode, full, flags, ld);
 }
-inline int occ_tiled(double, int vec, int shape, int mode, int full, int wide, int64_t ld) {
-  return vec == 2 ? occ_tiled_f64v2(shape, mode, full, wide, ld) : occ_tiled_f64v1(shape, mode, full, wide, ld);
+inline int occ_tiled(double, int vec, int shape, int mode, int full, int flags, int64_t ld) {
+  return vec == 2 ? occ_tiled_f64v2(shape, mode, full, flags, ld) : occ_tiled_f64v1(shape, mode, full, flags, ld);
 }
 inline int occ_rows(float, int vec, int shape, int mode) {
   return vec == 4 ? occ_rows_f32v4(shape, mode) : vec == 2 ? occ_rows_f32v2(shape, mode) : occ_rows_f32v1(shape, mode);

@@ -79,6 +79,9 @@ template <typename T> struct RowArgs {
   const int* heavy_rows; const int* heavy_segptr; T* seg_out; double* seg_cx;
   // optional processing order of the rows (general class, skewed degrees): position -> row, heaviest rows first
   const int* perm;
+  // k_rows_tiled: L2 cache policies (bit 0: per-row metadata copies evict_first; bit 1: X / X2 tile copies evict_first;
+  // bit 2: gathered neighbour rows evict_last; bit 3: output rows evict_first; bit 5: X tile copies evict_last)
+  int l2pol;
 };
 
 template <typename T> struct ConsArgs {
@@ -142,6 +145,84 @@ template <> __device__ __forceinline__ Pack<double, 1> ldg_pack<double, 1>(const
 template <typename T, int VEC> __device__ __forceinline__ void st_pack(T* p, const Pack<T, VEC>& x) {
   *reinterpret_cast<Pack<T, VEC>*>(p) = x;
 }
+
+// L2 cache policies (createpolicy) for the loads / stores / bulk copies of the tiled row kernel: kind 0 = evict_normal
+// (the default behaviour), 1 = evict_first (data read or written once per launch: slots, y, b, outputs), 2 = evict_last
+// (data other rows will gather again: the rows of X).  The policy is an operand, so one kernel serves all settings.
+__device__ __forceinline__ uint64_t l2_policy(int kind) {
+  uint64_t p;
+  if (kind == 1) asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
+  else if (kind == 2) asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p));
+  else asm volatile("createpolicy.fractional.L2::evict_normal.b64 %0, 1.0;" : "=l"(p));
+  return p;
+}
+#if ALORA_LD_L2HINT
+#define ALORA_LD_NCP "ld.global.nc.L2::cache_hint.L2::64B"
+#else
+#define ALORA_LD_NCP "ld.global.nc.L2::cache_hint"
+#endif
+template <typename T, int VEC> __device__ __forceinline__ Pack<T, VEC> ldg_pack_pol(const T* p, uint64_t pol);
+template <> __device__ __forceinline__ Pack<float, 4> ldg_pack_pol<float, 4>(const float* p, uint64_t pol) {
+  Pack<float, 4> o;
+  asm(ALORA_LD_NCP ".v4.f32 {%0,%1,%2,%3}, [%4], %5;" : "=f"(o.v[0]), "=f"(o.v[1]), "=f"(o.v[2]), "=f"(o.v[3]) : "l"(p), "l"(pol));
+  return o; }
+template <> __device__ __forceinline__ Pack<float, 2> ldg_pack_pol<float, 2>(const float* p, uint64_t pol) {
+  Pack<float, 2> o;
+  asm(ALORA_LD_NCP ".v2.f32 {%0,%1}, [%2], %3;" : "=f"(o.v[0]), "=f"(o.v[1]) : "l"(p), "l"(pol));
+  return o; }
+template <> __device__ __forceinline__ Pack<float, 1> ldg_pack_pol<float, 1>(const float* p, uint64_t pol) {
+  Pack<float, 1> o;
+  asm(ALORA_LD_NCP ".f32 %0, [%1], %2;" : "=f"(o.v[0]) : "l"(p), "l"(pol));
+  return o; }
+template <> __device__ __forceinline__ Pack<double, 2> ldg_pack_pol<double, 2>(const double* p, uint64_t pol) {
+  Pack<double, 2> o;
+  asm(ALORA_LD_NCP ".v2.f64 {%0,%1}, [%2], %3;" : "=d"(o.v[0]), "=d"(o.v[1]) : "l"(p), "l"(pol));
+  return o; }
+template <> __device__ __forceinline__ Pack<double, 1> ldg_pack_pol<double, 1>(const double* p, uint64_t pol) {
+  Pack<double, 1> o;
+  asm(ALORA_LD_NCP ".f64 %0, [%1], %2;" : "=d"(o.v[0]) : "l"(p), "l"(pol));
+  return o; }
+// One pack from shared memory (ps != 0: 32-bit shared address sa) or from global memory (pg != 0: read-only path with
+// the L2::64B fetch size and cache policy pol), or zeros (neither) -- as two PREDICATED loads instead of a branch: a
+// warp whose lanes disagree (one row's neighbour sits in the staged tile, the next row's does not) otherwise pays a
+// BSSY / BRA / BSYNC group per neighbour load.  volatile: the shared-memory stage is rewritten between iterations.
+template <typename T, int VEC> __device__ __forceinline__ Pack<T, VEC> ld_sel(uint32_t sa, const T* gp, int ps, int pg, uint64_t pol);
+template <> __device__ __forceinline__ Pack<float, 4> ld_sel<float, 4>(uint32_t sa, const float* gp, int ps, int pg, uint64_t pol) {
+  Pack<float, 4> o;
+  asm volatile("{\n .reg .pred ps, pg;\n setp.ne.s32 ps, %6, 0;\n setp.ne.s32 pg, %7, 0;\n mov.f32 %0, 0f00000000;\n mov.f32 %1, 0f00000000;\n mov.f32 %2, 0f00000000;\n mov.f32 %3, 0f00000000;\n @ps ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];\n @pg " ALORA_LD_NCP ".v4.f32 {%0,%1,%2,%3}, [%5], %8;\n}"
+               : "=&f"(o.v[0]), "=&f"(o.v[1]), "=&f"(o.v[2]), "=&f"(o.v[3]) : "r"(sa), "l"(gp), "r"(ps), "r"(pg), "l"(pol));
+  return o; }
+template <> __device__ __forceinline__ Pack<float, 2> ld_sel<float, 2>(uint32_t sa, const float* gp, int ps, int pg, uint64_t pol) {
+  Pack<float, 2> o;
+  asm volatile("{\n .reg .pred ps, pg;\n setp.ne.s32 ps, %4, 0;\n setp.ne.s32 pg, %5, 0;\n mov.f32 %0, 0f00000000;\n mov.f32 %1, 0f00000000;\n @ps ld.shared.v2.f32 {%0,%1}, [%2];\n @pg " ALORA_LD_NCP ".v2.f32 {%0,%1}, [%3], %6;\n}"
+               : "=&f"(o.v[0]), "=&f"(o.v[1]) : "r"(sa), "l"(gp), "r"(ps), "r"(pg), "l"(pol));
+  return o; }
+template <> __device__ __forceinline__ Pack<float, 1> ld_sel<float, 1>(uint32_t sa, const float* gp, int ps, int pg, uint64_t pol) {
+  Pack<float, 1> o;
+  asm volatile("{\n .reg .pred ps, pg;\n setp.ne.s32 ps, %3, 0;\n setp.ne.s32 pg, %4, 0;\n mov.f32 %0, 0f00000000;\n @ps ld.shared.f32 %0, [%1];\n @pg " ALORA_LD_NCP ".f32 %0, [%2], %5;\n}"
+               : "=&f"(o.v[0]) : "r"(sa), "l"(gp), "r"(ps), "r"(pg), "l"(pol));
+  return o; }
+template <> __device__ __forceinline__ Pack<double, 2> ld_sel<double, 2>(uint32_t sa, const double* gp, int ps, int pg, uint64_t pol) {
+  Pack<double, 2> o;
+  asm volatile("{\n .reg .pred ps, pg;\n setp.ne.s32 ps, %4, 0;\n setp.ne.s32 pg, %5, 0;\n mov.f64 %0, 0d0000000000000000;\n mov.f64 %1, 0d0000000000000000;\n @ps ld.shared.v2.f64 {%0,%1}, [%2];\n @pg " ALORA_LD_NCP ".v2.f64 {%0,%1}, [%3], %6;\n}"
+               : "=&d"(o.v[0]), "=&d"(o.v[1]) : "r"(sa), "l"(gp), "r"(ps), "r"(pg), "l"(pol));
+  return o; }
+template <> __device__ __forceinline__ Pack<double, 1> ld_sel<double, 1>(uint32_t sa, const double* gp, int ps, int pg, uint64_t pol) {
+  Pack<double, 1> o;
+  asm volatile("{\n .reg .pred ps, pg;\n setp.ne.s32 ps, %3, 0;\n setp.ne.s32 pg, %4, 0;\n mov.f64 %0, 0d0000000000000000;\n @ps ld.shared.f64 %0, [%1];\n @pg " ALORA_LD_NCP ".f64 %0, [%2], %5;\n}"
+               : "=&d"(o.v[0]) : "r"(sa), "l"(gp), "r"(ps), "r"(pg), "l"(pol));
+  return o; }
+template <typename T, int VEC> __device__ __forceinline__ void st_pack_pol(T* p, const Pack<T, VEC>& x, uint64_t pol);
+template <> __device__ __forceinline__ void st_pack_pol<float, 4>(float* p, const Pack<float, 4>& x, uint64_t pol) {
+  asm volatile("st.global.L2::cache_hint.v4.f32 [%0], {%1,%2,%3,%4}, %5;" ::"l"(p), "f"(x.v[0]), "f"(x.v[1]), "f"(x.v[2]), "f"(x.v[3]), "l"(pol) : "memory"); }
+template <> __device__ __forceinline__ void st_pack_pol<float, 2>(float* p, const Pack<float, 2>& x, uint64_t pol) {
+  asm volatile("st.global.L2::cache_hint.v2.f32 [%0], {%1,%2}, %3;" ::"l"(p), "f"(x.v[0]), "f"(x.v[1]), "l"(pol) : "memory"); }
+template <> __device__ __forceinline__ void st_pack_pol<float, 1>(float* p, const Pack<float, 1>& x, uint64_t pol) {
+  asm volatile("st.global.L2::cache_hint.f32 [%0], %1, %2;" ::"l"(p), "f"(x.v[0]), "l"(pol) : "memory"); }
+template <> __device__ __forceinline__ void st_pack_pol<double, 2>(double* p, const Pack<double, 2>& x, uint64_t pol) {
+  asm volatile("st.global.L2::cache_hint.v2.f64 [%0], {%1,%2}, %3;" ::"l"(p), "d"(x.v[0]), "d"(x.v[1]), "l"(pol) : "memory"); }
+template <> __device__ __forceinline__ void st_pack_pol<double, 1>(double* p, const Pack<double, 1>& x, uint64_t pol) {
+  asm volatile("st.global.L2::cache_hint.f64 [%0], %1, %2;" ::"l"(p), "d"(x.v[0]), "l"(pol) : "memory"); }
 
 template <int GS> __device__ __forceinline__ unsigned group_mask() {
   if (GS >= 32) return 0xffffffffu;

@@ -85,6 +85,11 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t by
                "l"(src), "r"(bytes), "r"(smem_u32(bar))
                : "memory");
 }
+__device__ __forceinline__ void bulk_g2s_pol(void* dst, const void* src, uint32_t bytes, uint64_t* bar, uint64_t pol) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;" ::"r"(smem_u32(dst)),
+               "l"(src), "r"(bytes), "r"(smem_u32(bar)), "l"(pol)
+               : "memory");
+}
 
 template <int GS> __device__ __forceinline__ float gsum(float v) {
 #pragma unroll
@@ -188,16 +193,27 @@ __host__ __device__ constexpr int tiled_min_blocks(int row_regs, int mode, bool 
 // row vector of a neighbour: from the staged tile when the neighbour is one of the tile's own rows, else gathered
 // from global memory.  sp / gp point at the lane's first pack of that row; mask: packs owned by the lane.
 template <typename T, int VEC, int GS, int NIT>
-__device__ __forceinline__ void row_nbr(RowReg<T, VEC, GS, NIT>& x, bool loc, const unsigned char* sp, const char* gp, unsigned mask) {
+__device__ __forceinline__ void row_nbr(RowReg<T, VEC, GS, NIT>& x, bool loc, const unsigned char* sp, const char* gp, unsigned mask, uint64_t pol) {
 #pragma unroll
   for (int it = 0; it < NIT; ++it) {
     if (mask == ~0u || (mask & (1u << it))) {
       if (loc) x.p[it] = *reinterpret_cast<const Pack<T, VEC>*>(sp + it * GS * VEC * sizeof(T));
-      else x.p[it] = ldg_pack<T, VEC>(reinterpret_cast<const T*>(gp) + it * GS * VEC);
+      else x.p[it] = ldg_pack_pol<T, VEC>(reinterpret_cast<const T*>(gp) + it * GS * VEC, pol);
     } else {
 #pragma unroll
       for (int i = 0; i < VEC; ++i) x.p[it].v[i] = T(0);
     }
+  }
+}
+
+// the same with the choice made per lane by predication (ld_sel): sa = 32-bit shared address of the lane's first pack
+// of that row in the stage (only used when loc), gp as above
+template <typename T, int VEC, int GS, int NIT>
+__device__ __forceinline__ void row_nbr_sel(RowReg<T, VEC, GS, NIT>& x, bool loc, uint32_t sa, const char* gp, unsigned mask, uint64_t pol) {
+#pragma unroll
+  for (int it = 0; it < NIT; ++it) {
+    const bool own = mask == ~0u || (mask & (1u << it));
+    x.p[it] = ld_sel<T, VEC>(sa + it * GS * VEC * (uint32_t)sizeof(T), reinterpret_cast<const T*>(gp) + it * GS * VEC, loc && own, !loc && own, pol);
   }
 }
 
@@ -207,7 +223,8 @@ __device__ __forceinline__ void row_nbr(RowReg<T, VEC, GS, NIT>& x, bool loc, co
 // the matrix (< TR rows) is processed by the consumer warps of the last block from global memory.  FULL: 1 = some lanes of a group own no pack (lane mask), 2 = all lanes busy.
 // CLD: the leading dimension equals the row length GS * NIT * VEC (dense rows, FULL == 2), known at compile time, so
 // every stage offset and row pitch is an immediate.
-template <typename T, int VEC, int GS, int NIT, int MODE, int FULL, bool CLD = false, bool WIDE = false>
+// SEL: neighbour rows by predicated load pairs (ld_sel) instead of a branch per neighbour.
+template <typename T, int VEC, int GS, int NIT, int MODE, int FULL, bool CLD = false, bool WIDE = false, bool SEL = true>
 __global__ void __launch_bounds__(kTiledThreads, tiled_min_blocks(VEC * NIT * (int)sizeof(T) / 4, MODE, WIDE)) k_rows_tiled(const RowArgs<T> a) {
   using Row = RowReg<T, VEC, GS, NIT>;
   constexpr int TR = tile_rows(GS), GPW = 32 / GS, NCW = kBlock / 32;
@@ -247,19 +264,21 @@ __global__ void __launch_bounds__(kTiledThreads, tiled_min_blocks(VEC * NIT * (i
     const uint32_t bytes = xbytes * (LS ? 2u : 1u) + TR * (uint32_t)ESZ + TR * 8u * (MODE == ROWS_ADJ ? 1u : 2u) +
                            TR * NU * (4u + (uint32_t)ESZ);
     uint32_t s = 0, ph = 0;
+    const uint64_t pol_m = l2_policy((a.l2pol & 1) ? 1 : 0);
+    const uint64_t pol_x = l2_policy((a.l2pol & 2) ? 1 : (a.l2pol & 32) ? 2 : 0);
     for (int64_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
       if (lane32 == 0) {
         const int64_t t0 = tile * TR;
         mbar_wait(&empty[s], ph ^ 1u);
         unsigned char* sb = smem_raw + (size_t)s * stage_sz;
         mbar_expect_tx(&full[s], bytes);
-        bulk_g2s(sb, a.X + t0 * ld, xbytes, &full[s]);
-        if (LS) bulk_g2s(sb + xbytes, a.X2 + t0 * ld, xbytes, &full[s]);
-        bulk_g2s(sb + off_dc, a.dC + t0, TR * (uint32_t)ESZ, &full[s]);
-        bulk_g2s(sb + off_y, (MODE == ROWS_ADJ ? a.w : a.y) + t0, TR * 8u, &full[s]);
-        if (MODE != ROWS_ADJ) bulk_g2s(sb + off_b, a.b + t0, TR * 8u, &full[s]);
-        bulk_g2s(sb + off_ec, a.ell_col + t0 * NU, TR * NU * 4u, &full[s]);
-        bulk_g2s(sb + off_ev, a.ell_val + t0 * NU, TR * NU * (uint32_t)ESZ, &full[s]);
+        bulk_g2s_pol(sb, a.X + t0 * ld, xbytes, &full[s], pol_x);
+        if (LS) bulk_g2s_pol(sb + xbytes, a.X2 + t0 * ld, xbytes, &full[s], pol_x);
+        bulk_g2s_pol(sb + off_dc, a.dC + t0, TR * (uint32_t)ESZ, &full[s], pol_m);
+        bulk_g2s_pol(sb + off_y, (MODE == ROWS_ADJ ? a.w : a.y) + t0, TR * 8u, &full[s], pol_m);
+        if (MODE != ROWS_ADJ) bulk_g2s_pol(sb + off_b, a.b + t0, TR * 8u, &full[s], pol_m);
+        bulk_g2s_pol(sb + off_ec, a.ell_col + t0 * NU, TR * NU * 4u, &full[s], pol_m);
+        bulk_g2s_pol(sb + off_ev, a.ell_val + t0 * NU, TR * NU * (uint32_t)ESZ, &full[s], pol_m);
       }
       __syncwarp();
       if (++s == kStages) { s = 0; ph ^= 1u; }
@@ -282,6 +301,7 @@ __global__ void __launch_bounds__(kTiledThreads, tiled_min_blocks(VEC * NIT * (i
     for (int i2 = 0; i2 < NIT; ++i2) if (FULL == 2 || lane + i2 * GS < nvec) lmask |= 1u << i2;
     const unsigned pmask = FULL == 2 ? ~0u : lmask;
     double* const zout = a.z;
+    const uint64_t pol_g = l2_policy((a.l2pol & 4) ? 2 : 0), pol_o = l2_policy((a.l2pol & 8) ? 1 : 0);
     const double sigma = a.sigma;
     const T sc = (T)a.scale;
     // one row: `staged` = its streaming inputs sit in stage `sb` (tile rows [row0, row0 + TR)), else they are read
@@ -290,9 +310,16 @@ __global__ void __launch_bounds__(kTiledThreads, tiled_min_blocks(VEC * NIT * (i
       Row x, d;
       T dc; double yv, bv = 0.0;
       int ck[NU]; T cw[NU];
+      // neighbour row: OFF = byte offset of the lane's first pack inside the stage (used when LOC), GP = global address
+      const uint32_t sb32 = (SEL && staged) ? smem_u32(sb) : 0u;
+#define NBR(DST, LOC, OFF, GP)                                                     \
+  do {                                                                             \
+    if constexpr (SEL) row_nbr_sel(DST, LOC, sb32 + (OFF), GP, pmask, pol_g);      \
+    else row_nbr(DST, LOC, sb + (OFF), GP, pmask, pol_g);                          \
+  } while (0)
       if (staged) {
-        row_nbr(x, true, sb + xme, nullptr, pmask);
-        if (LS) row_nbr(d, true, sb + xbytes + xme, nullptr, pmask);
+        row_nbr(x, true, sb + xme, nullptr, pmask, pol_g);
+        if (LS) row_nbr(d, true, sb + xbytes + xme, nullptr, pmask, pol_g);
         dc = reinterpret_cast<const T*>(sb + off_dc)[lr];
         yv = reinterpret_cast<const double*>(sb + off_y)[lr];
         if (MODE != ROWS_ADJ) bv = reinterpret_cast<const double*>(sb + off_b)[lr];
@@ -302,8 +329,8 @@ __global__ void __launch_bounds__(kTiledThreads, tiled_min_blocks(VEC * NIT * (i
           cw[u] = reinterpret_cast<const T*>(sb + off_ev)[lr * NU + u];
         }
       } else {
-        row_nbr(x, false, nullptr, Xl + (uint64_t)row * ldb, pmask);
-        if (LS) row_nbr(d, false, nullptr, X2l + (uint64_t)row * ldb, pmask);
+        row_nbr(x, false, nullptr, Xl + (uint64_t)row * ldb, pmask, pol_g);
+        if (LS) row_nbr(d, false, nullptr, X2l + (uint64_t)row * ldb, pmask, pol_g);
         dc = __ldg(a.dC + row);
         yv = __ldg((MODE == ROWS_ADJ ? a.w : a.y) + row);
         if (MODE != ROWS_ADJ) bv = __ldg(a.b + row);
@@ -327,7 +354,7 @@ __global__ void __launch_bounds__(kTiledThreads, tiled_min_blocks(VEC * NIT * (i
 #pragma unroll
             for (int u = 0; u < NU; ++u) {
               const uint32_t rel = (uint32_t)ck[u] - row0;
-              row_nbr(xk[u], staged && rel < (uint32_t)TR, sb + rel * ldb + loff, Xl + (uint64_t)(uint32_t)ck[u] * ldb, pmask);
+              NBR(xk[u], staged && rel < (uint32_t)TR, rel * ldb + loff, Xl + (uint64_t)(uint32_t)ck[u] * ldb);
             }
 #pragma unroll
             for (int u = 0; u < NU; ++u) uacc.axpy(cw[u], xk[u]);
@@ -337,7 +364,7 @@ __global__ void __launch_bounds__(kTiledThreads, tiled_min_blocks(VEC * NIT * (i
 #pragma unroll
             for (int u = 0; u < NU; ++u) {
               const uint32_t rel = (uint32_t)ck[u] - row0;
-              row_nbr(dk[u], staged && rel < (uint32_t)TR, sb + xbytes + rel * ldb + loff, X2l + (uint64_t)(uint32_t)ck[u] * ldb, pmask);
+              NBR(dk[u], staged && rel < (uint32_t)TR, xbytes + rel * ldb + loff, X2l + (uint64_t)(uint32_t)ck[u] * ldb);
             }
 #pragma unroll
             for (int u = 0; u < NU; ++u) wacc.axpy(cw[u], dk[u]);
@@ -348,8 +375,8 @@ __global__ void __launch_bounds__(kTiledThreads, tiled_min_blocks(VEC * NIT * (i
           for (int u = 0; u < NU; ++u) {
             const uint32_t rel = (uint32_t)ck[u] - row0;
             const bool loc = staged && rel < (uint32_t)TR;
-            row_nbr(xk[u], loc, sb + rel * ldb + loff, Xl + (uint64_t)(uint32_t)ck[u] * ldb, pmask);
-            row_nbr(dk[u], loc, sb + xbytes + rel * ldb + loff, X2l + (uint64_t)(uint32_t)ck[u] * ldb, pmask);
+            NBR(xk[u], loc, rel * ldb + loff, Xl + (uint64_t)(uint32_t)ck[u] * ldb);
+            NBR(dk[u], loc, xbytes + rel * ldb + loff, X2l + (uint64_t)(uint32_t)ck[u] * ldb);
           }
 #pragma unroll
           for (int u = 0; u < NU; ++u) { uacc.axpy(cw[u], xk[u]); wacc.axpy(cw[u], dk[u]); }
@@ -394,7 +421,7 @@ __global__ void __launch_bounds__(kTiledThreads, tiled_min_blocks(VEC * NIT * (i
 #pragma unroll
         for (int u = 0; u < NU; ++u) {
           const uint32_t rel = (uint32_t)ck[u] - row0;
-          row_nbr(xn[u], staged && rel < (uint32_t)TR, sb + rel * ldb + loff, Xl + (uint64_t)(uint32_t)ck[u] * ldb, pmask);
+          NBR(xn[u], staged && rel < (uint32_t)TR, rel * ldb + loff, Xl + (uint64_t)(uint32_t)ck[u] * ldb);
         }
         double coef;
         if (MODE == ROWS_FUSED_EVAL) {
@@ -435,12 +462,13 @@ __global__ void __launch_bounds__(kTiledThreads, tiled_min_blocks(VEC * NIT * (i
             char* const orow = Outl + (uint64_t)row * ldb;
 #pragma unroll
             for (int i2 = 0; i2 < NIT; ++i2)
-              if (FULL == 2 || (lmask & (1u << i2))) st_pack<T, VEC>(reinterpret_cast<T*>(orow) + i2 * GS * VEC, acc.p[i2]);
+              if (FULL == 2 || (lmask & (1u << i2))) st_pack_pol<T, VEC>(reinterpret_cast<T*>(orow) + i2 * GS * VEC, acc.p[i2], pol_o);
           }
         }
       }
     };
 
+#undef NBR
     uint32_t s = 0, ph = 0;
     const unsigned char* sb = smem_raw;
     for (int64_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
