@@ -154,8 +154,10 @@ alora_status alora_step_host(alora_ctx *ctx, const void *R_host, const void *D_h
  *   r, ld, same y and sigma, R not written since); the library may then reuse that state instead of recomputing
  *   it (p0 is taken from the evaluation's f, and q-only sums from its scalars).  ALORA_ESTATE if no such evaluation
  *   is on record (different R pointer / r / ld, or alora_set_dual called since).  Results equal the cold form to
- *   rounding.  (DESIGN.md section 6 says what is and is not worth reusing: keeping C R across the line search does
- *   not reduce the bytes of an inner iteration on this layout.) */
+ *   rounding.  If that evaluation wrote a gradient G (G != NULL there, and != D here), the caller also vouches that G
+ *   has not been written since: for the diagonal class the library then streams G and takes p1 = <G,D> -- the
+ *   directional derivative -- and <C,RR^T> from the evaluation, so the pass gathers only the D operand of each
+ *   neighbour pair, half the random row reads of the cold form. */
 alora_status alora_linesearch(alora_ctx *ctx, const void *R, const void *D, int32_t r, int64_t ld, int32_t warm,
                               double p[5]);
 alora_status alora_get_linesearch(alora_ctx *ctx, double p[5]);

@@ -203,14 +203,16 @@ FinArgs make_fin(const alora_ctx* c, const double* p0, int n0, const double* p1,
 FinArgs no_fin() { FinArgs f; f.p[0] = f.p[1] = f.p[2] = nullptr; f.n[0] = f.n[1] = f.n[2] = 0; f.out = nullptr; f.ticket = nullptr; return f; }
 
 template <typename T>
-alora_status launch_diag_rows(alora_ctx* c, int vec, int nvec, int exact, int shape, int mode, RowArgs<T>& a,
+alora_status launch_diag_rows(alora_ctx* c, int vec, int nvec, int exact, int shape, int mode_in, RowArgs<T>& a,
                               const void* dual, double* out) {
+  int mode = mode_in;   // ROWS_LS_WARM falls back to ROWS_LS_FUSED when the tiled kernel is not eligible (a.X3 is then cleared)
   const int gs = tiled_shape(mode, shape, c->ell_wide).gs, nit = tiled_shape(mode, shape, c->ell_wide).nit, tr = tile_rows(gs);
   // 1: whole packs, some lanes of a group idle (lane mask); 2: whole packs, all lanes busy.  Rows whose last
   // pack is partially filled (r not a multiple of the vector width) take k_rows.
   const int full = nvec == gs * nit ? 2 : 1;
   const int64_t tiles = c->n / tr;
   bool elig = c->ell_col && exact && tiles > 0 && !((uintptr_t)a.X % 16) && !((uintptr_t)a.X2 % 16) && !((uintptr_t)dual % 16);
+  if (mode == ROWS_LS_WARM && (!elig || !a.X3 || ((uintptr_t)a.X3 % 16))) { mode = ROWS_LS_FUSED; a.X3 = nullptr; }   // the warm form exists in the tiled kernel only
   int occ = 0;
   // Share of a row's neighbours that are far (beyond a quarter of L2 in rows of this width): the gathers of such a
   // problem miss L2, their latency is what the pass waits for, and issuing them as predicated load pairs instead of
@@ -219,7 +221,7 @@ alora_status launch_diag_rows(alora_ctx* c, int vec, int nvec, int exact, int sh
   bool sel = c->sel > 0;
   if (c->sel < 0) {
     const int64_t far_rows = std::max<int64_t>(1, (int64_t)(c->l2_bytes / 4) / std::max<int64_t>(1, a.ld * (int64_t)c->esz));
-    const int64_t* h = c->ell_hist[mode == ROWS_LS_FUSED ? 1 : 0];
+    const int64_t* h = c->ell_hist[(mode == ROWS_LS_FUSED || mode == ROWS_LS_WARM) ? 1 : 0];
     int64_t tot = 0, far = 0;
     for (int b = 0; b < 34; ++b) { tot += h[b]; if (b > 0 && ((int64_t)1 << (b - 1)) >= far_rows) far += h[b]; }
     sel = far * 20 > tot;
@@ -231,12 +233,16 @@ alora_status launch_diag_rows(alora_ctx* c, int vec, int nvec, int exact, int sh
   if (c->l2pol < 0)
     a.l2pol = (mode == ROWS_ADJ && (size_t)c->n * (size_t)(ell_slots(c->ell_wide) * (4 + c->esz)) > c->l2_bytes &&
                (size_t)c->n * (size_t)a.ld * c->esz * 2 <= c->l2_bytes * 3) ? 13 : 0;
-  if (elig) {
+  auto probe = [&]() {
     int& oc = c->occ_cache[vec_slot(vec)][shape][8 + mode];
     int64_t& key = c->occ_ld[vec_slot(vec)][shape][mode];
     const int64_t want = (a.ld * 4 + full) * 2 + (sel ? 1 : 0);
     if (!oc || key != want) { oc = occ_tiled(T(), vec, shape, mode, full, flags, a.ld); key = want; if (!oc) oc = -1; }
-    occ = oc;
+    return oc;
+  };
+  if (elig) {
+    occ = probe();
+    if (occ <= 0 && mode == ROWS_LS_WARM) { mode = ROWS_LS_FUSED; a.X3 = nullptr; occ = probe(); }   // the three-tile stage does not fit: cold form
     elig = occ > 0;
   }
   if (!elig) {
@@ -339,7 +345,7 @@ alora_status geometry(alora_ctx* c, int32_t r, int64_t ld, const void* p0, const
 }
 
 template <typename T> void fill_rows(alora_ctx* c, RowArgs<T>& a, const Geo& g, const T* X, int r, int64_t ld) {
-  a.n = c->n; a.r = r; a.ld = ld; a.nvec = g.nvec; a.exact = g.exact; a.X = X; a.X2 = nullptr; a.Out = nullptr;
+  a.n = c->n; a.r = r; a.ld = ld; a.nvec = g.nvec; a.exact = g.exact; a.X = X; a.X2 = nullptr; a.X3 = nullptr; a.Out = nullptr;
   a.perm = nullptr; a.l2pol = c->l2pol < 0 ? 0 : c->l2pol;
   a.c_rowptr = c->c_rowptr; a.c_col = c->c_col; a.c_val = (const T*)c->c_val; a.dC = (const T*)c->dC;
   a.dcons = c->dcons; a.da = (const T*)c->da;
@@ -484,17 +490,18 @@ alora_status fetch_stats(alora_ctx* c, int r_lowrank, double stats[8]) {
   return ALORA_OK;
 }
 
-template <typename T> alora_status ls_impl(alora_ctx* c, const T* R, const T* D, int32_t r, int64_t ld) {
+template <typename T> alora_status ls_impl(alora_ctx* c, const T* R, const T* D, int32_t r, int64_t ld, const T* G_warm) {
   Geo g;
   alora_status s = geometry(c, r, ld, R, D, nullptr, g);
   if (s != ALORA_OK) return s;
   if (c->cls == 0) {
     RowArgs<T> a;
     fill_rows(c, a, g, R, r, ld);
-    a.X2 = D;
+    a.X2 = D; a.X3 = G_warm;
     a.ell_col = c->ellu_col; a.ell_val = (const T*)c->ellu_val;
-    s = launch_diag_rows<T>(c, g.vec, g.nvec, g.exact, g.shape, ROWS_LS_FUSED, a, c->y, c->ls_dev);
+    s = launch_diag_rows<T>(c, g.vec, g.nvec, g.exact, g.shape, G_warm ? ROWS_LS_WARM : ROWS_LS_FUSED, a, c->y, c->ls_dev);
     if (s != ALORA_OK) return s;
+    c->ls_used_g = a.X3 != nullptr;   // launch_diag_rows drops it when the tiled kernel is not eligible
   } else {
     if (c->pC) {
       s = lowrank<T>(c, R, r, ld, c->TmR, false); if (s != ALORA_OK) return s;
@@ -570,7 +577,8 @@ alora_status fetch_ls(alora_ctx* c, int r, double p[5]) {
     if (lr) for (int q = 0; q < c->pC; ++q) { const double* tr = s + 64 + q * r; double rr = 0; for (int k = 0; k < r; ++k) rr += tr[k] * tr[k]; cx += c->s_host[q] * rr; }
     p[0] = cx - e[ES_YQ] + 0.5 * sg * e[ES_QQ];
   }
-  p[1] = 2.0 * cRD - s[LS_YQ1] + sg * s[LS_QQ1];
+  p[1] = c->ls_used_g ? s[LS_CRD]   // warm form with the evaluation's gradient: the slot carries <G,D> = d/d alpha f(R + alpha D) at 0
+                      : 2.0 * cRD - s[LS_YQ1] + sg * s[LS_QQ1];
   p[2] = cDD - s[LS_YQ2] + 0.5 * sg * s[LS_Q11] + sg * s[LS_QQ2];
   p[3] = sg * s[LS_Q12];
   p[4] = 0.5 * sg * s[LS_Q22];
@@ -610,7 +618,7 @@ extern "C" alora_status alora_eval(alora_ctx* c, const void* R, int32_t r, int64
   alora_status s = c->dtype == ALORA_F32 ? eval_impl<float>(c, (const float*)R, r, ld, (float*)G, z_dev)
                                          : eval_impl<double>(c, (const double*)R, r, ld, (double*)G, z_dev);
   if (s != ALORA_OK) return s;
-  c->last_eval_r = r; c->last_eval_R = R; c->last_eval_ld = ld;
+  c->last_eval_r = r; c->last_eval_R = R; c->last_eval_ld = ld; c->last_eval_G = G;
   return stats ? fetch_stats(c, r, stats) : ALORA_OK;
 }
 
@@ -710,8 +718,10 @@ extern "C" alora_status alora_linesearch(alora_ctx* c, const void* R, const void
   if (warm && !(c->have_eval && c->last_eval_R == R && c->last_eval_r == r && c->last_eval_ld == ld))
     return fail(c, ALORA_ESTATE, "alora_linesearch(warm): no alora_eval of this R (same pointer, r, ld, dual) is on record");
   ALORA_CUDA(c, cudaSetDevice(c->device));
-  alora_status s = c->dtype == ALORA_F32 ? ls_impl<float>(c, (const float*)R, (const float*)D, r, ld)
-                                         : ls_impl<double>(c, (const double*)R, (const double*)D, r, ld);
+  c->ls_used_g = false;
+  const void* Gw = (warm && c->last_eval_G != D) ? c->last_eval_G : nullptr;   // the gradient of the evaluation on record, if it wrote one
+  alora_status s = c->dtype == ALORA_F32 ? ls_impl<float>(c, (const float*)R, (const float*)D, r, ld, (const float*)Gw)
+                                         : ls_impl<double>(c, (const double*)R, (const double*)D, r, ld, (const double*)Gw);
   if (s != ALORA_OK) return s;
   c->last_ls_r = r;
   c->ls_warm = warm != 0;

@@ -103,6 +103,8 @@ struct alora_ctx {
   bool have_eval = false, have_ls = false;
   int last_eval_r = 0, last_ls_r = 0;
   const void* last_eval_R = nullptr; int64_t last_eval_ld = 0;   // what a warm alora_linesearch must match
+  const void* last_eval_G = nullptr;                              // gradient that evaluation wrote (null: value-only call)
+  bool ls_used_g = false;                                         // the last line search took p1 = <G,D> from that gradient
   bool ls_warm = false; double* ls_warm_stats = nullptr;          // copy of the evaluation's scalars taken by a warm call
   double* lam_auto = nullptr;   // diagonal class: lambda of the last evaluation, formed on demand (mu_dev == NULL)
   int64_t launches = 0;

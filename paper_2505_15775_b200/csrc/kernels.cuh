@@ -32,7 +32,7 @@ constexpr int kChunk = 16;           // entries per chunk of a long constraint /
 __host__ __device__ constexpr int ell_slots(bool wide) { return wide ? 8 : 4; }
 __host__ __device__ constexpr int ell_slots_ls(bool wide) { return wide ? 6 : 3; }
 
-enum RowsMode { ROWS_FUSED_EVAL = 0, ROWS_ADJ = 1, ROWS_LS_FUSED = 2 };
+enum RowsMode { ROWS_FUSED_EVAL = 0, ROWS_ADJ = 1, ROWS_LS_FUSED = 2, ROWS_LS_WARM = 3 };   // LS_WARM: k_rows_tiled only (RowArgs::X3)
 enum ConsMode { CONS_EVAL = 0, CONS_LS = 1 };
 
 // stat slots written by the kernels (per-block partial rows have this many doubles)
@@ -55,6 +55,7 @@ template <typename T> struct RowArgs {
   int64_t n; int r; int64_t ld; int nvec; int exact;  // exact: r == nvec*VEC (no tail masking)
   const T* X;    // R (or V)
   const T* X2;   // D (ROWS_LS_FUSED)
+  const T* X3;   // k_rows_tiled<ROWS_LS_WARM>: G = grad f(R) of the evaluation on record
   T* Out;        // G / W, may be null
   const int* c_rowptr; const int* c_col; const T* c_val; const T* dC;  // off-diagonal C (full pattern) + diag
   const int* dcons; const T* da;       // diagonal class: constraint on row j and its coefficient (null: j / 1)
@@ -1131,6 +1132,6 @@ constexpr Shape kShapes[7] = {{1, 1}, {2, 1}, {4, 1}, {8, 1}, {8, 2}, {16, 2}, {
 // per group, so fewer lanes per row means fewer warp instructions per row; a lane holds up to 4 packs
 constexpr Shape kTShapes[7] = {{1, 1}, {2, 1}, {2, 2}, {4, 2}, {8, 2}, {8, 4}, {16, 4}};     // f + grad, adjoint
 constexpr Shape kTShapesLS[7] = {{1, 1}, {2, 1}, {4, 1}, {4, 2}, {8, 2}, {8, 4}, {16, 4}};   // line search (two operands per row; measured: 2 lanes per row is slower there, 50.7 vs 48.4 us), wide ELL
-__host__ inline Shape tiled_shape(int mode, int idx, bool wide) { return (mode == ROWS_LS_FUSED || wide) ? kTShapesLS[idx] : kTShapes[idx]; }
+__host__ inline Shape tiled_shape(int mode, int idx, bool wide) { return (mode == ROWS_LS_FUSED || mode == ROWS_LS_WARM || wide) ? kTShapesLS[idx] : kTShapes[idx]; }
 
 }  // namespace alora

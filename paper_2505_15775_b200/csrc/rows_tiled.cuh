@@ -38,10 +38,11 @@ constexpr int kStages = ALORA_KSTAGES;   // tiles in flight per block (tuning kn
 constexpr int kTiledThreads = kBlock + 32;   // 8 consumer warps + 1 producer warp
 
 __host__ __device__ constexpr int tile_rows(int gs) { return kBlock / gs; }   // one row per group per tile
-// per-stage shared memory: [X tile][D tile (line search)][dC][y|w][b][ELL col][ELL val], 16-byte aligned pieces
+// per-stage shared memory: [X tile][D tile (line search)][G tile (warm line search)][dC][y|w][b][ELL col][ELL val], 16-byte aligned pieces
 __host__ __device__ inline size_t tiled_stage_bytes(int gs, int esz, int64_t ld, int mode, bool wide) {
-  const size_t tr = tile_rows(gs), nu = (mode == ROWS_LS_FUSED ? ell_slots_ls(wide) : ell_slots(wide));
-  size_t b = tr * (size_t)ld * esz * (mode == ROWS_LS_FUSED ? 2 : 1);
+  const bool ls = mode == ROWS_LS_FUSED || mode == ROWS_LS_WARM;
+  const size_t tr = tile_rows(gs), nu = (ls ? ell_slots_ls(wide) : ell_slots(wide));
+  size_t b = tr * (size_t)ld * esz * (mode == ROWS_LS_WARM ? 3 : ls ? 2 : 1);
   b = (b + 15) & ~(size_t)15;
   b += tr * esz;                 // dC
   b = (b + 15) & ~(size_t)15;
@@ -228,8 +229,9 @@ template <typename T, int VEC, int GS, int NIT, int MODE, int FULL, bool CLD = f
 __global__ void __launch_bounds__(kTiledThreads, tiled_min_blocks(VEC * NIT * (int)sizeof(T) / 4, MODE, WIDE)) k_rows_tiled(const RowArgs<T> a) {
   using Row = RowReg<T, VEC, GS, NIT>;
   constexpr int TR = tile_rows(GS), GPW = 32 / GS, NCW = kBlock / 32;
-  constexpr int NST = (MODE == ROWS_LS_FUSED) ? 12 : 6;
-  constexpr bool LS = (MODE == ROWS_LS_FUSED);
+  constexpr bool LS = (MODE == ROWS_LS_FUSED || MODE == ROWS_LS_WARM);
+  constexpr bool WG = (MODE == ROWS_LS_WARM);   // warm line search, see below
+  constexpr int NST = LS ? 12 : 6;
   constexpr int NU = LS ? ell_slots_ls(WIDE) : ell_slots(WIDE);
   constexpr int NSL = (LS && GS >= 4) ? 6 : NST;   // accumulators kept in the loop (line search spreads the 9 q-sums over lanes)
   constexpr int ESZ = (int)sizeof(T);
@@ -241,8 +243,12 @@ __global__ void __launch_bounds__(kTiledThreads, tiled_min_blocks(VEC * NIT * (i
   const int64_t ntiles = a.tiles;
 
   // stage layout (must match tiled_stage_bytes)
+  // Warm line search (ROWS_LS_WARM; a.X3 = G of the evaluation on record, reading 31): p1 = <G,D> is streamed
+  // instead of formed from <C,RD^T>, <C,RR^T> is the evaluation's, so only the D operand of the upper neighbours is
+  // gathered (half the random row reads of the cold form); the G tile rides in the stage behind the D tile.
   const uint32_t xbytes = (uint32_t)(TR * ld * ESZ);
-  const uint32_t off_dc = (xbytes * (LS ? 2u : 1u) + 15u) & ~15u;
+  constexpr uint32_t ntile = WG ? 3u : LS ? 2u : 1u;
+  const uint32_t off_dc = (xbytes * ntile + 15u) & ~15u;
   const uint32_t off_y = (off_dc + TR * (uint32_t)ESZ + 15u) & ~15u;
   const uint32_t off_b = off_y + TR * 8, off_ec = off_b + TR * 8, off_ev = off_ec + TR * NU * 4;
   const uint32_t stage_sz = (off_ev + TR * NU * (uint32_t)ESZ + 15u) & ~15u;
@@ -261,7 +267,7 @@ __global__ void __launch_bounds__(kTiledThreads, tiled_min_blocks(VEC * NIT * (i
   if (warp == NCW) {
     // ================= producer warp: streams the tiles of this block into the ring ===========================
     // (the whole warp walks the loop, lane 0 issues: a diverged producer warp was measured 5 - 10 % slower)
-    const uint32_t bytes = xbytes * (LS ? 2u : 1u) + TR * (uint32_t)ESZ + TR * 8u * (MODE == ROWS_ADJ ? 1u : 2u) +
+    const uint32_t bytes = xbytes * ntile + TR * (uint32_t)ESZ + TR * 8u * (MODE == ROWS_ADJ ? 1u : 2u) +
                            TR * NU * (4u + (uint32_t)ESZ);
     uint32_t s = 0, ph = 0;
     const uint64_t pol_m = l2_policy((a.l2pol & 1) ? 1 : 0);
@@ -274,6 +280,7 @@ __global__ void __launch_bounds__(kTiledThreads, tiled_min_blocks(VEC * NIT * (i
         mbar_expect_tx(&full[s], bytes);
         bulk_g2s_pol(sb, a.X + t0 * ld, xbytes, &full[s], pol_x);
         if (LS) bulk_g2s_pol(sb + xbytes, a.X2 + t0 * ld, xbytes, &full[s], pol_x);
+        if (WG) bulk_g2s_pol(sb + 2u * xbytes, a.X3 + t0 * ld, xbytes, &full[s], pol_x);
         bulk_g2s_pol(sb + off_dc, a.dC + t0, TR * (uint32_t)ESZ, &full[s], pol_m);
         bulk_g2s_pol(sb + off_y, (MODE == ROWS_ADJ ? a.w : a.y) + t0, TR * 8u, &full[s], pol_m);
         if (MODE != ROWS_ADJ) bulk_g2s_pol(sb + off_b, a.b + t0, TR * 8u, &full[s], pol_m);
@@ -294,6 +301,7 @@ __global__ void __launch_bounds__(kTiledThreads, tiled_min_blocks(VEC * NIT * (i
     const uint32_t xme = (uint32_t)lr * ldb + loff;    // this lane's first pack inside a staged X tile
     const char* const Xl = reinterpret_cast<const char*>(a.X) + loff;    // lane's first pack of row 0
     const char* const X2l = LS ? reinterpret_cast<const char*>(a.X2) + loff : nullptr;
+    const char* const X3l = WG ? reinterpret_cast<const char*>(a.X3) + loff : nullptr;
     char* const Outl = a.Out ? reinterpret_cast<char*>(a.Out) + loff : nullptr;
     const uint32_t full0 = smem_u32(full), empty0 = smem_u32(empty);
     unsigned lmask = 0;   // packs of a row owned by this lane (FULL == 2: all of them, known at compile time)
@@ -307,7 +315,7 @@ __global__ void __launch_bounds__(kTiledThreads, tiled_min_blocks(VEC * NIT * (i
     // one row: `staged` = its streaming inputs sit in stage `sb` (tile rows [row0, row0 + TR)), else they are read
     // from global memory (ragged tail of the matrix); live == false: padding lane of the tail, nothing is kept
     auto do_row = [&](const bool staged, const unsigned char* sb, const uint32_t row0, const uint32_t row, const bool live) {
-      Row x, d;
+      Row x, d, gv;
       T dc; double yv, bv = 0.0;
       int ck[NU]; T cw[NU];
       // neighbour row: OFF = byte offset of the lane's first pack inside the stage (used when LOC), GP = global address
@@ -320,6 +328,7 @@ __global__ void __launch_bounds__(kTiledThreads, tiled_min_blocks(VEC * NIT * (i
       if (staged) {
         row_nbr(x, true, sb + xme, nullptr, pmask, pol_g);
         if (LS) row_nbr(d, true, sb + xbytes + xme, nullptr, pmask, pol_g);
+        if (WG) row_nbr(gv, true, sb + 2u * xbytes + xme, nullptr, pmask, pol_g);
         dc = reinterpret_cast<const T*>(sb + off_dc)[lr];
         yv = reinterpret_cast<const double*>(sb + off_y)[lr];
         if (MODE != ROWS_ADJ) bv = reinterpret_cast<const double*>(sb + off_b)[lr];
@@ -331,6 +340,7 @@ __global__ void __launch_bounds__(kTiledThreads, tiled_min_blocks(VEC * NIT * (i
       } else {
         row_nbr(x, false, nullptr, Xl + (uint64_t)row * ldb, pmask, pol_g);
         if (LS) row_nbr(d, false, nullptr, X2l + (uint64_t)row * ldb, pmask, pol_g);
+        if (WG) row_nbr(gv, false, nullptr, X3l + (uint64_t)row * ldb, pmask, pol_g);
         dc = __ldg(a.dC + row);
         yv = __ldg((MODE == ROWS_ADJ ? a.w : a.y) + row);
         if (MODE != ROWS_ADJ) bv = __ldg(a.b + row);
@@ -347,7 +357,16 @@ __global__ void __launch_bounds__(kTiledThreads, tiled_min_blocks(VEC * NIT * (i
         // vectors in flight would spill).
         constexpr bool SEQ = VEC * NIT * (int)sizeof(T) / 4 > 4;
         Row uacc, wacc; uacc.zero(); wacc.zero();
-        if (SEQ) {
+        if (WG) {   // warm form: the D operand only
+          Row dk[NU];
+#pragma unroll
+          for (int u = 0; u < NU; ++u) {
+            const uint32_t rel = (uint32_t)ck[u] - row0;
+            NBR(dk[u], staged && rel < (uint32_t)TR, xbytes + rel * ldb + loff, X2l + (uint64_t)(uint32_t)ck[u] * ldb);
+          }
+#pragma unroll
+          for (int u = 0; u < NU; ++u) wacc.axpy(cw[u], dk[u]);
+        } else if (SEQ) {
           // two phases (R operand, then D operand): NU row vectors in flight instead of 2 NU
           {
             Row xk[NU];
@@ -405,16 +424,22 @@ __global__ void __launch_bounds__(kTiledThreads, tiled_min_blocks(VEC * NIT * (i
             if ((uint32_t)k <= row) break;
             const T cv = __ldg(a.c_val + e);
             Row xe, de;
-            xe.load(a.X + (int64_t)k * ld, lane, nvec, r, exact);
+            if (!WG) { xe.load(a.X + (int64_t)k * ld, lane, nvec, r, exact); uacc.axpy(cv, xe); }
             de.load(a.X2 + (int64_t)k * ld, lane, nvec, r, exact);
-            uacc.axpy(cv, xe); wacc.axpy(cv, de);
+            wacc.axpy(cv, de);
           }
         }
-        const T sRR = x.dot(uacc), sRD = x.dot(wacc) + d.dot(uacc), sDD = d.dot(wacc);
-        if (live) {
-          st[LS_CRR] += (double)dc * (double)rr_l + 2.0 * (double)sRR;
-          st[LS_CRD] += (double)dc * (double)rd_l + (double)sRD;
-          st[LS_CDD] += (double)dc * (double)dd_l + 2.0 * (double)sDD;
+        const T sDD = d.dot(wacc);
+        if (WG) {   // slot LS_CRD carries <G,D> (= p1), slot LS_CRR stays zero (the evaluation's <C,RR^T> is used)
+          const T gd = gv.dot(d);
+          if (live) { st[LS_CRD] += (double)gd; st[LS_CDD] += (double)dc * (double)dd_l + 2.0 * (double)sDD; }
+        } else {
+          const T sRR = x.dot(uacc), sRD = x.dot(wacc) + d.dot(uacc);
+          if (live) {
+            st[LS_CRR] += (double)dc * (double)rr_l + 2.0 * (double)sRR;
+            st[LS_CRD] += (double)dc * (double)rd_l + (double)sRD;
+            st[LS_CDD] += (double)dc * (double)dd_l + 2.0 * (double)sDD;
+          }
         }
       } else {
         Row xn[NU];

@@ -119,6 +119,10 @@ def check_workload(torch, binding, oracle_mod, w, ld=None, label="", split_scale
     assert np.abs(p - po).max() <= tol * np.abs(po).sum(), (label, p, po)
     pw = ctx.linesearch(R, D, r, ld, warm=True)
     assert np.abs(pw - po).max() <= tol * np.abs(po).sum(), (label, pw, po)
+    ctx.eval(R, r, ld, None, None)                        # a value-only evaluation on record: warm without a gradient
+    pw2 = ctx.linesearch(R, D, r, ld, warm=True)
+    assert np.abs(pw2 - po).max() <= tol * np.abs(po).sum(), (label, pw2, po)
+    ctx.eval(R, r, ld, G, z)
     with pytest.raises(binding.AloraError) as e:          # no evaluation of D on record
         ctx.linesearch(D, R, r, ld, warm=True)
     assert e.value.status == binding.ESTATE
