@@ -216,8 +216,9 @@ alora_status launch_diag_rows(alora_ctx* c, int vec, int nvec, int exact, int sh
   int occ = 0;
   // Share of a row's neighbours that are far (beyond a quarter of L2 in rows of this width): the gathers of such a
   // problem miss L2, their latency is what the pass waits for, and issuing them as predicated load pairs instead of
-  // a branch per neighbour pays (config 4: line search 1 283 -> 1 108 us); the dense line-search variant of an
-  // L2-resident grid is 4 % faster with branches (config 1), so that variant exists in both forms.
+  // a branch per neighbour pays (config 4: f + grad 1 124 -> 1 039 us, line search 1 283 -> 1 108 us); on a grid,
+  // whose neighbours are near, the dense variants are faster with branches (torus, n = 1e6: line search 49.1 -> 47.1
+  // us; n = 1.6e7: f + grad 597 -> 522 us), so the dense variants exist in both forms.
   bool sel = c->sel > 0;
   if (c->sel < 0) {
     const int64_t far_rows = std::max<int64_t>(1, (int64_t)(c->l2_bytes / 4) / std::max<int64_t>(1, a.ld * (int64_t)c->esz));

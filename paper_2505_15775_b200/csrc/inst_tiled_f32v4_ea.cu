@@ -1,0 +1,6 @@
+// tiled row kernel, float rows, 4-element vector loads, f + grad and adjoint
+#define ALORA_T float
+#define ALORA_VEC 4
+#define ALORA_SUF f32v4
+#define ALORA_TILED_LS 0
+#include "inst_tiled.inc"

@@ -1,0 +1,6 @@
+// tiled row kernel, double rows, 2-element vector loads, f + grad and adjoint
+#define ALORA_T double
+#define ALORA_VEC 2
+#define ALORA_SUF f64v2
+#define ALORA_TILED_LS 0
+#include "inst_tiled.inc"
