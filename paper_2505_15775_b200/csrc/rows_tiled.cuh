@@ -193,13 +193,16 @@ __host__ __device__ constexpr int tiled_min_blocks(int row_regs, int mode, bool 
 
 // row vector of a neighbour: from the staged tile when the neighbour is one of the tile's own rows, else gathered
 // from global memory.  sp / gp point at the lane's first pack of that row; mask: packs owned by the lane.
+// pstr: byte distance between the lane's consecutive packs (GS * VEC * sizeof(T), or its negative for a lane whose two
+// packs are taken in the opposite order -- the bank-conflict swizzle of the dense variants, see k_rows_tiled)
 template <typename T, int VEC, int GS, int NIT>
-__device__ __forceinline__ void row_nbr(RowReg<T, VEC, GS, NIT>& x, bool loc, const unsigned char* sp, const char* gp, unsigned mask, uint64_t pol) {
+__device__ __forceinline__ void row_nbr(RowReg<T, VEC, GS, NIT>& x, bool loc, const unsigned char* sp, const char* gp, unsigned mask, uint64_t pol,
+                                        int pstr = GS * VEC * (int)sizeof(T)) {
 #pragma unroll
   for (int it = 0; it < NIT; ++it) {
     if (mask == ~0u || (mask & (1u << it))) {
-      if (loc) x.p[it] = *reinterpret_cast<const Pack<T, VEC>*>(sp + it * GS * VEC * sizeof(T));
-      else x.p[it] = ldg_pack_pol<T, VEC>(reinterpret_cast<const T*>(gp) + it * GS * VEC, pol);
+      if (loc) x.p[it] = *reinterpret_cast<const Pack<T, VEC>*>(sp + it * pstr);
+      else x.p[it] = ldg_pack_pol<T, VEC>(reinterpret_cast<const T*>(gp + it * pstr), pol);
     } else {
 #pragma unroll
       for (int i = 0; i < VEC; ++i) x.p[it].v[i] = T(0);
@@ -210,11 +213,12 @@ __device__ __forceinline__ void row_nbr(RowReg<T, VEC, GS, NIT>& x, bool loc, co
 // the same with the choice made per lane by predication (ld_sel): sa = 32-bit shared address of the lane's first pack
 // of that row in the stage (only used when loc), gp as above
 template <typename T, int VEC, int GS, int NIT>
-__device__ __forceinline__ void row_nbr_sel(RowReg<T, VEC, GS, NIT>& x, bool loc, uint32_t sa, const char* gp, unsigned mask, uint64_t pol) {
+__device__ __forceinline__ void row_nbr_sel(RowReg<T, VEC, GS, NIT>& x, bool loc, uint32_t sa, const char* gp, unsigned mask, uint64_t pol,
+                                            int pstr = GS * VEC * (int)sizeof(T)) {
 #pragma unroll
   for (int it = 0; it < NIT; ++it) {
     const bool own = mask == ~0u || (mask & (1u << it));
-    x.p[it] = ld_sel<T, VEC>(sa + it * GS * VEC * (uint32_t)sizeof(T), reinterpret_cast<const T*>(gp) + it * GS * VEC, loc && own, !loc && own, pol);
+    x.p[it] = ld_sel<T, VEC>(sa + (uint32_t)(it * pstr), reinterpret_cast<const T*>(gp + it * pstr), loc && own, !loc && own, pol);
   }
 }
 
@@ -297,7 +301,16 @@ __global__ void __launch_bounds__(kTiledThreads, tiled_min_blocks(VEC * NIT * (i
     const int lane = lane32 % GS;
     const int lr = warp * GPW + lane32 / GS;           // row of the tile handled by this group
     const uint32_t ldb = (uint32_t)(ld * ESZ);         // row pitch in bytes
-    const uint32_t loff = (uint32_t)(lane * VEC * ESZ);
+    // Bank-conflict swizzle of the dense variants with two 16-byte packs per lane (r = 16 at 2 lanes per row, r = 32 at
+    // 4): a quarter warp (8 lanes = one shared-memory wavefront of a 16-byte load) spans 8 / GS rows whose pitch is a
+    // multiple of 64 bytes, so rows 4 / GS apart hit the same banks with their first packs (ncu, config 1: 2-way
+    // conflict on every row load, 3.7 M wavefronts for 2.2 M ideal).  Every other such row takes its two packs in the
+    // opposite order; all vectors of a group (own row, neighbours, output) share the order, and dot products and
+    // axpys do not care which register holds which pack.
+    constexpr bool SWZ = CLD && NIT == 2 && VEC * ESZ == 16 && (GS == 2 || GS == 4);
+    const int flip = SWZ ? ((lr / (4 / (GS > 4 ? 4 : GS))) & 1) : 0;
+    const int pstr = (SWZ && flip) ? -(GS * VEC * ESZ) : GS * VEC * ESZ;   // byte distance between the lane's packs
+    const uint32_t loff = (uint32_t)((lane + flip * GS) * VEC * ESZ);
     const uint32_t xme = (uint32_t)lr * ldb + loff;    // this lane's first pack inside a staged X tile
     const char* const Xl = reinterpret_cast<const char*>(a.X) + loff;    // lane's first pack of row 0
     const char* const X2l = LS ? reinterpret_cast<const char*>(a.X2) + loff : nullptr;
@@ -322,13 +335,13 @@ __global__ void __launch_bounds__(kTiledThreads, tiled_min_blocks(VEC * NIT * (i
       const uint32_t sb32 = (SEL && staged) ? smem_u32(sb) : 0u;
 #define NBR(DST, LOC, OFF, GP)                                                     \
   do {                                                                             \
-    if constexpr (SEL) row_nbr_sel(DST, LOC, sb32 + (OFF), GP, pmask, pol_g);      \
-    else row_nbr(DST, LOC, sb + (OFF), GP, pmask, pol_g);                          \
+    if constexpr (SEL) row_nbr_sel(DST, LOC, sb32 + (OFF), GP, pmask, pol_g, pstr); \
+    else row_nbr(DST, LOC, sb + (OFF), GP, pmask, pol_g, pstr);                    \
   } while (0)
       if (staged) {
-        row_nbr(x, true, sb + xme, nullptr, pmask, pol_g);
-        if (LS) row_nbr(d, true, sb + xbytes + xme, nullptr, pmask, pol_g);
-        if (WG) row_nbr(gv, true, sb + 2u * xbytes + xme, nullptr, pmask, pol_g);
+        row_nbr(x, true, sb + xme, nullptr, pmask, pol_g, pstr);
+        if (LS) row_nbr(d, true, sb + xbytes + xme, nullptr, pmask, pol_g, pstr);
+        if (WG) row_nbr(gv, true, sb + 2u * xbytes + xme, nullptr, pmask, pol_g, pstr);
         dc = reinterpret_cast<const T*>(sb + off_dc)[lr];
         yv = reinterpret_cast<const double*>(sb + off_y)[lr];
         if (MODE != ROWS_ADJ) bv = reinterpret_cast<const double*>(sb + off_b)[lr];
@@ -338,9 +351,9 @@ __global__ void __launch_bounds__(kTiledThreads, tiled_min_blocks(VEC * NIT * (i
           cw[u] = reinterpret_cast<const T*>(sb + off_ev)[lr * NU + u];
         }
       } else {
-        row_nbr(x, false, nullptr, Xl + (uint64_t)row * ldb, pmask, pol_g);
-        if (LS) row_nbr(d, false, nullptr, X2l + (uint64_t)row * ldb, pmask, pol_g);
-        if (WG) row_nbr(gv, false, nullptr, X3l + (uint64_t)row * ldb, pmask, pol_g);
+        row_nbr(x, false, nullptr, Xl + (uint64_t)row * ldb, pmask, pol_g, pstr);
+        if (LS) row_nbr(d, false, nullptr, X2l + (uint64_t)row * ldb, pmask, pol_g, pstr);
+        if (WG) row_nbr(gv, false, nullptr, X3l + (uint64_t)row * ldb, pmask, pol_g, pstr);
         dc = __ldg(a.dC + row);
         yv = __ldg((MODE == ROWS_ADJ ? a.w : a.y) + row);
         if (MODE != ROWS_ADJ) bv = __ldg(a.b + row);
@@ -424,8 +437,8 @@ __global__ void __launch_bounds__(kTiledThreads, tiled_min_blocks(VEC * NIT * (i
             if ((uint32_t)k <= row) break;
             const T cv = __ldg(a.c_val + e);
             Row xe, de;
-            if (!WG) { xe.load(a.X + (int64_t)k * ld, lane, nvec, r, exact); uacc.axpy(cv, xe); }
-            de.load(a.X2 + (int64_t)k * ld, lane, nvec, r, exact);
+            if (!WG) { row_nbr(xe, false, nullptr, Xl + (uint64_t)(uint32_t)k * ldb, pmask, pol_g, pstr); uacc.axpy(cv, xe); }
+            row_nbr(de, false, nullptr, X2l + (uint64_t)(uint32_t)k * ldb, pmask, pol_g, pstr);
             wacc.axpy(cv, de);
           }
         }
@@ -469,7 +482,7 @@ __global__ void __launch_bounds__(kTiledThreads, tiled_min_blocks(VEC * NIT * (i
         if (rem) {   // rows with more than NU neighbours: the CSR tail beyond the slots
           const int eb = __ldg(a.c_rowptr + row), ee = __ldg(a.c_rowptr + row + 1);
           for (int e = eb + NU; e < ee; ++e) {
-            Row xe; xe.load(a.X + (int64_t)__ldg(a.c_col + e) * ld, lane, nvec, r, exact);
+            Row xe; row_nbr(xe, false, nullptr, Xl + (uint64_t)(uint32_t)__ldg(a.c_col + e) * ldb, pmask, pol_g, pstr);
             acc.axpy(__ldg(a.c_val + e), xe);
           }
         }
@@ -487,7 +500,7 @@ __global__ void __launch_bounds__(kTiledThreads, tiled_min_blocks(VEC * NIT * (i
             char* const orow = Outl + (uint64_t)row * ldb;
 #pragma unroll
             for (int i2 = 0; i2 < NIT; ++i2)
-              if (FULL == 2 || (lmask & (1u << i2))) st_pack_pol<T, VEC>(reinterpret_cast<T*>(orow) + i2 * GS * VEC, acc.p[i2], pol_o);
+              if (FULL == 2 || (lmask & (1u << i2))) st_pack_pol<T, VEC>(reinterpret_cast<T*>(orow + i2 * pstr), acc.p[i2], pol_o);
           }
         }
       }
