@@ -1131,7 +1131,13 @@ constexpr Shape kShapes[7] = {{1, 1}, {2, 1}, {4, 1}, {8, 1}, {8, 2}, {16, 2}, {
 // tiled row kernel: few lanes per row -- the per-row bookkeeping (addresses, scalars, fp64 sums) is issued once
 // per group, so fewer lanes per row means fewer warp instructions per row; a lane holds up to 4 packs
 constexpr Shape kTShapes[7] = {{1, 1}, {2, 1}, {2, 2}, {4, 2}, {8, 2}, {8, 4}, {16, 4}};     // f + grad, adjoint
-constexpr Shape kTShapesLS[7] = {{1, 1}, {2, 1}, {4, 1}, {4, 2}, {8, 2}, {8, 4}, {16, 4}};   // line search (two operands per row; measured: 2 lanes per row is slower there, 50.7 vs 48.4 us), wide ELL
-__host__ inline Shape tiled_shape(int mode, int idx, bool wide) { return (mode == ROWS_LS_FUSED || mode == ROWS_LS_WARM || wide) ? kTShapesLS[idx] : kTShapes[idx]; }
+// wide ELL (all modes) and the warm line search: more lanes per row (two operands per row or 8 slots per row in registers)
+constexpr Shape kTShapesW[7] = {{1, 1}, {2, 1}, {4, 1}, {4, 2}, {8, 2}, {8, 4}, {16, 4}};
+// cold line search: as above, but 2 lanes x 2 packs for 3 - 4 packs per row (config 1, r = 16: 46.8 -> 43.1 us once the
+// dense variant's bank swizzle made that shape conflict-free; the warm form and the wide variants are slower with it)
+constexpr Shape kTShapesLS[7] = {{1, 1}, {2, 1}, {2, 2}, {4, 2}, {8, 2}, {8, 4}, {16, 4}};
+__host__ inline Shape tiled_shape(int mode, int idx, bool wide) {
+  return (wide || mode == ROWS_LS_WARM) ? kTShapesW[idx] : mode == ROWS_LS_FUSED ? kTShapesLS[idx] : kTShapes[idx];
+}
 
 }  // namespace alora
