@@ -195,13 +195,25 @@ def test_padded_leading_dimension(torch, binding, oracle_mod, idx, ld):
     check_workload(torch, binding, oracle_mod, inputs.small(idx), ld=ld, label=f"small{idx}/ld{ld}")
 
 
-@pytest.mark.parametrize("r", [1, 2, 3, 5, 7, 13, 33, 64])
+@pytest.mark.parametrize("r", [1, 2, 3, 5, 7, 8, 13, 16, 32, 33, 64])   # 8 / 16 / 32: the dense (compile-time ld) variants incl. the bank-swizzled ones
 def test_ranks(torch, binding, oracle_mod, r):
     """every (GS, NIT) shape and ragged tails, both classes and dtypes."""
     for maker in (lambda: inputs.config1(side=23, r=r), lambda: inputs.config6(side=19, r=r),
                   lambda: inputs.config3(n=700, m=900, nnzC=2000, r=r),
                   lambda: inputs.config2(n=300, M=900, r=r), lambda: inputs.config0(n=300, M=700, r=r)):
         check_workload(torch, binding, oracle_mod, maker(), label=f"r{r}")
+
+
+@pytest.mark.parametrize("sel", ["0", "1"])
+def test_dense_variants_both_neighbour_load_forms(torch, binding, oracle_mod, monkeypatch, sel):
+    """The dense (compile-time ld) variants of the tiled kernel exist with a branch per neighbour load and with predicated
+    load pairs; a call picks by the share of far neighbours, which small problems never have.  ALORA_SEL (read at
+    alora_create) forces either form: both must match the oracle, on the bank-swizzled shapes (r = 16, 32 in fp32; 8, 16 in
+    fp64) and a plain one, with rows that have more neighbours than ELL slots (G(n,M)) and without (torus)."""
+    monkeypatch.setenv("ALORA_SEL", sel)
+    for maker in (lambda: inputs.config1(side=23, r=16), lambda: inputs.config1(side=23, r=32), lambda: inputs.config1(side=23, r=8),
+                  lambda: inputs.config0(n=300, M=700, r=8), lambda: inputs.config0(n=300, M=700, r=16)):
+        check_workload(torch, binding, oracle_mod, maker(), label=f"sel{sel}")
 
 
 @pytest.mark.parametrize("idx", [1, 2, 3, 4, 5, 6, 7])
