@@ -418,6 +418,7 @@ extern "C" alora_status alora_create(const alora_problem* P, alora_dtype dtype, 
   c->esz = dtype == ALORA_F32 ? 4 : 8; c->n = P->n; c->m = P->m;
   if (const char* e = std::getenv("ALORA_CW")) c->cw = std::atoi(e);   // measurement switch: 0 never, 1 default, 2 always
   if (const char* e = std::getenv("ALORA_SEL")) c->sel = std::atoi(e);       // measurement switch: dense line-search variant, 0 branches, 1 predicated loads, -1 by far share
+  if (const char* e = std::getenv("ALORA_PDL")) c->pdl = std::atoi(e);       // measurement switch: programmatic dependent launch of the tiled kernel
   if (const char* e = std::getenv("ALORA_L2POL")) c->l2pol = std::atoi(e);   // measurement switch: L2 policies of the tiled kernel (RowArgs::l2pol), -1 = by size
   std::memset(c->occ_cache, 0, sizeof(c->occ_cache));
   std::memset(c->occ_ld, 0, sizeof(c->occ_ld));

@@ -348,6 +348,10 @@ alora_status geometry(alora_ctx* c, int32_t r, int64_t ld, const void* p0, const
 template <typename T> void fill_rows(alora_ctx* c, RowArgs<T>& a, const Geo& g, const T* X, int r, int64_t ld) {
   a.n = c->n; a.r = r; a.ld = ld; a.nvec = g.nvec; a.exact = g.exact; a.X = X; a.X2 = nullptr; a.X3 = nullptr; a.Out = nullptr;
   a.perm = nullptr; a.l2pol = c->l2pol < 0 ? 0 : c->l2pol;
+  // programmatic dependent launch of the tiled kernel: the next kernel's blocks become resident and run their prologue
+  // while this one drains (config 0: 32.9 -> 28.0 us per step, config 1: 96.3 -> 93.0 us, config 6: 134.6 -> 131.9 us);
+  // at n = 2^24 the step was 1 % SLOWER with it (2 498 -> 2 528 us), so only while the rows are within a few L2 sizes
+  a.pdl = c->pdl == 2 || (c->pdl == 1 && (size_t)c->n * (size_t)ld * c->esz <= 4 * c->l2_bytes);
   a.c_rowptr = c->c_rowptr; a.c_col = c->c_col; a.c_val = (const T*)c->c_val; a.dC = (const T*)c->dC;
   a.dcons = c->dcons; a.da = (const T*)c->da;
   a.a_rowptr = c->a_rowptr; a.a_col = c->a_col; a.a_val = (const T*)c->a_val; a.a_cons = c->a_cons;

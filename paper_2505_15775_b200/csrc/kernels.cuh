@@ -83,6 +83,7 @@ template <typename T> struct RowArgs {
   // k_rows_tiled: L2 cache policies (bit 0: per-row metadata copies evict_first; bit 1: X / X2 tile copies evict_first;
   // bit 2: gathered neighbour rows evict_last; bit 3: output rows evict_first; bit 5: X tile copies evict_last)
   int l2pol;
+  int pdl;   // host only: launch k_rows_tiled with programmatic stream serialisation (alora_ctx::pdl)
 };
 
 template <typename T> struct ConsArgs {

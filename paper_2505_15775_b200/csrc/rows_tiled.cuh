@@ -263,6 +263,13 @@ __global__ void __launch_bounds__(kTiledThreads, tiled_min_blocks(VEC * NIT * (i
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
   }
   __syncthreads();
+  // Programmatic dependent launch (the host launches this kernel with programmatic stream serialisation when
+  // RowArgs::pdl is set): the blocks of this grid may become resident while the previous kernel of the stream is still
+  // draining; nothing above touches global memory.  From here on the kernel reads buffers the previous kernel may have
+  // written (R, D, G, the partial rows, the ticket), so it waits for that kernel to complete and flush -- and lets its
+  // own successor start its prologue as early.  Both instructions are no-ops in a normal launch.
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
 
   double st[NSL];
 #pragma unroll
