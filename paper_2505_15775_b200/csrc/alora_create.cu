@@ -330,7 +330,9 @@ template <typename T> alora_status build(alora_ctx* c, const alora_problem* P) {
     c->s_host.assign(P->C_s, P->C_s + P->pC);
     ALORA_CUDA(c, upload(c, (void**)&c->s_dev, c->s_host));
     c->lr_grid = (int)std::min<int64_t>(2 * c->num_sms, std::max<int64_t>(1, n / 64));
-    ALORA_CUDA(c, c->pool.alloc((void**)&c->lr_part, sizeof(double) * c->lr_grid * P->pC * c->lr_rmax));
+    ALORA_CUDA(c, c->pool.alloc((void**)&c->lr_part, sizeof(double) * 2 * c->lr_grid * P->pC * c->lr_rmax));   // two matrices per launch
+    ALORA_CUDA(c, c->pool.alloc((void**)&c->lr_ticket, sizeof(unsigned int) * 2));
+    ALORA_CUDA(c, cudaMemset(c->lr_ticket, 0, sizeof(unsigned int) * 2));
     ALORA_CUDA(c, c->pool.alloc((void**)&c->TmR, sizeof(double) * P->pC * c->lr_rmax));
     ALORA_CUDA(c, c->pool.alloc((void**)&c->TmD, sizeof(double) * P->pC * c->lr_rmax));
     ALORA_CUDA(c, c->pool.alloc((void**)&c->Ts, sizeof(double) * P->pC * c->lr_rmax));

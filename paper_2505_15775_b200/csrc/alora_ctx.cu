@@ -51,11 +51,17 @@ __global__ void k_long_finish(int mode, int64_t m, const int* long_cons, const i
 
 // Low-rank cost term: T = U^T X (pC x r).  Per-block partials, then the block that finishes last (ticket) sums
 // them in block order: Tm[p][c], and optionally Ts = s_p * Tm.  blockDim.x = r * rpb.
+// gridDim.y = 2: two matrices in one launch (the line search: R -> Tm, D -> Tm2), each with its own partial rows and
+// its own ticket word.
 template <typename T>
-__global__ void k_lowrank(const T* X, int64_t n, int r, int64_t ld, const T* U, int pC, double* part, const double* s,
-                          double* Tm, double* Ts, unsigned int* ticket) {
+__global__ void k_lowrank(const T* X0, const T* X1, int64_t n, int r, int64_t ld, const T* U, int pC, double* part0, const double* s,
+                          double* Tm0, double* Tm1, double* Ts, unsigned int* ticket0) {
   extern __shared__ double lsm[];  // [pC][blockDim.x]
   __shared__ unsigned int s_last;
+  const T* const X = blockIdx.y ? X1 : X0;
+  double* const Tm = blockIdx.y ? Tm1 : Tm0;
+  double* const part = part0 + (size_t)blockIdx.y * gridDim.x * pC * r;
+  unsigned int* const ticket = ticket0 + blockIdx.y;
   const int c = threadIdx.x % r, slot = threadIdx.x / r, rpb = blockDim.x / r;
   double acc[8];
   for (int p = 0; p < 8; ++p) acc[p] = 0.0;
@@ -373,11 +379,17 @@ template <typename T> void fill_cons(alora_ctx* c, ConsArgs<T>& a, const Geo& g,
 }
 
 // T = U^T X (pC x r) into Tm, optionally Ts = s * Tm
-template <typename T> alora_status lowrank(alora_ctx* c, const T* X, int r, int64_t ld, double* Tm, bool want_Ts) {
+template <typename T> alora_status lowrank(alora_ctx* c, const T* X, int r, int64_t ld, double* Tm, bool want_Ts,
+                                           const T* X2 = nullptr, double* Tm2 = nullptr) {
   if (r > c->lr_rmax) return fail(c, ALORA_EINVAL, "low-rank cost term supports r <= 256");
-  const int rpb = std::max(1, kBlock / r), threads = r * rpb;
-  k_lowrank<T><<<c->lr_grid, threads, sizeof(double) * c->pC * threads, c->stream>>>(X, c->n, r, ld, (const T*)c->U, c->pC, c->lr_part,
-                                                                                    c->s_dev, Tm, want_Ts ? c->Ts : nullptr, c->ticket);
+  // Large blocks (up to 1024 threads, shared memory pC * threads doubles <= 48 KB) and a grid of about 8 rows per thread:
+  // both phases of the kernel are latency chains (the row loop, then the last block's ordered sum over the blocks), and
+  // this keeps both short (config 2, n = 20 000, r = 24: 296 blocks of 240 threads took 14 us, 78 blocks of 768 take 11 under ncu).
+  const int tmax = std::min(1024, 6144 / std::max(1, c->pC));
+  const int rpb = std::max(1, std::min(32, tmax / r)), threads = r * rpb;   // <= 32 row slots: their sums are added by one thread per column
+  const int grid = (int)std::max<int64_t>(1, std::min<int64_t>(c->lr_grid, (c->n + (int64_t)rpb * 8 - 1) / ((int64_t)rpb * 8)));
+  k_lowrank<T><<<dim3(grid, X2 ? 2 : 1), threads, sizeof(double) * c->pC * threads, c->stream>>>(
+      X, X2, c->n, r, ld, (const T*)c->U, c->pC, c->lr_part, c->s_dev, Tm, Tm2, want_Ts ? c->Ts : nullptr, c->lr_ticket);
   c->launches++;
   ALORA_CUDA(c, cudaGetLastError());
   return ALORA_OK;
@@ -410,8 +422,8 @@ alora_status forward_cw(alora_ctx* c, const Geo& g, int mode, ConsArgs<T>& ca, i
     c->launches++;
     if (longs) {
       ca.fin = last_out ? fin_all() : no_fin();
-      if (mode == CONS_EVAL) k_long_fin_e<T, CONS_EVAL><<<c->nlong_A, kBlock, 0, c->stream>>>(ca, c->part_long);
-      else k_long_fin_e<T, CONS_LS><<<c->nlong_A, kBlock, 0, c->stream>>>(ca, c->part_long);
+      if (mode == CONS_EVAL) k_long_fin_e<T, CONS_EVAL><<<c->nlong_A, kLongFinThreads, 0, c->stream>>>(ca, c->part_long);
+      else k_long_fin_e<T, CONS_LS><<<c->nlong_A, kLongFinThreads, 0, c->stream>>>(ca, c->part_long);
       c->launches++;
     }
   }
@@ -509,8 +521,7 @@ template <typename T> alora_status ls_impl(alora_ctx* c, const T* R, const T* D,
     c->ls_used_g = a.X3 != nullptr;   // launch_diag_rows drops it when the tiled kernel is not eligible
   } else {
     if (c->pC) {
-      s = lowrank<T>(c, R, r, ld, c->TmR, false); if (s != ALORA_OK) return s;
-      s = lowrank<T>(c, D, r, ld, c->TmD, false); if (s != ALORA_OK) return s;
+      s = lowrank<T>(c, R, r, ld, c->TmR, false, D, c->TmD); if (s != ALORA_OK) return s;   // both in one launch
     }
     ConsArgs<T> ca;
     fill_cons(c, ca, g, R, D, r, ld);

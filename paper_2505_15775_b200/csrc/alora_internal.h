@@ -94,7 +94,7 @@ struct alora_ctx {
   // low-rank cost
   int pC = 0; void* U = nullptr; double* s_dev = nullptr; std::vector<double> s_host;
   double* lr_part = nullptr; double* TmR = nullptr; double* TmD = nullptr; double* Ts = nullptr; double* lr_scal = nullptr;
-  int lr_grid = 0; int lr_rmax = 256;
+  int lr_grid = 0; int lr_rmax = 256; unsigned int* lr_ticket = nullptr;   // k_lowrank: one ticket word per matrix of a launch
   // partial sums / results
   int part_cap = 0;
   double* part_rows = nullptr; double* part_cons = nullptr; double* part_long = nullptr; double* part_chunk = nullptr;

@@ -1058,20 +1058,23 @@ __global__ void __launch_bounds__(kBlock) k_cons_fin(const ConsArgs<T> a) {
   finish_partials(a.fin);
 }
 
-// the same for one long constraint per block: thread t adds entries t, t + 256, ... in order, then an ordered block sum
+// the same for one long constraint per block of kLongFinThreads threads: thread t adds entries t, t + 1024, ... in order,
+// then an ordered block sum (one block per constraint: the trace row of the theta SDP has n entries, and with 256
+// threads this kernel took 14 / 38 us on config 2 -- ten dependent round trips; 1024 threads make it three)
+constexpr int kLongFinThreads = 1024;
 template <typename T, int MODE>
-__global__ void __launch_bounds__(kBlock) k_long_fin_e(const ConsArgs<T> a, double* part_long) {
-  constexpr int K = (MODE == CONS_LS) ? 3 : 1;
-  __shared__ double sm[3][kBlock / 32];
+__global__ void __launch_bounds__(kLongFinThreads) k_long_fin_e(const ConsArgs<T> a, double* part_long) {
+  constexpr int K = (MODE == CONS_LS) ? 3 : 1, BT = kLongFinThreads;
+  __shared__ double sm[3][BT / 32];
   const int slot = blockIdx.x, lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int64_t i = a.long_cons[slot], e0 = a.ptr[i], e1 = a.ptr[i + 1];
   double v[3] = {0.0, 0.0, 0.0};
   constexpr int U = 8;   // loads in flight per thread (the sums stay in entry order)
-  for (int64_t eb = e0 + threadIdx.x; eb < e1; eb += (int64_t)kBlock * U) {
+  for (int64_t eb = e0 + threadIdx.x; eb < e1; eb += (int64_t)BT * U) {
     T t[U][K];
 #pragma unroll
     for (int u = 0; u < U; ++u) {
-      const int64_t e = eb + (int64_t)u * kBlock;
+      const int64_t e = eb + (int64_t)u * BT;
 #pragma unroll
       for (int k = 0; k < K; ++k) t[u][k] = e < e1 ? __ldcg(a.e_out + e * K + k) : T(0);
     }
@@ -1084,7 +1087,7 @@ __global__ void __launch_bounds__(kBlock) k_long_fin_e(const ConsArgs<T> a, doub
   __syncthreads();
   if (threadIdx.x == 0) {
     double t[3] = {0.0, 0.0, 0.0};
-    for (int k = 0; k < 3; ++k) for (int wv = 0; wv < kBlock / 32; ++wv) t[k] += sm[k][wv];
+    for (int k = 0; k < 3; ++k) for (int wv = 0; wv < BT / 32; ++wv) t[k] += sm[k][wv];
     double st[kNStat];
     for (int s = 0; s < kNStat; ++s) st[s] = 0.0;
     cons_finish<MODE>(st, i, t[0], t[1], t[2], a.y, a.b, a.sigma, a.z, a.lam);
