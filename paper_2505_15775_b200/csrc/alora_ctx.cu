@@ -23,6 +23,7 @@ __global__ void k_long_finish(int mode, int64_t m, const int* long_cons, const i
                               const double* ch_out, const double* y, const double* b, double sigma,
                               double* z, double* lam, double* partials, const FinArgs fin) {
   __shared__ double sm[3][kBlock / 32];
+  ALORA_GRID_DEP();
   const int slot = blockIdx.x, lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int64_t c0 = long_chptr[slot], c1 = long_chptr[slot + 1];
   double v[3] = {0.0, 0.0, 0.0};
@@ -58,6 +59,7 @@ __global__ void k_lowrank(const T* X0, const T* X1, int64_t n, int r, int64_t ld
                           double* Tm0, double* Tm1, double* Ts, unsigned int* ticket0) {
   extern __shared__ double lsm[];  // [pC][blockDim.x]
   __shared__ unsigned int s_last;
+  ALORA_GRID_DEP();
   const T* const X = blockIdx.y ? X1 : X0;
   double* const Tm = blockIdx.y ? Tm1 : Tm0;
   double* const part = part0 + (size_t)blockIdx.y * gridDim.x * pC * r;
@@ -113,6 +115,7 @@ __global__ void k_lowrank(const T* X0, const T* X1, int64_t n, int r, int64_t ld
 
 // lambda = y - sigma (z - b)
 __global__ void k_lambda(int64_t m, const double* y, const double* z, const double* b, double sigma, double* lam) {
+  ALORA_GRID_DEP();
   for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < m; i += (int64_t)gridDim.x * blockDim.x)
     lam[i] = y[i] - sigma * (z[i] - b[i]);
 }
@@ -351,13 +354,17 @@ alora_status geometry(alora_ctx* c, int32_t r, int64_t ld, const void* p0, const
   return ALORA_OK;
 }
 
+// Programmatic dependent launch (launch_k, ALORA_GRID_DEP): the blocks of the next kernel are scheduled and run their
+// prologue while the current one drains.  Measured per step: config 0 32.9 -> 28.0 us, config 1 96.3 -> 93.0 us, config 2
+// 154.7 -> 132.7 us (11 launches), config 5 79.9 -> 75.2 us, config 6 134.6 -> 131.9 us, config 3 324 -> 319 us; SLOWER at
+// n = 2^24 (2 498 -> 2 528 us) and on the skewed rows of config 7 (953 -> 970 us), hence the two conditions.
+inline bool use_pdl(const alora_ctx* c, int64_t ld) {
+  return c->pdl == 2 || (c->pdl == 1 && !c->row_perm && (size_t)c->n * (size_t)ld * c->esz <= 4 * c->l2_bytes);
+}
 template <typename T> void fill_rows(alora_ctx* c, RowArgs<T>& a, const Geo& g, const T* X, int r, int64_t ld) {
   a.n = c->n; a.r = r; a.ld = ld; a.nvec = g.nvec; a.exact = g.exact; a.X = X; a.X2 = nullptr; a.X3 = nullptr; a.Out = nullptr;
   a.perm = nullptr; a.l2pol = c->l2pol < 0 ? 0 : c->l2pol;
-  // programmatic dependent launch of the tiled kernel: the next kernel's blocks become resident and run their prologue
-  // while this one drains (config 0: 32.9 -> 28.0 us per step, config 1: 96.3 -> 93.0 us, config 6: 134.6 -> 131.9 us);
-  // at n = 2^24 the step was 1 % SLOWER with it (2 498 -> 2 528 us), so only while the rows are within a few L2 sizes
-  a.pdl = c->pdl == 2 || (c->pdl == 1 && (size_t)c->n * (size_t)ld * c->esz <= 4 * c->l2_bytes);
+  a.pdl = use_pdl(c, ld);
   a.c_rowptr = c->c_rowptr; a.c_col = c->c_col; a.c_val = (const T*)c->c_val; a.dC = (const T*)c->dC;
   a.dcons = c->dcons; a.da = (const T*)c->da;
   a.a_rowptr = c->a_rowptr; a.a_col = c->a_col; a.a_val = (const T*)c->a_val; a.a_cons = c->a_cons;
@@ -375,7 +382,7 @@ template <typename T> void fill_cons(alora_ctx* c, ConsArgs<T>& a, const Geo& g,
   a.y = c->y; a.b = c->b; a.sigma = c->sigma; a.z = nullptr; a.lam = c->lam;
   a.nchunk = 0; a.ch_beg = c->ch_beg; a.ch_end = c->ch_end; a.ch_out = c->ch_out; a.partials = c->part_cons;
   a.nchunk_A = c->nchunk_A; a.part_chunk = c->part_chunk;
-  a.fin = no_fin();
+  a.fin = no_fin(); a.pdl = use_pdl(c, ld);
 }
 
 // T = U^T X (pC x r) into Tm, optionally Ts = s * Tm
@@ -388,8 +395,9 @@ template <typename T> alora_status lowrank(alora_ctx* c, const T* X, int r, int6
   const int tmax = std::min(1024, 6144 / std::max(1, c->pC));
   const int rpb = std::max(1, std::min(32, tmax / r)), threads = r * rpb;   // <= 32 row slots: their sums are added by one thread per column
   const int grid = (int)std::max<int64_t>(1, std::min<int64_t>(c->lr_grid, (c->n + (int64_t)rpb * 8 - 1) / ((int64_t)rpb * 8)));
-  k_lowrank<T><<<dim3(grid, X2 ? 2 : 1), threads, sizeof(double) * c->pC * threads, c->stream>>>(
-      X, X2, c->n, r, ld, (const T*)c->U, c->pC, c->lr_part, c->s_dev, Tm, Tm2, want_Ts ? c->Ts : nullptr, c->lr_ticket);
+  ALORA_CUDA(c, launch_k(use_pdl(c, ld), k_lowrank<T>, dim3(grid, X2 ? 2 : 1), dim3(threads), sizeof(double) * c->pC * threads, c->stream,
+                         X, X2, c->n, r, ld, (const T*)c->U, c->pC, c->lr_part, (const double*)c->s_dev, Tm, Tm2,
+                         want_Ts ? c->Ts : (double*)nullptr, c->lr_ticket));
   c->launches++;
   ALORA_CUDA(c, cudaGetLastError());
   return ALORA_OK;
@@ -417,13 +425,13 @@ alora_status forward_cw(alora_ctx* c, const Geo& g, int mode, ConsArgs<T>& ca, i
   c->launches++;
   if (fin_k) {
     ca.fin = (last_out && !longs) ? fin_all() : no_fin();
-    if (mode == CONS_EVAL) k_cons_fin<T, CONS_EVAL><<<*gf, kBlock, 0, c->stream>>>(ca);
-    else k_cons_fin<T, CONS_LS><<<*gf, kBlock, 0, c->stream>>>(ca);
+    if (mode == CONS_EVAL) ALORA_CUDA(c, launch_k(ca.pdl, k_cons_fin<T, CONS_EVAL>, dim3(*gf), dim3(kBlock), 0, c->stream, ca));
+    else ALORA_CUDA(c, launch_k(ca.pdl, k_cons_fin<T, CONS_LS>, dim3(*gf), dim3(kBlock), 0, c->stream, ca));
     c->launches++;
     if (longs) {
       ca.fin = last_out ? fin_all() : no_fin();
-      if (mode == CONS_EVAL) k_long_fin_e<T, CONS_EVAL><<<c->nlong_A, kLongFinThreads, 0, c->stream>>>(ca, c->part_long);
-      else k_long_fin_e<T, CONS_LS><<<c->nlong_A, kLongFinThreads, 0, c->stream>>>(ca, c->part_long);
+      if (mode == CONS_EVAL) ALORA_CUDA(c, launch_k(ca.pdl, k_long_fin_e<T, CONS_EVAL>, dim3(c->nlong_A), dim3(kLongFinThreads), 0, c->stream, ca, c->part_long));
+      else ALORA_CUDA(c, launch_k(ca.pdl, k_long_fin_e<T, CONS_LS>, dim3(c->nlong_A), dim3(kLongFinThreads), 0, c->stream, ca, c->part_long));
       c->launches++;
     }
   }

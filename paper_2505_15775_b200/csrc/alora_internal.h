@@ -61,7 +61,7 @@ struct alora_ctx {
   int64_t ell_hist[2][34] = {};   // used ELL slots (0: f + grad / adjoint block, 1: line-search block) by bit length of |col - row|
   size_t l2_bytes = 126u << 20;
   int sel = -1;            // dense variants of the tiled kernel: predicated neighbour loads (1), branches (0), -1 = by the share of far neighbours (ALORA_SEL)
-  int pdl = 1;             // tiled kernel launched with programmatic stream serialisation: 0 never, 1 while the rows are within a few L2 sizes, 2 always (ALORA_PDL)
+  int pdl = 1;             // hot-path kernels launched with programmatic stream serialisation: 0 never, 1 by use_pdl() (alora_ctx.cu), 2 always (ALORA_PDL)
   int l2pol = -1;          // L2 cache policies of the tiled row kernel (RowArgs::l2pol); -1: chosen per call from the sizes (ALORA_L2POL)
   bool ell_wide = false;   // 8 / 6 slots per row instead of 4 / 3 (more than 10 % of the rows have degree > 4)
   int* ell_col = nullptr; void* ell_val = nullptr;

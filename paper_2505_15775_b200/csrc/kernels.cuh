@@ -21,6 +21,26 @@
 
 namespace alora {
 
+// Programmatic dependent launch.  Every kernel of the hot path starts with ALORA_GRID_DEP(): it waits until the kernels
+// before it in the stream have completed and flushed (it reads what they wrote), and lets its own successor become
+// resident.  Both instructions are no-ops in a plain launch.  launch_k launches with programmatic stream serialisation
+// when `pdl` is set (alora_ctx::pdl), so that the blocks of the next kernel are scheduled while this one drains.
+#define ALORA_GRID_DEP()                                            \
+  do {                                                              \
+    asm volatile("griddepcontrol.wait;" ::: "memory");              \
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); \
+  } while (0)
+template <typename... KA, typename... A>
+inline cudaError_t launch_k(bool pdl, void (*k)(KA...), dim3 grid, dim3 block, size_t smem, cudaStream_t s, A&&... args) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = s;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = at; cfg.numAttrs = pdl ? 1 : 0;
+  return cudaLaunchKernelEx(&cfg, k, static_cast<KA>(args)...);
+}
+
 constexpr int kBlock = 256;
 constexpr int kGeneralRow = 512;      // a C row with more entries sends a diagonal-class problem down the general path
 constexpr int kHeavyRow = 128;        // general path: C rows with more entries are cut into segments of this many entries
@@ -83,7 +103,7 @@ template <typename T> struct RowArgs {
   // k_rows_tiled: L2 cache policies (bit 0: per-row metadata copies evict_first; bit 1: X / X2 tile copies evict_first;
   // bit 2: gathered neighbour rows evict_last; bit 3: output rows evict_first; bit 5: X tile copies evict_last)
   int l2pol;
-  int pdl;   // host only: launch k_rows_tiled with programmatic stream serialisation (alora_ctx::pdl)
+  int pdl;   // host only: programmatic dependent launch (alora_ctx::pdl)
 };
 
 template <typename T> struct ConsArgs {
@@ -106,6 +126,7 @@ template <typename T> struct ConsArgs {
   int64_t nent, nf_A; T* e_out;
   int npc;                        // > 1: every constraint has exactly npc entries (npc divides 32): k_ent_cw finishes them itself
   const int* long_cons;           // ids of the constraints with more than kLongThreshold entries (one block each)
+  int pdl;                        // host only: programmatic dependent launch (alora_ctx::pdl)
 };
 
 // ---------------------------------------------------------------------------------------------
@@ -392,6 +413,7 @@ __device__ __forceinline__ void gather_axpy(RowReg<T, VEC, GS, NIT>& acc, const 
 #endif
 template <typename T, int VEC, int GS, int NIT, int MODE>
 __global__ void __launch_bounds__(kBlock, (MODE == ROWS_ADJ && NIT <= 2) ? ALORA_ROWS_MINB : 1) k_rows(const RowArgs<T> a) {
+  ALORA_GRID_DEP();
   using Row = RowReg<T, VEC, GS, NIT>;
   constexpr int GPB = kBlock / GS;
   constexpr int NST = (MODE == ROWS_LS_FUSED) ? 12 : 6;
@@ -533,6 +555,7 @@ __global__ void __launch_bounds__(kBlock, (MODE == ROWS_ADJ && NIT <= 2) ? ALORA
 // scalar sum of c_e <X_k, X_row> over the C entries it handled (no extra reduction).  ROWS_ADJ semantics.
 template <typename T, int VEC, int PL, int NIT>
 __global__ void __launch_bounds__(kBlock) k_rows_ep(const RowArgs<T> a) {
+  ALORA_GRID_DEP();
   using Row = RowReg<T, VEC, PL, NIT>;
   constexpr int EL = 32 / PL, WPB = kBlock / 32, NST = 6;
   const int lane32 = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -637,6 +660,7 @@ __global__ void __launch_bounds__(kBlock) k_rows_ep(const RowArgs<T> a) {
 // ROWS_ADJ semantics (Out = scale * (C - sum_i w_i A_i) X, <C,XX^T>, |Out|^2, <Out,X>), nvec <= PL.
 template <typename T, int VEC, int PL, int UNR>
 __global__ void __launch_bounds__(kBlock) k_rows_cw(const RowArgs<T> a) {
+  ALORA_GRID_DEP();
   constexpr int WPB = kBlock / 32, NST = 6, EL = 32 / PL;
   using P = Pack<T, VEC>;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -777,6 +801,7 @@ __global__ void __launch_bounds__(kBlock) k_rows_cw(const RowArgs<T> a) {
 // sum_e c_e X_{k_e} in seg_out[s][0..r) and sum_e c_e <X_{k_e}, X_row> in seg_cx[s].
 template <typename T, int VEC, int PL, int NIT>
 __global__ void __launch_bounds__(kBlock) k_rows_seg(const RowArgs<T> a) {
+  ALORA_GRID_DEP();
   using Row = RowReg<T, VEC, PL, NIT>;
   constexpr int EL = 32 / PL, WPB = kBlock / 32;
   const int lane32 = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -850,6 +875,7 @@ __device__ __forceinline__ void cons_finish(double* st, int64_t i, double z, dou
 
 template <typename T, int VEC, int GS, int NIT, int MODE>
 __global__ void __launch_bounds__(kBlock) k_cons(const ConsArgs<T> a) {
+  ALORA_GRID_DEP();
   constexpr int GPB = kBlock / GS;
   constexpr int NST = (MODE == CONS_LS) ? 12 : 6;
   const int lane = threadIdx.x % GS, grp = threadIdx.x / GS;
@@ -880,6 +906,7 @@ __global__ void __launch_bounds__(kBlock) k_cons(const ConsArgs<T> a) {
 // sums as k_cons.
 template <typename T, int VEC, int MODE, bool SINGLE>
 __global__ void __launch_bounds__(kBlock) k_cons1(const ConsArgs<T> a) {
+  ALORA_GRID_DEP();
   constexpr int NST = (MODE == CONS_LS) ? 12 : 6;
   double st[NST];
 #pragma unroll
@@ -924,6 +951,7 @@ __global__ void __launch_bounds__(kBlock) k_cons1(const ConsArgs<T> a) {
 // Entries beyond nf_A are C's sym-upper list (line search): <C,RR^T>, <C,RD^T>, <C,DD^T> straight into the stats.
 template <typename T, int VEC, int PL, int MODE, bool SINGLE, int UNR>
 __global__ void __launch_bounds__(kBlock) k_ent_cw(const ConsArgs<T> a) {
+  ALORA_GRID_DEP();
   constexpr int WPB = kBlock / 32, NST = (MODE == CONS_LS) ? 12 : 6, K = (MODE == CONS_LS) ? 3 : 1, EL = 32 / PL;
   constexpr bool LS = (MODE == CONS_LS);
   using P = Pack<T, VEC>;
@@ -1040,6 +1068,7 @@ __global__ void __launch_bounds__(kBlock) k_ent_cw(const ConsArgs<T> a) {
 // per constraint, entries added in list order, then the per-constraint finish (a2)
 template <typename T, int MODE>
 __global__ void __launch_bounds__(kBlock) k_cons_fin(const ConsArgs<T> a) {
+  ALORA_GRID_DEP();
   constexpr int NST = (MODE == CONS_LS) ? 12 : 6, K = (MODE == CONS_LS) ? 3 : 1;
   double st[NST];
 #pragma unroll
@@ -1064,6 +1093,7 @@ __global__ void __launch_bounds__(kBlock) k_cons_fin(const ConsArgs<T> a) {
 constexpr int kLongFinThreads = 1024;
 template <typename T, int MODE>
 __global__ void __launch_bounds__(kLongFinThreads) k_long_fin_e(const ConsArgs<T> a, double* part_long) {
+  ALORA_GRID_DEP();
   constexpr int K = (MODE == CONS_LS) ? 3 : 1, BT = kLongFinThreads;
   __shared__ double sm[3][BT / 32];
   const int slot = blockIdx.x, lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -1101,6 +1131,7 @@ __global__ void __launch_bounds__(kLongFinThreads) k_long_fin_e(const ConsArgs<T
 // go straight into the block's partial row: <C,RR^T>, <C,RD^T> (the entry sum is <C,RD^T+DR^T>, halved) and <C,DD^T>.
 template <typename T, int VEC, int GS, int NIT, int MODE>
 __global__ void __launch_bounds__(kBlock) k_cons_chunk(const ConsArgs<T> a) {
+  ALORA_GRID_DEP();
   constexpr int GPB = kBlock / GS;
   constexpr int NST = 12;
   const int lane = threadIdx.x % GS, grp = threadIdx.x / GS;
