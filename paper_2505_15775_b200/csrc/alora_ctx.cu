@@ -302,7 +302,11 @@ template <typename T> alora_status launch_adj_general(alora_ctx* c, const Geo& g
     a.nseg = c->nseg;
     const int gs = (int)std::min<int64_t>((c->nseg + kBlock / 32 - 1) / (kBlock / 32), (int64_t)c->num_sms * 8);
     ALORA_CUDA(c, launch_rows_seg(g.vec, g.shape, a, gs, c->stream));
-    c->launches++;
+    // second level: a warp per heavy row adds its segments' results into the first segment's slot
+    const int gh = (int)std::min<int64_t>((c->nheavy + kBlock / 32 - 1) / (kBlock / 32), (int64_t)c->num_sms * 8);
+    ALORA_CUDA(c, launch_k(a.pdl != 0, k_heavy_sum<T>, dim3(std::max(1, gh)), dim3(kBlock), 0, c->stream, c->nheavy, (const int*)c->heavy_segptr,
+                           (T*)c->seg_out, c->seg_cx, g.nvec * g.vec));
+    c->launches += 2;
   }
   if (use_cw(c, g, a.r, a.ld) && !c->row_perm && !c->ep_wide) {
     // cooperative warp per row (k_rows_cw): coalesced entry metadata, one request per gathered row; not for skewed row

@@ -478,16 +478,15 @@ __global__ void __launch_bounds__(kBlock, (MODE == ROWS_ADJ && NIT <= 2) ? ALORA
       // (C X)_row : diagonal + off-diagonal gathers
       Row acc; acc.zero(); acc.axpy(dc, x);
       if (MODE == ROWS_ADJ && a.nseg > 0 && ce - cb > kHeavyRow) {
-        // heavy row: its off-diagonal C part was summed per segment by k_rows_seg; add the results in order
+        // heavy row: its off-diagonal C part was summed per segment by k_rows_seg and over the segments by k_heavy_sum
         int lo = 0, hi = a.nheavy - 1;
         while (lo < hi) { const int mid = (lo + hi) >> 1; if (__ldg(a.heavy_rows + mid) < (int)row) lo = mid + 1; else hi = mid; }
         const int s0 = __ldg(a.heavy_segptr + lo), s1 = __ldg(a.heavy_segptr + lo + 1);
         st[ES_CX] += (double)acc.dot(x);
-        for (int sg = s0; sg < s1; ++sg) {
-          Row part; part.load(a.seg_out + (int64_t)sg * (nvec * VEC), lane, nvec, r, exact);
-          acc.axpy(T(1), part);
-          if (lane == 0) st[ES_CX] += a.seg_cx[sg];
-        }
+        (void)s1;   // k_heavy_sum left the sum over the row's segments in its first segment's slot
+        Row part; part.load(a.seg_out + (int64_t)s0 * (nvec * VEC), lane, nvec, r, exact);
+        acc.axpy(T(1), part);
+        if (lane == 0) st[ES_CX] += a.seg_cx[s0];
       } else {
         gather_axpy<T, VEC, GS, NIT>(acc, a.X, a.ld, a.c_col, a.c_val, cb, ce, lane, nvec, r, exact);
         st[ES_CX] += (double)acc.dot(x);
@@ -571,16 +570,15 @@ __global__ void __launch_bounds__(kBlock) k_rows_ep(const RowArgs<T> a) {
     T cxl = T(0);
     const int cb = __ldg(a.c_rowptr + row), ce = __ldg(a.c_rowptr + row + 1);
     if (a.nseg > 0 && ce - cb > kHeavyRow) {
-      // heavy row: its C part was summed per segment by k_rows_seg; add the segment results in order
+      // heavy row: its C part was summed per segment by k_rows_seg and over the segments by k_heavy_sum
       int lo = 0, hi = a.nheavy - 1;
       while (lo < hi) { const int mid = (lo + hi) >> 1; if (__ldg(a.heavy_rows + mid) < (int)row) lo = mid + 1; else hi = mid; }
       const int s0 = __ldg(a.heavy_segptr + lo), s1 = __ldg(a.heavy_segptr + lo + 1);
+      (void)s1;   // k_heavy_sum left the sum over the row's segments in its first segment's slot
       if (el == 0) {
-        for (int sg = s0; sg < s1; ++sg) {
-          Row part; part.load(a.seg_out + (int64_t)sg * (nvec * VEC), pl, nvec, r, exact);
-          acc.axpy(T(1), part);
-        }
-        if (pl == 0) { double t = 0.0; for (int sg = s0; sg < s1; ++sg) t += a.seg_cx[sg]; st[ES_CX] += t; }
+        Row part; part.load(a.seg_out + (int64_t)s0 * (nvec * VEC), pl, nvec, r, exact);
+        acc.axpy(T(1), part);
+        if (pl == 0) st[ES_CX] += a.seg_cx[s0];
       }
     } else {
 #pragma unroll 2
@@ -730,17 +728,16 @@ __global__ void __launch_bounds__(kBlock) k_rows_cw(const RowArgs<T> a) {
     };
     const int cb = __ldg(a.c_rowptr + row), ce = __ldg(a.c_rowptr + row + 1);
     if (a.nseg > 0 && ce - cb > kHeavyRow) {
-      // heavy row: its C part was summed per segment by k_rows_seg; entry lane 0 adds the segment results in order
+      // heavy row: its C part was summed per segment by k_rows_seg and over the segments by k_heavy_sum
       int lo = 0, hi = a.nheavy - 1;
       while (lo < hi) { const int mid = (lo + hi) >> 1; if (__ldg(a.heavy_rows + mid) < (int)row) lo = mid + 1; else hi = mid; }
       const int s0 = __ldg(a.heavy_segptr + lo), s1 = __ldg(a.heavy_segptr + lo + 1);
+      (void)s1;   // k_heavy_sum left the sum over the row's segments in its first segment's slot
       if (el == 0) {
-        for (int sg = s0; sg < s1; ++sg) {
-          const P part = load_pack(a.seg_out + (int64_t)sg * (nvec * VEC) + plc * VEC);
+        const P part = load_pack(a.seg_out + (int64_t)s0 * (nvec * VEC) + plc * VEC);
 #pragma unroll
-          for (int i = 0; i < VEC; ++i) acc.v[i] += part.v[i];
-        }
-        if (lane == 0) { double t = 0.0; for (int sg = s0; sg < s1; ++sg) t += a.seg_cx[sg]; st[ES_CX] += t; }
+        for (int i = 0; i < VEC; ++i) acc.v[i] += part.v[i];
+        if (lane == 0) st[ES_CX] += a.seg_cx[s0];
       }
     } else {
       walk(a.c_col, a.c_val, nullptr, cb, ce);
@@ -830,6 +827,45 @@ __global__ void __launch_bounds__(kBlock) k_rows_seg(const RowArgs<T> a) {
     const double cx = warp_sum((double)cxl);
     if (el == 0) acc.store(a.seg_out + (int64_t)sg * (nvec * VEC), pl, nvec, r, exact);
     if (lane32 == 0) a.seg_cx[sg] = cx;
+  }
+}
+
+// Second level of the heavy-row sums: a warp per heavy row adds the partial rows (and the <C X, X> parts) of the row's
+// segments in a fixed order and leaves the total in the FIRST segment's slot, which is all the row kernels then read.
+// Before, the group that owned the row added its segments one dependent load at a time -- 308 segments for the
+// largest row of config 7 -- and the whole grid waited for that group (ncu: the SMs were active for 42 % of the
+// adjoint kernel's duration).  Lanes: PW = smallest power of two >= P elements of a partial row (capped at 32) take the
+// elements, the 32 / PW lane groups take every (32 / PW)-th segment; the groups' sums are then added in group order.
+template <typename T>
+__global__ void __launch_bounds__(kBlock) k_heavy_sum(int nheavy, const int* __restrict__ heavy_segptr, T* seg_out, double* seg_cx, int P) {
+  ALORA_GRID_DEP();
+  constexpr int WPB = kBlock / 32;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  int PW = 1; while (PW < P && PW < 32) PW <<= 1;
+  const int NG = 32 / PW, g = lane / PW, el0 = lane % PW;
+  for (int h = blockIdx.x * WPB + warp; h < nheavy; h += gridDim.x * WPB) {
+    const int s0 = __ldg(heavy_segptr + h), s1 = __ldg(heavy_segptr + h + 1);
+    double cx = 0.0;
+    for (int sg = s0 + lane; sg < s1; sg += 32) cx += __ldcg(seg_cx + sg);
+    cx = warp_sum(cx);
+    for (int eb = 0; eb < P; eb += PW) {   // one pass unless a partial row has more than 32 elements
+      const int el = eb + el0;
+      T acc = T(0);
+      if (el < P) {
+        int sg = s0 + g;
+        for (; sg + 3 * NG < s1; sg += 4 * NG) {   // four loads in flight, added in segment order
+          const T v0 = __ldcg(seg_out + (int64_t)sg * P + el), v1 = __ldcg(seg_out + (int64_t)(sg + NG) * P + el);
+          const T v2 = __ldcg(seg_out + (int64_t)(sg + 2 * NG) * P + el), v3 = __ldcg(seg_out + (int64_t)(sg + 3 * NG) * P + el);
+          acc += v0; acc += v1; acc += v2; acc += v3;
+        }
+        for (; sg < s1; sg += NG) acc += __ldcg(seg_out + (int64_t)sg * P + el);
+      }
+      T tot = T(0);
+      for (int q = 0; q < NG; ++q) tot += __shfl_sync(0xffffffffu, acc, q * PW + el0);   // groups in order
+      __syncwarp();   // every lane has read its segments before the first slot is overwritten
+      if (g == 0 && el < P) seg_out[(int64_t)s0 * P + el] = tot;
+    }
+    if (lane == 0) seg_cx[s0] = cx;
   }
 }
 
