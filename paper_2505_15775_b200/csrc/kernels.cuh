@@ -853,10 +853,12 @@ __global__ void __launch_bounds__(kBlock) k_heavy_sum(int nheavy, const int* __r
       T acc = T(0);
       if (el < P) {
         int sg = s0 + g;
-        for (; sg + 3 * NG < s1; sg += 4 * NG) {   // four loads in flight, added in segment order
-          const T v0 = __ldcg(seg_out + (int64_t)sg * P + el), v1 = __ldcg(seg_out + (int64_t)(sg + NG) * P + el);
-          const T v2 = __ldcg(seg_out + (int64_t)(sg + 2 * NG) * P + el), v3 = __ldcg(seg_out + (int64_t)(sg + 3 * NG) * P + el);
-          acc += v0; acc += v1; acc += v2; acc += v3;
+        for (; sg + 7 * NG < s1; sg += 8 * NG) {   // eight loads in flight, added in segment order
+          T v[8];
+#pragma unroll
+          for (int u = 0; u < 8; ++u) v[u] = __ldcg(seg_out + (int64_t)(sg + u * NG) * P + el);
+#pragma unroll
+          for (int u = 0; u < 8; ++u) acc += v[u];
         }
         for (; sg < s1; sg += NG) acc += __ldcg(seg_out + (int64_t)sg * P + el);
       }
