@@ -438,13 +438,29 @@ def main():
     ms = aggregate_ms(ms, world)
     value = whole_job_value(args.steps, world, ms)
 
+    # the same step with the WARM line search (what alora_solve and alora_step_host run: the line search follows an
+    # evaluation of the same R and streams its gradient, reading 31) -- reported beside the cold-form `value`
+    pls = ctx.get_linesearch()    # coefficients of the last cold line search of the timed region
+    def step_warm():
+        ctx.eval(R, r, ld, G, z, stats=False)
+        ctx.linesearch(R, D, r, ld, fetch=False, warm=True)
+        ctx.smatvec(lam, V, 1, W, fetch=False)
+    for _ in range(3):
+        step_warm()
+    barrier(); e0.record()
+    for _ in range(args.steps):
+        step_warm()
+    e1.record(); barrier()
+    ms_warm = aggregate_ms(e0.elapsed_time(e1), world)
+    pls_warm = ctx.get_linesearch()
+
     # eval-only rate (the metric's bare "f+grad evals/s"), same hygiene
     barrier(); e0.record()
     for _ in range(args.steps):
         ctx.eval(R, r, ld, G, z, stats=False)
     e1.record(); barrier()
     eval_only = args.steps / (e0.elapsed_time(e1) * 1e-3)
-    st = ctx.get_stats(); pls = ctx.get_linesearch()
+    st = ctx.get_stats()
 
     # L2-flushed figures (configs whose arrays fit in L2): a 256 MB scratch write before every step, each step timed
     # by its own event pair so that the flush is outside the timed spans
@@ -514,9 +530,12 @@ def main():
                         "l2": ("no flush: the step's arrays (%.0f MB per evaluation) exceed the 126 MB L2 several times" % (B_eval / 1e6))
                         if not resident else "value is L2-warm (the evaluation's %.0f MB fit in L2); see `flushed`" % (B_eval / 1e6),
                         "timing": "CUDA events on the ctx stream around K steps; dominant kernel by event pairs inside alora_eval"},
-                "eval_only_per_s": eval_only, "roofline": roof, "flushed": flushed,
+                "eval_only_per_s": eval_only,
+                "warm_linesearch": {"value": whole_job_value(args.steps, world, ms_warm), "unit": UNIT, "ms_per_step": ms_warm / args.steps,
+                                    "what": "same step with alora_linesearch(warm=1): p1 = <G,D> from the evaluation's gradient, only the D operand gathered"},
+                "roofline": roof, "flushed": flushed,
                 "gpu_launches": int(launches), "clocks": clocks, "e2e": e2e,
-                "check": {"f": st[0], "gnorm": float(np.sqrt(st[4])), "p": [float(x) for x in pls]}}
+                "check": {"f": st[0], "gnorm": float(np.sqrt(st[4])), "p": [float(x) for x in pls], "p_warm": [float(x) for x in pls_warm]}}
         if not args.no_cpu_baseline and world == 1:
             sec, k = oracle_step_seconds(w)
             cb = {"value": 1.0 / sec, "unit": UNIT, "cores": 1, "kind": "oracle",
