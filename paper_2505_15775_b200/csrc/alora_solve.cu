@@ -96,52 +96,79 @@ struct LbCoef { double cg; double cs[kLbMax]; double cy[kLbMax]; };
 //   [j] S_j.G   [np + j] Y_j.G   [2np + j] S_new.Y_j   [3np + j] S_j.Y_new   [4np + j] Y_new.Y_j   [5np] S_new.S_new
 // (the last four only if have_new).  Partial rows of kLbW doubles per block; the block that finishes last adds
 // them in block order into out[kLbW].
-template <typename T, int NP>
-__global__ void __launch_bounds__(kBlock) k_lbfgs_dots(int64_t N, int have_new, double alpha, const T* D, const T* G, const T* Gp,
-                                                       LbVecs v, T* Snew, T* Ynew, double* part, double* out,
-                                                       unsigned int* ticket) {
-  constexpr int VEC = 16 / (int)sizeof(T);
-  double sg[NP], yg[NP], sny[NP], syn[NP], yyn[NP], ss = 0.0;
+// The two halves of a block (threads 0..127 / 128..255) take the same 128 packs of an iteration and the even / odd pairs
+// of the list, so a thread carries the sums of at most (NP + 1) / 2 pairs: about 70 registers and three blocks per SM
+// instead of 128 - 142 registers and one or two (ncu, config 4 inside alora_solve: 3.2 TB/s with every product in fp64,
+// 4.3 TB/s with pack-local sums, both bound by registers / the fp64 pipe rather than HBM; over 40 % of the solve's GPU
+// time).  G, D, Gp are read by both halves (the second read hits L1 / L2).
+// The VEC products of a pack are summed in the vector type (fp32 contexts: FFMA) and enter the fp64 sums once per pack:
+// the library's precision model -- products and short local sums in the context type, everything that crosses rows in
+// fp64.
+template <typename T, int NP, int PAR>
+__device__ __forceinline__ void lbfgs_dots_half(int64_t nv, int have_new, double alpha, const T* D, const T* G, const T* Gp, const LbVecs& v,
+                                                T* Snew, T* Ynew, double (*sm)[kBlock / 32]) {
+  constexpr int VEC = 16 / (int)sizeof(T), HB = kBlock / 2;
+  constexpr int NH = (NP - PAR + 1) / 2;        // pairs j = PAR, PAR + 2, ... < NP
+  double sg[NH > 0 ? NH : 1], yg[NH > 0 ? NH : 1], sny[NH > 0 ? NH : 1], syn[NH > 0 ? NH : 1], yyn[NH > 0 ? NH : 1], ss = 0.0;
 #pragma unroll
-  for (int j = 0; j < NP; ++j) { sg[j] = yg[j] = sny[j] = syn[j] = yyn[j] = 0.0; }
-  const int64_t nv = N / VEC;
-  for (int64_t i = (int64_t)blockIdx.x * kBlock + threadIdx.x; i < nv; i += (int64_t)gridDim.x * kBlock) {
+  for (int h = 0; h < NH; ++h) { sg[h] = yg[h] = sny[h] = syn[h] = yyn[h] = 0.0; }
+  const int tx = threadIdx.x % HB;
+  for (int64_t i = (int64_t)blockIdx.x * HB + tx; i < nv; i += (int64_t)gridDim.x * HB) {
     const Pack<T, VEC> g = reinterpret_cast<const Pack<T, VEC>*>(G)[i];
     Pack<T, VEC> sn, yn;
     if (have_new) {
       const Pack<T, VEC> d = reinterpret_cast<const Pack<T, VEC>*>(D)[i], gp = reinterpret_cast<const Pack<T, VEC>*>(Gp)[i];
 #pragma unroll
       for (int k = 0; k < VEC; ++k) { sn.v[k] = (T)(alpha * (double)d.v[k]); yn.v[k] = (T)((double)g.v[k] - (double)gp.v[k]); }
-      reinterpret_cast<Pack<T, VEC>*>(Snew)[i] = sn;
-      reinterpret_cast<Pack<T, VEC>*>(Ynew)[i] = yn;
+      if (PAR == 0) {
+        reinterpret_cast<Pack<T, VEC>*>(Snew)[i] = sn;
+        reinterpret_cast<Pack<T, VEC>*>(Ynew)[i] = yn;
+      }
     }
 #pragma unroll
-    for (int j = 0; j < NP; ++j) {
+    for (int h = 0; h < NH; ++h) {
+      const int j = PAR + 2 * h;
       Pack<T, VEC> sj, yj;
       if (have_new && j == NP - 1) { sj = sn; yj = yn; }
       else { sj = reinterpret_cast<const Pack<T, VEC>*>(v.S[j])[i]; yj = reinterpret_cast<const Pack<T, VEC>*>(v.Y[j])[i]; }
+      T a0 = T(0), a1 = T(0), a2 = T(0), a3 = T(0), a4 = T(0);
 #pragma unroll
       for (int k = 0; k < VEC; ++k) {
-        const double gs = (double)g.v[k], s_ = (double)sj.v[k], y_ = (double)yj.v[k];
-        sg[j] += s_ * gs; yg[j] += y_ * gs;
-        if (have_new) {
-          const double sn_ = (double)sn.v[k], yn_ = (double)yn.v[k];
-          sny[j] += sn_ * y_; syn[j] += s_ * yn_; yyn[j] += yn_ * y_;
-        }
+        a0 = fma(sj.v[k], g.v[k], a0); a1 = fma(yj.v[k], g.v[k], a1);
+        if (have_new) { a2 = fma(sn.v[k], yj.v[k], a2); a3 = fma(sj.v[k], yn.v[k], a3); a4 = fma(yn.v[k], yj.v[k], a4); }
       }
+      sg[h] += (double)a0; yg[h] += (double)a1;
+      if (have_new) { sny[h] += (double)a2; syn[h] += (double)a3; yyn[h] += (double)a4; }
     }
-    if (have_new) {
+    if (PAR == 0 && have_new) {
+      T a = T(0);
 #pragma unroll
-      for (int k = 0; k < VEC; ++k) ss += (double)sn.v[k] * (double)sn.v[k];
+      for (int k = 0; k < VEC; ++k) a = fma(sn.v[k], sn.v[k], a);
+      ss += (double)a;
     }
   }
-  __shared__ double sm[kLbW][kBlock / 32];
-  __shared__ unsigned int s_last;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   auto put = [&](int slot, double val) { const double t = warp_sum(val); if (lane == 0) sm[slot][warp] = t; };
 #pragma unroll
-  for (int j = 0; j < NP; ++j) { put(j, sg[j]); put(NP + j, yg[j]); put(2 * NP + j, sny[j]); put(3 * NP + j, syn[j]); put(4 * NP + j, yyn[j]); }
-  put(5 * NP, ss);
+  for (int h = 0; h < NH; ++h) {
+    const int j = PAR + 2 * h;
+    put(j, sg[h]); put(NP + j, yg[h]); put(2 * NP + j, sny[h]); put(3 * NP + j, syn[h]); put(4 * NP + j, yyn[h]);
+  }
+  if (PAR == 0) put(5 * NP, ss);
+}
+
+template <typename T, int NP>
+__global__ void __launch_bounds__(kBlock, 3) k_lbfgs_dots(int64_t N, int have_new, double alpha, const T* D, const T* G, const T* Gp,
+                                                          LbVecs v, T* Snew, T* Ynew, double* part, double* out,
+                                                          unsigned int* ticket) {
+  constexpr int VEC = 16 / (int)sizeof(T);
+  __shared__ double sm[kLbW][kBlock / 32];
+  __shared__ unsigned int s_last;
+  for (int t = threadIdx.x; t < kLbW * (kBlock / 32); t += kBlock) (&sm[0][0])[t] = 0.0;   // a warp fills only its half's slots
+  __syncthreads();
+  const int64_t nv = N / VEC;
+  if (threadIdx.x < kBlock / 2) lbfgs_dots_half<T, NP, 0>(nv, have_new, alpha, D, G, Gp, v, Snew, Ynew, sm);
+  else lbfgs_dots_half<T, NP, 1>(nv, have_new, alpha, D, G, Gp, v, Snew, Ynew, sm);
   __syncthreads();
   if (threadIdx.x < kLbW) {
     double t = 0.0;
@@ -207,35 +234,63 @@ template <typename T> __global__ void k_axpy2(int64_t N, const double* a_dev, co
   for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (int64_t)gridDim.x * blockDim.x)
     w[i] = (T)((double)w[i] - a * (double)v[i] - (u ? b * (double)u[i] : 0.0));
 }
-// c[j] = <V_j, w> for j < k: V is k x N (row j contiguous), blockIdx.y = j, nchunk blocks per j leave partial sums;
-// the block that draws the last ticket adds the chunks of every j in order (no separate reduction launch)
+// c[j] = <V_j, w> for j < k: V is k x N (row j contiguous).  blockIdx.y takes kBasisJB consecutive vectors j (w is read
+// once for all of them, 16-byte loads when N is a multiple of the pack), nchunk blocks per group leave partial sums;
+// the block that draws the last ticket adds the chunks of every j in order (no separate reduction launch).
+// (Before: one vector per blockIdx.y and 4-byte loads -- w was re-read for every j and the kernel ran at 2.8 TB/s.)
+constexpr int kBasisJB = 4;
 template <typename T>
 __global__ void __launch_bounds__(kBlock) k_basis_dots(int64_t N, const T* V, const T* w, double* part, int nchunk, int k,
                                                        double* c, unsigned int* ticket) {
-  const int j = blockIdx.y;
-  const T* vj = V + (int64_t)j * N;
-  double st[1] = {0.0};
-  for (int64_t i = (int64_t)blockIdx.x * kBlock + threadIdx.x; i < N; i += (int64_t)gridDim.x * kBlock)
-    st[0] += (double)vj[i] * (double)w[i];
-  __shared__ double sm[kBlock / 32];
+  constexpr int VEC = 16 / (int)sizeof(T), JB = kBasisJB;
+  const int j0 = blockIdx.y * JB, nj = min(JB, k - j0);
+  double st[JB];
+#pragma unroll
+  for (int q = 0; q < JB; ++q) st[q] = 0.0;
+  if (N % VEC == 0) {
+    const int64_t nv = N / VEC;
+    for (int64_t i = (int64_t)blockIdx.x * kBlock + threadIdx.x; i < nv; i += (int64_t)gridDim.x * kBlock) {
+      const Pack<T, VEC> wv = reinterpret_cast<const Pack<T, VEC>*>(w)[i];
+      Pack<T, VEC> vv[JB];
+#pragma unroll
+      for (int q = 0; q < JB; ++q) if (q < nj) vv[q] = reinterpret_cast<const Pack<T, VEC>*>(V + (int64_t)(j0 + q) * N)[i];
+#pragma unroll
+      for (int q = 0; q < JB; ++q) if (q < nj) {
+        T a = T(0);
+#pragma unroll
+        for (int e = 0; e < VEC; ++e) a = fma(vv[q].v[e], wv.v[e], a);
+        st[q] += (double)a;
+      }
+    }
+  } else {
+    for (int64_t i = (int64_t)blockIdx.x * kBlock + threadIdx.x; i < N; i += (int64_t)gridDim.x * kBlock) {
+      const double wi = (double)w[i];
+#pragma unroll
+      for (int q = 0; q < JB; ++q) if (q < nj) st[q] += (double)V[(int64_t)(j0 + q) * N + i] * wi;
+    }
+  }
+  __shared__ double sm[JB][kBlock / 32];
   __shared__ unsigned int s_last;
-  const double v = warp_sum(st[0]);
-  if ((threadIdx.x & 31) == 0) sm[threadIdx.x >> 5] = v;
+#pragma unroll
+  for (int q = 0; q < JB; ++q) { const double v = warp_sum(st[q]); if ((threadIdx.x & 31) == 0) sm[q][threadIdx.x >> 5] = v; }
   __syncthreads();
   if (threadIdx.x == 0) {
-    double t = 0.0;
-    for (int wv = 0; wv < kBlock / 32; ++wv) t += sm[wv];
-    part[(int64_t)j * nchunk + blockIdx.x] = t;
+    for (int q = 0; q < nj; ++q) {
+      double t = 0.0;
+      for (int wv = 0; wv < kBlock / 32; ++wv) t += sm[q][wv];
+      part[(int64_t)(j0 + q) * nchunk + blockIdx.x] = t;
+    }
     __threadfence();
     s_last = (atomicAdd(ticket, 1u) == gridDim.x * gridDim.y - 1) ? 1u : 0u;
   }
   __syncthreads();
   if (!s_last) return;
   __threadfence();
-  for (int jj = threadIdx.x; jj < k; jj += kBlock) {
+  for (int jj = threadIdx.x >> 5; jj < k; jj += kBlock / 32) {   // a warp per vector: lanes over the chunks, then an ordered warp sum
     double t = 0.0;
-    for (int i = 0; i < nchunk; ++i) t += __ldcg(part + (int64_t)jj * nchunk + i);
-    c[jj] = t;
+    for (int i = threadIdx.x & 31; i < nchunk; i += 32) t += __ldcg(part + (int64_t)jj * nchunk + i);
+    t = warp_sum(t);
+    if ((threadIdx.x & 31) == 0) c[jj] = t;
   }
   if (threadIdx.x == 0) *ticket = 0u;
 }
@@ -245,12 +300,48 @@ template <typename T>
 __global__ void __launch_bounds__(kBlock) k_basis_combine(int64_t N, int k, const T* V, const double* c, double beta, double sign, T* out,
                                                           double* part, double* nrm, unsigned int* ticket) {
   double st[1] = {0.0};
-  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (int64_t)gridDim.x * blockDim.x) {
-    double t = 0.0;
-    for (int j = 0; j < k; ++j) t += c[j] * (double)V[(int64_t)j * N + i];
-    const T o = (T)((beta != 0.0 ? beta * (double)out[i] : 0.0) + sign * t);
-    out[i] = o;
-    st[0] += (double)o * (double)o;
+  constexpr int VEC = 16 / (int)sizeof(T);
+  if (N % VEC == 0) {   // 16-byte loads, four basis vectors in flight per thread (the scalar form ran at 3.1 TB/s)
+    const int64_t nv = N / VEC;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < nv; i += (int64_t)gridDim.x * blockDim.x) {
+      double t[VEC];
+#pragma unroll
+      for (int e = 0; e < VEC; ++e) t[e] = 0.0;
+      int j = 0;
+      for (; j + 4 <= k; j += 4) {
+        Pack<T, VEC> vv[4];
+#pragma unroll
+        for (int q = 0; q < 4; ++q) vv[q] = reinterpret_cast<const Pack<T, VEC>*>(V + (int64_t)(j + q) * N)[i];
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+          const double cj = __ldg(c + j + q);
+#pragma unroll
+          for (int e = 0; e < VEC; ++e) t[e] += cj * (double)vv[q].v[e];
+        }
+      }
+      for (; j < k; ++j) {
+        const Pack<T, VEC> vv = reinterpret_cast<const Pack<T, VEC>*>(V + (int64_t)j * N)[i];
+        const double cj = __ldg(c + j);
+#pragma unroll
+        for (int e = 0; e < VEC; ++e) t[e] += cj * (double)vv.v[e];
+      }
+      Pack<T, VEC> o;
+      if (beta != 0.0) o = reinterpret_cast<const Pack<T, VEC>*>(out)[i];
+#pragma unroll
+      for (int e = 0; e < VEC; ++e) {
+        o.v[e] = (T)((beta != 0.0 ? beta * (double)o.v[e] : 0.0) + sign * t[e]);
+        st[0] += (double)o.v[e] * (double)o.v[e];
+      }
+      reinterpret_cast<Pack<T, VEC>*>(out)[i] = o;
+    }
+  } else {
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (int64_t)gridDim.x * blockDim.x) {
+      double t = 0.0;
+      for (int j = 0; j < k; ++j) t += c[j] * (double)V[(int64_t)j * N + i];
+      const T o = (T)((beta != 0.0 ? beta * (double)out[i] : 0.0) + sign * t);
+      out[i] = o;
+      st[0] += (double)o * (double)o;
+    }
   }
   if (!nrm) return;
   __shared__ double sm[kBlock / 32];
@@ -345,6 +436,7 @@ struct SolveWorkspace {
   double* bd_part = nullptr; double* cvec = nullptr; int bd_chunks = 0;
   double* red_part = nullptr; double* red_out = nullptr;
   double* lb_part = nullptr; double* lb_out = nullptr;   // k_lbfgs_dots partial rows / result
+  int occ_dots[kLbMax + 1] = {}, occ_comb[kLbMax + 1] = {};   // resident blocks per SM of k_lbfgs_dots / k_lbfgs_combine by pair count
   // solve
   static constexpr int kNBuf = 5 + 2 * (kMemMax + 1);   // R, G, D, Gprev, Rtmp + (mem + 1) slots each of S and Y
   void* buf[kNBuf] = {}; int nbuf = 0; int64_t buf_elems = 0;
@@ -672,7 +764,7 @@ alora_status lanczos_impl(alora_ctx* c, const double* mu, int kmax, double tol_a
   kmax = (int)std::min<int64_t>(std::max(1, kmax), n);
   if (w->V_cap < kmax) {
     if (w->V) { c->pool.release(w->V); c->pool.release(w->bd_part); c->pool.release(w->cvec); }
-    w->bd_chunks = (int)std::max<int64_t>(1, std::min<int64_t>((n + kBlock * 8 - 1) / (kBlock * 8), 64));
+    w->bd_chunks = (int)std::max<int64_t>(1, std::min<int64_t>((n + kBlock * 8 - 1) / (kBlock * 8), 256));   // x ceil(k / kBasisJB) blocks
     ALORA_CUDA(c, c->pool.alloc(&w->V, c->esz * (size_t)n * kmax));
     ALORA_CUDA(c, c->pool.alloc((void**)&w->bd_part, sizeof(double) * (size_t)kmax * w->bd_chunks));
     ALORA_CUDA(c, c->pool.alloc((void**)&w->cvec, sizeof(double) * kmax));
@@ -700,7 +792,7 @@ alora_status lanczos_impl(alora_ctx* c, const double* mu, int kmax, double tol_a
     k_axpy2<T><<<g, 256, 0, c->stream>>>(n, c->mv_dev + ES_GR, vk, k ? be.back() : 0.0, k ? vk - n : (const T*)nullptr, wv);
     c->launches++;
     for (int pass = 0; pass < 2; ++pass) {  // classical Gram-Schmidt against V[0..k], twice
-      k_basis_dots<T><<<dim3(w->bd_chunks, k + 1), kBlock, 0, c->stream>>>(n, V, wv, w->bd_part, w->bd_chunks, k + 1, w->cvec, c->ticket);
+      k_basis_dots<T><<<dim3(w->bd_chunks, (k + 1 + kBasisJB - 1) / kBasisJB), kBlock, 0, c->stream>>>(n, V, wv, w->bd_part, w->bd_chunks, k + 1, w->cvec, c->ticket);
       k_basis_combine<T><<<g, kBlock, 0, c->stream>>>(n, k + 1, V, w->cvec, 1.0, -1.0, wv, w->red_part, pass ? w->red_out : nullptr, c->ticket);
       c->launches += 2;
     }
@@ -888,12 +980,24 @@ template <typename T>
 alora_status lbfgs_dots_enqueue(alora_ctx* c, int64_t N, int np, bool have_new, double alpha, const T* D, const T* G, const T* Gp,
                                 const LbVecs& v, T* Snew, T* Ynew) {
   SolveWorkspace* w = c->ws;
-  const int grid = (int)std::max<int64_t>(1, std::min<int64_t>((N / (16 / (int64_t)sizeof(T)) + kBlock - 1) / kBlock, kRedBlocks));
+  if (np < 1 || np > kLbMax) return fail(c, ALORA_EINVAL, "lbfgs_dots: too many pairs");
+  // A grid-stride kernel is launched with exactly the blocks that are resident at once: a fixed 592 (four per SM) left
+  // a partial second wave as soon as three fitted (ncu, config 4: SMs active 79 % of the kernel, 4.1 TB/s).
+  int& occ = w->occ_dots[np];
+  if (!occ) {
+    switch (np) {
+#define X(NP) case NP: cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_lbfgs_dots<T, NP>, kBlock, 0); break;
+      X(1) X(2) X(3) X(4) X(5) X(6) X(7) X(8)
+#undef X
+    }
+    occ = std::max(1, occ);
+  }
+  const int grid = (int)std::max<int64_t>(1, std::min<int64_t>((N / (16 / (int64_t)sizeof(T)) + kBlock / 2 - 1) / (kBlock / 2),   // 128 packs per block and pass
+                                                               std::min<int64_t>((int64_t)c->num_sms * occ, kRedBlocks)));
   switch (np) {
 #define X(NP) case NP: k_lbfgs_dots<T, NP><<<grid, kBlock, 0, c->stream>>>(N, have_new ? 1 : 0, alpha, D, G, Gp, v, Snew, Ynew, w->lb_part, w->lb_out, c->ticket); break;
     X(1) X(2) X(3) X(4) X(5) X(6) X(7) X(8)
 #undef X
-    default: return fail(c, ALORA_EINVAL, "lbfgs_dots: too many pairs");
   }
   c->launches++;
   ALORA_CUDA(c, cudaMemcpyAsync(c->pinned + kLbPinned, w->lb_out, sizeof(double) * kLbW, cudaMemcpyDeviceToHost, c->stream));
@@ -901,12 +1005,21 @@ alora_status lbfgs_dots_enqueue(alora_ctx* c, int64_t N, int np, bool have_new, 
 }
 template <typename T>
 alora_status lbfgs_combine(alora_ctx* c, int64_t N, int np, const T* G, const LbVecs& v, const LbCoef& cf, T* D) {
-  const int grid = (int)std::max<int64_t>(1, std::min<int64_t>((N / (16 / (int64_t)sizeof(T)) + kBlock - 1) / kBlock, (int64_t)c->num_sms * 8));
+  if (np < 1 || np > kLbMax) return fail(c, ALORA_EINVAL, "lbfgs_combine: too many pairs");
+  int& occ = c->ws->occ_comb[np];
+  if (!occ) {
+    switch (np) {
+#define X(NP) case NP: cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_lbfgs_combine<T, NP>, kBlock, 0); break;
+      X(1) X(2) X(3) X(4) X(5) X(6) X(7) X(8)
+#undef X
+    }
+    occ = std::max(1, occ);
+  }
+  const int grid = (int)std::max<int64_t>(1, std::min<int64_t>((N / (16 / (int64_t)sizeof(T)) + kBlock - 1) / kBlock, (int64_t)c->num_sms * occ));
   switch (np) {
 #define X(NP) case NP: k_lbfgs_combine<T, NP><<<grid, kBlock, 0, c->stream>>>(N, G, v, cf, D); break;
     X(1) X(2) X(3) X(4) X(5) X(6) X(7) X(8)
 #undef X
-    default: return fail(c, ALORA_EINVAL, "lbfgs_combine: too many pairs");
   }
   c->launches++;
   ALORA_CUDA(c, cudaGetLastError());
