@@ -48,13 +48,17 @@ template <typename T, bool READ_Y, typename F> __device__ __forceinline__ void e
   const bool al = (((uintptr_t)x | (uintptr_t)y) & 15) == 0;
   const int64_t nv = al ? N / VEC : 0;
   const int64_t tid = (int64_t)blockIdx.x * blockDim.x + threadIdx.x, nth = (int64_t)gridDim.x * blockDim.x;
-  for (int64_t i = tid; i < nv; i += nth) {
-    const Pack<T, VEC> xv = reinterpret_cast<const Pack<T, VEC>*>(x)[i];
-    Pack<T, VEC> yv;
-    if (READ_Y) yv = reinterpret_cast<Pack<T, VEC>*>(y)[i];
+  for (int64_t i = tid; i < nv; i += 2 * nth) {   // two packs per thread in flight (the grid is four blocks per SM, see ew_grid)
+    const int64_t i1 = i + nth;
+    const bool two = i1 < nv;
+    const Pack<T, VEC> xv0 = reinterpret_cast<const Pack<T, VEC>*>(x)[i];
+    Pack<T, VEC> xv1 = xv0, yv0, yv1;
+    if (two) xv1 = reinterpret_cast<const Pack<T, VEC>*>(x)[i1];
+    if (READ_Y) { yv0 = reinterpret_cast<Pack<T, VEC>*>(y)[i]; if (two) yv1 = reinterpret_cast<Pack<T, VEC>*>(y)[i1]; }
 #pragma unroll
-    for (int k = 0; k < VEC; ++k) yv.v[k] = f(xv.v[k], READ_Y ? yv.v[k] : T(0));
-    reinterpret_cast<Pack<T, VEC>*>(y)[i] = yv;
+    for (int k = 0; k < VEC; ++k) { yv0.v[k] = f(xv0.v[k], READ_Y ? yv0.v[k] : T(0)); yv1.v[k] = f(xv1.v[k], READ_Y ? yv1.v[k] : T(0)); }
+    reinterpret_cast<Pack<T, VEC>*>(y)[i] = yv0;
+    if (two) reinterpret_cast<Pack<T, VEC>*>(y)[i1] = yv1;
   }
   for (int64_t i = nv * VEC + tid; i < N; i += nth) y[i] = f(x[i], READ_Y ? y[i] : T(0));
 }
@@ -639,8 +643,11 @@ void jacobi_eigh(std::vector<double>& M, int r, std::vector<double>& mu, std::ve
   Q.swap(Qs);
 }
 
+// grid of the element-wise / streaming kernels: four blocks of 256 threads per SM are resident at once for every kernel of
+// this file with <= 64 registers; with eight (the former value) the 40 - 44 register kernels (k_axpy, k_basis_combine) had six
+// or five resident and ran a partial second wave (ncu: R += alpha D at 5.9 TB/s)
 inline int ew_grid(alora_ctx* c, int64_t N) {
-  return (int)std::max<int64_t>(1, std::min<int64_t>((N + 255) / 256, (int64_t)c->num_sms * 8));
+  return (int)std::max<int64_t>(1, std::min<int64_t>((N + 255) / 256, (int64_t)c->num_sms * 4));
 }
 
 }  // namespace
@@ -789,7 +796,7 @@ alora_status lanczos_impl(alora_ctx* c, const double* mu, int kmax, double tol_a
     T* vk = V + (int64_t)k * n;
     s = alora_smatvec(c, mu, vk, 1, wv, nullptr); if (s != ALORA_OK) return s;
     if (n_matvec) ++*n_matvec;
-    k_axpy2<T><<<g, 256, 0, c->stream>>>(n, c->mv_dev + ES_GR, vk, k ? be.back() : 0.0, k ? vk - n : (const T*)nullptr, wv);
+    k_axpy2<T><<<2 * g, 256, 0, c->stream>>>(   /* scalar loads, 30 - 32 registers: eight blocks per SM are resident */n, c->mv_dev + ES_GR, vk, k ? be.back() : 0.0, k ? vk - n : (const T*)nullptr, wv);
     c->launches++;
     for (int pass = 0; pass < 2; ++pass) {  // classical Gram-Schmidt against V[0..k], twice
       k_basis_dots<T><<<dim3(w->bd_chunks, (k + 1 + kBasisJB - 1) / kBasisJB), kBlock, 0, c->stream>>>(n, V, wv, w->bd_part, w->bd_chunks, k + 1, w->cvec, c->ticket);
